@@ -1,0 +1,127 @@
+/* fx.h -- C ABI of libfx.so: the data-parallel hot path of arXiv:1807.01971 (Feltor) on one B200.
+ *
+ * The preconditioned conjugate-gradient solve of the 2-D discontinuous-Galerkin elliptic equation
+ *     div( chi grad phi ) = rho            (the gyro-fluid form div(N grad_perp phi) = n - N is Eq. (1c))
+ * built, as the paper prescribes for its "Level 2" algorithms, from "Level 1" vector and matrix primitives only
+ * (PAPER.md:75-76): the exactly rounded dot product (section 3.1), axpby and pointwise multiply
+ * with a fixed order of explicitly fused operations (section 3.2), and the dG block-stencil
+ * matrix-vector product (section 4.1).  "P:n" below = PAPER.md line n; "D:x" = DESIGN.md section x.
+ *
+ * Conventions for every call
+ *   - pointers named *_dev / documented "device" are CUDA device pointers on the current device, owned by the caller,
+ *     never retained or freed by the library; pointers documented "host" are ordinary host memory.
+ *   - vectors are dense fp64 arrays.  A dG vector of a grid {Nx,Ny,P} has n = P*P*Nx*Ny entries laid out as a
+ *     row-major (Ny*P) x (Nx*P) image, x fastest:  idx = ((j*P + l)*Nx + i)*P + k   for cell (i,j), node (k,l)   (D:4).
+ *   - all work is enqueued on the stream set with fx_set_stream (default: the legacy default stream).  Calls are
+ *     asynchronous except where "synchronises" is stated.
+ *   - return value: fx_status.  < 0 is an error (nothing useful was computed), >= 0 is success.  No exceptions,
+ *     no aborts.  fx_last_error() returns a thread-local message for the last error.
+ *   - there is no CPU fallback: without a CUDA device every compute call returns FX_ECUDA.
+ */
+#ifndef FX_H
+#define FX_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    FX_OK = 0,
+    FX_MAXIT = 1,          /* fx_cg_solve: maxit iterations done without meeting tol (not an error)            */
+    FX_EINVAL = -1,        /* bad argument (null pointer with n>0, P outside 1..5, overlap where forbidden ...)  */
+    FX_ECUDA = -2,         /* CUDA runtime failure; fx_last_error() holds the CUDA string                      */
+    FX_ENOMEM = -3,        /* device allocation of library scratch failed                                     */
+    FX_EBREAKDOWN = -4     /* fx_cg_solve: p.Sp <= 0 or non-finite (operator not positive definite on p)       */
+} fx_status;
+
+typedef enum { FX_BC_PER = 0, FX_BC_DIR = 1 } fx_bc;   /* periodic / homogeneous Dirichlet                     */
+
+/* Grid of Fig. 2 `CartesianGrid2d(x0,x1,y0,y1,P,Nx,Ny)` on the domain [0,lx] x [0,ly]:
+ * Nx x Ny cells, P Gauss-Legendre nodes per cell and direction (P = number of polynomial coefficients). */
+typedef struct {
+    int32_t Nx, Ny, P;     /* Nx,Ny >= 1; 1 <= P <= 5                                                           */
+    double lx, ly;         /* > 0                                                                               */
+    int32_t bcx, bcy;      /* fx_bc                                                                             */
+} fx_grid;
+
+typedef struct {
+    int32_t iterations;    /* operator applications inside the loop                                             */
+    int32_t status;        /* FX_OK, FX_MAXIT or FX_EBREAKDOWN                                                  */
+    double rel_residual;   /* sqrt(r.V.r) / sqrt(b.W.b) at exit                                                  */
+} fx_cg_info;
+
+/* ---- housekeeping ---------------------------------------------------------------------------------------- */
+
+/* Stream (a cudaStream_t passed as void*) used by all later calls of this process; NULL = legacy default.     */
+fx_status fx_set_stream(void* cuda_stream);
+const char* fx_last_error(void);
+/* Release all library scratch (device digits, CG work vectors).  Optional; safe to call repeatedly.           */
+void fx_shutdown(void);
+
+/* Test hook for the launch-shape invariance tests (north star: results identical "regardless of grid and block
+ * shape").  kernel_id: 0 = exdot, 1 = axpby/pointwise, 2 = dG apply, 3 = fused CG kernels.  grid_dim = number of
+ * CTAs (0 = default), block_dim = threads per CTA (0 = default; must be a multiple of 32, <= 1024; the dG apply
+ * reads it as warps-per-CTA*32 and grid_dim as rows-per-segment).                                              */
+fx_status fx_set_launch(int32_t kernel_id, int32_t grid_dim, int32_t block_dim);
+/* 1 = fx_cg_solve uses the fused kernels (default), 0 = one kernel per primitive.  Results are bit-identical.  */
+fx_status fx_set_cg_fused(int32_t fused);
+
+/* ---- exactly rounded dot product (P:9) ----------------------------------------------------------
+ * result = RN( sum_i x[i]*y[i] ), products and sum over the reals, one rounding to nearest-even at the end; the
+ * full range of products of doubles is exact (subnormal*subnormal, 2^1000*2^1000 that cancel ...), exact zero
+ * gives +0.0, n == 0 gives +0.0; NaN if any input is NaN, any product is 0*inf, or +inf and -inf products both
+ * occur; else +-inf if an infinite product occurs or the exact sum rounds beyond DBL_MAX        (D:3.1, Q1-Q6).
+ * Bitwise identical for every launch shape.  x, y: device, may alias, n >= 0.                                  */
+
+/* Synchronises; returns the value (NaN and fx_last_error() on failure). */
+double fx_exdot(const double* x_dev, const double* y_dev, int64_t n);
+/* Asynchronous form: writes the double to result_dev (device, 8 bytes). */
+fx_status fx_exdot_async(const double* x_dev, const double* y_dev, int64_t n, double* result_dev);
+/* The long accumulator itself: 68 limbs, two's complement, limb k weighs 2^(64k-2176), plus flags
+ * {nan, +inf, -inf}.  limbs_host: host uint64[68]; flags_host: host int32[3] or NULL.  Synchronises.          */
+fx_status fx_exdot_digits(const double* x_dev, const double* y_dev, int64_t n, uint64_t* limbs_host,
+                          int32_t* flags_host, double* result_host);
+/* Host-buffer convenience (the "e2e" path of bench.py): x, y are HOST arrays; copies them to device scratch in
+ * chunks on the library stream, accumulates, returns the value.  Synchronises.                                */
+double fx_exdot_host(const double* x_host, const double* y_host, int64_t n);
+
+/* ---- vector primitives in canonical order (D:3.2) ---------------------------------------------- */
+
+/* y[i] <- fma(alpha, x[i], RN(beta*y[i]));  beta == 0: y[i] <- RN(alpha*x[i]) and y is not read.
+ * x, y: device; x may equal y; partial overlap is undefined.                                                   */
+fx_status fx_axpby(double alpha, const double* x_dev, double beta, double* y_dev, int64_t n);
+/* u = RN(alpha*x1[i]); y[i] <- fma(u, x2[i], RN(beta*y[i]));  beta == 0: y[i] <- RN(u*x2[i]), y not read.      */
+fx_status fx_pointwise_dot(double alpha, const double* x1_dev, const double* x2_dev, double beta, double* y_dev,
+                           int64_t n);
+
+/* ---- dG elliptic operator (construction D:3.3, operation order D:3.4) -------------------------
+ * S = Fx^T diag(W chi) Fx + Fy^T diag(W chi) Fy + (jump terms), symmetric; A = diag(V) S ~ -div(chi grad .),
+ * V = 1/W the inverse dG weights.  chi, x, y: device vectors of the grid; y must not overlap x or chi.         */
+fx_status fx_dg_elliptic_apply(const fx_grid* grid, const double* chi_dev, const double* x_dev, double* y_dev);     /* y = A x */
+fx_status fx_dg_elliptic_apply_sym(const fx_grid* grid, const double* chi_dev, const double* x_dev, double* y_dev); /* y = S x */
+/* dG weights W ("volume" of Fig. 2) and V = 1/W; either pointer may be NULL.  Device vectors.           */
+fx_status fx_dg_weights(const fx_grid* grid, double* w_dev, double* v_dev);
+/* The reference-element tables the kernels use, for the cross-check against the oracle's own tables.
+ * out_host: host double[5*P + 4*P*P] = xi,w,L,R,B (P each) then T0,T0L,WW,D (P*P each, row-major).  No GPU.   */
+fx_status fx_dg_tables(int32_t P, double* out_host);
+
+/* ---- preconditioned CG (algorithm D:3.5) ------------------------------------------------------
+ * Solves div(chi grad phi) = rho as S phi = W o (-rho) with preconditioner V; every dot product exactly rounded;
+ * stops when sqrt(r.V.r) <= tol*sqrt(b.W.b) (tested after every iteration) or after maxit iterations.
+ * chi, rho: device (read only); phi: device, in = phi0, out = phi; info: host or NULL.  Synchronises.
+ * Returns info->status.                                                                                       */
+fx_status fx_cg_solve(const fx_grid* grid, const double* chi_dev, const double* rho_dev, double* phi_dev,
+                      double tol, int32_t maxit, fx_cg_info* info);
+/* Host-buffer convenience (bench.py "e2e"): chi, rho, phi are HOST arrays of the grid's n doubles.            */
+fx_status fx_cg_solve_host(const fx_grid* grid, const double* chi_host, const double* rho_host, double* phi_host,
+                           double tol, int32_t maxit, fx_cg_info* info);
+
+/* Number of kernels this library has launched since load (bench.py's "gpu_launches").                          */
+int64_t fx_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FX_H */

@@ -1,0 +1,229 @@
+"""paper_1807_01971_b200 -- thin Python binding of libfx.so (C ABI: include/fx.h).
+
+Argument marshalling only: every step of the hot path (exact dot, axpby, pointwise_dot, dG elliptic apply, CG) runs in
+the hand-written sm_100a kernels of csrc/.  torch is used for device memory and streams.  There is no CPU fallback and
+nothing here imports oracle/: if the library cannot be built/loaded or no CUDA device is present, calls raise.
+"""
+import ctypes as C
+import os
+
+from . import build as _build
+
+PER, DIR = 0, 1
+OK, MAXIT, EINVAL, ECUDA, ENOMEM, EBREAKDOWN = 0, 1, -1, -2, -3, -4
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+class Grid(C.Structure):
+    """fx_grid: Nx x Ny cells on [0,lx] x [0,ly], P Gauss-Legendre nodes per cell and direction (Fig. 2)."""
+    _fields_ = [("Nx", C.c_int32), ("Ny", C.c_int32), ("P", C.c_int32),
+                ("lx", C.c_double), ("ly", C.c_double), ("bcx", C.c_int32), ("bcy", C.c_int32)]
+
+    @property
+    def n(self):
+        return self.Nx * self.Ny * self.P * self.P
+
+
+class CGInfo(C.Structure):
+    _fields_ = [("iterations", C.c_int32), ("status", C.c_int32), ("rel_residual", C.c_double)]
+
+
+class FxError(RuntimeError):
+    pass
+
+
+_lib = None
+_vp, _dp = C.c_void_p, C.POINTER(C.c_double)
+
+# name -> (restype, argtypes): every symbol include/fx.h declares
+_SIGNATURES = {
+    "fx_set_stream": (C.c_int, [_vp]),
+    "fx_last_error": (C.c_char_p, []),
+    "fx_shutdown": (None, []),
+    "fx_set_launch": (C.c_int, [C.c_int32, C.c_int32, C.c_int32]),
+    "fx_set_cg_fused": (C.c_int, [C.c_int32]),
+    "fx_exdot": (C.c_double, [_vp, _vp, C.c_int64]),
+    "fx_exdot_async": (C.c_int, [_vp, _vp, C.c_int64, _vp]),
+    "fx_exdot_digits": (C.c_int, [_vp, _vp, C.c_int64, _vp, _vp, _vp]),
+    "fx_exdot_host": (C.c_double, [_vp, _vp, C.c_int64]),
+    "fx_axpby": (C.c_int, [C.c_double, _vp, C.c_double, _vp, C.c_int64]),
+    "fx_pointwise_dot": (C.c_int, [C.c_double, _vp, _vp, C.c_double, _vp, C.c_int64]),
+    "fx_dg_elliptic_apply": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp]),
+    "fx_dg_elliptic_apply_sym": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp]),
+    "fx_dg_weights": (C.c_int, [C.POINTER(Grid), _vp, _vp]),
+    "fx_dg_tables": (C.c_int, [C.c_int32, _dp]),
+    "fx_cg_solve": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp, C.c_double, C.c_int32, C.POINTER(CGInfo)]),
+    "fx_cg_solve_host": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp, C.c_double, C.c_int32, C.POINTER(CGInfo)]),
+    "fx_launch_count": (C.c_int64, []),
+}
+
+
+def lib_path():
+    return os.path.join(_HERE, "libfx.so")
+
+
+def lib():
+    """Load libfx.so (building it in-tree first if it is missing or stale).  Raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(L, name)          # AttributeError if the ABI lost a symbol
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _check(rc, what):
+    if rc < 0:
+        raise FxError("%s failed (%d): %s" % (what, rc, lib().fx_last_error().decode()))
+    return rc
+
+
+def _ptr(t, n=None):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError("expected a contiguous float64 CUDA tensor")
+    if n is not None and t.numel() != n:
+        raise ValueError("tensor has %d elements, expected %d" % (t.numel(), n))
+    return t.data_ptr()
+
+
+def _use_torch_stream():
+    import torch
+    _check(lib().fx_set_stream(torch.cuda.current_stream().cuda_stream), "fx_set_stream")
+
+
+def make_grid(Nx, Ny, P, lx, ly, bcx, bcy):
+    return Grid(int(Nx), int(Ny), int(P), float(lx), float(ly), int(bcx), int(bcy))
+
+
+def set_launch(kernel_id, grid_dim=0, block_dim=0):
+    _check(lib().fx_set_launch(kernel_id, grid_dim, block_dim), "fx_set_launch")
+
+
+def set_cg_fused(fused):
+    _check(lib().fx_set_cg_fused(int(bool(fused))), "fx_set_cg_fused")
+
+
+def launch_count():
+    return int(lib().fx_launch_count())
+
+
+def exdot(x, y):
+    """RN(sum x_i*y_i) as a Python float (synchronises).  PAPER.md:170-176."""
+    _use_torch_stream()
+    n = x.numel()
+    v = lib().fx_exdot(_ptr(x), _ptr(y, n), n)
+    if v != v and lib().fx_last_error():
+        raise FxError(lib().fx_last_error().decode())
+    return v
+
+
+def exdot_async(x, y, out):
+    """Stream-ordered form: writes the double into out[0] (a float64 CUDA tensor)."""
+    _use_torch_stream()
+    n = x.numel()
+    _check(lib().fx_exdot_async(_ptr(x), _ptr(y, n), n, _ptr(out)), "fx_exdot_async")
+    return out
+
+
+def exdot_digits(x, y):
+    """-> (value, limbs uint64[68] numpy, flags int32[3] numpy): the long accumulator itself."""
+    import numpy as np
+    _use_torch_stream()
+    n = x.numel()
+    limbs = np.zeros(68, dtype=np.uint64)
+    flags = np.zeros(3, dtype=np.int32)
+    res = C.c_double(0.0)
+    _check(lib().fx_exdot_digits(_ptr(x), _ptr(y, n), n, limbs.ctypes.data, flags.ctypes.data, C.addressof(res)), "fx_exdot_digits")
+    return res.value, limbs, flags
+
+
+def exdot_host(x, y):
+    """x, y: CPU float64 tensors (pinned for full speed) or numpy arrays; copies inside the call."""
+    n, px, py = _host_ptrs(x, y)
+    v = lib().fx_exdot_host(px, py, n)
+    if v != v and lib().fx_last_error():
+        raise FxError(lib().fx_last_error().decode())
+    return v
+
+
+def _host_ptrs(*arrs):
+    import numpy as np
+    import torch
+    ptrs, n = [], None
+    for a in arrs:
+        if isinstance(a, torch.Tensor):
+            assert (not a.is_cuda) and a.dtype == torch.float64 and a.is_contiguous()
+            ptrs.append(a.data_ptr()); m = a.numel()
+        else:
+            assert isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags.c_contiguous
+            ptrs.append(a.ctypes.data); m = a.size
+        assert n is None or n == m
+        n = m
+    return (n, *ptrs)
+
+
+def axpby(alpha, x, beta, y):
+    """y <- alpha*x + beta*y in the canonical order of DESIGN.md 3.2 (in place; returns y).  PAPER.md:184-186."""
+    _use_torch_stream()
+    n = y.numel()
+    _check(lib().fx_axpby(float(alpha), _ptr(x, n), float(beta), _ptr(y), n), "fx_axpby")
+    return y
+
+
+def pointwise_dot(alpha, x1, x2, beta, y):
+    """y <- alpha*x1*x2 + beta*y (in place; returns y).  PAPER.md:238."""
+    _use_torch_stream()
+    n = y.numel()
+    _check(lib().fx_pointwise_dot(float(alpha), _ptr(x1, n), _ptr(x2, n), float(beta), _ptr(y), n), "fx_pointwise_dot")
+    return y
+
+
+def dg_elliptic_apply(grid, chi, x, y, sym=False):
+    """y = A x (normed, default) or y = S x (sym=True): the dG discretisation of -div(chi grad .).  PAPER.md:73, 240."""
+    _use_torch_stream()
+    fn = lib().fx_dg_elliptic_apply_sym if sym else lib().fx_dg_elliptic_apply
+    _check(fn(C.byref(grid), _ptr(chi, grid.n), _ptr(x, grid.n), _ptr(y, grid.n)), "fx_dg_elliptic_apply")
+    return y
+
+
+def dg_weights(grid, w=None, v=None):
+    _use_torch_stream()
+    _check(lib().fx_dg_weights(C.byref(grid), _ptr(w, grid.n) if w is not None else None,
+                               _ptr(v, grid.n) if v is not None else None), "fx_dg_weights")
+    return w, v
+
+
+def dg_tables(P):
+    """The kernels' reference-element tables (host only, no GPU): dict(xi,w,L,R,B: [P]; T0,T0L,WW,D: [P,P])."""
+    import numpy as np
+    out = np.zeros(5 * P + 4 * P * P)
+    _check(lib().fx_dg_tables(P, out.ctypes.data_as(_dp)), "fx_dg_tables")
+    d, o = {}, 0
+    for name in ("xi", "w", "L", "R", "B"):
+        d[name] = out[o:o + P].copy(); o += P
+    for name in ("T0", "T0L", "WW", "D"):
+        d[name] = out[o:o + P * P].reshape(P, P).copy(); o += P * P
+    return d
+
+
+def cg_solve(grid, chi, rho, phi, tol, maxit):
+    """Solve div(chi grad phi) = rho in place in phi (in: phi0).  Returns CGInfo.  PAPER.md:29, 75, 212."""
+    _use_torch_stream()
+    info = CGInfo()
+    _check(lib().fx_cg_solve(C.byref(grid), _ptr(chi, grid.n), _ptr(rho, grid.n), _ptr(phi, grid.n), float(tol), int(maxit),
+                             C.byref(info)), "fx_cg_solve")
+    return info
+
+
+def cg_solve_host(grid, chi, rho, phi, tol, maxit):
+    """Same with HOST buffers (CPU tensors / numpy); phi is updated in place."""
+    n, pc, pr, pp = _host_ptrs(chi, rho, phi)
+    assert n == grid.n
+    info = CGInfo()
+    _check(lib().fx_cg_solve_host(C.byref(grid), pc, pr, pp, float(tol), int(maxit), C.byref(info)), "fx_cg_solve_host")
+    return info

@@ -1,0 +1,348 @@
+// fx_cg.cu -- preconditioned conjugate gradient (a Level-2 algorithm built from Level-1 calls only;
+// the exact dot "is for example important in a conjugate gradient method").  Algorithm: DESIGN.md 3.5.
+//
+// Two drivers that produce bit-identical iterates:
+//   * unfused: one kernel per primitive, both dot results visit the host every iteration -- the structure the paper
+//     benchmarks (its GPU dot latency IS that host round trip);
+//   * fused (default; the paper's remedy "fewer calls, fewer passes"): three kernels per iteration
+//       K1  q = S p  and the exact dot p.q accumulated while q is produced      -> alpha = rz / pq   (device)
+//       K2  phi += alpha p;  r -= alpha q;  z = V o r on the fly;  exact dot r.z -> convergence test, beta (device)
+//       K3  p = z + beta p   (z recomputed from r)
+//     12 vector passes instead of 19.  The scalars never leave the device; a `done` flag turns the kernels that
+//     were enqueued past convergence into no-ops, and the host looks at it once per batch of iterations.
+
+#include <math.h>
+#include <string.h>
+
+#include "fx_internal.h"
+
+struct CgScal {
+    double rz, pq, alpha, beta, bz, thresh, dot;
+    int done, status, iters, pad;
+};
+
+#define CG_K 4
+#define CG_W 40
+typedef ExAcc<CG_K, CG_W> CgAcc;
+
+// ---- K1: apply + dot -----------------------------------------------------------------------------------------
+template <int P>
+__global__ void __launch_bounds__(256) k_cg_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi,
+                                                      const double* __restrict__ p, double* __restrict__ q, ExGlobal ex,
+                                                      CgScal* sc) {
+    if (*(volatile int*)&sc->done) return;
+    __shared__ ExShared sh;
+    ex_shared_init(&sh);
+    CgAcc acc;
+    acc.init();
+    const int wpb = blockDim.x >> 5;
+    const long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
+    if (w < (long long)g.nstrip * g.nseg) {
+        const int seg = (int)(w / g.nstrip), strip = (int)(w % g.nstrip);
+        const int j0 = seg * g.rows_per_seg;
+        int j1 = j0 + g.rows_per_seg;
+        if (j1 > g.Ny) j1 = g.Ny;
+        dg_warp_strip<P, true, CgAcc>(g, chi, p, q, strip, j0, j1, &acc, &sh);
+    }
+    acc.flush(&sh);
+    if (ex_block_finish(&sh, ex, 1, 1, &sc->pq) && threadIdx.x == 0) {
+        const double pq = sc->pq;
+        sc->iters += 1;
+        if (!(pq > 0.0) || isinf(pq)) { sc->status = FX_EBREAKDOWN; sc->done = 1; }
+        else sc->alpha = __ddiv_rn(sc->rz, pq);
+    }
+}
+
+// ---- K2: phi += alpha p; r -= alpha q; z = V o r; dot(r, z) ----------------------------------------------------
+#define CG_U 4
+template <int P>
+__global__ void __launch_bounds__(256) k_cg_update(const __grid_constant__ DgParams g, const double* __restrict__ p,
+                                                   const double* __restrict__ q, double* phi, double* r, ExGlobal ex,
+                                                   CgScal* sc) {
+    if (*(volatile int*)&sc->done) return;
+    __shared__ ExShared sh;
+    ex_shared_init(&sh);
+    CgAcc acc;
+    acc.init();
+    const double alpha = sc->alpha, nalpha = -alpha;
+    const int pitch = g.Nx * P, rows = g.Ny * P;
+    const int cw = blockDim.x * CG_U;                        // columns per chunk
+    const int cpr = (pitch + cw - 1) / cw;                   // chunks per row
+    const long long nchunk = (long long)rows * cpr;
+    for (long long c = blockIdx.x; c < nchunk; c += gridDim.x) {
+        const int row = (int)(c / cpr), cb = (int)(c - (long long)row * cpr);
+        const int l = row % P;
+        const long long base = (long long)row * pitch;
+        double pv[CG_U], qv[CG_U], fv[CG_U], rv[CG_U];
+        int col[CG_U];
+#pragma unroll
+        for (int u = 0; u < CG_U; ++u) {
+            col[u] = cb * cw + u * blockDim.x + threadIdx.x;
+            if (col[u] < pitch) { pv[u] = p[base + col[u]]; qv[u] = q[base + col[u]]; fv[u] = phi[base + col[u]]; rv[u] = r[base + col[u]]; }
+        }
+        double rr[CG_U], zz[CG_U];
+#pragma unroll
+        for (int u = 0; u < CG_U; ++u) {
+            if (col[u] < pitch) {
+                const int k = col[u] % P;
+                phi[base + col[u]] = __fma_rn(alpha, pv[u], fv[u]);          // axpby(alpha, p, 1, phi)
+                const double rn = __fma_rn(nalpha, qv[u], rv[u]);            // axpby(-alpha, q, 1, r)
+                r[base + col[u]] = rn;
+                rr[u] = rn;
+                zz[u] = __dmul_rn(g.V[l][k], rn);                            // pointwise_dot(1, V, r, 0, z)
+            } else { rr[u] = 0.0; zz[u] = 0.0; }
+        }
+        acc.add<CG_U>(rr, zz, &sh);
+    }
+    acc.flush(&sh);
+    if (ex_block_finish(&sh, ex, 1, 1, &sc->dot) && threadIdx.x == 0) {
+        const double rzn = sc->dot;
+        if (__dsqrt_rn(rzn) <= sc->thresh) { sc->rz = rzn; sc->status = FX_OK; sc->done = 1; }
+        else { sc->beta = __ddiv_rn(rzn, sc->rz); sc->rz = rzn; }
+    }
+}
+
+// ---- K3: p = z + beta p,  z = V o r -----------------------------------------------------------------------------
+template <int P>
+__global__ void __launch_bounds__(256) k_cg_dir(const __grid_constant__ DgParams g, const double* __restrict__ r, double* p,
+                                                const CgScal* sc) {
+    if (*(volatile const int*)&sc->done) return;
+    const double beta = sc->beta;
+    const int pitch = g.Nx * P, rows = g.Ny * P;
+    const int cw = blockDim.x * CG_U;
+    const int cpr = (pitch + cw - 1) / cw;
+    const long long nchunk = (long long)rows * cpr;
+    for (long long c = blockIdx.x; c < nchunk; c += gridDim.x) {
+        const int row = (int)(c / cpr), cb = (int)(c - (long long)row * cpr);
+        const int l = row % P;
+        const long long base = (long long)row * pitch;
+        double pv[CG_U], rv[CG_U];
+        int col[CG_U];
+#pragma unroll
+        for (int u = 0; u < CG_U; ++u) {
+            col[u] = cb * cw + u * blockDim.x + threadIdx.x;
+            if (col[u] < pitch) { pv[u] = p[base + col[u]]; rv[u] = r[base + col[u]]; }
+        }
+#pragma unroll
+        for (int u = 0; u < CG_U; ++u)
+            if (col[u] < pitch) {
+                const double z = __dmul_rn(g.V[l][col[u] % P], rv[u]);
+                p[base + col[u]] = __fma_rn(1.0, z, __dmul_rn(beta, pv[u]));    // axpby(1, z, beta, p)
+            }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+
+static fx_status cg_workspace(FxCtx* c, int64_t n) {
+    if (c->cg_cap < n) {
+        if (c->cg_vec) { cudaStreamSynchronize(c->stream); cudaFree(c->cg_vec); c->cg_vec = nullptr; c->cg_cap = 0; }
+        if (cudaMalloc(&c->cg_vec, (size_t)7 * n * sizeof(double)) != cudaSuccess) {
+            fx_set_error("CG work space: %s", cudaGetErrorString(cudaGetLastError())); return FX_ENOMEM;
+        }
+        c->cg_cap = n;
+    }
+    if (!c->cg_scal) {
+        if (cudaMalloc(&c->cg_scal, sizeof(CgScal)) != cudaSuccess || cudaMallocHost(&c->cg_scal_pinned, sizeof(CgScal)) != cudaSuccess) {
+            fx_set_error("CG scalars: %s", cudaGetErrorString(cudaGetLastError())); return FX_ENOMEM;
+        }
+    }
+    return FX_OK;
+}
+
+static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int* apply_grid, int* apply_block, int* ew_grid, int* ew_block) {
+    const int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
+    p->nstrip = (g->Nx + FX_STRIP - 1) / FX_STRIP;
+    int rps = c->launch[2][0];
+    if (rps <= 0) {
+        const long long target = (long long)c->num_sms * 32;
+        long long nseg = target / p->nstrip;
+        if (nseg < 1) nseg = 1;
+        rps = (int)((g->Ny + nseg - 1) / nseg);
+        if (rps < 8) rps = 8;
+    }
+    if (rps > g->Ny) rps = g->Ny;
+    p->rows_per_seg = rps;
+    p->nseg = (g->Ny + rps - 1) / rps;
+    const long long warps = (long long)p->nstrip * p->nseg;
+    *apply_grid = (int)((warps + wpb - 1) / wpb);
+    *apply_block = wpb * 32;
+    const int bd = c->launch[3][1] ? c->launch[3][1] : 256;
+    const int pitch = g->Nx * g->P;
+    const long long cpr = (pitch + (long long)bd * CG_U - 1) / ((long long)bd * CG_U);
+    long long chunks = cpr * g->Ny * g->P;
+    long long gmax = (long long)c->num_sms * (1024 / bd) * 2;
+    if (chunks > gmax) chunks = gmax;
+    if (c->launch[3][0]) chunks = c->launch[3][0];
+    *ew_grid = (int)chunks; *ew_block = bd;
+}
+
+template <int P>
+static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, int eg, int eb, const double* chi, double* phi,
+                                  double* r, double* p, double* q, CgScal* sc, int iters) {
+    for (int i = 0; i < iters; ++i) {
+        k_cg_apply_dot<P><<<ag, ab, 0, c->stream>>>(dp, chi, p, q, c->ex, sc);
+        k_cg_update<P><<<eg, eb, 0, c->stream>>>(dp, p, q, phi, r, c->ex, sc);
+        k_cg_dir<P><<<eg, eb, 0, c->stream>>>(dp, r, p, sc);
+        c->launches += 3;
+    }
+    FX_CUDA(cudaGetLastError());
+    return FX_OK;
+}
+
+extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const double* rho, double* phi, double tol, int32_t maxit,
+                                 fx_cg_info* info) {
+    if (!fx_grid_ok(g) || !chi || !rho || !phi || maxit < 0 || !(tol >= 0)) { fx_set_error("fx_cg_solve: bad arguments"); return FX_EINVAL; }
+    FxCtx* c = fx_ctx();
+    if (!c) return FX_ECUDA;
+    const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
+    fx_status s = cg_workspace(c, n);
+    if (s != FX_OK) return s;
+    double *W = c->cg_vec, *V = W + n, *rhs = V + n, *r = rhs + n, *z = r + n, *p = z + n, *q = p + n;
+    const size_t bytes = (size_t)n * sizeof(double);
+
+    // setup with the public primitives (lines before the loop)
+    if ((s = fx_dg_weights(g, W, V)) != FX_OK) return s;
+    if ((s = fx_pointwise_dot(-1.0, W, rho, 0.0, rhs, n)) != FX_OK) return s;
+    if ((s = fx_launch_apply(c, g, chi, phi, q, 0)) != FX_OK) return s;
+    FX_CUDA(cudaMemcpyAsync(r, rhs, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    if ((s = fx_axpby(-1.0, q, 1.0, r, n)) != FX_OK) return s;
+    if ((s = fx_pointwise_dot(1.0, V, rhs, 0.0, z, n)) != FX_OK) return s;
+    const double bz = fx_exdot(rhs, z, n);
+    if (bz == 0.0) {
+        FX_CUDA(cudaMemsetAsync(phi, 0, bytes, c->stream));
+        FX_CUDA(cudaStreamSynchronize(c->stream));
+        if (info) { info->iterations = 0; info->status = FX_OK; info->rel_residual = 0.0; }
+        return FX_OK;
+    }
+    if ((s = fx_pointwise_dot(1.0, V, r, 0.0, z, n)) != FX_OK) return s;
+    double rz = fx_exdot(r, z, n);
+    FX_CUDA(cudaMemcpyAsync(p, z, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    const double thresh = tol * sqrt(bz);
+    int it = 0, status = FX_OK;
+    if (!(sqrt(rz) <= thresh)) {
+        status = FX_MAXIT;
+        if (!c->cg_fused) {
+            for (it = 1; it <= maxit; ++it) {
+                if ((s = fx_launch_apply(c, g, chi, p, q, 0)) != FX_OK) return s;
+                const double pq = fx_exdot(p, q, n);
+                if (!(pq > 0.0) || !isfinite(pq)) { status = FX_EBREAKDOWN; break; }
+                const double alpha = rz / pq;
+                if ((s = fx_axpby(alpha, p, 1.0, phi, n)) != FX_OK) return s;
+                if ((s = fx_axpby(-alpha, q, 1.0, r, n)) != FX_OK) return s;
+                if ((s = fx_pointwise_dot(1.0, V, r, 0.0, z, n)) != FX_OK) return s;
+                const double rz_new = fx_exdot(r, z, n);
+                if (sqrt(rz_new) <= thresh) { rz = rz_new; status = FX_OK; break; }
+                const double beta = rz_new / rz;
+                if ((s = fx_axpby(1.0, z, beta, p, n)) != FX_OK) return s;
+                rz = rz_new;
+            }
+            if (it > maxit) it = maxit;
+        } else {
+            DgParams dp;
+            if ((s = fx_make_dg_params(g, 0, &dp, nullptr)) != FX_OK) return s;
+            int ag, ab, eg, eb;
+            cg_shapes(c, g, &dp, &ag, &ab, &eg, &eb);
+            CgScal* sc = (CgScal*)c->cg_scal;
+            CgScal* hs = (CgScal*)c->cg_scal_pinned;
+            memset(hs, 0, sizeof(*hs));
+            hs->rz = rz; hs->bz = bz; hs->thresh = thresh; hs->status = FX_MAXIT;
+            FX_CUDA(cudaMemcpyAsync(sc, hs, sizeof(CgScal), cudaMemcpyHostToDevice, c->stream));
+            FX_CUDA(cudaStreamSynchronize(c->stream));           // hs is reused as the read-back buffer
+            int enq = 0;
+            int batch = 8;
+            while (enq < maxit) {
+                const int m = (maxit - enq < batch) ? (maxit - enq) : batch;
+                switch (g->P) {
+                case 1: s = cg_enqueue_iters<1>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
+                case 2: s = cg_enqueue_iters<2>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
+                case 3: s = cg_enqueue_iters<3>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
+                case 4: s = cg_enqueue_iters<4>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
+                default: s = cg_enqueue_iters<5>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
+                }
+                if (s != FX_OK) return s;
+                enq += m;
+                FX_CUDA(cudaMemcpyAsync(hs, sc, sizeof(CgScal), cudaMemcpyDeviceToHost, c->stream));
+                FX_CUDA(cudaStreamSynchronize(c->stream));
+                if (hs->done) break;
+                if (batch < 64) batch *= 2;
+            }
+            it = hs->iters; status = hs->status; rz = hs->rz;
+        }
+    }
+    FX_CUDA(cudaStreamSynchronize(c->stream));
+    if (info) { info->iterations = it; info->status = status; info->rel_residual = sqrt(rz) / sqrt(bz); }
+    return (fx_status)status;
+}
+
+// ---- host-buffer entry points (bench.py "e2e") ------------------------------------------------------------------
+
+static fx_status stage_alloc(FxCtx* c, int64_t cap) {
+    if (c->stage_cap < cap) {
+        cudaStreamSynchronize(c->stream);
+        for (int i = 0; i < 4; ++i) { if (c->stage[i]) cudaFree(c->stage[i]); c->stage[i] = nullptr; }
+        c->stage_cap = 0;
+        for (int i = 0; i < 4; ++i)
+            if (cudaMalloc(&c->stage[i], (size_t)cap * sizeof(double)) != cudaSuccess) {
+                fx_set_error("staging buffers: %s", cudaGetErrorString(cudaGetLastError())); return FX_ENOMEM;
+            }
+        c->stage_cap = cap;
+    }
+    if (!c->copy_stream) {
+        FX_CUDA(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            FX_CUDA(cudaEventCreateWithFlags(&c->ev_copy[i], cudaEventDisableTiming));
+            FX_CUDA(cudaEventCreateWithFlags(&c->ev_comp[i], cudaEventDisableTiming));
+        }
+    }
+    return FX_OK;
+}
+
+extern "C" fx_status fx_cg_solve_host(const fx_grid* g, const double* chi, const double* rho, double* phi, double tol,
+                                      int32_t maxit, fx_cg_info* info) {
+    if (!fx_grid_ok(g) || !chi || !rho || !phi) { fx_set_error("fx_cg_solve_host: bad arguments"); return FX_EINVAL; }
+    FxCtx* c = fx_ctx();
+    if (!c) return FX_ECUDA;
+    const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
+    fx_status s = stage_alloc(c, n);
+    if (s != FX_OK) return s;
+    const size_t bytes = (size_t)n * sizeof(double);
+    FX_CUDA(cudaMemcpyAsync(c->stage[0], chi, bytes, cudaMemcpyHostToDevice, c->stream));
+    FX_CUDA(cudaMemcpyAsync(c->stage[1], rho, bytes, cudaMemcpyHostToDevice, c->stream));
+    FX_CUDA(cudaMemcpyAsync(c->stage[2], phi, bytes, cudaMemcpyHostToDevice, c->stream));
+    s = fx_cg_solve(g, c->stage[0], c->stage[1], c->stage[2], tol, maxit, info);
+    if (s < 0) return s;
+    FX_CUDA(cudaMemcpyAsync(phi, c->stage[2], bytes, cudaMemcpyDeviceToHost, c->stream));
+    FX_CUDA(cudaStreamSynchronize(c->stream));
+    return s;
+}
+
+// double-buffered: the copy of chunk i+1 overlaps the accumulation of chunk i
+extern "C" double fx_exdot_host(const double* x, const double* y, int64_t n) {
+    if (n < 0 || (n > 0 && (!x || !y))) { fx_set_error("fx_exdot_host: bad arguments"); return NAN; }
+    fx_set_error("%s", "");
+    FxCtx* c = fx_ctx();
+    if (!c) return NAN;
+    const int64_t CH = (int64_t)1 << 23;                       // 64 MB per array and chunk
+    if (stage_alloc(c, n < CH ? (n > 0 ? n : 1) : CH) != FX_OK) return NAN;
+    const int64_t cap = c->stage_cap < CH ? c->stage_cap : CH;
+    const int64_t nch = n == 0 ? 1 : (n + cap - 1) / cap;
+    cudaEventRecord(c->ev_comp[0], c->stream);
+    cudaEventRecord(c->ev_comp[1], c->stream);
+    for (int64_t i = 0; i < nch; ++i) {
+        const int b = (int)(i & 1);
+        const int64_t off = i * cap, m = (n - off < cap) ? (n - off) : cap;
+        cudaStreamWaitEvent(c->copy_stream, c->ev_comp[b], 0);       // buffer b free again
+        if (m > 0) {
+            cudaMemcpyAsync(c->stage[2 * b], x + off, (size_t)m * sizeof(double), cudaMemcpyHostToDevice, c->copy_stream);
+            cudaMemcpyAsync(c->stage[2 * b + 1], y + off, (size_t)m * sizeof(double), cudaMemcpyHostToDevice, c->copy_stream);
+        }
+        cudaEventRecord(c->ev_copy[b], c->copy_stream);
+        cudaStreamWaitEvent(c->stream, c->ev_copy[b], 0);
+        if (fx_launch_exdot_part(c, c->stage[2 * b], c->stage[2 * b + 1], m, i == 0, i == nch - 1, c->result_dev) != FX_OK) return NAN;
+        cudaEventRecord(c->ev_comp[b], c->stream);
+    }
+    if (cudaMemcpyAsync(c->result_pinned, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess) { fx_cuda_fail(cudaGetLastError(), "fx_exdot_host"); return NAN; }
+    return c->result_pinned[0];
+}

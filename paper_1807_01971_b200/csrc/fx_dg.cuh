@@ -1,0 +1,246 @@
+// fx_dg.cuh -- the dG elliptic operator y = S x (or A x = V o S x) as one fused block-stencil kernel.
+//
+// Paper: the dG derivatives are block-sparse matrices with few distinct P x P blocks, kept out of the memory
+// traffic so that the product is bandwidth bound like axpby; P is a compile-time
+// parameter for tight inner loops; no divergent branches; fixed operation order with explicit
+// FMAs for bitwise reproducibility.  The paper applies dx, dy and jump matrices one call at a time
+// (6 mat-vecs per elliptic apply) and names that modularity a factor 2-5 loss.
+//
+// Here: ONE kernel reads x and chi once and writes y once (24 B per unknown).  A warp owns a
+// strip of 30 cells in x (lanes 1..30; lanes 0 and 31 are the one-cell halo and recompute only traces and flux
+// traces) and marches through a segment of cell rows in y.  A lane holds its cell's P*P values in registers.
+// Everything that couples neighbouring cells is a *trace* (P numbers per cell side): in x they travel by warp
+// shuffle, in y they are carried in registers from one marching step to the next.  No shared memory, no
+// __syncthreads, no tensor cores (this is a bandwidth-bound stencil, not a dense contraction).
+// The operation sequence per node is exactly DESIGN.md 3.4; every intermediate has a single defining
+// expression, so halo recomputation and any launch shape give the same bits.
+
+#ifndef FX_DG_CUH
+#define FX_DG_CUH
+
+#include "fx_exdot.cuh"
+#include "fx_tables.h"
+
+struct DgParams {
+    int Nx, Ny, bcx, bcy;          // bc: 0 = periodic, 1 = Dirichlet
+    int rows_per_seg, nseg, nstrip;
+    int normed;
+    double cxx, cyy;               // hy/hx, hx/hy
+    double T0[FX_PMAX][FX_PMAX], T0L[FX_PMAX][FX_PMAX], WW[FX_PMAX][FX_PMAX], V[FX_PMAX][FX_PMAX];
+    double B[FX_PMAX], L[FX_PMAX], R[FX_PMAX], JX[FX_PMAX], JY[FX_PMAX];
+};
+
+#define FX_STRIP 30
+
+template <int P>
+struct DgCell { double v[P][P]; };     // [l][k]: row l (y node), column k (x node)
+
+// load one cell's P x P values; `zero` lanes get +0.0 without touching memory
+template <int P>
+__device__ __forceinline__ void dg_load(DgCell<P>& c, const double* __restrict__ a, long long pitch, int col0, int j,
+                                        bool zero) {
+    const double* q = a + (long long)j * P * pitch + col0;
+#pragma unroll
+    for (int l = 0; l < P; ++l)
+#pragma unroll
+        for (int k = 0; k < P; ++k) c.v[l][k] = zero ? 0.0 : __ldg(q + l * pitch + k);
+}
+
+// chain over m:  acc = c[0]*v[0]; acc = fma(c[m], v[m], acc)
+#define FX_CHAIN(acc, COEF, VAL)                         \
+    {                                                    \
+        acc = __dmul_rn(COEF(0), VAL(0));                \
+        _Pragma("unroll") for (int m_ = 1; m_ < P; ++m_) \
+            acc = __fma_rn(COEF(m_), VAL(m_), acc);      \
+    }
+
+// One warp: strip `strip` of 30 cells, cell rows [j0, j1).  FUSE: feed (x, y) pairs of the produced rows into the
+// exact-dot accumulator `acc` (the CG's p.Sp).
+template <int P, bool FUSE, class ACC>
+__device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* __restrict__ chi,
+                                              const double* __restrict__ x, double* __restrict__ y, int strip, int j0,
+                                              int j1, ACC* acc, ExShared* sh) {
+    const int lane = threadIdx.x & 31;
+    const int Nx = g.Nx, Ny = g.Ny;
+    const long long pitch = (long long)Nx * P;
+    const int ci = strip * FX_STRIP - 1 + lane;                    // this lane's cell column (may be outside)
+    const bool outside = ci < 0 || ci >= Nx;
+    const bool dirx = g.bcx == 1, diry = g.bcy == 1;
+    // periodic: wrap once; lanes further out are never used but must read valid memory
+    int cw = ci;
+    if (outside) { cw = ci % Nx; if (cw < 0) cw += Nx; }
+    const bool xghost = outside && (dirx || ci < -1 || ci > Nx);   // contributes zero traces
+    const bool produce = lane >= 1 && lane <= FX_STRIP && ci < Nx; // ci >= 0 holds for lanes >= 1
+    const bool firstx = dirx && ci == 0;                           // T0L instead of T0 along x
+    const int col0 = cw * P;
+
+    DgCell<P> uc, un, cc;
+    double tLy[P], tRyp[P], tByp[P];                               // own bottom trace; previous cell's top / flux trace
+
+    // ---- prologue: state of cell row j0-1 ------------------------------------------------------------------
+    dg_load<P>(uc, x, pitch, col0, j0, xghost);
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+#define CL(m) g.L[m]
+#define UC(m) uc.v[m][k]
+        FX_CHAIN(tLy[k], CL, UC)
+#undef UC
+    }
+    if (j0 == 0 && diry) {
+#pragma unroll
+        for (int k = 0; k < P; ++k) { tRyp[k] = 0.0; tByp[k] = 0.0; }
+    } else {
+        const int jp = (j0 == 0) ? Ny - 1 : j0 - 1;
+        const bool firsty = diry && jp == 0;
+        DgCell<P> up, cp;
+        dg_load<P>(up, x, pitch, col0, jp, xghost);
+        dg_load<P>(cp, chi, pitch, col0, jp, xghost);
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+#define CR(m) g.R[m]
+#define UP(m) up.v[m][k]
+            FX_CHAIN(tRyp[k], CR, UP)
+            double f[P];
+#pragma unroll
+            for (int l = 0; l < P; ++l) {
+                double a;
+#define CT(m) (firsty ? g.T0L[l][m] : g.T0[l][m])
+                FX_CHAIN(a, CT, UP)
+#undef CT
+                const double gh = __fma_rn(g.B[l], tLy[k], a);
+                f[l] = __dmul_rn(__dmul_rn(g.WW[l][k], cp.v[l][k]), gh);
+            }
+#define CB(m) g.B[m]
+#define FF(m) f[m]
+            FX_CHAIN(tByp[k], CB, FF)
+#undef UP
+        }
+    }
+    dg_load<P>(cc, chi, pitch, col0, j0, xghost);
+
+    // ---- march ---------------------------------------------------------------------------------------------
+    for (int j = j0; j < j1; ++j) {
+        int jn = j + 1;
+        bool yghost = false;
+        if (jn == Ny) { jn = 0; yghost = diry; }
+        dg_load<P>(un, x, pitch, col0, jn, xghost || yghost);
+        DgCell<P> cn;
+        const bool more = (j + 1 < j1);
+        if (more) dg_load<P>(cn, chi, pitch, col0, j + 1, xghost);
+
+        const bool firsty = diry && j == 0;
+        double tRy[P], tLyn[P], tLx[P], tRx[P];
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+#define UC(m) uc.v[m][k]
+#define UN(m) un.v[m][k]
+            FX_CHAIN(tRy[k], CR, UC)
+            FX_CHAIN(tLyn[k], CL, UN)
+            if (yghost) tLyn[k] = 0.0;
+#undef UC
+#undef UN
+        }
+#pragma unroll
+        for (int l = 0; l < P; ++l) {
+#define UC(m) uc.v[l][m]
+            FX_CHAIN(tLx[l], CL, UC)
+            FX_CHAIN(tRx[l], CR, UC)
+#undef UC
+            if (xghost) { tLx[l] = 0.0; tRx[l] = 0.0; }
+        }
+        // c = RN(WW * chi), jumps first (DESIGN.md 3.4 combine order: JY*jy, then + JX*jx, + cyy*sy, + cxx*sx)
+        double acc_[P][P];
+        double tLxr[P], tRxl[P];
+#pragma unroll
+        for (int l = 0; l < P; ++l) {
+            tLxr[l] = __shfl_down_sync(0xffffffffu, tLx[l], 1);
+            tRxl[l] = __shfl_up_sync(0xffffffffu, tRx[l], 1);
+        }
+#pragma unroll
+        for (int l = 0; l < P; ++l)
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                cc.v[l][k] = __dmul_rn(g.WW[l][k], cc.v[l][k]);
+                const double jy = __fma_rn(g.L[l], __dsub_rn(tLy[k], tRyp[k]), __dmul_rn(g.R[l], __dsub_rn(tRy[k], tLyn[k])));
+                const double jx = __fma_rn(g.L[k], __dsub_rn(tLx[l], tRxl[l]), __dmul_rn(g.R[k], __dsub_rn(tRx[l], tLxr[l])));
+                acc_[l][k] = __fma_rn(g.JX[l], jx, __dmul_rn(g.JY[k], jy));
+            }
+        // y lines: one column k at a time
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            double f[P];
+#pragma unroll
+            for (int l = 0; l < P; ++l) {
+                double a;
+#define UC(m) uc.v[m][k]
+#define CT(m) (firsty ? g.T0L[l][m] : g.T0[l][m])
+                FX_CHAIN(a, CT, UC)
+#undef CT
+#undef UC
+                f[l] = __dmul_rn(cc.v[l][k], __fma_rn(g.B[l], tLyn[k], a));
+            }
+            double tB;
+            FX_CHAIN(tB, CB, FF)
+#pragma unroll
+            for (int l = 0; l < P; ++l) {
+                double a;
+#define CT(m) (firsty ? g.T0L[m][l] : g.T0[m][l])
+                FX_CHAIN(a, CT, FF)
+#undef CT
+                const double sy = __fma_rn(g.L[l], tByp[k], a);
+                acc_[l][k] = __fma_rn(g.cyy, sy, acc_[l][k]);
+            }
+            tByp[k] = tB; tRyp[k] = tRy[k]; tLy[k] = tLyn[k];
+        }
+        // x lines: one row l at a time
+        double* yrow = y + (long long)j * P * pitch + col0;
+#pragma unroll
+        for (int l = 0; l < P; ++l) {
+            double f[P];
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                double a;
+#define UC(m) uc.v[l][m]
+#define CT(m) (firstx ? g.T0L[k][m] : g.T0[k][m])
+                FX_CHAIN(a, CT, UC)
+#undef CT
+#undef UC
+                f[k] = __dmul_rn(cc.v[l][k], __fma_rn(g.B[k], tLxr[l], a));
+            }
+            double tB;
+            FX_CHAIN(tB, CB, FF)
+            if (xghost) tB = 0.0;
+            const double tBl = __shfl_up_sync(0xffffffffu, tB, 1);
+            double out[P];
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                double a;
+#define CT(m) (firstx ? g.T0L[m][k] : g.T0[m][k])
+                FX_CHAIN(a, CT, FF)
+#undef CT
+                const double sx = __fma_rn(g.L[k], tBl, a);
+                double o = __fma_rn(g.cxx, sx, acc_[l][k]);
+                if (g.normed) o = __dmul_rn(g.V[l][k], o);
+                out[k] = o;
+            }
+            if (produce) {
+#pragma unroll
+                for (int k = 0; k < P; ++k) yrow[l * pitch + k] = out[k];
+            }
+            if (FUSE) {
+                double xs[P], ys[P];
+#pragma unroll
+                for (int k = 0; k < P; ++k) { xs[k] = produce ? uc.v[l][k] : 0.0; ys[k] = produce ? out[k] : 0.0; }
+                acc->template add<P>(xs, ys, sh);
+            }
+        }
+        uc = un;
+        if (more) cc = cn;
+    }
+#undef CL
+#undef CR
+#undef CB
+#undef FF
+}
+
+#endif

@@ -1,0 +1,320 @@
+// fx_exdot.cuh -- device side of the exactly rounded dot product (section 3.1).
+//
+// The paper's scheme: TwoProd splits every product error-free into (p, e); p and e are accumulated in
+// floating-point expansions held in registers; what an expansion cannot hold goes to a long accumulator
+// ("a very long fixed point number") which is "rarely invoked"; partial results are merged
+// "on various levels" and rounded once.
+//
+// What is kept and what differs on sm_100a:
+//   * kept: TwoProd by FMA, register-resident expansions in front of an integer long accumulator, integer
+//     merging (associative -> result independent of thread, warp, block and grid shape);
+//   * differs: the expansion is a BINNED one.  A warp keeps a common window top 2^T; bin k is a double S[k] that
+//     sits in the binade [2^(E_k+52), 2^(E_k+53)], E_k = T - W*(k+1), so that ulp(S[k]) = 2^E_k.  Adding a value
+//     v (|v| <= |S[k]|) is FastTwoSum(S[k], v):  s = S[k]+v; q = s-S[k]; r = v-q  -- always error-free; r
+//     (|r| <= 2^(E_k-1)) drops into the next bin.  That is 3 fp64 operations per bin and value instead of the
+//     6 of a TwoSum, with no data-dependent branch in the common case, which is what fits B200's ratio of
+//     ~2.3 fp64 issue slots per HBM byte.  A non-zero remainder below the last bin, and products outside the
+//     range where TwoProd is error-free, take a slow path that deposits exact integer chunks into the shared
+//     long accumulator.
+//
+// Long accumulator: 136 signed 64-bit digits spaced 32 bit apart, digit d weighs 2^(32 d - 2176) (the same
+// fixed-point grid as 68 limbs x 64 bit with the LSB at 2^-2176: below the smallest product bit 2^-2148, above
+// 2^2048 * n).  One copy in shared memory per CTA, one in global memory per context.
+
+#ifndef FX_EXDOT_CUH
+#define FX_EXDOT_CUH
+
+#include <stdint.h>
+
+#define FX_NDIG 136
+#define FX_NLIMB 68
+#define FX_BIAS 2176
+#define FX_FLAG_NAN 1
+#define FX_FLAG_PINF 2
+#define FX_FLAG_NINF 4
+
+typedef unsigned long long fx_u64;
+
+struct ExShared {
+    fx_u64 dig[FX_NDIG];     // signed digits, two's complement wrap-around arithmetic
+    int flags;
+    int is_last;
+};
+
+struct ExGlobal {            // device scratch of one context
+    fx_u64* dig;             // [FX_NDIG]   merged CTA digits of the running launch (zero between launches)
+    fx_u64* limbs;           // [FX_NLIMB]  canonical two's complement accumulator of the running call
+    int* flags;              // [1]
+    unsigned int* ticket;    // [1]         CTAs finished (zero between launches)
+};
+
+// add (-1)^neg * (hi:lo) * 2^(b - FX_BIAS) into a digit array with atomics (shared or global)
+__device__ __forceinline__ void ex_deposit(fx_u64* dig, int b, fx_u64 hi, fx_u64 lo, bool neg) {
+    const int d = b >> 5, s = b & 31;
+    fx_u64 w0 = lo << s;
+    fx_u64 w1 = (hi << s) | (s ? (lo >> (64 - s)) : 0ull);
+    fx_u64 w2 = s ? (hi >> (64 - s)) : 0ull;
+    fx_u64 c[5] = {w0 & 0xffffffffull, w0 >> 32, w1 & 0xffffffffull, w1 >> 32, w2};
+#pragma unroll
+    for (int i = 0; i < 5; ++i)
+        if (c[i]) atomicAdd(&dig[d + i], neg ? (0ull - c[i]) : c[i]);
+}
+
+// any finite double v (exactly), DESIGN.md 6.1 "slow path 1"
+static __device__ __noinline__ void ex_deposit_double(ExShared* sh, double v) {
+    const fx_u64 bits = (fx_u64)__double_as_longlong(v);
+    const int be = (int)((bits >> 52) & 0x7ff);
+    fx_u64 m = bits & 0xfffffffffffffull;
+    if (be) m |= 1ull << 52;
+    if (m == 0) return;
+    const int E = (be ? be : 1) - 1075;
+    ex_deposit(sh->dig, E + FX_BIAS, 0ull, m, (bits >> 63) != 0);
+}
+
+// exact product of any two doubles, DESIGN.md 6.1 "slow path 2": integer mantissa product (106 bit)
+static __device__ __noinline__ void ex_deposit_product(ExShared* sh, double x, double y) {
+    const fx_u64 bx = (fx_u64)__double_as_longlong(x), by = (fx_u64)__double_as_longlong(y);
+    const int ex = (int)((bx >> 52) & 0x7ff), ey = (int)((by >> 52) & 0x7ff);
+    const fx_u64 fx = bx & 0xfffffffffffffull, fy = by & 0xfffffffffffffull;
+    const bool neg = ((bx ^ by) >> 63) != 0;
+    if (ex == 0x7ff || ey == 0x7ff) {
+        const bool nan = (ex == 0x7ff && fx) || (ey == 0x7ff && fy) || (ex == 0 && fx == 0) || (ey == 0 && fy == 0);
+        atomicOr(&sh->flags, nan ? FX_FLAG_NAN : (neg ? FX_FLAG_NINF : FX_FLAG_PINF));
+        return;
+    }
+    const fx_u64 mx = ex ? (fx | (1ull << 52)) : fx, my = ey ? (fy | (1ull << 52)) : fy;
+    const fx_u64 lo = mx * my, hi = __umul64hi(mx, my);
+    if ((lo | hi) == 0) return;
+    const int E = (ex ? ex : 1) + (ey ? ey : 1) - 2150;          // value = mx*my * 2^E, E >= -2148
+    ex_deposit(sh->dig, E + FX_BIAS, hi, lo, neg);
+}
+
+__device__ __forceinline__ long long ex_warp_sum(long long v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Per-thread binned expansion with a warp-uniform window.  K bins of W bit.
+template <int K, int W>
+struct ExAcc {
+    static constexpr int CAP = 1 << (50 - W);            // deposits per bin before S[k] must be re-centred
+    static constexpr int MARGIN = 6;                     // head-room (bit) above the largest product seen
+    static constexpr int TB_MIN = -1074 + K * W + 1022;  // lowest bin stays a normal double with ulp >= 2^-1074
+    static constexpr int BE_LO = 63;                     // fast path: 2^-960 <= |p| < 2^1000 (TwoProd error-free,
+    static constexpr int BE_HI = 2022;                   //   no overflow of the top bin)
+    double S[K];
+    long long C[K];
+    int Tb;          // T + 1022; |p| < 2^T  <=>  biased exponent of p <= Tb.   INT_MIN/2 = no window yet
+    int cnt, ren;
+
+    __device__ __forceinline__ void init() {
+#pragma unroll
+        for (int k = 0; k < K; ++k) { S[k] = 0.0; C[k] = 0; }
+        Tb = -(1 << 29); cnt = 0; ren = 0;
+    }
+    __device__ __forceinline__ long long mbits(int k) const {      // bit pattern of 1.5 * 2^(E_k + 52)
+        const int be = Tb - 1022 - W * (k + 1) + 52 + 1023;
+        return ((long long)be << 52) | (1ll << 51);
+    }
+    __device__ __forceinline__ void recentre() {                    // S[k] -> centre, integer part -> C[k]
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const long long m = mbits(k);
+            C[k] += __double_as_longlong(S[k]) - m;                 // same binade: bit patterns are linear in value
+            S[k] = __longlong_as_double(m);
+        }
+        cnt = 0; ++ren;
+    }
+    // all 32 lanes: merge the warp's bins by shuffles, lane 0 deposits into the CTA's long accumulator
+    __device__ __noinline__ void flush(ExShared* sh) {
+        if (Tb > -(1 << 28)) {
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                long long c = C[k] + (__double_as_longlong(S[k]) - mbits(k));
+                c = ex_warp_sum(c);
+                if ((threadIdx.x & 31) == 0 && c != 0) {
+                    const int Ek = Tb - 1022 - W * (k + 1);
+                    ex_deposit(sh->dig, Ek + FX_BIAS, 0ull, (fx_u64)(c < 0 ? -c : c), c < 0);
+                }
+                C[k] = 0;
+                S[k] = __longlong_as_double(mbits(k));
+            }
+        }
+        cnt = 0; ren = 0;
+    }
+    __device__ __noinline__ void reanchor(ExShared* sh, int bemax) {
+        flush(sh);
+        int t = bemax + MARGIN;
+        Tb = t < TB_MIN ? TB_MIN : t;
+#pragma unroll
+        for (int k = 0; k < K; ++k) { S[k] = __longlong_as_double(mbits(k)); C[k] = 0; }
+    }
+
+    // U products per lane; must be called by all 32 lanes of the warp together
+    template <int U>
+    __device__ __forceinline__ void add(const double (&x)[U], const double (&y)[U], ExShared* sh) {
+        double p[U], e[U];
+        int bemax = 0;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            p[u] = __dmul_rn(x[u], y[u]);
+            e[u] = __fma_rn(x[u], y[u], -p[u]);                      // TwoProd
+            const int be = (__double2hiint(p[u]) >> 20) & 0x7ff;
+            if (be < BE_LO || be > BE_HI) {                          // outside TwoProd's error-free range
+                if (be == 0x7ff || (x[u] != 0.0 && y[u] != 0.0)) ex_deposit_product(sh, x[u], y[u]);
+                p[u] = 0.0; e[u] = 0.0;
+            } else bemax = be > bemax ? be : bemax;
+        }
+        if (__any_sync(0xffffffffu, bemax > Tb)) reanchor(sh, __reduce_max_sync(0xffffffffu, bemax));
+        if (cnt + U > CAP) { recentre(); if (__any_sync(0xffffffffu, ren >= 32)) flush(sh); }
+        cnt += U;
+        unsigned rest = 0;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            double v = p[u], w = e[u];
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                const double s = __dadd_rn(S[k], v);
+                const double q = __dsub_rn(s, S[k]);
+                v = __dsub_rn(v, q);
+                S[k] = s;
+            }
+#pragma unroll
+            for (int k = 1; k < K; ++k) {                            // |e| < ulp(S[0])/2: bin 0 cannot take any of it
+                const double s = __dadd_rn(S[k], w);
+                const double q = __dsub_rn(s, S[k]);
+                w = __dsub_rn(w, q);
+                S[k] = s;
+            }
+            p[u] = v; e[u] = w;
+            rest |= (unsigned)__double2loint(v) | (unsigned)__double2loint(w) |
+                    (((unsigned)__double2hiint(v) | (unsigned)__double2hiint(w)) & 0x7fffffffu);
+        }
+        if (rest) {                                                  // bits below the window: exact, but slow
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                if (p[u] != 0.0) ex_deposit_double(sh, p[u]);
+                if (e[u] != 0.0) ex_deposit_double(sh, e[u]);
+            }
+        }
+    }
+};
+
+__device__ __forceinline__ void ex_shared_init(ExShared* sh) {
+    for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) sh->dig[i] = 0ull;
+    if (threadIdx.x == 0) { sh->flags = 0; sh->is_last = 0; }
+    __syncthreads();
+}
+
+// ---- final stage, one thread: merge digits into the canonical limbs, round once ----------------------------
+
+__device__ inline fx_u64 ex_get64(const fx_u64* mag, int bit) {     // bits [bit, bit+63]
+    const int k = bit >> 6, s = bit & 63;
+    fx_u64 v = mag[k] >> s;
+    if (s && k + 1 < FX_NLIMB) v |= mag[k + 1] << (64 - s);
+    return v;
+}
+
+// RN(limbs) with ties to even, gradual underflow, overflow to inf; exact zero -> +0.0   (DESIGN.md 3.1 step 4)
+__device__ inline double ex_round(const fx_u64* limbs, int flags) {
+    if ((flags & FX_FLAG_NAN) || ((flags & FX_FLAG_PINF) && (flags & FX_FLAG_NINF)))
+        return __longlong_as_double(0x7FF8000000000000ll);
+    if (flags & FX_FLAG_PINF) return __longlong_as_double(0x7FF0000000000000ll);
+    if (flags & FX_FLAG_NINF) return __longlong_as_double((long long)0xFFF0000000000000ull);
+    fx_u64 mag[FX_NLIMB];
+    const bool neg = (limbs[FX_NLIMB - 1] >> 63) != 0;
+    fx_u64 carry = neg ? 1ull : 0ull;
+    int top = -1;
+    for (int k = 0; k < FX_NLIMB; ++k) {
+        fx_u64 v = neg ? ~limbs[k] : limbs[k];
+        const fx_u64 s = v + carry;
+        carry = (s < v) ? 1ull : 0ull;
+        mag[k] = s;
+        if (s) top = k;
+    }
+    if (top < 0) return 0.0;
+    const int t = 64 * top + 63 - __clzll((long long)mag[top]);
+    const int PMIN = -1074 + FX_BIAS;
+    const bool normal = (t - 52) >= PMIN;
+    const int p = normal ? (t - 52) : PMIN;
+    fx_u64 mant = ex_get64(mag, p);                                   // < 2^53
+    const fx_u64 round_bit = (mag[(p - 1) >> 6] >> ((p - 1) & 63)) & 1ull;
+    bool sticky = false;
+    {
+        const int b = p - 1;                                          // bits [0, b) below the round bit
+        const int k = b >> 6, s = b & 63;
+        for (int i = 0; i < k; ++i) sticky |= (mag[i] != 0);
+        if (s) sticky |= (mag[k] & ((1ull << s) - 1ull)) != 0;
+    }
+    if (round_bit && (sticky || (mant & 1ull))) mant += 1ull;
+    fx_u64 bits;
+    if (normal) {
+        const long long be = (long long)(t - FX_BIAS) + 1023;
+        if (be >= 2047) bits = 0x7FF0000000000000ull;
+        else bits = ((fx_u64)be << 52) + (mant - (1ull << 52));       // mant == 2^53 carries into the exponent
+    } else bits = mant;                                               // mant == 2^52 is the smallest normal
+    if (neg) bits |= 1ull << 63;
+    return __longlong_as_double((long long)bits);
+}
+
+// last CTA, thread 0.  first: limbs start from zero; last: round and publish.
+__device__ inline void ex_finalize(const ExGlobal& g, int first, int last, double* result) {
+    volatile fx_u64* dig = g.dig;
+    long long carry = 0;
+    fx_u64 c2 = 0;
+    fx_u64 limbs[FX_NLIMB];
+    for (int k = 0; k < FX_NLIMB; ++k) {
+        long long v = (long long)dig[2 * k] + carry;
+        const fx_u64 lo = (fx_u64)v & 0xffffffffull;
+        carry = v >> 32;
+        v = (long long)dig[2 * k + 1] + carry;
+        const fx_u64 hi = (fx_u64)v & 0xffffffffull;
+        carry = v >> 32;
+        dig[2 * k] = 0ull; dig[2 * k + 1] = 0ull;
+        const fx_u64 word = lo | (hi << 32);
+        const fx_u64 old = first ? 0ull : g.limbs[k];
+        fx_u64 s = old + word;
+        fx_u64 c = (s < old) ? 1ull : 0ull;
+        const fx_u64 s2 = s + c2;
+        c |= (s2 < s) ? 1ull : 0ull;
+        c2 = c;
+        limbs[k] = s2;
+        g.limbs[k] = s2;
+    }
+    if (last) {
+        const int flags = *(volatile int*)g.flags;
+        g.flags[1] = flags;                       // kept for fx_exdot_digits
+        g.flags[0] = 0;
+        if (result) *result = ex_round(limbs, flags);
+    }
+}
+
+// End of a CTA: digits -> global, the last CTA to arrive finalises.  Returns true in every thread of the last CTA
+// after the result has been written.  `first`/`last`: position of this launch in a multi-launch call.
+__device__ __forceinline__ bool ex_block_finish(ExShared* sh, const ExGlobal& g, int first, int last, double* result) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) {
+        const fx_u64 v = sh->dig[i];
+        if (v) atomicAdd(&g.dig[i], v);
+    }
+    if (threadIdx.x == 0 && sh->flags) atomicOr(g.flags, sh->flags);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned int t = atomicAdd(g.ticket, 1u);
+        sh->is_last = (t == gridDim.x * gridDim.y - 1);
+    }
+    __syncthreads();
+    if (!sh->is_last) return false;
+    if (threadIdx.x == 0) {
+        __threadfence();
+        ex_finalize(g, first, last, result);
+        *g.ticket = 0u;
+        __threadfence();
+    }
+    __syncthreads();
+    return true;
+}
+
+#endif

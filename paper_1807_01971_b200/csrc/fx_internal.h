@@ -1,0 +1,56 @@
+// fx_internal.h -- host-side state shared by the translation units of libfx.so (not part of the ABI).
+#ifndef FX_INTERNAL_H
+#define FX_INTERNAL_H
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/fx.h"
+#include "fx_dg.cuh"
+#include "fx_exdot.cuh"
+#include "fx_tables.h"
+
+#define FX_NUM_SMS_DEFAULT 148
+
+struct FxCtx {
+    bool ready;
+    int device, num_sms;
+    cudaStream_t stream;
+    ExGlobal ex;                 // device scratch of the exact dot
+    double* result_dev;          // [8] scratch doubles (dot results of the synchronous calls)
+    double* result_pinned;       // [8] pinned host mirror
+    // launch-shape overrides (fx_set_launch): [kernel_id][0]=grid, [1]=block
+    int launch[4][2];
+    int cg_fused;
+    // CG work space
+    double* cg_vec; int64_t cg_cap;   // 7 vectors of cg_cap doubles
+    void* cg_scal;                     // CgScal on the device
+    void* cg_scal_pinned;
+    // host staging for the *_host entry points
+    double* stage[4]; int64_t stage_cap;
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_copy[2], ev_comp[2];
+    int64_t launches;
+};
+
+FxCtx* fx_ctx();                               // lazily initialised; NULL (and last error set) on failure
+void fx_set_error(const char* fmt, ...);
+fx_status fx_cuda_fail(cudaError_t e, const char* what);
+
+#define FX_CUDA(call)                                           \
+    do {                                                        \
+        cudaError_t e_ = (call);                                \
+        if (e_ != cudaSuccess) return fx_cuda_fail(e_, #call);  \
+    } while (0)
+
+static inline bool aligned16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
+int fx_grid_ok(const fx_grid* g);
+fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* out, double* vol4_out);
+
+// internal launchers (stream-ordered, no synchronisation)
+fx_status fx_launch_exdot(FxCtx* c, const double* x, const double* y, int64_t n, double* result_dev);
+fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64_t m, int first, int last, double* result_dev);
+fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const double* x, double* y, int normed);
+
+#endif

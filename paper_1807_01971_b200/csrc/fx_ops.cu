@@ -1,0 +1,256 @@
+// fx_ops.cu -- exact-dot kernel, dG apply kernel, dG weights, and their C ABI entry points (include/fx.h).
+
+#include <math.h>
+#include <string.h>
+
+#include "fx_internal.h"
+
+// ------------------------------------------------------------------------------------------------------------
+// exact dot  (design in fx_exdot.cuh / DESIGN.md 6.1).  HBM roofline: 16 B per element.
+// ------------------------------------------------------------------------------------------------------------
+
+#define EX_K 4
+#define EX_W 40
+#define EX_U 4
+
+template <bool VEC>
+__global__ void __launch_bounds__(1024) k_exdot(const double* __restrict__ x, const double* __restrict__ y, long long n,
+                                                ExGlobal g, int first, int last, double* result) {
+    __shared__ ExShared sh;
+    ex_shared_init(&sh);
+    ExAcc<EX_K, EX_W> acc;
+    acc.init();
+    const long long tile = (long long)blockDim.x * EX_U;
+    const long long ntiles = (n + tile - 1) / tile;
+    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        double xv[EX_U], yv[EX_U];
+        if (VEC) {
+#pragma unroll
+            for (int u = 0; u < EX_U / 2; ++u) {
+                const long long e0 = t * tile + 2 * ((long long)u * blockDim.x + threadIdx.x);
+                if (e0 + 1 < n) {
+                    const double2 a = *reinterpret_cast<const double2*>(x + e0);
+                    const double2 b = *reinterpret_cast<const double2*>(y + e0);
+                    xv[2 * u] = a.x; xv[2 * u + 1] = a.y; yv[2 * u] = b.x; yv[2 * u + 1] = b.y;
+                } else {
+                    const bool in = e0 < n;
+                    xv[2 * u] = in ? x[e0] : 0.0; yv[2 * u] = in ? y[e0] : 0.0;
+                    xv[2 * u + 1] = 0.0; yv[2 * u + 1] = 0.0;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < EX_U; ++u) {
+                const long long e0 = t * tile + (long long)u * blockDim.x + threadIdx.x;
+                const bool in = e0 < n;
+                xv[u] = in ? x[e0] : 0.0; yv[u] = in ? y[e0] : 0.0;
+            }
+        }
+        acc.add<EX_U>(xv, yv, &sh);
+    }
+    acc.flush(&sh);
+    ex_block_finish(&sh, g, first, last, result);
+}
+
+// one launch over m <= 2^28 elements (keeps every 64-bit digit far from overflow); first/last: position in the call
+fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64_t m, int first, int last, double* result_dev) {
+    const bool vec = aligned16(x) && aligned16(y);
+    const int bd = c->launch[0][1] ? c->launch[0][1] : 256;
+    const long long tile = (long long)bd * EX_U;
+    long long grid = (m + tile - 1) / tile;
+    const long long gmax = (long long)c->num_sms * (1024 / bd) * 2;
+    if (grid > gmax) grid = gmax;
+    if (grid < 1) grid = 1;
+    if (c->launch[0][0]) grid = c->launch[0][0];
+    if (vec) k_exdot<true><<<(int)grid, bd, 0, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
+    else k_exdot<false><<<(int)grid, bd, 0, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
+    c->launches++;
+    FX_CUDA(cudaGetLastError());
+    return FX_OK;
+}
+
+fx_status fx_launch_exdot(FxCtx* c, const double* x, const double* y, int64_t n, double* result_dev) {
+    const int64_t CHUNK = (int64_t)1 << 28;
+    int64_t done = 0;
+    do {
+        const int64_t m = (n - done < CHUNK) ? (n - done) : CHUNK;
+        fx_status s = fx_launch_exdot_part(c, x + done, y + done, m, done == 0, done + m == n, result_dev);
+        if (s != FX_OK) return s;
+        done += m;
+    } while (done < n);
+    return FX_OK;
+}
+
+extern "C" fx_status fx_exdot_async(const double* x, const double* y, int64_t n, double* result_dev) {
+    if (n < 0 || (n > 0 && (!x || !y)) || !result_dev) { fx_set_error("fx_exdot_async: bad arguments"); return FX_EINVAL; }
+    FxCtx* c = fx_ctx();
+    if (!c) return FX_ECUDA;
+    return fx_launch_exdot(c, x, y, n, result_dev);
+}
+
+extern "C" double fx_exdot(const double* x, const double* y, int64_t n) {
+    if (n < 0 || (n > 0 && (!x || !y))) { fx_set_error("fx_exdot: bad arguments"); return NAN; }
+    fx_set_error("%s", "");                 // a NaN result with an empty fx_last_error() is a genuine NaN
+    FxCtx* c = fx_ctx();
+    if (!c) return NAN;
+    if (fx_launch_exdot(c, x, y, n, c->result_dev) != FX_OK) return NAN;
+    if (cudaMemcpyAsync(c->result_pinned, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess) {
+        fx_cuda_fail(cudaGetLastError(), "fx_exdot result copy");
+        return NAN;
+    }
+    return c->result_pinned[0];
+}
+
+extern "C" fx_status fx_exdot_digits(const double* x, const double* y, int64_t n, uint64_t* limbs_host, int32_t* flags_host,
+                                     double* result_host) {
+    if (n < 0 || (n > 0 && (!x || !y)) || !limbs_host) { fx_set_error("fx_exdot_digits: bad arguments"); return FX_EINVAL; }
+    FxCtx* c = fx_ctx();
+    if (!c) return FX_ECUDA;
+    // flags are cleared by the finaliser after rounding; read them through the result instead: launch, then copy
+    fx_status s = fx_launch_exdot(c, x, y, n, c->result_dev);
+    if (s != FX_OK) return s;
+    FX_CUDA(cudaStreamSynchronize(c->stream));
+    FX_CUDA(cudaMemcpy(limbs_host, c->ex.limbs, FX_NLIMB * sizeof(fx_u64), cudaMemcpyDeviceToHost));
+    int fl[2] = {0, 0};
+    FX_CUDA(cudaMemcpy(fl, c->ex.flags, 2 * sizeof(int), cudaMemcpyDeviceToHost));
+    if (flags_host) { flags_host[0] = (fl[1] & FX_FLAG_NAN) != 0; flags_host[1] = (fl[1] & FX_FLAG_PINF) != 0; flags_host[2] = (fl[1] & FX_FLAG_NINF) != 0; }
+    if (result_host) FX_CUDA(cudaMemcpy(result_host, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost));
+    return FX_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// dG elliptic apply  (fx_dg.cuh / DESIGN.md 6.2).  HBM roofline: 24 B per unknown.
+// ------------------------------------------------------------------------------------------------------------
+
+struct NoAcc { template <int U> __device__ void add(const double (&)[U], const double (&)[U], ExShared*) {} };
+
+template <int P>
+__global__ void __launch_bounds__(256) k_dg_apply(const __grid_constant__ DgParams g, const double* __restrict__ chi,
+                                                  const double* __restrict__ x, double* __restrict__ y) {
+    const int wpb = blockDim.x >> 5;
+    const long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
+    if (w >= (long long)g.nstrip * g.nseg) return;
+    // consecutive warps take consecutive strips of the same row segment: neighbouring halo columns are L1/L2 hits
+    const int seg = (int)(w / g.nstrip), strip = (int)(w % g.nstrip);
+    const int j0 = seg * g.rows_per_seg;
+    int j1 = j0 + g.rows_per_seg;
+    if (j1 > g.Ny) j1 = g.Ny;
+    dg_warp_strip<P, false, NoAcc>(g, chi, x, y, strip, j0, j1, nullptr, nullptr);
+}
+
+int fx_grid_ok(const fx_grid* g) {
+    return g && g->Nx >= 1 && g->Ny >= 1 && g->P >= 1 && g->P <= FX_PMAX && g->lx > 0 && g->ly > 0 &&
+           (g->bcx == FX_BC_PER || g->bcx == FX_BC_DIR) && (g->bcy == FX_BC_PER || g->bcy == FX_BC_DIR) &&
+           (int64_t)g->Nx * g->P < (1ll << 30) && (int64_t)g->Ny * g->P < (1ll << 30);
+}
+
+// host scalars and tables exactly as DESIGN.md 3.4 writes them (plain IEEE double operations, no contraction)
+fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* o, double* vol4_out) {
+    fx_tables t;
+    if (fx_make_tables(g->P, &t) != 0) { fx_set_error("P outside 1..5"); return FX_EINVAL; }
+    memset(o, 0, sizeof(*o));
+    const int P = g->P;
+    volatile double hx = g->lx / g->Nx, hy = g->ly / g->Ny;
+    volatile double hxhy = hx * hy;
+    const double vol4 = hxhy / 4;
+    o->Nx = g->Nx; o->Ny = g->Ny; o->bcx = g->bcx; o->bcy = g->bcy; o->normed = normed;
+    o->cxx = hy / hx; o->cyy = hx / hy;
+    volatile double hy2 = hy / 2, hx2 = hx / 2;
+    for (int k = 0; k < P; ++k) {
+        o->B[k] = t.B[k]; o->L[k] = t.L[k]; o->R[k] = t.R[k];
+        o->JX[k] = hy2 * t.w[k]; o->JY[k] = hx2 * t.w[k];          // jump factor jf = 1 (Q8)
+        for (int m = 0; m < P; ++m) {
+            o->T0[k][m] = t.T0[k][m]; o->T0L[k][m] = t.T0L[k][m]; o->WW[k][m] = t.WW[k][m];
+            volatile double w = vol4 * t.WW[k][m];
+            o->V[k][m] = 1.0 / w;
+        }
+    }
+    if (vol4_out) *vol4_out = vol4;
+    return FX_OK;
+}
+
+fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const double* x, double* y, int normed) {
+    DgParams p;
+    fx_status s = fx_make_dg_params(g, normed, &p, nullptr);
+    if (s != FX_OK) return s;
+    const int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
+    p.nstrip = (g->Nx + FX_STRIP - 1) / FX_STRIP;
+    // rows per segment: aim at >= 2 waves of 16 warps per SM, but keep the per-segment prologue (one extra cell row) small
+    int rps = c->launch[2][0];
+    if (rps <= 0) {
+        const long long target = (long long)c->num_sms * 32;
+        long long nseg = target / p.nstrip;
+        if (nseg < 1) nseg = 1;
+        rps = (int)((g->Ny + nseg - 1) / nseg);
+        if (rps < 8) rps = 8;
+    }
+    if (rps > g->Ny) rps = g->Ny;
+    p.rows_per_seg = rps;
+    p.nseg = (g->Ny + rps - 1) / rps;
+    const long long warps = (long long)p.nstrip * p.nseg;
+    const int grid = (int)((warps + wpb - 1) / wpb);
+    switch (g->P) {
+    case 1: k_dg_apply<1><<<grid, wpb * 32, 0, c->stream>>>(p, chi, x, y); break;
+    case 2: k_dg_apply<2><<<grid, wpb * 32, 0, c->stream>>>(p, chi, x, y); break;
+    case 3: k_dg_apply<3><<<grid, wpb * 32, 0, c->stream>>>(p, chi, x, y); break;
+    case 4: k_dg_apply<4><<<grid, wpb * 32, 0, c->stream>>>(p, chi, x, y); break;
+    case 5: k_dg_apply<5><<<grid, wpb * 32, 0, c->stream>>>(p, chi, x, y); break;
+    }
+    c->launches++;
+    FX_CUDA(cudaGetLastError());
+    return FX_OK;
+}
+
+static fx_status apply_checked(const fx_grid* g, const double* chi, const double* x, double* y, int normed) {
+    if (!fx_grid_ok(g) || !chi || !x || !y) { fx_set_error("fx_dg_elliptic_apply: bad grid or null pointer"); return FX_EINVAL; }
+    const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
+    const double *ye = y + n;
+    if ((x < ye && y < x + n) || (chi < ye && y < chi + n)) { fx_set_error("fx_dg_elliptic_apply: y overlaps an input"); return FX_EINVAL; }
+    FxCtx* c = fx_ctx();
+    if (!c) return FX_ECUDA;
+    return fx_launch_apply(c, g, chi, x, y, normed);
+}
+extern "C" fx_status fx_dg_elliptic_apply(const fx_grid* g, const double* chi, const double* x, double* y) { return apply_checked(g, chi, x, y, 1); }
+extern "C" fx_status fx_dg_elliptic_apply_sym(const fx_grid* g, const double* chi, const double* x, double* y) { return apply_checked(g, chi, x, y, 0); }
+
+// W[idx] = RN(vol4 * WW[l][k]),  V[idx] = RN(1 / W[idx])     (Fig. 2 "volume")
+__global__ void k_dg_weights(const __grid_constant__ DgParams g, int P, double vol4, double* W, double* V) {
+    const long long pitch = (long long)g.Nx * P, n = pitch * g.Ny * P;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int l = (int)((i / pitch) % P), k = (int)((i % pitch) % P);
+        if (W) W[i] = __dmul_rn(vol4, g.WW[l][k]);
+        if (V) V[i] = g.V[l][k];
+    }
+}
+
+extern "C" fx_status fx_dg_weights(const fx_grid* g, double* W, double* V) {
+    if (!fx_grid_ok(g)) { fx_set_error("fx_dg_weights: bad grid"); return FX_EINVAL; }
+    FxCtx* c = fx_ctx();
+    if (!c) return FX_ECUDA;
+    DgParams p; double vol4;
+    fx_status s = fx_make_dg_params(g, 0, &p, &vol4);
+    if (s != FX_OK) return s;
+    const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
+    int grid = (int)((n + 255) / 256); if (grid > c->num_sms * 32) grid = c->num_sms * 32;
+    k_dg_weights<<<grid, 256, 0, c->stream>>>(p, g->P, vol4, W, V);
+    c->launches++;
+    FX_CUDA(cudaGetLastError());
+    return FX_OK;
+}
+
+extern "C" fx_status fx_dg_tables(int32_t P, double* out) {
+    fx_tables t;
+    if (!out || fx_make_tables(P, &t) != 0) { fx_set_error("fx_dg_tables: bad arguments"); return FX_EINVAL; }
+    double* o = out;
+    for (int k = 0; k < P; ++k) *o++ = t.xi[k];
+    for (int k = 0; k < P; ++k) *o++ = t.w[k];
+    for (int k = 0; k < P; ++k) *o++ = t.L[k];
+    for (int k = 0; k < P; ++k) *o++ = t.R[k];
+    for (int k = 0; k < P; ++k) *o++ = t.B[k];
+    for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m) *o++ = t.T0[k][m];
+    for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m) *o++ = t.T0L[k][m];
+    for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m) *o++ = t.WW[k][m];
+    for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m) *o++ = t.D[k][m];
+    return FX_OK;
+}

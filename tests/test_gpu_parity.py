@@ -1,0 +1,362 @@
+"""GPU parity: libfx.so (through its C ABI) against the CPU oracle, element by element, on the same seeded inputs.
+
+Bars (BASELINE.json north_star / DESIGN.md 7): exact dot and every integer digit bit-exact; axpby, pointwise_dot, dG
+weights and the dG apply bit-exact against the oracle's canonical order (so also <= 1e-14), the apply additionally
+<= 1e-14 * scale against the 113-bit definition; CG: identical iteration count, relative L2 <= 1e-10 (expected: 0),
+bitwise identical across repeats, fused/unfused drivers and launch shapes.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import fxinputs as fi
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def fx():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    import paper_1807_01971_b200 as fx
+    fx.lib()
+    return fx
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+
+
+def bits(a):
+    return np.ascontiguousarray(a, dtype=np.float64).view(np.uint64)
+
+
+def same_bits(a, b):
+    return np.array_equal(bits(a), bits(b))
+
+
+def fbits(v):
+    return np.float64(v).view(np.uint64)
+
+
+@pytest.fixture(autouse=True)
+def _default_launch(fx):
+    yield
+    for k in range(4):
+        fx.set_launch(k, 0, 0)
+    fx.set_cg_fused(True)
+
+
+# ---- exact dot ----------------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("n", [0, 1, 2, 3, 31, 32, 33, 255, 1024, 1025, 4099, 100003, (1 << 20) + 7])
+def test_exdot_uniform_sizes(fx, oracle, n):
+    x, y = fi.uniform(11, n), fi.uniform(12, n)
+    want = oracle.exdot(x, y) if n else 0.0
+    got = fx.exdot(dev(x), dev(y)) if n else fx.exdot(dev(np.zeros(0)), dev(np.zeros(0)))
+    assert fbits(got) == fbits(want)
+
+
+@pytest.mark.parametrize("k", [10, 13, 17, 20])
+@pytest.mark.parametrize("ci", range(6))
+def test_exdot_condition_family(fx, oracle, k, ci):
+    x, y, expected = fi.dot_family_a(k, ci)
+    want, limbs, flags = oracle.exdot_digits(x, y)
+    if expected is not None:
+        assert want == expected                      # closed form by construction: 26 * 2^-e
+    got, glimbs, gflags = fx.exdot_digits(dev(x), dev(y))
+    assert fbits(got) == fbits(want)
+    assert np.array_equal(glimbs, limbs)             # the long accumulator itself, digit for digit
+    assert np.array_equal(gflags, flags)
+
+
+def test_exdot_special_cases(fx, oracle):
+    for name, x, y in fi.dot_special_cases():
+        want, limbs, flags = oracle.exdot_digits(x, y)
+        got, glimbs, gflags = fx.exdot_digits(dev(x), dev(y))
+        if math.isnan(want):
+            assert math.isnan(got), name
+        else:
+            assert fbits(got) == fbits(want), (name, got, want)
+        assert np.array_equal(gflags, flags), name
+        if not flags.any():
+            assert np.array_equal(glimbs, limbs), name
+
+
+def test_exdot_paper_example_and_closed_forms(fx):
+    import itertools
+    for perm in itertools.permutations([-1.0, 1.0, 2.0 ** -53]):
+        assert fx.exdot(dev(np.array(perm)), dev(np.ones(3))) == 2.0 ** -53
+    n = 300000                                                          # sum i^2 beyond 2^53
+    i = np.arange(1, n + 1, dtype=np.float64)
+    exact = n * (n + 1) * (2 * n + 1) // 6
+    assert fx.exdot(dev(i), dev(i)) == float(exact)
+    x = np.ldexp(1.0, -np.arange(1, 55))                                # sum 2^-i, i=1..54 is a tie -> 1.0
+    assert fx.exdot(dev(x), dev(np.ones(54))) == 1.0
+    assert fx.exdot(dev(x[:53]), dev(np.ones(53))) == 1.0 - 2.0 ** -53
+
+
+def test_exdot_wide_exponent_spread(fx, oracle):
+    """products far below the warp's window take the slow path; all of config 1's range in one vector"""
+    g = fi.rng(77)
+    n = 20000
+    x = np.ldexp(1.0 + g.random(n), g.integers(-500, 500, n)) * np.where(g.random(n) < 0.5, -1, 1)
+    y = np.ldexp(1.0 + g.random(n), g.integers(-500, 500, n))
+    want, limbs, _ = oracle.exdot_digits(x, y)
+    got, glimbs, _ = fx.exdot_digits(dev(x), dev(y))
+    assert fbits(got) == fbits(want)
+    assert np.array_equal(glimbs, limbs)
+
+
+def test_exdot_launch_shape_and_alignment_invariance(fx, oracle):
+    n = 300007
+    x, y = fi.uniform(21, n + 1), fi.uniform(22, n + 1)
+    x[:100] *= 1e-30
+    y[5000:5100] *= 1e25
+    dx, dy = dev(x), dev(y)
+    want = oracle.exdot(x[:n], y[:n])
+    for grid, block in [(0, 0), (1, 32), (3, 64), (148, 128), (1000, 256), (7, 1024), (296, 512)]:
+        fx.set_launch(0, grid, block)
+        assert fbits(fx.exdot(dx[:n], dy[:n])) == fbits(want), (grid, block)
+    fx.set_launch(0, 0, 0)
+    assert fbits(fx.exdot(dx[1:], dy[1:])) == fbits(oracle.exdot(x[1:], y[1:]))        # both 8-byte aligned only
+    assert fbits(fx.exdot(dx[1:], dy[:n])) == fbits(oracle.exdot(x[1:], y[:n]))        # mixed alignment
+    assert fbits(fx.exdot(dx, dx)) == fbits(oracle.exdot(x, x))                        # aliasing (norm)
+
+
+def test_exdot_async_and_host(fx, oracle):
+    import torch
+    n = 70001
+    x, y = fi.uniform(31, n), fi.uniform(32, n)
+    out = torch.zeros(1, dtype=torch.float64, device="cuda")
+    fx.exdot_async(dev(x), dev(y), out)
+    want = oracle.exdot(x, y)
+    assert fbits(out.cpu().numpy()[0]) == fbits(want)
+    assert fbits(fx.exdot_host(torch.from_numpy(x).pin_memory(), torch.from_numpy(y).pin_memory())) == fbits(want)
+
+
+@pytest.mark.parametrize("ci", [0, 3, 5])
+def test_exdot_full_size_config1(fx, oracle, ci):
+    """n = 2^27 (the largest size of config 1, the launch configuration bench.py times)"""
+    x, y, expected = fi.dot_family_a(27, ci)
+    got = fx.exdot(dev(x), dev(y))
+    if expected is not None:
+        assert got == expected
+    assert fbits(got) == fbits(oracle.exdot(x, y))
+
+
+# ---- axpby / pointwise_dot / weights ------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("n", [1, 2, 7, 1023, 2048, 2049, 100003, (1 << 21) + 5])
+@pytest.mark.parametrize("alpha,beta", [(0.7, -0.3), (1.25, 1.0), (-2.5, 0.0)])
+def test_axpby_bit_exact(fx, oracle, n, alpha, beta):
+    x, y = fi.uniform(41, n), fi.uniform(42, n)
+    want = oracle.axpby(alpha, x, beta, y)
+    got = fx.axpby(alpha, dev(x), beta, dev(y)).cpu().numpy()
+    assert same_bits(got, want)
+
+
+@pytest.mark.parametrize("n", [1, 5, 2047, 100003])
+@pytest.mark.parametrize("alpha,beta", [(1.0, 0.0), (0.3, 0.9), (-1.0, 1.0)])
+def test_pointwise_dot_bit_exact(fx, oracle, n, alpha, beta):
+    x1, x2, y = fi.uniform(43, n), fi.uniform(44, n), fi.uniform(45, n)
+    want = oracle.pointwise_dot(alpha, x1, x2, beta, y)
+    got = fx.pointwise_dot(alpha, dev(x1), dev(x2), beta, dev(y)).cpu().numpy()
+    assert same_bits(got, want)
+
+
+def test_elementwise_unaligned_alias_and_shapes(fx, oracle):
+    n = 5001
+    x, y = fi.uniform(46, n + 1), fi.uniform(47, n + 1)
+    dx, dy = dev(x), dev(y)
+    got = fx.axpby(0.5, dx[1:], 2.0, dy[1:]).cpu().numpy()
+    assert same_bits(got, oracle.axpby(0.5, x[1:], 2.0, y[1:]))
+    dz = dev(x)
+    assert same_bits(fx.axpby(3.0, dz, -1.5, dz).cpu().numpy(), oracle.axpby(3.0, x, -1.5, x))      # x is y
+    for grid, block in [(1, 32), (5, 1024), (999, 64)]:
+        fx.set_launch(1, grid, block)
+        assert same_bits(fx.axpby(0.7, dev(x), -0.3, dev(y)).cpu().numpy(), oracle.axpby(0.7, x, -0.3, y))
+    beta0 = fx.axpby(2.0, dev(x), 0.0, dev(np.full(n + 1, np.nan))).cpu().numpy()                   # y not read
+    assert same_bits(beta0, oracle.axpby(2.0, x, 0.0, y))
+
+
+GRIDS = [(1, 1), (2, 3), (3, 2), (31, 5), (30, 9), (61, 17), (64, 64)]
+BCS = [(0, 0), (0, 1), (1, 0), (1, 1)]
+
+
+def _grid(fx, oracle, Nx, Ny, P, bcx, bcy, lx=2 * math.pi, ly=3.0):
+    return fx.make_grid(Nx, Ny, P, lx, ly, bcx, bcy), oracle.Grid(Nx, Ny, P, lx, ly, bcx, bcy)
+
+
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
+def test_dg_weights_bit_exact(fx, oracle, P):
+    import torch
+    g, og = _grid(fx, oracle, 7, 5, P, 0, 1)
+    w = torch.empty(g.n, dtype=torch.float64, device="cuda"); v = torch.empty_like(w)
+    fx.dg_weights(g, w, v)
+    W, V = oracle.dg_weights(og)
+    assert same_bits(w.cpu().numpy(), W) and same_bits(v.cpu().numpy(), V)
+
+
+# ---- dG apply -----------------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("bc", BCS)
+def test_dg_apply_bit_exact_small_grids(fx, oracle, P, bc):
+    import torch
+    for (Nx, Ny) in GRIDS:
+        g, og = _grid(fx, oracle, Nx, Ny, P, *bc)
+        x = fi.uniform(51 + P, g.n); chi = 1.0 + 0.5 * fi.uniform(61 + P, g.n)
+        for sym in (True, False):
+            want = oracle.dg_apply_canonical(og, chi, x, normed=not sym)
+            y = torch.full((g.n,), float("nan"), dtype=torch.float64, device="cuda")
+            fx.dg_elliptic_apply(g, dev(chi), dev(x), y, sym=sym)
+            got = y.cpu().numpy()
+            assert np.array_equal(got, want), (Nx, Ny, P, bc, sym, np.abs(got - want).max())
+            assert same_bits(got + 0.0, want + 0.0)
+
+
+@pytest.mark.parametrize("P", [2, 3, 5])
+def test_dg_apply_against_definition(fx, oracle, P):
+    """|y - y_def| <= 1e-14 * (|F^T||W chi||F| + |J|)|x|, y_def from explicit block matrices in 113-bit arithmetic"""
+    import torch
+    g, og = _grid(fx, oracle, 12, 9, P, 0, 1)
+    x = fi.uniform(71, g.n); chi = 1.0 + 0.5 * fi.uniform(72, g.n)
+    for sym in (True, False):
+        ydef, scale = oracle.dg_apply_definition(og, chi, x, normed=not sym)
+        y = torch.empty(g.n, dtype=torch.float64, device="cuda")
+        fx.dg_elliptic_apply(g, dev(chi), dev(x), y, sym=sym)
+        assert np.all(np.abs(y.cpu().numpy() - ydef) <= 1e-14 * scale)
+
+
+def test_dg_apply_launch_shape_invariance(fx, oracle):
+    import torch
+    g, og = _grid(fx, oracle, 95, 40, 3, 0, 1)
+    x = fi.uniform(73, g.n); chi = 1.0 + 0.5 * fi.uniform(74, g.n)
+    want = oracle.dg_apply_canonical(og, chi, x, normed=False)
+    for rows, block in [(0, 0), (1, 32), (3, 64), (7, 256), (40, 128), (1000, 1024)]:
+        fx.set_launch(2, rows, block)
+        y = torch.empty(g.n, dtype=torch.float64, device="cuda")
+        fx.dg_elliptic_apply(g, dev(chi), dev(x), y, sym=True)
+        assert np.array_equal(y.cpu().numpy(), want), (rows, block)
+
+
+def test_dg_apply_rejects_overlap_and_bad_grid(fx):
+    import torch
+    g = fx.make_grid(4, 4, 3, 1.0, 1.0, 0, 1)
+    x = torch.zeros(g.n, dtype=torch.float64, device="cuda")
+    with pytest.raises(fx.FxError):
+        fx.dg_elliptic_apply(g, x, x, x)
+    bad = fx.make_grid(4, 4, 6, 1.0, 1.0, 0, 1)
+    with pytest.raises(fx.FxError):
+        fx.dg_elliptic_apply(bad, torch.zeros(bad.n, dtype=torch.float64, device="cuda"), torch.zeros(bad.n, dtype=torch.float64, device="cuda"),
+                             torch.zeros(bad.n, dtype=torch.float64, device="cuda"))
+
+
+def test_dg_apply_full_size_config3(fx, oracle):
+    """1024 x 1024 cells, P = 3: every element against the canonical oracle (default launch shape = bench.py's)"""
+    import torch
+    c = fi.config3()
+    g, og = fx.make_grid(**c["grid"]), oracle.Grid(**c["grid"])
+    x = fi.uniform(75, g.n)
+    want = oracle.dg_apply_canonical(og, c["chi"], x, normed=False)
+    y = torch.empty(g.n, dtype=torch.float64, device="cuda")
+    fx.dg_elliptic_apply(g, dev(c["chi"]), dev(x), y, sym=True)
+    assert np.array_equal(y.cpu().numpy(), want)
+
+
+# ---- CG -----------------------------------------------------------------------------------------------------------
+
+def _solve(fx, c, tol=None, maxit=None):
+    g = fx.make_grid(**c["grid"])
+    phi = dev(c["phi0"])
+    info = fx.cg_solve(g, dev(c["chi"]), dev(c["rho"]), phi, c["tol"] if tol is None else tol, c["maxit"] if maxit is None else maxit)
+    return phi.cpu().numpy(), info
+
+
+def test_cg_config0_matches_oracle(fx, oracle):
+    c = fi.config0()
+    og = oracle.Grid(**c["grid"])
+    want, oinfo = oracle.cg_solve(og, c["chi"], c["rho"], c["phi0"], c["tol"], c["maxit"])
+    got, info = _solve(fx, c)
+    assert info.iterations == oinfo.iterations and info.status == oinfo.status == 0
+    rel = np.linalg.norm(got - want) / np.linalg.norm(want)
+    assert rel <= 1e-10
+    assert same_bits(got, want), "expected a bit-identical trajectory (rel = %g)" % rel
+    assert info.rel_residual == oinfo.rel_residual
+    # the manufactured solution: discretisation error of order P (Q7)
+    W, _ = oracle.dg_weights(og)
+    err = math.sqrt(np.sum(W * (got - c["phi_exact"]) ** 2) / np.sum(W * c["phi_exact"] ** 2))
+    assert err < 1e-5
+
+
+def test_cg_reproducible_across_runs_drivers_and_shapes(fx):
+    c = fi.config0(N=32)
+    ref, info0 = _solve(fx, c)
+    for _ in range(2):
+        got, info = _solve(fx, c)
+        assert same_bits(got, ref) and info.iterations == info0.iterations
+    fx.set_cg_fused(False)
+    got, info = _solve(fx, c)
+    assert same_bits(got, ref) and info.iterations == info0.iterations
+    fx.set_cg_fused(True)
+    for (rows, ablock, egrid, eblock, dgrid, dblock) in [(1, 32, 1, 32, 1, 32), (5, 128, 37, 512, 300, 64), (100, 1024, 999, 128, 2, 1024)]:
+        fx.set_launch(2, rows, ablock); fx.set_launch(3, egrid, eblock); fx.set_launch(0, dgrid, dblock)
+        got, info = _solve(fx, c)
+        assert same_bits(got, ref) and info.iterations == info0.iterations
+
+
+@pytest.mark.parametrize("P", [1, 2, 4, 5])
+def test_cg_other_orders(fx, oracle, P):
+    c = fi.config0(N=12, P=P)
+    og = oracle.Grid(**c["grid"])
+    want, oinfo = oracle.cg_solve(og, c["chi"], c["rho"], c["phi0"], 1e-9, 3000)
+    got, info = _solve(fx, c, tol=1e-9, maxit=3000)
+    assert info.iterations == oinfo.iterations and info.status == oinfo.status
+    assert same_bits(got, want)
+
+
+def test_cg_config2_reduced_and_maxit(fx, oracle):
+    c = fi.config2(N=48)
+    og = oracle.Grid(**c["grid"])
+    want, oinfo = oracle.cg_solve(og, c["chi"], c["rho"], c["phi0"], c["tol"], c["maxit"])
+    got, info = _solve(fx, c)
+    assert info.iterations == oinfo.iterations and info.status == oinfo.status == 0
+    assert same_bits(got, want)
+    want, oinfo = oracle.cg_solve(og, c["chi"], c["rho"], c["phi0"], 0.0, 37)        # fixed iteration count (config 3's mode)
+    got, info = _solve(fx, c, tol=0.0, maxit=37)
+    assert info.iterations == oinfo.iterations == 37 and info.status == oinfo.status == 1
+    assert same_bits(got, want)
+
+
+def test_cg_zero_rhs_and_nonzero_start(fx, oracle):
+    c = fi.config0(N=8)
+    og = oracle.Grid(**c["grid"])
+    z = np.zeros_like(c["rho"])
+    got, info = _solve(fx, dict(c, rho=z, phi0=fi.uniform(81, z.size)))
+    assert info.iterations == 0 and np.all(got == 0.0)
+    phi0 = 0.1 * fi.uniform(82, z.size)
+    want, oinfo = oracle.cg_solve(og, c["chi"], c["rho"], phi0, 1e-9, 2000)
+    got, info = _solve(fx, dict(c, phi0=phi0), tol=1e-9, maxit=2000)
+    assert info.iterations == oinfo.iterations and same_bits(got, want)
+
+
+def test_cg_full_size_config3_first_iterations(fx, oracle):
+    """config 3 at full size, the launch shape bench.py times; 6 iterations against the oracle, bit for bit"""
+    c = fi.config3()
+    og = oracle.Grid(**c["grid"])
+    want, oinfo = oracle.cg_solve(og, c["chi"], c["rho"], c["phi0"], 0.0, 6)
+    got, info = _solve(fx, c, tol=0.0, maxit=6)
+    assert info.iterations == oinfo.iterations == 6 and info.status == 1
+    assert same_bits(got, want)
+
+
+def test_cg_host_entry(fx, oracle):
+    c = fi.config0(N=8)
+    og = oracle.Grid(**c["grid"])
+    want, oinfo = oracle.cg_solve(og, c["chi"], c["rho"], c["phi0"], 1e-9, 2000)
+    phi = c["phi0"].copy()
+    info = fx.cg_solve_host(fx.make_grid(**c["grid"]), c["chi"], c["rho"], phi, 1e-9, 2000)
+    assert info.iterations == oinfo.iterations and same_bits(phi, want)

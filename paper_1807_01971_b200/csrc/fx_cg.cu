@@ -151,7 +151,8 @@ static fx_status cg_workspace(FxCtx* c, int64_t n) {
 }
 
 static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int* apply_grid, int* apply_block, int* ew_grid, int* ew_block) {
-    const int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
+    int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
+    if (wpb > 8) wpb = 8;
     p->nstrip = (g->Nx + FX_STRIP - 1) / FX_STRIP;
     int rps = c->launch[2][0];
     if (rps <= 0) {
@@ -167,7 +168,8 @@ static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int* apply_grid, 
     const long long warps = (long long)p->nstrip * p->nseg;
     *apply_grid = (int)((warps + wpb - 1) / wpb);
     *apply_block = wpb * 32;
-    const int bd = c->launch[3][1] ? c->launch[3][1] : 256;
+    int bd = c->launch[3][1] ? c->launch[3][1] : 256;
+    if (bd > 256) bd = 256;
     const int pitch = g->Nx * g->P;
     const long long cpr = (pitch + (long long)bd * CG_U - 1) / ((long long)bd * CG_U);
     long long chunks = cpr * g->Ny * g->P;

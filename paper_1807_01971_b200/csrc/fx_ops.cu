@@ -174,7 +174,8 @@ fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const d
     DgParams p;
     fx_status s = fx_make_dg_params(g, normed, &p, nullptr);
     if (s != FX_OK) return s;
-    const int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
+    int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
+    if (wpb > 8) wpb = 8;                       // the kernels are compiled for <= 256 threads per CTA
     p.nstrip = (g->Nx + FX_STRIP - 1) / FX_STRIP;
     // rows per segment: aim at >= 2 waves of 16 warps per SM, but keep the per-segment prologue (one extra cell row) small
     int rps = c->launch[2][0];

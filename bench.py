@@ -1,0 +1,293 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the driver (contract: task prompt "bench.py" + tier section 4).
+
+A "step" is one pass of the whole hot path = ONE preconditioned-CG iteration (dG apply + exact dot, the two vector
+updates + preconditioner + exact dot, the direction update) on BASELINE.json configs[3]: 1024 x 1024 cells, P = 3
+(9.4 M fp64 unknowns, 75.5 MB per vector, working set 7 vectors = 528 MB > L2), chi / rho as configs[2].
+value = algorithmic GB/s of the iteration: 12 vector passes x 8 B x n per iteration / device time.
+Extra keys report the metric's other parts: exact-dot, dG-apply and axpby GB/s at >= 100 MB vectors.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--quick]
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+PASSES_FUSED = 12          # vector passes of one fused CG iteration: K1 3, K2 6, K3 3
+METRIC = "CG-iteration algorithmic bandwidth (dG apply + exact dots + vector updates; 12 vector passes x 8 B x n per iteration)"
+UNIT = "GB/s"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md 'clocks' line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            self.t.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); mx = max(mx, float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, col in (("hw_slowdown", 5), ("hw_thermal_slowdown", 6), ("sw_thermal_slowdown", 7), ("sw_power_cap", 8)):
+                if len(r) > col and r[col].lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def reduce_over_ranks(ms_local, units_local, world):
+    """max time over ranks, sum of units (replicas only: DESIGN.md 8).  Uses torch.distributed when world > 1."""
+    if world == 1:
+        return ms_local, units_local
+    import torch
+    import torch.distributed as dist
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([ms_local], dtype=torch.float64, device=dev)
+    u = torch.tensor([units_local], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def time_events(fn, reps, torch):
+    """CUDA-event time per call (ms) of fn over `reps` back-to-back calls on torch's current stream."""
+    s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    s.record()
+    for _ in range(reps):
+        fn()
+    e.record()
+    torch.cuda.synchronize()
+    return s.elapsed_time(e) / reps
+
+
+def run_fx(args):
+    import numpy as np
+    import torch
+
+    import fxinputs as fi
+    import paper_1807_01971_b200 as fx
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (libfx has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    fx.lib()
+    K, Wm = args.steps, max(args.warmup, 3)
+    N = 256 if args.quick else 1024
+    cfg = fi.config3(N=N)
+    g = fx.make_grid(**cfg["grid"])
+    n = g.n
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        chi = torch.from_numpy(cfg["chi"]).cuda(); rho = torch.from_numpy(cfg["rho"]).cuda()
+        phi = torch.zeros(n, dtype=torch.float64, device="cuda")
+        # ---- warm-up: W iterations through the same call (also allocates the library's work space) -------------
+        fx.cg_solve(g, chi, rho, phi, 0.0, Wm)
+        phi.zero_()
+        fx.cg_profile(True)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        l0 = fx.launch_count()
+        with ClockSampler(local) as clk:
+            # ---- timed region: exactly K iterations; events on the library's stream around every loop kernel ---
+            info = fx.cg_solve(g, chi, rho, phi, 0.0, K)
+            torch.cuda.synchronize()
+            if world > 1:
+                dist.barrier()
+        prof = fx.cg_last_profile()
+        launches = fx.launch_count() - l0
+        fx.cg_profile(False)
+        assert info.iterations == K and prof["iterations"] == K, (info.iterations, prof)
+        loop_ms = prof["loop_ms"]
+        ms, units = reduce_over_ranks(loop_ms, float(K) * PASSES_FUSED * 8.0 * n, world)
+        value = units / (ms * 1e-3) / 1e9
+        peak, peak_src = peaks()
+
+        # ---- roofline of the dominant kernel (K1: dG apply fused with the exact dot p.Sp) ------------------------
+        k_ms = {k: prof[k + "_ms"] / K for k in ("k1", "k2", "k3")}
+        dom = max(k_ms, key=k_ms.get)
+        bytes_per_launch = {"k1": 24.0 * n, "k2": 48.0 * n, "k3": 24.0 * n}
+        achieved = bytes_per_launch[dom] / (k_ms[dom] * 1e-3) / 1e9
+        names = {"k1": "k_cg_apply_dot<3> (q = S p fused with exact dot p.q; 24 B/unknown)",
+                 "k2": "k_cg_update<3> (phi,r updates + preconditioner + exact dot r.z; 48 B/unknown)",
+                 "k3": "k_cg_dir<3> (p = z + beta p; 24 B/unknown)"}
+        roofline = {"bound": "hbm", "kernel": names[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "peak_source": peak_src, "traffic": None,
+                    "frac_of_nominal_8TBs": achieved / 8000.0,
+                    "per_kernel_ms": k_ms,
+                    "per_kernel_GBs": {k: bytes_per_launch[k] / (k_ms[k] * 1e-3) / 1e9 for k in k_ms},
+                    "kernel_share_of_step": {k: k_ms[k] / (loop_ms / K) for k in k_ms}}
+        traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(traffic_file):
+            roofline["traffic"] = json.load(open(traffic_file)).get(dom)
+
+        # ---- the metric's other parts: primitives on >= 100 MB vectors (inputs larger than L2) --------------------
+        prim = {}
+        if rank == 0 and not args.no_primitives:
+            nd = (1 << 22) if args.quick else (1 << 27)
+            x = torch.from_numpy(fi.uniform(9001, nd)).cuda(); y = torch.from_numpy(fi.uniform(9002, nd)).cuda()
+            out = torch.zeros(1, dtype=torch.float64, device="cuda")
+            for _ in range(3):
+                fx.exdot_async(x, y, out)
+            t = time_events(lambda: fx.exdot_async(x, y, out), 20, torch)
+            prim["exdot"] = {"n": nd, "MB_per_vector": 8e-6 * nd, "ms": t, "GBps": 16.0 * nd / t / 1e6, "frac_of_peak": 16.0 * nd / t / 1e6 / peak}
+            for _ in range(3):
+                fx.axpby(0.7, x, -0.3, y)
+            t = time_events(lambda: fx.axpby(0.7, x, -0.3, y), 20, torch)
+            prim["axpby"] = {"n": nd, "ms": t, "GBps": 24.0 * nd / t / 1e6, "frac_of_peak": 24.0 * nd / t / 1e6 / peak}
+            for _ in range(3):
+                fx.pointwise_dot(1.0, x, y, 0.0, x)
+            y.copy_(torch.from_numpy(fi.uniform(9002, nd)))
+            z = torch.empty_like(x)
+            t = time_events(lambda: fx.pointwise_dot(1.0, x, y, 0.0, z), 20, torch)
+            prim["pointwise_dot"] = {"n": nd, "ms": t, "GBps": 24.0 * nd / t / 1e6, "frac_of_peak": 24.0 * nd / t / 1e6 / peak}
+            del x, y, z
+            q = torch.empty(n, dtype=torch.float64, device="cuda")
+            pvec = torch.from_numpy(fi.uniform(9003, n)).cuda()
+            for _ in range(3):
+                fx.dg_elliptic_apply(g, chi, pvec, q, sym=True)
+            t = time_events(lambda: fx.dg_elliptic_apply(g, chi, pvec, q, sym=True), 20, torch)
+            prim["dg_apply"] = {"grid": "%dx%d P=3" % (N, N), "n": n, "MB_per_vector": 8e-6 * n, "ms": t, "GBps": 24.0 * n / t / 1e6,
+                                "frac_of_peak": 24.0 * n / t / 1e6 / peak, "note": "3 x 75.5 MB partly L2-resident between repeats"}
+
+        # ---- e2e: the public host-buffer call; H2D of chi, rho, phi0 and D2H of phi inside the timed region -------
+        hchi = torch.from_numpy(cfg["chi"]).pin_memory(); hrho = torch.from_numpy(cfg["rho"]).pin_memory()
+        hphi = torch.zeros(n, dtype=torch.float64).pin_memory()
+        fx.cg_solve_host(g, hchi, hrho, hphi, 0.0, 3)
+        hphi.zero_()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        info2 = fx.cg_solve_host(g, hchi, hrho, hphi, 0.0, K)
+        t1 = time.perf_counter()
+        e_ms, e_units = reduce_over_ranks((t1 - t0) * 1e3, float(K) * PASSES_FUSED * 8.0 * n, world)
+        assert info2.iterations == K
+        same = bool(torch.equal(hphi, phi.cpu()))
+        e2e = {"value": e_units / (e_ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": 3 * 8.0 * n / K, "d2h_bytes_per_step": 8.0 * n / K,
+               "ms_total": e_ms, "region": "one fx_cg_solve_host call: H2D chi,rho,phi0 (pinned) + setup + K iterations + D2H phi; bytes per step = per call / K",
+               "bitwise_equal_to_device_run": same}
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+           "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic (seeded; fxinputs.config3: chi = 1+0.5 exp(-r^2/0.5), rho = n-N with 1e-3 uniform noise; stands in for the paper's datasets [58],[59])",
+           "config": {"workload": "BASELINE.json configs[3]: dG elliptic PCG, %dx%d cells, P=3, %d fp64 unknowns, DIRxDIR, tol=0, fixed K iterations" % (N, N, n),
+                      "step": "one fused PCG iteration (3 kernels)", "l2": "inputs larger than L2 (7 vectors x %.1f MB)" % (8e-6 * n),
+                      "multi_gpu": "replicas only (north star: one GPU, no sharding)", "algorithmic_bytes_per_step": PASSES_FUSED * 8.0 * n},
+           "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+           "cg": {"iterations": int(info.iterations), "status": int(info.status), "rel_residual": info.rel_residual},
+           "primitives": prim}
+    if rank == 0:
+        if not args.no_cpu_baseline and world == 1:
+            out["cpu_baseline"] = cpu_baseline(cfg, n, quick=args.quick)
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def cpu_baseline(cfg, n, quick=False):
+    """The oracle as it stands, on the host cores, bounded sample: 5 CG iterations of the same grid (t(6) - t(1))."""
+    import oracle as o
+    og = o.Grid(**cfg["grid"])
+    its = 2 if quick else 5
+    t0 = time.perf_counter(); o.cg_solve(og, cfg["chi"], cfg["rho"], cfg["phi0"], 0.0, 1); t1 = time.perf_counter()
+    o.cg_solve(og, cfg["chi"], cfg["rho"], cfg["phi0"], 0.0, 1 + its); t2 = time.perf_counter()
+    per_it = ((t2 - t1) - (t1 - t0)) / its
+    return {"value": PASSES_FUSED * 8.0 * n / per_it / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "ms_per_step": per_it * 1e3,
+            "sample": "%d CG iterations of the same %dx%d P=3 problem (time of 1+%d iterations minus time of 1), oracle/fxo.cpp single-threaded"
+                      % (its, og.Nx, og.Ny, its)}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric/unit; each step = one oracle CG iteration on a
+    256 x 256-cell sub-sample of the workload (1/16 of the unknowns), so that K steps end within minutes."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import fxinputs as fi
+    import oracle as o
+    K, Wm = args.steps, max(args.warmup, 1)
+    N = 256
+    cfg = fi.config3(N=N)
+    og = o.Grid(**cfg["grid"])
+    n = og.n
+    o.cg_solve(og, cfg["chi"], cfg["rho"], cfg["phi0"], 0.0, Wm)
+    t0 = time.perf_counter(); o.cg_solve(og, cfg["chi"], cfg["rho"], cfg["phi0"], 0.0, 0); t_setup = time.perf_counter() - t0
+    t0 = time.perf_counter(); _, info = o.cg_solve(og, cfg["chi"], cfg["rho"], cfg["phi0"], 0.0, K); t = time.perf_counter() - t0
+    ms = max(t - t_setup, 1e-9) * 1e3
+    value = K * PASSES_FUSED * 8.0 * n / (ms * 1e-3) / 1e9
+    sample = "each step = one oracle CG iteration on a 256x256-cell, P=3 sub-sample (1/16 of configs[3]); setup time subtracted"
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": K, "warmup": Wm,
+                      "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                      "data": "synthetic (fxinputs.config3 at N=256)",
+                      "config": {"workload": "BASELINE.json configs[3] (bounded sample: 256x256 cells, P=3, %d unknowns)" % n},
+                      "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+                      "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                      "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="fx", choices=["fx", "reference"])
+    ap.add_argument("--quick", action="store_true", help="256x256 grid and small vectors (smoke runs)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-primitives", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_fx(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -55,6 +55,8 @@ _SIGNATURES = {
     "fx_dg_tables": (C.c_int, [C.c_int32, _dp]),
     "fx_cg_solve": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp, C.c_double, C.c_int32, C.POINTER(CGInfo)]),
     "fx_cg_solve_host": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp, C.c_double, C.c_int32, C.POINTER(CGInfo)]),
+    "fx_cg_profile": (C.c_int, [C.c_int32]),
+    "fx_cg_last_profile": (C.c_int, [_dp, C.POINTER(C.c_int32)]),
     "fx_launch_count": (C.c_int64, []),
 }
 
@@ -218,6 +220,18 @@ def cg_solve(grid, chi, rho, phi, tol, maxit):
     _check(lib().fx_cg_solve(C.byref(grid), _ptr(chi, grid.n), _ptr(rho, grid.n), _ptr(phi, grid.n), float(tol), int(maxit),
                              C.byref(info)), "fx_cg_solve")
     return info
+
+
+def cg_profile(enable):
+    _check(lib().fx_cg_profile(int(bool(enable))), "fx_cg_profile")
+
+
+def cg_last_profile():
+    """-> dict(loop_ms, k1_ms, k2_ms, k3_ms, iterations) of the most recent profiled fused solve (device times)."""
+    ms = (C.c_double * 4)()
+    it = C.c_int32(0)
+    _check(lib().fx_cg_last_profile(ms, C.byref(it)), "fx_cg_last_profile")
+    return dict(loop_ms=ms[0], k1_ms=ms[1], k2_ms=ms[2], k3_ms=ms[3], iterations=it.value)
 
 
 def cg_solve_host(grid, chi, rho, phi, tol, maxit):

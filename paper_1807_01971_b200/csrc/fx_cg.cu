@@ -12,6 +12,7 @@
 //     were enqueued past convergence into no-ops, and the host looks at it once per batch of iterations.
 
 #include <math.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "fx_internal.h"
@@ -143,7 +144,9 @@ static fx_status cg_workspace(FxCtx* c, int64_t n) {
         c->cg_cap = n;
     }
     if (!c->cg_scal) {
-        if (cudaMalloc(&c->cg_scal, sizeof(CgScal)) != cudaSuccess || cudaMallocHost(&c->cg_scal_pinned, sizeof(CgScal)) != cudaSuccess) {
+        if (cudaMalloc(&c->cg_scal, sizeof(CgScal)) != cudaSuccess || cudaMallocHost(&c->cg_scal_pinned, 2 * sizeof(CgScal)) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->cg_ev[0], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->cg_ev[1], cudaEventDisableTiming) != cudaSuccess) {
             fx_set_error("CG scalars: %s", cudaGetErrorString(cudaGetLastError())); return FX_ENOMEM;
         }
     }
@@ -183,12 +186,55 @@ template <int P>
 static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, int eg, int eb, const double* chi, double* phi,
                                   double* r, double* p, double* q, CgScal* sc, int iters) {
     for (int i = 0; i < iters; ++i) {
+        cudaEvent_t* ev = nullptr;
+        if (c->prof_on && c->prof_iters < c->prof_cap) { ev = c->prof_ev + 4 * c->prof_iters; c->prof_iters++; }
+        if (ev) cudaEventRecord(ev[0], c->stream);
         k_cg_apply_dot<P><<<ag, ab, 0, c->stream>>>(dp, chi, p, q, c->ex, sc);
+        if (ev) cudaEventRecord(ev[1], c->stream);
         k_cg_update<P><<<eg, eb, 0, c->stream>>>(dp, p, q, phi, r, c->ex, sc);
+        if (ev) cudaEventRecord(ev[2], c->stream);
         k_cg_dir<P><<<eg, eb, 0, c->stream>>>(dp, r, p, sc);
+        if (ev) cudaEventRecord(ev[3], c->stream);
         c->launches += 3;
     }
     FX_CUDA(cudaGetLastError());
+    return FX_OK;
+}
+
+extern "C" fx_status fx_cg_profile(int32_t enable) {
+    FxCtx* c = fx_ctx();
+    if (!c) return FX_ECUDA;
+    if (enable && !c->prof_ev) {
+        c->prof_cap = 1024;
+        c->prof_ev = (cudaEvent_t*)calloc((size_t)4 * c->prof_cap, sizeof(cudaEvent_t));
+        for (int i = 0; i < 4 * c->prof_cap; ++i) FX_CUDA(cudaEventCreate(&c->prof_ev[i]));
+    }
+    c->prof_on = enable ? 1 : 0;
+    return FX_OK;
+}
+
+extern "C" fx_status fx_cg_last_profile(double* ms, int32_t* iters) {
+    FxCtx* c = fx_ctx();
+    if (!c) return FX_ECUDA;
+    if (!ms) { fx_set_error("fx_cg_last_profile: null pointer"); return FX_EINVAL; }
+    for (int i = 0; i < 4; ++i) ms[i] = c->prof_ms[i];
+    if (iters) *iters = c->prof_iters;
+    return FX_OK;
+}
+
+static fx_status cg_collect_profile(FxCtx* c, int iters_done) {
+    for (int i = 0; i < 4; ++i) c->prof_ms[i] = 0.0;
+    int m = c->prof_iters < iters_done ? c->prof_iters : iters_done;
+    c->prof_iters = m;
+    if (m <= 0) return FX_OK;
+    float t;
+    FX_CUDA(cudaEventElapsedTime(&t, c->prof_ev[0], c->prof_ev[4 * (m - 1) + 3]));
+    c->prof_ms[0] = t;
+    for (int i = 0; i < m; ++i)
+        for (int k = 0; k < 3; ++k) {
+            FX_CUDA(cudaEventElapsedTime(&t, c->prof_ev[4 * i + k], c->prof_ev[4 * i + k + 1]));
+            c->prof_ms[1 + k] += t;
+        }
     return FX_OK;
 }
 
@@ -240,7 +286,7 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
                 rz = rz_new;
             }
             if (it > maxit) it = maxit;
-        } else {
+        } else if (maxit > 0) {
             DgParams dp;
             if ((s = fx_make_dg_params(g, 0, &dp, nullptr)) != FX_OK) return s;
             int ag, ab, eg, eb;
@@ -251,24 +297,37 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
             hs->rz = rz; hs->bz = bz; hs->thresh = thresh; hs->status = FX_MAXIT;
             FX_CUDA(cudaMemcpyAsync(sc, hs, sizeof(CgScal), cudaMemcpyHostToDevice, c->stream));
             FX_CUDA(cudaStreamSynchronize(c->stream));           // hs is reused as the read-back buffer
-            int enq = 0;
-            int batch = 8;
-            while (enq < maxit) {
-                const int m = (maxit - enq < batch) ? (maxit - enq) : batch;
-                switch (g->P) {
-                case 1: s = cg_enqueue_iters<1>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
-                case 2: s = cg_enqueue_iters<2>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
-                case 3: s = cg_enqueue_iters<3>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
-                case 4: s = cg_enqueue_iters<4>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
-                default: s = cg_enqueue_iters<5>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
-                }
-                if (s != FX_OK) return s;
-                enq += m;
-                FX_CUDA(cudaMemcpyAsync(hs, sc, sizeof(CgScal), cudaMemcpyDeviceToHost, c->stream));
-                FX_CUDA(cudaStreamSynchronize(c->stream));
-                if (hs->done) break;
-                if (batch < 64) batch *= 2;
+            // batches of iterations; the host looks at the `done` flag of batch b only after batch b+1 is enqueued,
+            // so the device never idles while the flag travels
+            CgScal* slot[2] = {hs, hs + 1};
+            int enq = 0, batch = 8, nb = 0;
+            bool finished = false;
+            c->prof_iters = 0;
+            while (!finished) {
+                if (enq < maxit) {
+                    const int m = (maxit - enq < batch) ? (maxit - enq) : batch;
+                    switch (g->P) {
+                    case 1: s = cg_enqueue_iters<1>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
+                    case 2: s = cg_enqueue_iters<2>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
+                    case 3: s = cg_enqueue_iters<3>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
+                    case 4: s = cg_enqueue_iters<4>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
+                    default: s = cg_enqueue_iters<5>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
+                    }
+                    if (s != FX_OK) return s;
+                    enq += m;
+                    FX_CUDA(cudaMemcpyAsync(slot[nb & 1], sc, sizeof(CgScal), cudaMemcpyDeviceToHost, c->stream));
+                    FX_CUDA(cudaEventRecord(c->cg_ev[nb & 1], c->stream));
+                    ++nb;
+                    if (batch < 64) batch *= 2;
+                    if (nb >= 2) {
+                        FX_CUDA(cudaEventSynchronize(c->cg_ev[nb & 1]));         // the batch before the one just enqueued
+                        if (slot[nb & 1]->done) finished = true;
+                    }
+                } else finished = true;
             }
+            FX_CUDA(cudaStreamSynchronize(c->stream));
+            hs = slot[(nb - 1) & 1];                                             // state after the last enqueued batch
+            if (c->prof_on) { if ((s = cg_collect_profile(c, hs->iters)) != FX_OK) return s; }
             it = hs->iters; status = hs->status; rz = hs->rz;
         }
     }

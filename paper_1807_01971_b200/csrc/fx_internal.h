@@ -27,11 +27,16 @@ struct FxCtx {
     double* cg_vec; int64_t cg_cap;   // 7 vectors of cg_cap doubles
     void* cg_scal;                     // CgScal on the device
     void* cg_scal_pinned;
+    cudaEvent_t cg_ev[2];
     // host staging for the *_host entry points
     double* stage[4]; int64_t stage_cap;
     cudaStream_t copy_stream;
     cudaEvent_t ev_copy[2], ev_comp[2];
     int64_t launches;
+    // fx_cg_profile
+    int prof_on, prof_iters, prof_cap;
+    cudaEvent_t* prof_ev;
+    double prof_ms[4];
 };
 
 FxCtx* fx_ctx();                               // lazily initialised; NULL (and last error set) on failure

@@ -16,6 +16,7 @@
 #include <string.h>
 
 #include "fx_internal.h"
+#include "fx_stream.cuh"
 
 struct CgScal {
     double rz, pq, alpha, beta, bz, thresh, dot;
@@ -28,7 +29,7 @@ typedef ExAcc<CG_K, CG_W> CgAcc;
 
 // ---- K1: apply + dot -----------------------------------------------------------------------------------------
 template <int P>
-__global__ void __launch_bounds__(256) k_cg_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi,
+__global__ void __launch_bounds__(128, 3) k_cg_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi,
                                                       const double* __restrict__ p, double* __restrict__ q, ExGlobal ex,
                                                       CgScal* sc) {
     if (*(volatile int*)&sc->done) return;
@@ -54,47 +55,85 @@ __global__ void __launch_bounds__(256) k_cg_apply_dot(const __grid_constant__ Dg
     }
 }
 
-// ---- K2: phi += alpha p; r -= alpha q; z = V o r; dot(r, z) ----------------------------------------------------
-#define CG_U 4
+// ---- K2 / K3: streaming kernels over (row, column block) chunks --------------------------------------------------
+// A chunk is CG_U * blockDim.x consecutive columns of one image row, so that l = row % P is uniform and k = col % P
+// is cheap; chunks are taken grid-stride and iterated incrementally (no division in the loop).
+#define CG_U 2
+struct ChunkIter {
+    int row, cb, drow, dcb, cpr;
+    __device__ __forceinline__ void init(long long c0, int grid, int cpr_) {
+        cpr = cpr_; row = (int)(c0 / cpr_); cb = (int)(c0 - (long long)row * cpr_); drow = grid / cpr_; dcb = grid - drow * cpr_;
+    }
+    __device__ __forceinline__ void next() { row += drow; cb += dcb; if (cb >= cpr) { cb -= cpr; ++row; } }
+};
+
+template <int NA>
+__device__ __forceinline__ void cg_issue(double* buf, int stage, const double* const (&arr)[NA], int pitch, int rows,
+                                         const ChunkIter& it) {
+    const int bd = blockDim.x;
+    double* s0 = buf + (size_t)stage * NA * CG_U * bd;
+    if (it.row < rows) {
+        const long long base = (long long)it.row * pitch;
+#pragma unroll
+        for (int u = 0; u < CG_U; ++u) {
+            const int slot = u * bd + threadIdx.x;
+            const int col = it.cb * (CG_U * bd) + slot;
+            const bool in = col < pitch;
+            const long long e = in ? base + col : 0;
+#pragma unroll
+            for (int a = 0; a < NA; ++a) fx_cp_async8(fx_smem_addr(s0 + a * CG_U * bd + slot), arr[a] + e, in);
+        }
+    }
+    fx_cp_commit();
+}
+
+// K2: phi += alpha p; r -= alpha q; z = V o r; dot(r, z)
 template <int P>
-__global__ void __launch_bounds__(256) k_cg_update(const __grid_constant__ DgParams g, const double* __restrict__ p,
-                                                   const double* __restrict__ q, double* phi, double* r, ExGlobal ex,
-                                                   CgScal* sc) {
+__global__ void __launch_bounds__(256, 3) k_cg_update(const __grid_constant__ DgParams g, const double* __restrict__ p,
+                                                      const double* __restrict__ q, double* phi, double* r, ExGlobal ex,
+                                                      CgScal* sc) {
     if (*(volatile int*)&sc->done) return;
+    extern __shared__ __align__(16) double cg_buf[];
     __shared__ ExShared sh;
     ex_shared_init(&sh);
     CgAcc acc;
     acc.init();
     const double alpha = sc->alpha, nalpha = -alpha;
-    const int pitch = g.Nx * P, rows = g.Ny * P;
-    const int cw = blockDim.x * CG_U;                        // columns per chunk
-    const int cpr = (pitch + cw - 1) / cw;                   // chunks per row
-    const long long nchunk = (long long)rows * cpr;
-    for (long long c = blockIdx.x; c < nchunk; c += gridDim.x) {
-        const int row = (int)(c / cpr), cb = (int)(c - (long long)row * cpr);
-        const int l = row % P;
-        const long long base = (long long)row * pitch;
-        double pv[CG_U], qv[CG_U], fv[CG_U], rv[CG_U];
-        int col[CG_U];
+    const int pitch = g.Nx * P, rows = g.Ny * P, bd = blockDim.x;
+    const int cpr = (pitch + CG_U * bd - 1) / (CG_U * bd);
+    const double* const arr[4] = {p, q, phi, r};
+    ChunkIter iq, ic;
+    iq.init(blockIdx.x, gridDim.x, cpr); ic = iq;
 #pragma unroll
-        for (int u = 0; u < CG_U; ++u) {
-            col[u] = cb * cw + u * blockDim.x + threadIdx.x;
-            if (col[u] < pitch) { pv[u] = p[base + col[u]]; qv[u] = q[base + col[u]]; fv[u] = phi[base + col[u]]; rv[u] = r[base + col[u]]; }
-        }
+    for (int s = 0; s < FX_STAGES - 1; ++s) { cg_issue<4>(cg_buf, s, arr, pitch, rows, iq); iq.next(); }
+    int stage = 0;
+    for (; ic.row < rows; ic.next()) {
+        int sq = stage + FX_STAGES - 1; if (sq >= FX_STAGES) sq -= FX_STAGES;
+        cg_issue<4>(cg_buf, sq, arr, pitch, rows, iq); iq.next();
+        fx_cp_wait<FX_STAGES - 1>();
+        const double* s0 = cg_buf + (size_t)stage * 4 * CG_U * bd;
+        const int l = ic.row % P;
+        const long long base = (long long)ic.row * pitch;
         double rr[CG_U], zz[CG_U];
+        bool act[CG_U];
 #pragma unroll
         for (int u = 0; u < CG_U; ++u) {
-            if (col[u] < pitch) {
-                const int k = col[u] % P;
-                phi[base + col[u]] = __fma_rn(alpha, pv[u], fv[u]);          // axpby(alpha, p, 1, phi)
-                const double rn = __fma_rn(nalpha, qv[u], rv[u]);            // axpby(-alpha, q, 1, r)
-                r[base + col[u]] = rn;
-                rr[u] = rn;
-                zz[u] = __dmul_rn(g.V[l][k], rn);                            // pointwise_dot(1, V, r, 0, z)
-            } else { rr[u] = 0.0; zz[u] = 0.0; }
+            const int slot = u * bd + threadIdx.x;
+            const int col = ic.cb * (CG_U * bd) + slot;
+            act[u] = col < pitch;
+            const double pv = s0[slot], qv = s0[CG_U * bd + slot], fv = s0[2 * CG_U * bd + slot], rv = s0[3 * CG_U * bd + slot];
+            const double rn = __fma_rn(nalpha, qv, rv);                      // axpby(-alpha, q, 1, r)
+            if (act[u]) {
+                phi[base + col] = __fma_rn(alpha, pv, fv);                   // axpby(alpha, p, 1, phi)
+                r[base + col] = rn;
+            }
+            rr[u] = act[u] ? rn : 0.0;
+            zz[u] = act[u] ? __dmul_rn(g.V[l][col % P], rn) : 0.0;           // pointwise_dot(1, V, r, 0, z)
         }
-        acc.add<CG_U>(rr, zz, &sh);
+        acc.add<CG_U>(rr, zz, act, &sh);
+        if (++stage == FX_STAGES) stage = 0;
     }
+    fx_cp_wait<0>();
     acc.flush(&sh);
     if (ex_block_finish(&sh, ex, 1, 1, &sc->dot) && threadIdx.x == 0) {
         const double rzn = sc->dot;
@@ -103,29 +142,29 @@ __global__ void __launch_bounds__(256) k_cg_update(const __grid_constant__ DgPar
     }
 }
 
-// ---- K3: p = z + beta p,  z = V o r -----------------------------------------------------------------------------
+// K3: p = z + beta p,  z = V o r.  Two fp64 operations per element: plain coalesced loads, four chunks in flight.
+#define CG_U3 4
 template <int P>
 __global__ void __launch_bounds__(256) k_cg_dir(const __grid_constant__ DgParams g, const double* __restrict__ r, double* p,
                                                 const CgScal* sc) {
     if (*(volatile const int*)&sc->done) return;
     const double beta = sc->beta;
-    const int pitch = g.Nx * P, rows = g.Ny * P;
-    const int cw = blockDim.x * CG_U;
-    const int cpr = (pitch + cw - 1) / cw;
-    const long long nchunk = (long long)rows * cpr;
-    for (long long c = blockIdx.x; c < nchunk; c += gridDim.x) {
-        const int row = (int)(c / cpr), cb = (int)(c - (long long)row * cpr);
-        const int l = row % P;
-        const long long base = (long long)row * pitch;
-        double pv[CG_U], rv[CG_U];
-        int col[CG_U];
+    const int pitch = g.Nx * P, rows = g.Ny * P, bd = blockDim.x;
+    const int cpr = (pitch + CG_U3 * bd - 1) / (CG_U3 * bd);
+    ChunkIter ic;
+    ic.init(blockIdx.x, gridDim.x, cpr);
+    for (; ic.row < rows; ic.next()) {
+        const int l = ic.row % P;
+        const long long base = (long long)ic.row * pitch;
+        double pv[CG_U3], rv[CG_U3];
+        int col[CG_U3];
 #pragma unroll
-        for (int u = 0; u < CG_U; ++u) {
-            col[u] = cb * cw + u * blockDim.x + threadIdx.x;
+        for (int u = 0; u < CG_U3; ++u) {
+            col[u] = ic.cb * (CG_U3 * bd) + u * bd + threadIdx.x;
             if (col[u] < pitch) { pv[u] = p[base + col[u]]; rv[u] = r[base + col[u]]; }
         }
 #pragma unroll
-        for (int u = 0; u < CG_U; ++u)
+        for (int u = 0; u < CG_U3; ++u)
             if (col[u] < pitch) {
                 const double z = __dmul_rn(g.V[l][col[u] % P], rv[u]);
                 p[base + col[u]] = __fma_rn(1.0, z, __dmul_rn(beta, pv[u]));    // axpby(1, z, beta, p)
@@ -155,7 +194,7 @@ static fx_status cg_workspace(FxCtx* c, int64_t n) {
 
 static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int* apply_grid, int* apply_block, int* ew_grid, int* ew_block) {
     int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
-    if (wpb > 8) wpb = 8;
+    if (wpb > 4) wpb = 4;                       // the kernels are compiled for <= 128 threads per CTA
     p->nstrip = (g->Nx + FX_STRIP - 1) / FX_STRIP;
     int rps = c->launch[2][0];
     if (rps <= 0) {
@@ -176,24 +215,29 @@ static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int* apply_grid, 
     const int pitch = g->Nx * g->P;
     const long long cpr = (pitch + (long long)bd * CG_U - 1) / ((long long)bd * CG_U);
     long long chunks = cpr * g->Ny * g->P;
-    long long gmax = (long long)c->num_sms * (1024 / bd) * 2;
+    long long gmax = (long long)c->num_sms * (768 / bd);           // one resident wave
     if (chunks > gmax) chunks = gmax;
     if (c->launch[3][0]) chunks = c->launch[3][0];
     *ew_grid = (int)chunks; *ew_block = bd;
 }
 
 template <int P>
-static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, int eg, int eb, const double* chi, double* phi,
+static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, int eg, int eb, int dg, const double* chi, double* phi,
                                   double* r, double* p, double* q, CgScal* sc, int iters) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        FX_CUDA(cudaFuncSetAttribute(k_cg_update<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, FX_STAGES * 4 * CG_U * 256 * 8));
+        attr_done = true;
+    }
     for (int i = 0; i < iters; ++i) {
         cudaEvent_t* ev = nullptr;
         if (c->prof_on && c->prof_iters < c->prof_cap) { ev = c->prof_ev + 4 * c->prof_iters; c->prof_iters++; }
         if (ev) cudaEventRecord(ev[0], c->stream);
         k_cg_apply_dot<P><<<ag, ab, 0, c->stream>>>(dp, chi, p, q, c->ex, sc);
         if (ev) cudaEventRecord(ev[1], c->stream);
-        k_cg_update<P><<<eg, eb, 0, c->stream>>>(dp, p, q, phi, r, c->ex, sc);
+        k_cg_update<P><<<eg, eb, (size_t)FX_STAGES * 4 * CG_U * eb * 8, c->stream>>>(dp, p, q, phi, r, c->ex, sc);
         if (ev) cudaEventRecord(ev[2], c->stream);
-        k_cg_dir<P><<<eg, eb, 0, c->stream>>>(dp, r, p, sc);
+        k_cg_dir<P><<<dg, eb, 0, c->stream>>>(dp, r, p, sc);
         if (ev) cudaEventRecord(ev[3], c->stream);
         c->launches += 3;
     }
@@ -291,6 +335,14 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
             if ((s = fx_make_dg_params(g, 0, &dp, nullptr)) != FX_OK) return s;
             int ag, ab, eg, eb;
             cg_shapes(c, g, &dp, &ag, &ab, &eg, &eb);
+            int dgrid;                                   // K3: grid-stride over chunks of CG_U3*eb columns, ~4 waves
+            {
+                const long long cpr3 = ((long long)g->Nx * g->P + (long long)eb * CG_U3 - 1) / ((long long)eb * CG_U3);
+                long long ch = cpr3 * g->Ny * g->P, gm = (long long)c->num_sms * (2048 / eb) * 4;
+                if (ch > gm) ch = gm;
+                if (c->launch[3][0]) ch = c->launch[3][0];
+                dgrid = (int)ch;
+            }
             CgScal* sc = (CgScal*)c->cg_scal;
             CgScal* hs = (CgScal*)c->cg_scal_pinned;
             memset(hs, 0, sizeof(*hs));
@@ -307,11 +359,11 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
                 if (enq < maxit) {
                     const int m = (maxit - enq < batch) ? (maxit - enq) : batch;
                     switch (g->P) {
-                    case 1: s = cg_enqueue_iters<1>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
-                    case 2: s = cg_enqueue_iters<2>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
-                    case 3: s = cg_enqueue_iters<3>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
-                    case 4: s = cg_enqueue_iters<4>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
-                    default: s = cg_enqueue_iters<5>(c, dp, ag, ab, eg, eb, chi, phi, r, p, q, sc, m); break;
+                    case 1: s = cg_enqueue_iters<1>(c, dp, ag, ab, eg, eb, dgrid, chi, phi, r, p, q, sc, m); break;
+                    case 2: s = cg_enqueue_iters<2>(c, dp, ag, ab, eg, eb, dgrid, chi, phi, r, p, q, sc, m); break;
+                    case 3: s = cg_enqueue_iters<3>(c, dp, ag, ab, eg, eb, dgrid, chi, phi, r, p, q, sc, m); break;
+                    case 4: s = cg_enqueue_iters<4>(c, dp, ag, ab, eg, eb, dgrid, chi, phi, r, p, q, sc, m); break;
+                    default: s = cg_enqueue_iters<5>(c, dp, ag, ab, eg, eb, dgrid, chi, phi, r, p, q, sc, m); break;
                     }
                     if (s != FX_OK) return s;
                     enq += m;

@@ -46,6 +46,15 @@ __device__ __forceinline__ void dg_load(DgCell<P>& c, const double* __restrict__
         for (int k = 0; k < P; ++k) c.v[l][k] = zero ? 0.0 : __ldg(q + l * pitch + k);
 }
 
+// L1 prefetch of one cell (the first element of each of its P rows; a lane's P doubles span at most two 32-byte
+// sectors and the neighbouring lane touches the second one)
+template <int P>
+__device__ __forceinline__ void dg_prefetch(const double* __restrict__ a, long long pitch, int col0, int j) {
+    const double* q = a + (long long)j * P * pitch + col0;
+#pragma unroll
+    for (int l = 0; l < P; ++l) asm volatile("prefetch.global.L1 [%0];" ::"l"(q + l * pitch));
+}
+
 // chain over m:  acc = c[0]*v[0]; acc = fma(c[m], v[m], acc)
 #define FX_CHAIN(acc, COEF, VAL)                         \
     {                                                    \
@@ -53,8 +62,79 @@ __device__ __forceinline__ void dg_load(DgCell<P>& c, const double* __restrict__
         _Pragma("unroll") for (int m_ = 1; m_ < P; ++m_) \
             acc = __fma_rn(COEF(m_), VAL(m_), acc);      \
     }
+#define CL(m) g.L[m]
+#define CR(m) g.R[m]
+#define CB(m) g.B[m]
+#define FF(m) f[m]
 
-// One warp: strip `strip` of 30 cells, cell rows [j0, j1).  FUSE: feed (x, y) pairs of the produced rows into the
+// y lines of one cell: flux, flux trace, adjoint; acc_ += cyy * sy.  FIRST: first cell of a Dirichlet direction (T0L).
+// tByp: in = flux trace of the cell below, out = this cell's.
+template <int P, bool FIRST>
+__device__ __forceinline__ void dg_ylines(const DgParams& g, const DgCell<P>& uc, const DgCell<P>& cc, const double (&tLyn)[P],
+                                          double (&tByp)[P], double (&acc_)[P][P]) {
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+        double f[P];
+#pragma unroll
+        for (int l = 0; l < P; ++l) {
+            double a;
+#define UC(m) uc.v[m][k]
+#define CT(m) (FIRST ? g.T0L[l][m] : g.T0[l][m])
+            FX_CHAIN(a, CT, UC)
+#undef CT
+#undef UC
+            f[l] = __dmul_rn(cc.v[l][k], __fma_rn(g.B[l], tLyn[k], a));
+        }
+        double tB;
+        FX_CHAIN(tB, CB, FF)
+#pragma unroll
+        for (int l = 0; l < P; ++l) {
+            double a;
+#define CT(m) (FIRST ? g.T0L[m][l] : g.T0[m][l])
+            FX_CHAIN(a, CT, FF)
+#undef CT
+            acc_[l][k] = __fma_rn(g.cyy, __fma_rn(g.L[l], tByp[k], a), acc_[l][k]);
+        }
+        tByp[k] = tB;
+    }
+}
+
+// x lines of one cell.  SEL: this warp contains the first cell of a Dirichlet x direction (lane flag firstx).
+// out[l][k] = cxx * sx + acc_ (times V if normed)
+template <int P, bool SEL>
+__device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc, const DgCell<P>& cc, const double (&tLxr)[P],
+                                          bool firstx, bool xghost, double (&acc_)[P][P]) {
+#pragma unroll
+    for (int l = 0; l < P; ++l) {
+        double f[P];
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            double a;
+#define UC(m) uc.v[l][m]
+#define CT(m) ((SEL && firstx) ? g.T0L[k][m] : g.T0[k][m])
+            FX_CHAIN(a, CT, UC)
+#undef CT
+#undef UC
+            f[k] = __dmul_rn(cc.v[l][k], __fma_rn(g.B[k], tLxr[l], a));
+        }
+        double tB;
+        FX_CHAIN(tB, CB, FF)
+        if (xghost) tB = 0.0;
+        const double tBl = __shfl_up_sync(0xffffffffu, tB, 1);
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            double a;
+#define CT(m) ((SEL && firstx) ? g.T0L[m][k] : g.T0[m][k])
+            FX_CHAIN(a, CT, FF)
+#undef CT
+            double o = __fma_rn(g.cxx, __fma_rn(g.L[k], tBl, a), acc_[l][k]);
+            if (g.normed) o = __dmul_rn(g.V[l][k], o);
+            acc_[l][k] = o;
+        }
+    }
+}
+
+// One warp: strip `strip` of 30 cells, cell rows [j0, j1).  FUSE: feed (x, y) pairs of the produced cells into the
 // exact-dot accumulator `acc` (the CG's p.Sp).
 template <int P, bool FUSE, class ACC>
 __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* __restrict__ chi,
@@ -72,6 +152,7 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
     const bool xghost = outside && (dirx || ci < -1 || ci > Nx);   // contributes zero traces
     const bool produce = lane >= 1 && lane <= FX_STRIP && ci < Nx; // ci >= 0 holds for lanes >= 1
     const bool firstx = dirx && ci == 0;                           // T0L instead of T0 along x
+    const bool selx = dirx && strip == 0;                          // warp-uniform: some lane has firstx
     const int col0 = cw * P;
 
     DgCell<P> uc, un, cc;
@@ -79,9 +160,10 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
 
     // ---- prologue: state of cell row j0-1 ------------------------------------------------------------------
     dg_load<P>(uc, x, pitch, col0, j0, xghost);
+    dg_load<P>(cc, chi, pitch, col0, j0, xghost);
+    if (!xghost && j0 + 1 < Ny) { dg_prefetch<P>(x, pitch, col0, j0 + 1); dg_prefetch<P>(chi, pitch, col0, j0 + 1); }
 #pragma unroll
     for (int k = 0; k < P; ++k) {
-#define CL(m) g.L[m]
 #define UC(m) uc.v[m][k]
         FX_CHAIN(tLy[k], CL, UC)
 #undef UC
@@ -91,44 +173,38 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
         for (int k = 0; k < P; ++k) { tRyp[k] = 0.0; tByp[k] = 0.0; }
     } else {
         const int jp = (j0 == 0) ? Ny - 1 : j0 - 1;
-        const bool firsty = diry && jp == 0;
         DgCell<P> up, cp;
         dg_load<P>(up, x, pitch, col0, jp, xghost);
         dg_load<P>(cp, chi, pitch, col0, jp, xghost);
+        double dummy[P][P];
 #pragma unroll
         for (int k = 0; k < P; ++k) {
-#define CR(m) g.R[m]
 #define UP(m) up.v[m][k]
             FX_CHAIN(tRyp[k], CR, UP)
-            double f[P];
-#pragma unroll
-            for (int l = 0; l < P; ++l) {
-                double a;
-#define CT(m) (firsty ? g.T0L[l][m] : g.T0[l][m])
-                FX_CHAIN(a, CT, UP)
-#undef CT
-                const double gh = __fma_rn(g.B[l], tLy[k], a);
-                f[l] = __dmul_rn(__dmul_rn(g.WW[l][k], cp.v[l][k]), gh);
-            }
-#define CB(m) g.B[m]
-#define FF(m) f[m]
-            FX_CHAIN(tByp[k], CB, FF)
 #undef UP
+            tByp[k] = 0.0;
+#pragma unroll
+            for (int l = 0; l < P; ++l) { cp.v[l][k] = __dmul_rn(g.WW[l][k], cp.v[l][k]); dummy[l][k] = 0.0; }
         }
+        if (diry && jp == 0) dg_ylines<P, true>(g, up, cp, tLy, tByp, dummy);
+        else dg_ylines<P, false>(g, up, cp, tLy, tByp, dummy);
     }
-    dg_load<P>(cc, chi, pitch, col0, j0, xghost);
 
     // ---- march ---------------------------------------------------------------------------------------------
     for (int j = j0; j < j1; ++j) {
         int jn = j + 1;
         bool yghost = false;
         if (jn == Ny) { jn = 0; yghost = diry; }
-        dg_load<P>(un, x, pitch, col0, jn, xghost || yghost);
+        dg_load<P>(un, x, pitch, col0, jn, xghost || yghost);       // L1 hit: prefetched one step ago
         DgCell<P> cn;
         const bool more = (j + 1 < j1);
         if (more) dg_load<P>(cn, chi, pitch, col0, j + 1, xghost);
+        if (more && !xghost) {                                       // next step's loads
+            const int j2 = (j + 2 == Ny) ? 0 : j + 2;
+            if (!(j + 2 == Ny && diry)) dg_prefetch<P>(x, pitch, col0, j2);
+            if (j + 2 < j1) dg_prefetch<P>(chi, pitch, col0, j + 2);
+        }
 
-        const bool firsty = diry && j == 0;
         double tRy[P], tLyn[P], tLx[P], tRx[P];
 #pragma unroll
         for (int k = 0; k < P; ++k) {
@@ -165,82 +241,38 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
                 const double jx = __fma_rn(g.L[k], __dsub_rn(tLx[l], tRxl[l]), __dmul_rn(g.R[k], __dsub_rn(tRx[l], tLxr[l])));
                 acc_[l][k] = __fma_rn(g.JX[l], jx, __dmul_rn(g.JY[k], jy));
             }
-        // y lines: one column k at a time
+        if (diry && j == 0) dg_ylines<P, true>(g, uc, cc, tLyn, tByp, acc_);
+        else dg_ylines<P, false>(g, uc, cc, tLyn, tByp, acc_);
 #pragma unroll
-        for (int k = 0; k < P; ++k) {
-            double f[P];
+        for (int k = 0; k < P; ++k) { tRyp[k] = tRy[k]; tLy[k] = tLyn[k]; }
+        if (selx) dg_xlines<P, true>(g, uc, cc, tLxr, firstx, xghost, acc_);
+        else dg_xlines<P, false>(g, uc, cc, tLxr, firstx, xghost, acc_);
+
+        if (produce) {
+            double* yrow = y + (long long)j * P * pitch + col0;
 #pragma unroll
-            for (int l = 0; l < P; ++l) {
-                double a;
-#define UC(m) uc.v[m][k]
-#define CT(m) (firsty ? g.T0L[l][m] : g.T0[l][m])
-                FX_CHAIN(a, CT, UC)
-#undef CT
-#undef UC
-                f[l] = __dmul_rn(cc.v[l][k], __fma_rn(g.B[l], tLyn[k], a));
-            }
-            double tB;
-            FX_CHAIN(tB, CB, FF)
+            for (int l = 0; l < P; ++l)
 #pragma unroll
-            for (int l = 0; l < P; ++l) {
-                double a;
-#define CT(m) (firsty ? g.T0L[m][l] : g.T0[m][l])
-                FX_CHAIN(a, CT, FF)
-#undef CT
-                const double sy = __fma_rn(g.L[l], tByp[k], a);
-                acc_[l][k] = __fma_rn(g.cyy, sy, acc_[l][k]);
-            }
-            tByp[k] = tB; tRyp[k] = tRy[k]; tLy[k] = tLyn[k];
+                for (int k = 0; k < P; ++k) yrow[l * pitch + k] = acc_[l][k];
         }
-        // x lines: one row l at a time
-        double* yrow = y + (long long)j * P * pitch + col0;
+        if (FUSE) {
+            double xs[P * P], ys[P * P];
+            bool act[P * P];
 #pragma unroll
-        for (int l = 0; l < P; ++l) {
-            double f[P];
+            for (int l = 0; l < P; ++l)
 #pragma unroll
-            for (int k = 0; k < P; ++k) {
-                double a;
-#define UC(m) uc.v[l][m]
-#define CT(m) (firstx ? g.T0L[k][m] : g.T0[k][m])
-                FX_CHAIN(a, CT, UC)
-#undef CT
-#undef UC
-                f[k] = __dmul_rn(cc.v[l][k], __fma_rn(g.B[k], tLxr[l], a));
-            }
-            double tB;
-            FX_CHAIN(tB, CB, FF)
-            if (xghost) tB = 0.0;
-            const double tBl = __shfl_up_sync(0xffffffffu, tB, 1);
-            double out[P];
-#pragma unroll
-            for (int k = 0; k < P; ++k) {
-                double a;
-#define CT(m) (firstx ? g.T0L[m][k] : g.T0[m][k])
-                FX_CHAIN(a, CT, FF)
-#undef CT
-                const double sx = __fma_rn(g.L[k], tBl, a);
-                double o = __fma_rn(g.cxx, sx, acc_[l][k]);
-                if (g.normed) o = __dmul_rn(g.V[l][k], o);
-                out[k] = o;
-            }
-            if (produce) {
-#pragma unroll
-                for (int k = 0; k < P; ++k) yrow[l * pitch + k] = out[k];
-            }
-            if (FUSE) {
-                double xs[P], ys[P];
-#pragma unroll
-                for (int k = 0; k < P; ++k) { xs[k] = produce ? uc.v[l][k] : 0.0; ys[k] = produce ? out[k] : 0.0; }
-                acc->template add<P>(xs, ys, sh);
-            }
+                for (int k = 0; k < P; ++k) {
+                    xs[l * P + k] = produce ? uc.v[l][k] : 0.0; ys[l * P + k] = produce ? acc_[l][k] : 0.0; act[l * P + k] = produce;
+                }
+            acc->template add<P * P>(xs, ys, act, sh);
         }
         uc = un;
         if (more) cc = cn;
     }
+}
 #undef CL
 #undef CR
 #undef CB
 #undef FF
-}
 
 #endif

@@ -37,6 +37,7 @@ typedef unsigned long long fx_u64;
 
 struct ExShared {
     fx_u64 dig[FX_NDIG];     // signed digits, two's complement wrap-around arithmetic
+    fx_u64 lim[FX_NLIMB];    // last CTA only: the canonical limbs while they are normalised and rounded
     int flags;
     int is_last;
 };
@@ -95,17 +96,23 @@ __device__ __forceinline__ long long ex_warp_sum(long long v) {
     return v;
 }
 
-// Per-thread binned expansion with a warp-uniform window.  K bins of W bit.
+// lane 0 of a warp: add c * 2^(E - FX_BIAS + FX_BIAS) ... i.e. the signed count c at bit position b
+static __device__ __noinline__ void ex_deposit_count(ExShared* sh, int b, long long c) {
+    ex_deposit(sh->dig, b, 0ull, (fx_u64)(c < 0 ? -c : c), c < 0);
+}
+
+// Per-thread binned expansion with a warp-uniform window.  K bins of W bit.  All members are inlined so that the
+// state lives in registers; only the integer deposits are calls.
 template <int K, int W>
 struct ExAcc {
     static constexpr int CAP = 1 << (50 - W);            // deposits per bin before S[k] must be re-centred
     static constexpr int MARGIN = 6;                     // head-room (bit) above the largest product seen
     static constexpr int TB_MIN = -1074 + K * W + 1022;  // lowest bin stays a normal double with ulp >= 2^-1074
-    static constexpr int BE_LO = 63;                     // fast path: 2^-960 <= |p| < 2^1000 (TwoProd error-free,
-    static constexpr int BE_HI = 2022;                   //   no overflow of the top bin)
+    static constexpr unsigned BE_LO = 63;                // fast path: 2^-960 <= |p| < 2^1000 (TwoProd error-free,
+    static constexpr unsigned BE_HI = 2022;              //   no overflow of the top bin)
     double S[K];
     long long C[K];
-    int Tb;          // T + 1022; |p| < 2^T  <=>  biased exponent of p <= Tb.   INT_MIN/2 = no window yet
+    int Tb;          // T + 1022; |p| < 2^T  <=>  biased exponent of p <= Tb.   very negative = no window yet
     int cnt, ren;
 
     __device__ __forceinline__ void init() {
@@ -127,47 +134,52 @@ struct ExAcc {
         cnt = 0; ++ren;
     }
     // all 32 lanes: merge the warp's bins by shuffles, lane 0 deposits into the CTA's long accumulator
-    __device__ __noinline__ void flush(ExShared* sh) {
+    __device__ __forceinline__ void flush(ExShared* sh) {
         if (Tb > -(1 << 28)) {
 #pragma unroll
             for (int k = 0; k < K; ++k) {
                 long long c = C[k] + (__double_as_longlong(S[k]) - mbits(k));
                 c = ex_warp_sum(c);
-                if ((threadIdx.x & 31) == 0 && c != 0) {
-                    const int Ek = Tb - 1022 - W * (k + 1);
-                    ex_deposit(sh->dig, Ek + FX_BIAS, 0ull, (fx_u64)(c < 0 ? -c : c), c < 0);
-                }
+                if ((threadIdx.x & 31) == 0 && c != 0) ex_deposit_count(sh, Tb - 1022 - W * (k + 1) + FX_BIAS, c);
                 C[k] = 0;
                 S[k] = __longlong_as_double(mbits(k));
             }
         }
         cnt = 0; ren = 0;
     }
-    __device__ __noinline__ void reanchor(ExShared* sh, int bemax) {
+    __device__ __forceinline__ void reanchor(ExShared* sh, int bemax) {
         flush(sh);
-        int t = bemax + MARGIN;
+        const int t = bemax + MARGIN;
         Tb = t < TB_MIN ? TB_MIN : t;
 #pragma unroll
         for (int k = 0; k < K; ++k) { S[k] = __longlong_as_double(mbits(k)); C[k] = 0; }
     }
 
-    // U products per lane; must be called by all 32 lanes of the warp together
+    // U products per lane; must be called by all 32 lanes of the warp together.  Lanes/elements with active == false
+    // must pass x = y = 0 (padding); they are not inspected.
     template <int U>
-    __device__ __forceinline__ void add(const double (&x)[U], const double (&y)[U], ExShared* sh) {
+    __device__ __forceinline__ void add(const double (&x)[U], const double (&y)[U], const bool (&active)[U], ExShared* sh) {
         double p[U], e[U];
-        int bemax = 0;
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             p[u] = __dmul_rn(x[u], y[u]);
             e[u] = __fma_rn(x[u], y[u], -p[u]);                      // TwoProd
-            const int be = (__double2hiint(p[u]) >> 20) & 0x7ff;
-            if (be < BE_LO || be > BE_HI) {                          // outside TwoProd's error-free range
-                if (be == 0x7ff || (x[u] != 0.0 && y[u] != 0.0)) ex_deposit_product(sh, x[u], y[u]);
+            const unsigned be = ((unsigned)__double2hiint(p[u]) >> 20) & 0x7ffu;
+            if (active[u] && (be - BE_LO) > (BE_HI - BE_LO)) {       // outside TwoProd's error-free range (or zero)
+                const bool xz = (((unsigned)__double2hiint(x[u]) & 0x7fffffffu) | (unsigned)__double2loint(x[u])) == 0u;
+                const bool yz = (((unsigned)__double2hiint(y[u]) & 0x7fffffffu) | (unsigned)__double2loint(y[u])) == 0u;
+                if (be == 0x7ffu || !(xz || yz)) ex_deposit_product(sh, x[u], y[u]);
                 p[u] = 0.0; e[u] = 0.0;
-            } else bemax = be > bemax ? be : bemax;
+            }
+        }
+        int bemax = 0;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int be = (__double2hiint(p[u]) >> 20) & 0x7ff;
+            bemax = be > bemax ? be : bemax;
         }
         if (__any_sync(0xffffffffu, bemax > Tb)) reanchor(sh, __reduce_max_sync(0xffffffffu, bemax));
-        if (cnt + U > CAP) { recentre(); if (__any_sync(0xffffffffu, ren >= 32)) flush(sh); }
+        if (cnt + U > CAP) { recentre(); if (ren >= 32) flush(sh); }
         cnt += U;
         unsigned rest = 0;
 #pragma unroll
@@ -199,6 +211,13 @@ struct ExAcc {
             }
         }
     }
+    template <int U>
+    __device__ __forceinline__ void add(const double (&x)[U], const double (&y)[U], ExShared* sh) {
+        bool act[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) act[u] = true;
+        add<U>(x, y, act, sh);
+    }
 };
 
 __device__ __forceinline__ void ex_shared_init(ExShared* sh) {
@@ -217,12 +236,11 @@ __device__ inline fx_u64 ex_get64(const fx_u64* mag, int bit) {     // bits [bit
 }
 
 // RN(limbs) with ties to even, gradual underflow, overflow to inf; exact zero -> +0.0   (DESIGN.md 3.1 step 4)
-__device__ inline double ex_round(const fx_u64* limbs, int flags) {
+__device__ inline double ex_round(const fx_u64* limbs, int flags, fx_u64* mag /* scratch [FX_NLIMB] */) {
     if ((flags & FX_FLAG_NAN) || ((flags & FX_FLAG_PINF) && (flags & FX_FLAG_NINF)))
         return __longlong_as_double(0x7FF8000000000000ll);
     if (flags & FX_FLAG_PINF) return __longlong_as_double(0x7FF0000000000000ll);
     if (flags & FX_FLAG_NINF) return __longlong_as_double((long long)0xFFF0000000000000ull);
-    fx_u64 mag[FX_NLIMB];
     const bool neg = (limbs[FX_NLIMB - 1] >> 63) != 0;
     fx_u64 carry = neg ? 1ull : 0ull;
     int top = -1;
@@ -258,40 +276,10 @@ __device__ inline double ex_round(const fx_u64* limbs, int flags) {
     return __longlong_as_double((long long)bits);
 }
 
-// last CTA, thread 0.  first: limbs start from zero; last: round and publish.
-__device__ inline void ex_finalize(const ExGlobal& g, int first, int last, double* result) {
-    volatile fx_u64* dig = g.dig;
-    long long carry = 0;
-    fx_u64 c2 = 0;
-    fx_u64 limbs[FX_NLIMB];
-    for (int k = 0; k < FX_NLIMB; ++k) {
-        long long v = (long long)dig[2 * k] + carry;
-        const fx_u64 lo = (fx_u64)v & 0xffffffffull;
-        carry = v >> 32;
-        v = (long long)dig[2 * k + 1] + carry;
-        const fx_u64 hi = (fx_u64)v & 0xffffffffull;
-        carry = v >> 32;
-        dig[2 * k] = 0ull; dig[2 * k + 1] = 0ull;
-        const fx_u64 word = lo | (hi << 32);
-        const fx_u64 old = first ? 0ull : g.limbs[k];
-        fx_u64 s = old + word;
-        fx_u64 c = (s < old) ? 1ull : 0ull;
-        const fx_u64 s2 = s + c2;
-        c |= (s2 < s) ? 1ull : 0ull;
-        c2 = c;
-        limbs[k] = s2;
-        g.limbs[k] = s2;
-    }
-    if (last) {
-        const int flags = *(volatile int*)g.flags;
-        g.flags[1] = flags;                       // kept for fx_exdot_digits
-        g.flags[0] = 0;
-        if (result) *result = ex_round(limbs, flags);
-    }
-}
-
-// End of a CTA: digits -> global, the last CTA to arrive finalises.  Returns true in every thread of the last CTA
-// after the result has been written.  `first`/`last`: position of this launch in a multi-launch call.
+// End of a CTA: digits -> global, the last CTA to arrive finalises (single pass, no second launch): its threads fetch
+// the merged digits and the running limbs in parallel, thread 0 carry-normalises them in shared memory and rounds
+// once.  Returns true in every thread of the last CTA after the result has been written.
+// `first`/`last`: position of this launch in a multi-launch call (first: limbs start from zero; last: round).
 __device__ __forceinline__ bool ex_block_finish(ExShared* sh, const ExGlobal& g, int first, int last, double* result) {
     __syncthreads();
     for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) {
@@ -307,12 +295,40 @@ __device__ __forceinline__ bool ex_block_finish(ExShared* sh, const ExGlobal& g,
     }
     __syncthreads();
     if (!sh->is_last) return false;
+    __threadfence();
+    for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) { sh->dig[i] = __ldcg(&g.dig[i]); g.dig[i] = 0ull; }
+    for (int i = threadIdx.x; i < FX_NLIMB; i += blockDim.x) sh->lim[i] = first ? 0ull : __ldcg(&g.limbs[i]);
+    __syncthreads();
     if (threadIdx.x == 0) {
-        __threadfence();
-        ex_finalize(g, first, last, result);
+        long long carry = 0;
+        fx_u64 c2 = 0;
+        for (int k = 0; k < FX_NLIMB; ++k) {
+            long long v = (long long)sh->dig[2 * k] + carry;
+            const fx_u64 lo = (fx_u64)v & 0xffffffffull;
+            carry = v >> 32;
+            v = (long long)sh->dig[2 * k + 1] + carry;
+            const fx_u64 hi = (fx_u64)v & 0xffffffffull;
+            carry = v >> 32;
+            const fx_u64 word = lo | (hi << 32);
+            const fx_u64 old = sh->lim[k];
+            const fx_u64 s1 = old + word;
+            fx_u64 c = (s1 < old) ? 1ull : 0ull;
+            const fx_u64 s2 = s1 + c2;
+            c |= (s2 < s1) ? 1ull : 0ull;
+            c2 = c;
+            sh->lim[k] = s2;
+        }
+        if (last) {
+            const int flags = __ldcg(g.flags);
+            g.flags[1] = flags;                       // kept for fx_exdot_digits
+            g.flags[0] = 0;
+            if (result) *result = ex_round(sh->lim, flags, sh->dig);
+        }
         *g.ticket = 0u;
-        __threadfence();
     }
+    __syncthreads();
+    for (int i = threadIdx.x; i < FX_NLIMB; i += blockDim.x) g.limbs[i] = sh->lim[i];
+    __threadfence();
     __syncthreads();
     return true;
 }

@@ -4,6 +4,7 @@
 #include <string.h>
 
 #include "fx_internal.h"
+#include "fx_stream.cuh"
 
 // ------------------------------------------------------------------------------------------------------------
 // exact dot  (design in fx_exdot.cuh / DESIGN.md 6.1).  HBM roofline: 16 B per element.
@@ -13,41 +14,85 @@
 #define EX_W 40
 #define EX_U 4
 
+// Tiles of blockDim.x * EX_U elements, grid-stride; FX_STAGES-1 tiles in flight per thread through cp.async.
+// Shared layout (doubles): [stage][array 0..1][u][thread]   (VEC: [stage][array][u/2][thread] of 16 B)
 template <bool VEC>
-__global__ void __launch_bounds__(1024) k_exdot(const double* __restrict__ x, const double* __restrict__ y, long long n,
-                                                ExGlobal g, int first, int last, double* result) {
-    __shared__ ExShared sh;
-    ex_shared_init(&sh);
-    ExAcc<EX_K, EX_W> acc;
-    acc.init();
-    const long long tile = (long long)blockDim.x * EX_U;
-    const long long ntiles = (n + tile - 1) / tile;
-    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
-        double xv[EX_U], yv[EX_U];
+__device__ __forceinline__ void exdot_issue(double* buf, int stage, const double* __restrict__ x, const double* __restrict__ y,
+                                            long long n, long long base, bool live) {
+    const int bd = blockDim.x;
+    double* sx = buf + (size_t)stage * 2 * EX_U * bd;
+    double* sy = sx + EX_U * bd;
+    if (live) {
         if (VEC) {
 #pragma unroll
             for (int u = 0; u < EX_U / 2; ++u) {
-                const long long e0 = t * tile + 2 * ((long long)u * blockDim.x + threadIdx.x);
-                if (e0 + 1 < n) {
-                    const double2 a = *reinterpret_cast<const double2*>(x + e0);
-                    const double2 b = *reinterpret_cast<const double2*>(y + e0);
-                    xv[2 * u] = a.x; xv[2 * u + 1] = a.y; yv[2 * u] = b.x; yv[2 * u + 1] = b.y;
-                } else {
-                    const bool in = e0 < n;
-                    xv[2 * u] = in ? x[e0] : 0.0; yv[2 * u] = in ? y[e0] : 0.0;
-                    xv[2 * u + 1] = 0.0; yv[2 * u + 1] = 0.0;
-                }
+                const int slot = 2 * (u * bd + threadIdx.x);
+                const long long e0 = base + slot;
+                const long long left = n - e0;
+                const int bytes = left >= 2 ? 16 : (left == 1 ? 8 : 0);
+                const long long es = bytes ? e0 : 0;                 // keep the address valid when nothing is copied
+                fx_cp_async16(fx_smem_addr(sx + slot), x + es, bytes);
+                fx_cp_async16(fx_smem_addr(sy + slot), y + es, bytes);
             }
         } else {
 #pragma unroll
             for (int u = 0; u < EX_U; ++u) {
-                const long long e0 = t * tile + (long long)u * blockDim.x + threadIdx.x;
+                const int slot = u * bd + threadIdx.x;
+                const long long e0 = base + slot;
                 const bool in = e0 < n;
-                xv[u] = in ? x[e0] : 0.0; yv[u] = in ? y[e0] : 0.0;
+                fx_cp_async8(fx_smem_addr(sx + slot), x + (in ? e0 : 0), in);
+                fx_cp_async8(fx_smem_addr(sy + slot), y + (in ? e0 : 0), in);
             }
         }
-        acc.add<EX_U>(xv, yv, &sh);
     }
+    fx_cp_commit();
+}
+
+template <bool VEC>
+__global__ void __launch_bounds__(256, 3) k_exdot(const double* __restrict__ x, const double* __restrict__ y, long long n,
+                                                  ExGlobal g, int first, int last, double* result) {
+    extern __shared__ __align__(16) double ex_buf[];
+    __shared__ ExShared sh;
+    ex_shared_init(&sh);
+    ExAcc<EX_K, EX_W> acc;
+    acc.init();
+    const int bd = blockDim.x;
+    const long long tile = (long long)bd * EX_U;
+    const long long ntiles = (n + tile - 1) / tile;
+    long long tq = blockIdx.x;                                   // next tile to issue
+#pragma unroll
+    for (int s = 0; s < FX_STAGES - 1; ++s) { exdot_issue<VEC>(ex_buf, s, x, y, n, tq * tile, tq < ntiles); tq += gridDim.x; }
+    int stage = 0;
+    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        int sq = stage + FX_STAGES - 1; if (sq >= FX_STAGES) sq -= FX_STAGES;
+        exdot_issue<VEC>(ex_buf, sq, x, y, n, tq * tile, tq < ntiles); tq += gridDim.x;
+        fx_cp_wait<FX_STAGES - 1>();                             // the group of tile t has landed
+        const double* sx = ex_buf + (size_t)stage * 2 * EX_U * bd;
+        const double* sy = sx + EX_U * bd;
+        double xv[EX_U], yv[EX_U];
+        bool act[EX_U];
+        if (VEC) {
+#pragma unroll
+            for (int u = 0; u < EX_U / 2; ++u) {
+                const int slot = 2 * (u * bd + threadIdx.x);
+                const double2 a = *reinterpret_cast<const double2*>(sx + slot);
+                const double2 b = *reinterpret_cast<const double2*>(sy + slot);
+                xv[2 * u] = a.x; xv[2 * u + 1] = a.y; yv[2 * u] = b.x; yv[2 * u + 1] = b.y;
+                const long long e0 = t * tile + slot;
+                act[2 * u] = e0 < n; act[2 * u + 1] = e0 + 1 < n;
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < EX_U; ++u) {
+                const int slot = u * bd + threadIdx.x;
+                xv[u] = sx[slot]; yv[u] = sy[slot];
+                act[u] = t * tile + slot < n;
+            }
+        }
+        acc.add<EX_U>(xv, yv, act, &sh);
+        if (++stage == FX_STAGES) stage = 0;
+    }
+    fx_cp_wait<0>();
     acc.flush(&sh);
     ex_block_finish(&sh, g, first, last, result);
 }
@@ -55,15 +100,23 @@ __global__ void __launch_bounds__(1024) k_exdot(const double* __restrict__ x, co
 // one launch over m <= 2^28 elements (keeps every 64-bit digit far from overflow); first/last: position in the call
 fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64_t m, int first, int last, double* result_dev) {
     const bool vec = aligned16(x) && aligned16(y);
-    const int bd = c->launch[0][1] ? c->launch[0][1] : 256;
+    int bd = c->launch[0][1] ? c->launch[0][1] : 256;
+    if (bd > 256) bd = 256;                     // compiled for <= 256 threads per CTA
     const long long tile = (long long)bd * EX_U;
     long long grid = (m + tile - 1) / tile;
-    const long long gmax = (long long)c->num_sms * (1024 / bd) * 2;
+    const long long gmax = (long long)c->num_sms * (768 / bd);      // one resident wave: every CTA pays one flush + merge
     if (grid > gmax) grid = gmax;
     if (grid < 1) grid = 1;
     if (c->launch[0][0]) grid = c->launch[0][0];
-    if (vec) k_exdot<true><<<(int)grid, bd, 0, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
-    else k_exdot<false><<<(int)grid, bd, 0, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
+    const size_t smem = (size_t)FX_STAGES * 2 * EX_U * bd * sizeof(double);
+    static bool attr_done = false;
+    if (!attr_done) {
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, FX_STAGES * 2 * EX_U * 256 * 8));
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, FX_STAGES * 2 * EX_U * 256 * 8));
+        attr_done = true;
+    }
+    if (vec) k_exdot<true><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
+    else k_exdot<false><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
     c->launches++;
     FX_CUDA(cudaGetLastError());
     return FX_OK;
@@ -123,10 +176,10 @@ extern "C" fx_status fx_exdot_digits(const double* x, const double* y, int64_t n
 // dG elliptic apply  (fx_dg.cuh / DESIGN.md 6.2).  HBM roofline: 24 B per unknown.
 // ------------------------------------------------------------------------------------------------------------
 
-struct NoAcc { template <int U> __device__ void add(const double (&)[U], const double (&)[U], ExShared*) {} };
+struct NoAcc { template <int U> __device__ void add(const double (&)[U], const double (&)[U], const bool (&)[U], ExShared*) {} };
 
 template <int P>
-__global__ void __launch_bounds__(256) k_dg_apply(const __grid_constant__ DgParams g, const double* __restrict__ chi,
+__global__ void __launch_bounds__(128, 3) k_dg_apply(const __grid_constant__ DgParams g, const double* __restrict__ chi,
                                                   const double* __restrict__ x, double* __restrict__ y) {
     const int wpb = blockDim.x >> 5;
     const long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
@@ -175,7 +228,7 @@ fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const d
     fx_status s = fx_make_dg_params(g, normed, &p, nullptr);
     if (s != FX_OK) return s;
     int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
-    if (wpb > 8) wpb = 8;                       // the kernels are compiled for <= 256 threads per CTA
+    if (wpb > 4) wpb = 4;                       // the kernels are compiled for <= 128 threads per CTA
     p.nstrip = (g->Nx + FX_STRIP - 1) / FX_STRIP;
     // rows per segment: aim at >= 2 waves of 16 warps per SM, but keep the per-segment prologue (one extra cell row) small
     int rps = c->launch[2][0];

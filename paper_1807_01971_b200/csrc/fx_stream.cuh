@@ -1,0 +1,28 @@
+// fx_stream.cuh -- per-thread asynchronous staging of streamed vectors (cp.async / LDGSTS into shared memory).
+//
+// The streaming kernels (exact dot, the fused CG vector update) do 25-30 dependent fp64 operations per element, so a
+// thread that loads into registers and then computes keeps nothing in flight while it computes.  Here every thread
+// copies ITS OWN elements of the next FX_STAGES-1 tiles into its own shared-memory slots with cp.async and reads them
+// back when their group has completed: no barrier is needed (a thread only reads what it copied itself), no
+// registers are held by data in flight, and ~200 KB per SM stay in flight ("bytes in flight").
+// Out-of-range elements are zero-filled by the copy itself (src-size 0).
+
+#ifndef FX_STREAM_CUH
+#define FX_STREAM_CUH
+
+#define FX_STAGES 4
+
+__device__ __forceinline__ unsigned fx_smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void fx_cp_async8(unsigned dst, const void* src, bool valid) {
+    const int sz = valid ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void fx_cp_async16(unsigned dst, const void* src, int src_bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void fx_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void fx_cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+#endif

@@ -161,7 +161,7 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
     // ---- prologue: state of cell row j0-1 ------------------------------------------------------------------
     dg_load<P>(uc, x, pitch, col0, j0, xghost);
     dg_load<P>(cc, chi, pitch, col0, j0, xghost);
-    if (!xghost && j0 + 1 < Ny) { dg_prefetch<P>(x, pitch, col0, j0 + 1); dg_prefetch<P>(chi, pitch, col0, j0 + 1); }
+    if (!xghost && j0 + 1 < Ny) dg_prefetch<P>(x, pitch, col0, j0 + 1);
 #pragma unroll
     for (int k = 0; k < P; ++k) {
 #define UC(m) uc.v[m][k]
@@ -191,18 +191,19 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
     }
 
     // ---- march ---------------------------------------------------------------------------------------------
+    // Every cell row is fetched from HBM once, by an L1 prefetch one step ahead; the register loads below are L1
+    // hits.  u of a row is read twice (as the row above, for its bottom trace, then as the current row): holding it
+    // in registers across the step instead costs 2*P*P registers and a quarter of the occupancy.
     for (int j = j0; j < j1; ++j) {
         int jn = j + 1;
         bool yghost = false;
         if (jn == Ny) { jn = 0; yghost = diry; }
-        dg_load<P>(un, x, pitch, col0, jn, xghost || yghost);       // L1 hit: prefetched one step ago
-        DgCell<P> cn;
-        const bool more = (j + 1 < j1);
-        if (more) dg_load<P>(cn, chi, pitch, col0, j + 1, xghost);
-        if (more && !xghost) {                                       // next step's loads
+        if (j > j0) { dg_load<P>(uc, x, pitch, col0, j, xghost); dg_load<P>(cc, chi, pitch, col0, j, xghost); }
+        dg_load<P>(un, x, pitch, col0, jn, xghost || yghost);
+        if (j + 1 < j1 && !xghost) {                                 // next step's rows
             const int j2 = (j + 2 == Ny) ? 0 : j + 2;
             if (!(j + 2 == Ny && diry)) dg_prefetch<P>(x, pitch, col0, j2);
-            if (j + 2 < j1) dg_prefetch<P>(chi, pitch, col0, j + 2);
+            dg_prefetch<P>(chi, pitch, col0, j + 1);
         }
 
         double tRy[P], tLyn[P], tLx[P], tRx[P];
@@ -266,8 +267,6 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
                 }
             acc->template add<P * P>(xs, ys, act, sh);
         }
-        uc = un;
-        if (more) cc = cn;
     }
 }
 #undef CL

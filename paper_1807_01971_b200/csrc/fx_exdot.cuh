@@ -155,33 +155,46 @@ struct ExAcc {
         for (int k = 0; k < K; ++k) { S[k] = __longlong_as_double(mbits(k)); C[k] = 0; }
     }
 
-    // U products per lane; must be called by all 32 lanes of the warp together.  Lanes/elements with active == false
-    // must pass x = y = 0 (padding); they are not inspected.
-    template <int U>
+    // U products per lane; must be called by all 32 lanes of the warp together.  Elements with active == false must
+    // pass x = y = 0 (padding); they are not inspected.  ALLACT: every element is active (no selects).
+    // Instruction budget per element: 2 + 3K + 3(K-1) fp64 operations and ~5 integer ones; the range
+    // test and the below-window test are OR/MAX-reduced over the batch and branch once per batch.
+    template <int U, bool ALLACT>
     __device__ __forceinline__ void add(const double (&x)[U], const double (&y)[U], const bool (&active)[U], ExShared* sh) {
+        constexpr unsigned LOS = BE_LO << 20, RANGES = (BE_HI - BE_LO) << 20;
         double p[U], e[U];
+        unsigned tmax = 0;
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             p[u] = __dmul_rn(x[u], y[u]);
             e[u] = __fma_rn(x[u], y[u], -p[u]);                      // TwoProd
-            const unsigned be = ((unsigned)__double2hiint(p[u]) >> 20) & 0x7ffu;
-            if (active[u] && (be - BE_LO) > (BE_HI - BE_LO)) {       // outside TwoProd's error-free range (or zero)
-                const bool xz = (((unsigned)__double2hiint(x[u]) & 0x7fffffffu) | (unsigned)__double2loint(x[u])) == 0u;
-                const bool yz = (((unsigned)__double2hiint(y[u]) & 0x7fffffffu) | (unsigned)__double2loint(y[u])) == 0u;
-                if (be == 0x7ffu || !(xz || yz)) ex_deposit_product(sh, x[u], y[u]);
-                p[u] = 0.0; e[u] = 0.0;
+            unsigned hp = (unsigned)__double2hiint(p[u]) & 0x7ff00000u;
+            if (!ALLACT) hp = active[u] ? hp : LOS;
+            const unsigned t = hp - LOS;                             // wraps to huge below the range
+            tmax = t > tmax ? t : tmax;
+        }
+        if (tmax > RANGES) {                                         // some product outside TwoProd's error-free range, or zero
+            tmax = 0;
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const unsigned be = ((unsigned)__double2hiint(p[u]) >> 20) & 0x7ffu;
+                const bool act = ALLACT || active[u];
+                if (act && (be - BE_LO) > (BE_HI - BE_LO)) {
+                    const bool xz = (((unsigned)__double2hiint(x[u]) & 0x7fffffffu) | (unsigned)__double2loint(x[u])) == 0u;
+                    const bool yz = (((unsigned)__double2hiint(y[u]) & 0x7fffffffu) | (unsigned)__double2loint(y[u])) == 0u;
+                    if (be == 0x7ffu || !(xz || yz)) ex_deposit_product(sh, x[u], y[u]);
+                    p[u] = 0.0; e[u] = 0.0;
+                } else if (act) {
+                    const unsigned t = (be - BE_LO) << 20;
+                    tmax = t > tmax ? t : tmax;
+                }
             }
         }
-        int bemax = 0;
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const int be = (__double2hiint(p[u]) >> 20) & 0x7ff;
-            bemax = be > bemax ? be : bemax;
-        }
+        const int bemax = (int)(tmax >> 20) + (int)BE_LO;
         if (__any_sync(0xffffffffu, bemax > Tb)) reanchor(sh, __reduce_max_sync(0xffffffffu, bemax));
         if (cnt + U > CAP) { recentre(); if (ren >= 32) flush(sh); }
         cnt += U;
-        unsigned rest = 0;
+        unsigned rlo = 0, rhi = 0;
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             double v = p[u], w = e[u];
@@ -200,10 +213,10 @@ struct ExAcc {
                 S[k] = s;
             }
             p[u] = v; e[u] = w;
-            rest |= (unsigned)__double2loint(v) | (unsigned)__double2loint(w) |
-                    (((unsigned)__double2hiint(v) | (unsigned)__double2hiint(w)) & 0x7fffffffu);
+            rlo |= (unsigned)__double2loint(v) | (unsigned)__double2loint(w);
+            rhi |= (unsigned)__double2hiint(v) | (unsigned)__double2hiint(w);
         }
-        if (rest) {                                                  // bits below the window: exact, but slow
+        if (rlo | (rhi & 0x7fffffffu)) {                             // bits below the window: exact, but slow
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 if (p[u] != 0.0) ex_deposit_double(sh, p[u]);
@@ -212,11 +225,15 @@ struct ExAcc {
         }
     }
     template <int U>
-    __device__ __forceinline__ void add(const double (&x)[U], const double (&y)[U], ExShared* sh) {
+    __device__ __forceinline__ void add(const double (&x)[U], const double (&y)[U], const bool (&active)[U], ExShared* sh) {
+        add<U, false>(x, y, active, sh);
+    }
+    template <int U>
+    __device__ __forceinline__ void add_all(const double (&x)[U], const double (&y)[U], ExShared* sh) {
         bool act[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) act[u] = true;
-        add<U>(x, y, act, sh);
+        add<U, true>(x, y, act, sh);
     }
 };
 

@@ -48,6 +48,37 @@ __device__ __forceinline__ void exdot_issue(double* buf, int stage, const double
     fx_cp_commit();
 }
 
+// Consume one landed tile from shared memory (generic: bounds-checked).
+template <bool VEC>
+__device__ __forceinline__ void exdot_consume(const double* buf, int stage, long long n, long long base, ExAcc<EX_K, EX_W>& acc,
+                                              ExShared* sh) {
+    const int bd = blockDim.x;
+    const double* sx = buf + (size_t)stage * 2 * EX_U * bd;
+    const double* sy = sx + EX_U * bd;
+    double xv[EX_U], yv[EX_U];
+    bool act[EX_U];
+    if (VEC) {
+#pragma unroll
+        for (int u = 0; u < EX_U / 2; ++u) {
+            const int slot = 2 * (u * bd + threadIdx.x);
+            const double2 a = *reinterpret_cast<const double2*>(sx + slot);
+            const double2 b = *reinterpret_cast<const double2*>(sy + slot);
+            xv[2 * u] = a.x; xv[2 * u + 1] = a.y; yv[2 * u] = b.x; yv[2 * u + 1] = b.y;
+            act[2 * u] = base + slot < n; act[2 * u + 1] = base + slot + 1 < n;
+        }
+    } else {
+#pragma unroll
+        for (int u = 0; u < EX_U; ++u) {
+            const int slot = u * bd + threadIdx.x;
+            xv[u] = sx[slot]; yv[u] = sy[slot];
+            act[u] = base + slot < n;
+        }
+    }
+    acc.add<EX_U>(xv, yv, act, sh);
+}
+
+// The kernel.  CTA b takes tiles b, b+G, b+2G, ...; FX_STAGES-1 tiles are in flight per thread.
+// Hot loop (16-byte aligned inputs, full tiles): pointer increments only, compile-time stage offsets, no bounds.
 template <bool VEC>
 __global__ void __launch_bounds__(256, 3) k_exdot(const double* __restrict__ x, const double* __restrict__ y, long long n,
                                                   ExGlobal g, int first, int last, double* result) {
@@ -58,38 +89,50 @@ __global__ void __launch_bounds__(256, 3) k_exdot(const double* __restrict__ x, 
     acc.init();
     const int bd = blockDim.x;
     const long long tile = (long long)bd * EX_U;
-    const long long ntiles = (n + tile - 1) / tile;
+    const long long ntiles = (n + tile - 1) / tile, nfull = n / tile;
     long long tq = blockIdx.x;                                   // next tile to issue
+    long long t = blockIdx.x;                                    // next tile to consume
 #pragma unroll
     for (int s = 0; s < FX_STAGES - 1; ++s) { exdot_issue<VEC>(ex_buf, s, x, y, n, tq * tile, tq < ntiles); tq += gridDim.x; }
     int stage = 0;
-    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
-        int sq = stage + FX_STAGES - 1; if (sq >= FX_STAGES) sq -= FX_STAGES;
-        exdot_issue<VEC>(ex_buf, sq, x, y, n, tq * tile, tq < ntiles); tq += gridDim.x;
-        fx_cp_wait<FX_STAGES - 1>();                             // the group of tile t has landed
-        const double* sx = ex_buf + (size_t)stage * 2 * EX_U * bd;
-        const double* sy = sx + EX_U * bd;
-        double xv[EX_U], yv[EX_U];
-        bool act[EX_U];
-        if (VEC) {
+    if (VEC) {
+        // per-thread pointers of the tile to issue; shared slots of this thread
+        const long long step = (long long)gridDim.x * tile;
+        const double* gx = x + tq * tile + 2 * threadIdx.x;
+        const double* gy = y + tq * tile + 2 * threadIdx.x;
+        const unsigned s0 = fx_smem_addr(ex_buf) + 16u * threadIdx.x;
+        const unsigned stage_bytes = 2u * EX_U * bd * 8u, arr_bytes = (unsigned)EX_U * bd * 8u, u_bytes = 16u * bd;
+        unsigned so = 0;                                             // byte offset of the stage to consume
+        unsigned sqo = (FX_STAGES - 1) * stage_bytes;                // ... and of the stage to fill
+        while (tq < nfull) {                                         // the tile to issue is a full one
 #pragma unroll
             for (int u = 0; u < EX_U / 2; ++u) {
-                const int slot = 2 * (u * bd + threadIdx.x);
-                const double2 a = *reinterpret_cast<const double2*>(sx + slot);
-                const double2 b = *reinterpret_cast<const double2*>(sy + slot);
-                xv[2 * u] = a.x; xv[2 * u + 1] = a.y; yv[2 * u] = b.x; yv[2 * u + 1] = b.y;
-                const long long e0 = t * tile + slot;
-                act[2 * u] = e0 < n; act[2 * u + 1] = e0 + 1 < n;
+                fx_cp_async16_full(s0 + sqo + u * u_bytes, gx + 2 * u * bd);
+                fx_cp_async16_full(s0 + sqo + arr_bytes + u * u_bytes, gy + 2 * u * bd);
             }
-        } else {
+            fx_cp_commit();
+            gx += step; gy += step; tq += gridDim.x;
+            fx_cp_wait<FX_STAGES - 1>();
+            double xv[EX_U], yv[EX_U];
 #pragma unroll
-            for (int u = 0; u < EX_U; ++u) {
-                const int slot = u * bd + threadIdx.x;
-                xv[u] = sx[slot]; yv[u] = sy[slot];
-                act[u] = t * tile + slot < n;
+            for (int u = 0; u < EX_U / 2; ++u) {
+                double2 a, b;
+                fx_lds128(a, s0 + so + u * u_bytes);
+                fx_lds128(b, s0 + so + arr_bytes + u * u_bytes);
+                xv[2 * u] = a.x; xv[2 * u + 1] = a.y; yv[2 * u] = b.x; yv[2 * u + 1] = b.y;
             }
+            acc.add_all<EX_U>(xv, yv, &sh);                          // consumed tile < issued tile: full as well
+            t += gridDim.x;
+            sqo = so;
+            so += stage_bytes; if (so == FX_STAGES * stage_bytes) so = 0;
+            if (++stage == FX_STAGES) stage = 0;
         }
-        acc.add<EX_U>(xv, yv, act, &sh);
+    }
+    for (; t < ntiles; t += gridDim.x) {                                     // generic: tail tiles, unaligned inputs
+        int sq = stage + FX_STAGES - 1; if (sq >= FX_STAGES) sq -= FX_STAGES;
+        exdot_issue<VEC>(ex_buf, sq, x, y, n, tq * tile, tq < ntiles); tq += gridDim.x;
+        fx_cp_wait<FX_STAGES - 1>();
+        exdot_consume<VEC>(ex_buf, stage, n, t * tile, acc, &sh);
         if (++stage == FX_STAGES) stage = 0;
     }
     fx_cp_wait<0>();

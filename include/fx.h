@@ -125,6 +125,15 @@ fx_status fx_cg_solve_host(const fx_grid* grid, const double* chi_host, const do
 fx_status fx_cg_profile(int32_t enable);
 fx_status fx_cg_last_profile(double* ms_host, int32_t* iterations_host);
 
+/* Timing hook for the latency-bandwidth sweep (the paper reports average run times of back-to-back calls):
+ * launches one primitive `reps` times (after one untimed call) between two CUDA events on the library stream and
+ * returns the average milliseconds per call in *ms_host.  kind: 0 = exdot(a,b) result left on the device,
+ * 1 = axpby(0.7,a,-0.3,c), 2 = pointwise_dot(1,a,b,0,c), 3 = dG apply_sym(grid; chi=a, x=b, y=c), 4 = dG apply (normed),
+ * 5 = exdot(a,b) returned to the host every call (the paper's GPU dot latency), 6 = axpby(0.7,a,1,c).
+ * a, b, c: device vectors of n doubles (kinds 3,4: n must equal the grid's size).  Synchronises.               */
+fx_status fx_time_primitive(int32_t kind, const fx_grid* grid, const double* a_dev, const double* b_dev, double* c_dev,
+                            int64_t n, int32_t reps, double* ms_host);
+
 /* Number of kernels this library has launched since load (bench.py's "gpu_launches").                          */
 int64_t fx_launch_count(void);
 

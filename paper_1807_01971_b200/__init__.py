@@ -57,6 +57,7 @@ _SIGNATURES = {
     "fx_cg_solve_host": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp, C.c_double, C.c_int32, C.POINTER(CGInfo)]),
     "fx_cg_profile": (C.c_int, [C.c_int32]),
     "fx_cg_last_profile": (C.c_int, [_dp, C.POINTER(C.c_int32)]),
+    "fx_time_primitive": (C.c_int, [C.c_int32, C.POINTER(Grid), _vp, _vp, _vp, C.c_int64, C.c_int32, _dp]),
     "fx_launch_count": (C.c_int64, []),
 }
 
@@ -220,6 +221,19 @@ def cg_solve(grid, chi, rho, phi, tol, maxit):
     _check(lib().fx_cg_solve(C.byref(grid), _ptr(chi, grid.n), _ptr(rho, grid.n), _ptr(phi, grid.n), float(tol), int(maxit),
                              C.byref(info)), "fx_cg_solve")
     return info
+
+
+TIME_KINDS = {"exdot": 0, "axpby": 1, "pointwise_dot": 2, "dg_apply_sym": 3, "dg_apply": 4, "exdot_host": 5, "axpy": 6}
+
+
+def time_primitive(kind, a, b, c, reps, grid=None):
+    """Average milliseconds per call of `reps` back-to-back calls of one primitive, timed on the device (fx.h)."""
+    _use_torch_stream()
+    ms = C.c_double(0.0)
+    n = a.numel()
+    _check(lib().fx_time_primitive(TIME_KINDS[kind], C.byref(grid) if grid is not None else None, _ptr(a), _ptr(b, n), _ptr(c, n), n,
+                                   int(reps), C.byref(ms)), "fx_time_primitive")
+    return ms.value
 
 
 def cg_profile(enable):

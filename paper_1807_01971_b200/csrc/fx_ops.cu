@@ -351,3 +351,42 @@ extern "C" fx_status fx_dg_tables(int32_t P, double* out) {
     for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m) *o++ = t.D[k][m];
     return FX_OK;
 }
+
+// ------------------------------------------------------------------------------------------------------------
+// timing hook (include/fx.h): average time of back-to-back calls, measured on the device
+// ------------------------------------------------------------------------------------------------------------
+static fx_status time_one(FxCtx* c, int kind, const fx_grid* g, const double* a, const double* b, double* cc, int64_t n) {
+    switch (kind) {
+    case 0: return fx_launch_exdot(c, a, b, n, c->result_dev);
+    case 1: return fx_axpby(0.7, a, -0.3, cc, n);
+    case 2: return fx_pointwise_dot(1.0, a, b, 0.0, cc, n);
+    case 3: return fx_launch_apply(c, g, a, b, cc, 0);
+    case 4: return fx_launch_apply(c, g, a, b, cc, 1);
+    case 5: { const double v = fx_exdot(a, b, n); return (v != v && fx_last_error()[0]) ? FX_ECUDA : FX_OK; }
+    case 6: return fx_axpby(0.7, a, 1.0, cc, n);
+    }
+    return FX_EINVAL;
+}
+
+extern "C" fx_status fx_time_primitive(int32_t kind, const fx_grid* g, const double* a, const double* b, double* cc, int64_t n,
+                                       int32_t reps, double* ms_host) {
+    if (kind < 0 || kind > 6 || n < 0 || reps < 1 || !ms_host || !a || !b || !cc) { fx_set_error("fx_time_primitive: bad arguments"); return FX_EINVAL; }
+    if ((kind == 3 || kind == 4) && (!fx_grid_ok(g) || (int64_t)g->Nx * g->Ny * g->P * g->P != n)) { fx_set_error("fx_time_primitive: bad grid"); return FX_EINVAL; }
+    FxCtx* c = fx_ctx();
+    if (!c) return FX_ECUDA;
+    cudaEvent_t e0, e1;
+    FX_CUDA(cudaEventCreate(&e0)); FX_CUDA(cudaEventCreate(&e1));
+    fx_status s = time_one(c, kind, g, a, b, cc, n);
+    if (s == FX_OK) {
+        cudaStreamSynchronize(c->stream);
+        cudaEventRecord(e0, c->stream);
+        for (int i = 0; i < reps && s == FX_OK; ++i) s = time_one(c, kind, g, a, b, cc, n);
+        cudaEventRecord(e1, c->stream);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        *ms_host = (double)ms / reps;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    return s;
+}

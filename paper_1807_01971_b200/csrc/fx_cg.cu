@@ -142,6 +142,129 @@ __global__ void __launch_bounds__(256, 3) k_cg_update(const __grid_constant__ Dg
     }
 }
 
+// K2, fast path: all four vectors 16-byte aligned.  Linear tiles of 2*blockDim.x elements, one 16-byte vector per thread,
+// array and tile, FX_STAGES-1 tiles in flight through cp.async (as k_exdot).  The table indices l = row % P, k = col % P
+// of a thread's elements are advanced incrementally from tile to tile (no division in the loop).
+template <int P>
+__device__ __forceinline__ void cg_update_pair(const DgParams& g, double alpha, double nalpha, int l, int k, int col, int pitch,
+                                               const double2& pv, const double2& qv, const double2& fv, const double2& rv,
+                                               double2& fo, double2& ro, double (&zz)[2]) {
+    int k1 = k + 1, l1 = l;
+    if (k1 == P) k1 = 0;
+    if (col + 1 == pitch) { k1 = 0; l1 = l + 1; if (l1 == P) l1 = 0; }
+    fo.x = __fma_rn(alpha, pv.x, fv.x); fo.y = __fma_rn(alpha, pv.y, fv.y);       // axpby(alpha, p, 1, phi)
+    ro.x = __fma_rn(nalpha, qv.x, rv.x); ro.y = __fma_rn(nalpha, qv.y, rv.y);     // axpby(-alpha, q, 1, r)
+    zz[0] = __dmul_rn(g.V[l][k], ro.x); zz[1] = __dmul_rn(g.V[l1][k1], ro.y);     // pointwise_dot(1, V, r, 0, z)
+}
+
+template <int P>
+__global__ void __launch_bounds__(256, 3) k_cg_update_lin(const __grid_constant__ DgParams g, const double* __restrict__ p,
+                                                          const double* __restrict__ q, double* phi, double* r, ExGlobal ex,
+                                                          CgScal* sc) {
+    if (*(volatile int*)&sc->done) return;
+    extern __shared__ __align__(16) double cg_buf[];
+    __shared__ ExShared sh;
+    ex_shared_init(&sh);
+    CgAcc acc;
+    acc.init();
+    const double alpha = sc->alpha, nalpha = -alpha;
+    const int pitch = g.Nx * P, bd = blockDim.x;
+    const long long n = (long long)pitch * g.Ny * P;
+    const long long tile = 2ll * bd, ntiles = (n + tile - 1) / tile, nfull = n / tile;
+    const unsigned s0 = fx_smem_addr(cg_buf) + 16u * threadIdx.x;
+    const unsigned arr_bytes = 16u * bd, stage_bytes = 4u * arr_bytes;
+    long long tq = blockIdx.x, t = blockIdx.x;
+    const long long step = (long long)gridDim.x * tile;
+    // prologue (generic issue: zero-fills what lies beyond n)
+#pragma unroll
+    for (int s = 0; s < FX_STAGES - 1; ++s) {
+        if (tq < ntiles) {
+            const long long e0 = tq * tile + 2 * threadIdx.x;
+            const long long left = n - e0;
+            const int bytes = left >= 2 ? 16 : (left == 1 ? 8 : 0);
+            const long long es = bytes ? e0 : 0;
+            fx_cp_async16(s0 + s * stage_bytes, p + es, bytes);
+            fx_cp_async16(s0 + s * stage_bytes + arr_bytes, q + es, bytes);
+            fx_cp_async16(s0 + s * stage_bytes + 2 * arr_bytes, phi + es, bytes);
+            fx_cp_async16(s0 + s * stage_bytes + 3 * arr_bytes, r + es, bytes);
+        }
+        fx_cp_commit();
+        tq += gridDim.x;
+    }
+    // incremental (l, k, col) of this thread's first element of the tile to consume
+    long long i0 = t * tile + 2 * threadIdx.x;
+    int col = (int)(i0 % pitch), l = (int)((i0 / pitch) % P), k = col % P;
+    const int dcol = (int)(step % pitch), dl = (int)((step / pitch) % P), dk1 = dcol % P, dk2 = ((dcol % P) - (pitch % P) + P) % P;
+    const double* gp = p + tq * tile + 2 * threadIdx.x;
+    const double* gq = q + tq * tile + 2 * threadIdx.x;
+    const double* gf = phi + tq * tile + 2 * threadIdx.x;
+    const double* gr = r + tq * tile + 2 * threadIdx.x;
+    double* of = phi + i0;
+    double* orr = r + i0;
+    unsigned so = 0, sqo = (FX_STAGES - 1) * stage_bytes;
+    while (tq < nfull) {                                             // hot loop: tile to issue is full => so is the one consumed
+        fx_cp_async16_full(s0 + sqo, gp);
+        fx_cp_async16_full(s0 + sqo + arr_bytes, gq);
+        fx_cp_async16_full(s0 + sqo + 2 * arr_bytes, gf);
+        fx_cp_async16_full(s0 + sqo + 3 * arr_bytes, gr);
+        fx_cp_commit();
+        gp += step; gq += step; gf += step; gr += step; tq += gridDim.x;
+        fx_cp_wait<FX_STAGES - 1>();
+        double2 pv, qv, fv, rv, fo, ro;
+        fx_lds128(pv, s0 + so); fx_lds128(qv, s0 + so + arr_bytes); fx_lds128(fv, s0 + so + 2 * arr_bytes); fx_lds128(rv, s0 + so + 3 * arr_bytes);
+        double rr[2], zz[2];
+        cg_update_pair<P>(g, alpha, nalpha, l, k, col, pitch, pv, qv, fv, rv, fo, ro, zz);
+        *reinterpret_cast<double2*>(of) = fo;
+        *reinterpret_cast<double2*>(orr) = ro;
+        rr[0] = ro.x; rr[1] = ro.y;
+        acc.add_all<2>(rr, zz, &sh);
+        of += step; orr += step; t += gridDim.x;
+        col += dcol;
+        const bool wrapped = col >= pitch;
+        col -= wrapped ? pitch : 0;
+        k += wrapped ? dk2 : dk1; k -= (k >= P) ? P : 0;
+        l += dl + (wrapped ? 1 : 0); l -= (l >= P) ? P : 0;
+        sqo = so;
+        so += stage_bytes; if (so == FX_STAGES * stage_bytes) so = 0;
+    }
+    for (; t < ntiles; t += gridDim.x) {                             // the last FX_STAGES-1 issued tiles and the ragged tail
+        if (tq < ntiles) {
+            const long long e0 = tq * tile + 2 * threadIdx.x;
+            const long long left = n - e0;
+            const int bytes = left >= 2 ? 16 : (left == 1 ? 8 : 0);
+            const long long es = bytes ? e0 : 0;
+            fx_cp_async16(s0 + sqo, p + es, bytes);
+            fx_cp_async16(s0 + sqo + arr_bytes, q + es, bytes);
+            fx_cp_async16(s0 + sqo + 2 * arr_bytes, phi + es, bytes);
+            fx_cp_async16(s0 + sqo + 3 * arr_bytes, r + es, bytes);
+        }
+        fx_cp_commit();
+        tq += gridDim.x;
+        fx_cp_wait<FX_STAGES - 1>();
+        double2 pv, qv, fv, rv, fo, ro;
+        fx_lds128(pv, s0 + so); fx_lds128(qv, s0 + so + arr_bytes); fx_lds128(fv, s0 + so + 2 * arr_bytes); fx_lds128(rv, s0 + so + 3 * arr_bytes);
+        const long long e0 = t * tile + 2 * threadIdx.x;
+        const int c0 = (int)(e0 % pitch), l0 = (int)((e0 / pitch) % P);
+        double rr[2], zz[2];
+        bool act[2] = {e0 < n, e0 + 1 < n};
+        cg_update_pair<P>(g, alpha, nalpha, l0, c0 % P, c0, pitch, pv, qv, fv, rv, fo, ro, zz);
+        if (act[1]) { *reinterpret_cast<double2*>(phi + e0) = fo; *reinterpret_cast<double2*>(r + e0) = ro; }
+        else if (act[0]) { phi[e0] = fo.x; r[e0] = ro.x; }
+        rr[0] = act[0] ? ro.x : 0.0; rr[1] = act[1] ? ro.y : 0.0;
+        zz[0] = act[0] ? zz[0] : 0.0; zz[1] = act[1] ? zz[1] : 0.0;
+        acc.add<2>(rr, zz, act, &sh);
+        sqo = so;
+        so += stage_bytes; if (so == FX_STAGES * stage_bytes) so = 0;
+    }
+    fx_cp_wait<0>();
+    acc.flush(&sh);
+    if (ex_block_finish(&sh, ex, 1, 1, &sc->dot) && threadIdx.x == 0) {
+        const double rzn = sc->dot;
+        if (__dsqrt_rn(rzn) <= sc->thresh) { sc->rz = rzn; sc->status = FX_OK; sc->done = 1; }
+        else { sc->beta = __ddiv_rn(rzn, sc->rz); sc->rz = rzn; }
+    }
+}
+
 // K3: p = z + beta p,  z = V o r.  Two fp64 operations per element: plain coalesced loads, four chunks in flight.
 #define CG_U3 4
 template <int P>
@@ -227,7 +350,18 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, 
     static bool attr_done = false;
     if (!attr_done) {
         FX_CUDA(cudaFuncSetAttribute(k_cg_update<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, FX_STAGES * 4 * CG_U * 256 * 8));
+        FX_CUDA(cudaFuncSetAttribute(k_cg_update_lin<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, FX_STAGES * 4 * 2 * 256 * 8));
         attr_done = true;
+    }
+    // K2 fast path: 16-byte aligned vectors (the work vectors always are; phi is the caller's)
+    const bool lin = aligned16(phi) && aligned16(r) && aligned16(p) && aligned16(q);
+    int lg;
+    {
+        const long long n = (long long)dp.Nx * dp.Ny * P * P, tile = 2ll * eb;
+        long long nt = (n + tile - 1) / tile, gm = (long long)c->num_sms * (768 / eb);
+        if (nt > gm) nt = gm;
+        if (c->launch[3][0]) nt = c->launch[3][0];
+        lg = (int)nt;
     }
     for (int i = 0; i < iters; ++i) {
         cudaEvent_t* ev = nullptr;
@@ -235,7 +369,8 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, 
         if (ev) cudaEventRecord(ev[0], c->stream);
         k_cg_apply_dot<P><<<ag, ab, 0, c->stream>>>(dp, chi, p, q, c->ex, sc);
         if (ev) cudaEventRecord(ev[1], c->stream);
-        k_cg_update<P><<<eg, eb, (size_t)FX_STAGES * 4 * CG_U * eb * 8, c->stream>>>(dp, p, q, phi, r, c->ex, sc);
+        if (lin) k_cg_update_lin<P><<<lg, eb, (size_t)FX_STAGES * 4 * 2 * eb * 8, c->stream>>>(dp, p, q, phi, r, c->ex, sc);
+        else k_cg_update<P><<<eg, eb, (size_t)FX_STAGES * 4 * CG_U * eb * 8, c->stream>>>(dp, p, q, phi, r, c->ex, sc);
         if (ev) cudaEventRecord(ev[2], c->stream);
         k_cg_dir<P><<<dg, eb, 0, c->stream>>>(dp, r, p, sc);
         if (ev) cudaEventRecord(ev[3], c->stream);

@@ -343,6 +343,24 @@ def test_cg_zero_rhs_and_nonzero_start(fx, oracle):
     assert info.iterations == oinfo.iterations and same_bits(got, want)
 
 
+@pytest.mark.parametrize("Nx,Ny,P", [(15, 9, 3), (33, 7, 5), (7, 5, 1), (61, 4, 2)])
+def test_cg_odd_pitch_and_unaligned_phi(fx, oracle, Nx, Ny, P):
+    """rows that are not 16-byte aligned (odd Nx*P), ragged tiles, and a caller phi that is only 8-byte aligned"""
+    import torch
+    grid = dict(Nx=Nx, Ny=Ny, P=P, lx=2 * math.pi, ly=1.7, bcx=0, bcy=1)
+    g, og = fx.make_grid(**grid), oracle.Grid(**grid)
+    chi = 1.0 + 0.5 * fi.uniform(91, g.n); rho = fi.uniform(92, g.n); phi0 = 0.01 * fi.uniform(93, g.n)
+    want, oinfo = oracle.cg_solve(og, chi, rho, phi0, 1e-9, 400)
+    phi = dev(phi0)
+    info = fx.cg_solve(g, dev(chi), dev(rho), phi, 1e-9, 400)
+    assert info.iterations == oinfo.iterations and info.status == oinfo.status
+    assert same_bits(phi.cpu().numpy(), want)
+    buf = torch.zeros(g.n + 1, dtype=torch.float64, device="cuda")
+    buf[1:] = dev(phi0)
+    info = fx.cg_solve(g, dev(chi), dev(rho), buf[1:], 1e-9, 400)
+    assert info.iterations == oinfo.iterations and same_bits(buf[1:].cpu().numpy(), want)
+
+
 def test_cg_full_size_config3_first_iterations(fx, oracle):
     """config 3 at full size, the launch shape bench.py times; 6 iterations against the oracle, bit for bit"""
     c = fi.config3()

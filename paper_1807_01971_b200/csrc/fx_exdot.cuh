@@ -40,6 +40,7 @@ struct ExShared {
     fx_u64 lim[FX_NLIMB];    // last CTA only: the canonical limbs while they are normalised and rounded
     int flags;
     int is_last;
+    int dlo, dhi;            // last CTA only: range of non-zero merged digits
 };
 
 struct ExGlobal {            // device scratch of one context
@@ -245,43 +246,44 @@ __device__ __forceinline__ void ex_shared_init(ExShared* sh) {
 
 // ---- final stage, one thread: merge digits into the canonical limbs, round once ----------------------------
 
-__device__ inline fx_u64 ex_get64(const fx_u64* mag, int bit) {     // bits [bit, bit+63]
-    const int k = bit >> 6, s = bit & 63;
-    fx_u64 v = mag[k] >> s;
-    if (s && k + 1 < FX_NLIMB) v |= mag[k + 1] << (64 - s);
-    return v;
-}
-
-// RN(limbs) with ties to even, gradual underflow, overflow to inf; exact zero -> +0.0   (DESIGN.md 3.1 step 4)
-__device__ inline double ex_round(const fx_u64* limbs, int flags, fx_u64* mag /* scratch [FX_NLIMB] */) {
+// RN(limbs) with ties to even, gradual underflow, overflow to inf; exact zero -> +0.0   (DESIGN.md 3.1 step 4).
+// Only limbs [a, bb] are inspected: limbs below a are zero, limbs above bb repeat the sign of limb bb.
+__device__ inline double ex_round(const fx_u64* limbs, int flags, fx_u64* mag /* scratch [FX_NLIMB] */, int a, int bb) {
     if ((flags & FX_FLAG_NAN) || ((flags & FX_FLAG_PINF) && (flags & FX_FLAG_NINF)))
         return __longlong_as_double(0x7FF8000000000000ll);
     if (flags & FX_FLAG_PINF) return __longlong_as_double(0x7FF0000000000000ll);
     if (flags & FX_FLAG_NINF) return __longlong_as_double((long long)0xFFF0000000000000ull);
-    const bool neg = (limbs[FX_NLIMB - 1] >> 63) != 0;
+    const bool neg = (limbs[bb] >> 63) != 0;
     fx_u64 carry = neg ? 1ull : 0ull;
     int top = -1;
-    for (int k = 0; k < FX_NLIMB; ++k) {
-        fx_u64 v = neg ? ~limbs[k] : limbs[k];
+    for (int k = a; k <= bb; ++k) {
+        const fx_u64 v = neg ? ~limbs[k] : limbs[k];
         const fx_u64 s = v + carry;
         carry = (s < v) ? 1ull : 0ull;
         mag[k] = s;
         if (s) top = k;
     }
     if (top < 0) return 0.0;
+#define FX_MAG(k) (((k) >= a && (k) <= bb) ? mag[(k)] : 0ull)
     const int t = 64 * top + 63 - __clzll((long long)mag[top]);
     const int PMIN = -1074 + FX_BIAS;
     const bool normal = (t - 52) >= PMIN;
     const int p = normal ? (t - 52) : PMIN;
-    fx_u64 mant = ex_get64(mag, p);                                   // < 2^53
-    const fx_u64 round_bit = (mag[(p - 1) >> 6] >> ((p - 1) & 63)) & 1ull;
+    fx_u64 mant;                                                      // bits [p, p+63] (all above t are zero): < 2^53
+    {
+        const int k = p >> 6, sft = p & 63;
+        mant = FX_MAG(k) >> sft;
+        if (sft) mant |= FX_MAG(k + 1) << (64 - sft);
+    }
+    const fx_u64 round_bit = (FX_MAG((p - 1) >> 6) >> ((p - 1) & 63)) & 1ull;
     bool sticky = false;
     {
         const int b = p - 1;                                          // bits [0, b) below the round bit
-        const int k = b >> 6, s = b & 63;
-        for (int i = 0; i < k; ++i) sticky |= (mag[i] != 0);
-        if (s) sticky |= (mag[k] & ((1ull << s) - 1ull)) != 0;
+        const int k = b >> 6, sft = b & 63;
+        for (int i = a; i < k && i <= bb; ++i) sticky |= (mag[i] != 0);
+        if (sft) sticky |= (FX_MAG(k) & ((1ull << sft) - 1ull)) != 0;
     }
+#undef FX_MAG
     if (round_bit && (sticky || (mant & 1ull))) mant += 1ull;
     fx_u64 bits;
     if (normal) {
@@ -313,13 +315,25 @@ __device__ __forceinline__ bool ex_block_finish(ExShared* sh, const ExGlobal& g,
     __syncthreads();
     if (!sh->is_last) return false;
     __threadfence();
-    for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) { sh->dig[i] = __ldcg(&g.dig[i]); g.dig[i] = 0ull; }
+    if (threadIdx.x == 0) { sh->dlo = FX_NDIG; sh->dhi = -1; }
+    __syncthreads();
+    for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) {
+        const fx_u64 v = __ldcg(&g.dig[i]);
+        sh->dig[i] = v;
+        if (v) { g.dig[i] = 0ull; atomicMin(&sh->dlo, i); atomicMax(&sh->dhi, i); }
+    }
     for (int i = threadIdx.x; i < FX_NLIMB; i += blockDim.x) sh->lim[i] = first ? 0ull : __ldcg(&g.limbs[i]);
     __syncthreads();
+    // thread 0: carry-normalise.  In the first launch of a call the limbs start from zero, so only the limbs that hold
+    // non-zero digits (a handful: the data's exponent window) need the serial pass; above them the sign repeats.
     if (threadIdx.x == 0) {
+        int la = 0, lb = FX_NLIMB - 1;
+        if (first) { la = sh->dhi < 0 ? 0 : (sh->dlo >> 1); lb = sh->dhi < 0 ? 0 : (sh->dhi >> 1); }
         long long carry = 0;
         fx_u64 c2 = 0;
-        for (int k = 0; k < FX_NLIMB; ++k) {
+        int k = la;
+        for (; k < FX_NLIMB; ++k) {
+            if (k > lb && first && (carry == 0 || carry == -1) && c2 == 0) break;   // nothing but sign extension left
             long long v = (long long)sh->dig[2 * k] + carry;
             const fx_u64 lo = (fx_u64)v & 0xffffffffull;
             carry = v >> 32;
@@ -335,16 +349,25 @@ __device__ __forceinline__ bool ex_block_finish(ExShared* sh, const ExGlobal& g,
             c2 = c;
             sh->lim[k] = s2;
         }
+        // k = first limb not written; limbs k.. are 0 (carry 0) or all ones (carry -1)
+        const fx_u64 fill = (carry == -1) ? ~0ull : 0ull;
+        int bb = k;
+        if (k < FX_NLIMB) sh->lim[k] = fill; else bb = FX_NLIMB - 1;
+        sh->dlo = k; sh->dhi = (carry == -1) ? 1 : 0;                 // hand the fill range to the other threads
         if (last) {
             const int flags = __ldcg(g.flags);
             g.flags[1] = flags;                       // kept for fx_exdot_digits
             g.flags[0] = 0;
-            if (result) *result = ex_round(sh->lim, flags, sh->dig);
+            if (result) *result = ex_round(sh->lim, flags, sh->dig, la, bb);
         }
         *g.ticket = 0u;
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < FX_NLIMB; i += blockDim.x) g.limbs[i] = sh->lim[i];
+    {
+        const int kf = sh->dlo;
+        const fx_u64 fill = sh->dhi ? ~0ull : 0ull;
+        for (int i = threadIdx.x; i < FX_NLIMB; i += blockDim.x) g.limbs[i] = (i > kf) ? fill : sh->lim[i];
+    }
     __threadfence();
     __syncthreads();
     return true;

@@ -316,23 +316,7 @@ static fx_status cg_workspace(FxCtx* c, int64_t n) {
 }
 
 static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int* apply_grid, int* apply_block, int* ew_grid, int* ew_block) {
-    int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
-    if (wpb > 4) wpb = 4;                       // the kernels are compiled for <= 128 threads per CTA
-    p->nstrip = (g->Nx + FX_STRIP - 1) / FX_STRIP;
-    int rps = c->launch[2][0];
-    if (rps <= 0) {
-        const long long target = (long long)c->num_sms * 32;
-        long long nseg = target / p->nstrip;
-        if (nseg < 1) nseg = 1;
-        rps = (int)((g->Ny + nseg - 1) / nseg);
-        if (rps < 8) rps = 8;
-    }
-    if (rps > g->Ny) rps = g->Ny;
-    p->rows_per_seg = rps;
-    p->nseg = (g->Ny + rps - 1) / rps;
-    const long long warps = (long long)p->nstrip * p->nseg;
-    *apply_grid = (int)((warps + wpb - 1) / wpb);
-    *apply_block = wpb * 32;
+    fx_dg_shape(c, g, p, apply_grid, apply_block);
     int bd = c->launch[3][1] ? c->launch[3][1] : 256;
     if (bd > 256) bd = 256;
     const int pitch = g->Nx * g->P;

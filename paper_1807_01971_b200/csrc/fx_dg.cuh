@@ -35,15 +35,16 @@ struct DgParams {
 template <int P>
 struct DgCell { double v[P][P]; };     // [l][k]: row l (y node), column k (x node)
 
-// load one cell's P x P values; `zero` lanes get +0.0 without touching memory
+// load one cell's P x P values (always from valid memory: ghost lanes read their wrapped cell and have their traces
+// forced to +0.0 afterwards, which is all their neighbours ever see)
 template <int P>
 __device__ __forceinline__ void dg_load(DgCell<P>& c, const double* __restrict__ a, long long pitch, int col0, int j,
-                                        bool zero) {
+                                        bool) {
     const double* q = a + (long long)j * P * pitch + col0;
 #pragma unroll
     for (int l = 0; l < P; ++l)
 #pragma unroll
-        for (int k = 0; k < P; ++k) c.v[l][k] = zero ? 0.0 : __ldg(q + l * pitch + k);
+        for (int k = 0; k < P; ++k) c.v[l][k] = __ldg(q + l * pitch + k);
 }
 
 // L1 prefetch of one cell (the first element of each of its P rows; a lane's P doubles span at most two 32-byte

@@ -266,33 +266,47 @@ fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* o, double* v
     return FX_OK;
 }
 
+// Launch shape of the warp-strip kernels.  A warp = one strip of 30 cells x `rows_per_seg` cell rows; every segment pays
+// a prologue of about 0.6 steps (the flux trace of the row below it).  Choose rows_per_seg to minimise
+// waves * (rows_per_seg + 0.6), waves = ceil(warps / resident warps): whole waves, little redundant work, and for small
+// grids as many warps as there are rows.
+void fx_dg_shape(FxCtx* c, const fx_grid* g, DgParams* p, int* grid, int* block) {
+    int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
+    if (wpb > 4) wpb = 4;                       // the kernels are compiled for <= 128 threads per CTA
+    p->nstrip = (g->Nx + FX_STRIP - 1) / FX_STRIP;
+    int rps = c->launch[2][0];
+    if (rps <= 0) {
+        const long long resident = (long long)c->num_sms * 12;      // 3 CTAs x 4 warps per SM (168 registers per thread)
+        double best = 1e300;
+        rps = 1;
+        for (int r = 1; r <= g->Ny; ++r) {
+            const long long warps = (long long)p->nstrip * ((g->Ny + r - 1) / r);
+            const double cost = (double)((warps + resident - 1) / resident) * (r + 0.6);
+            if (cost <= best) { best = cost; rps = r; }
+            if (warps <= resident && r >= 2) break;                   // one wave: larger segments only cost more
+        }
+    }
+    if (rps > g->Ny) rps = g->Ny;
+    p->rows_per_seg = rps;
+    p->nseg = (g->Ny + rps - 1) / rps;
+    const long long warps = (long long)p->nstrip * p->nseg;
+    *grid = (int)((warps + wpb - 1) / wpb);
+    *block = wpb * 32;
+}
+
 fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const double* x, double* y, int normed) {
     DgParams p;
     fx_status s = fx_make_dg_params(g, normed, &p, nullptr);
     if (s != FX_OK) return s;
-    int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
-    if (wpb > 4) wpb = 4;                       // the kernels are compiled for <= 128 threads per CTA
-    p.nstrip = (g->Nx + FX_STRIP - 1) / FX_STRIP;
-    // rows per segment: aim at >= 2 waves of 16 warps per SM, but keep the per-segment prologue (one extra cell row) small
-    int rps = c->launch[2][0];
-    if (rps <= 0) {
-        const long long target = (long long)c->num_sms * 32;
-        long long nseg = target / p.nstrip;
-        if (nseg < 1) nseg = 1;
-        rps = (int)((g->Ny + nseg - 1) / nseg);
-        if (rps < 8) rps = 8;
-    }
-    if (rps > g->Ny) rps = g->Ny;
-    p.rows_per_seg = rps;
-    p.nseg = (g->Ny + rps - 1) / rps;
-    const long long warps = (long long)p.nstrip * p.nseg;
-    const int grid = (int)((warps + wpb - 1) / wpb);
+    int grid, block;
+    fx_dg_shape(c, g, &p, &grid, &block);
+    const int wpb = block / 32;
     switch (g->P) {
-    case 1: k_dg_apply<1><<<grid, wpb * 32, 0, c->stream>>>(p, chi, x, y); break;
-    case 2: k_dg_apply<2><<<grid, wpb * 32, 0, c->stream>>>(p, chi, x, y); break;
-    case 3: k_dg_apply<3><<<grid, wpb * 32, 0, c->stream>>>(p, chi, x, y); break;
-    case 4: k_dg_apply<4><<<grid, wpb * 32, 0, c->stream>>>(p, chi, x, y); break;
-    case 5: k_dg_apply<5><<<grid, wpb * 32, 0, c->stream>>>(p, chi, x, y); break;
+    case 1: k_dg_apply<1><<<grid, block, 0, c->stream>>>(p, chi, x, y); break;
+    case 2: k_dg_apply<2><<<grid, block, 0, c->stream>>>(p, chi, x, y); break;
+    case 3: k_dg_apply<3><<<grid, block, 0, c->stream>>>(p, chi, x, y); break;
+    case 4: k_dg_apply<4><<<grid, block, 0, c->stream>>>(p, chi, x, y); break;
+    case 5: k_dg_apply<5><<<grid, block, 0, c->stream>>>(p, chi, x, y); break;
     }
     c->launches++;
     FX_CUDA(cudaGetLastError());

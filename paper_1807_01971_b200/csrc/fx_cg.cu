@@ -29,7 +29,7 @@ typedef ExAcc<CG_K, CG_W> CgAcc;
 
 // ---- K1: apply + dot -----------------------------------------------------------------------------------------
 template <int P>
-__global__ void __launch_bounds__(128, 3) k_cg_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi,
+__global__ void __launch_bounds__(128, (P <= 2 ? 4 : P == 3 ? 3 : 2)) k_cg_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi,
                                                       const double* __restrict__ p, double* __restrict__ q, ExGlobal ex,
                                                       CgScal* sc) {
     if (*(volatile int*)&sc->done) return;
@@ -315,8 +315,8 @@ static fx_status cg_workspace(FxCtx* c, int64_t n) {
     return FX_OK;
 }
 
-static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int* apply_grid, int* apply_block, int* ew_grid, int* ew_block) {
-    fx_dg_shape(c, g, p, apply_grid, apply_block);
+static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int k1_warps_per_sm, int* apply_grid, int* apply_block, int* ew_grid, int* ew_block) {
+    fx_dg_shape(c, g, p, k1_warps_per_sm, apply_grid, apply_block);
     int bd = c->launch[3][1] ? c->launch[3][1] : 256;
     if (bd > 256) bd = 256;
     const int pitch = g->Nx * g->P;
@@ -453,7 +453,13 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
             DgParams dp;
             if ((s = fx_make_dg_params(g, 0, &dp, nullptr)) != FX_OK) return s;
             int ag, ab, eg, eb;
-            cg_shapes(c, g, &dp, &ag, &ab, &eg, &eb);
+            int occb = 0;
+            {
+                const void* f = g->P == 1 ? (const void*)k_cg_apply_dot<1> : g->P == 2 ? (const void*)k_cg_apply_dot<2>
+                              : g->P == 3 ? (const void*)k_cg_apply_dot<3> : g->P == 4 ? (const void*)k_cg_apply_dot<4> : (const void*)k_cg_apply_dot<5>;
+                FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occb, f, 128, 0));
+            }
+            cg_shapes(c, g, &dp, occb > 0 ? occb * 4 : 4, &ag, &ab, &eg, &eb);
             int dgrid;                                   // K3: grid-stride over chunks of CG_U3*eb columns, ~4 waves
             {
                 const long long cpr3 = ((long long)g->Nx * g->P + (long long)eb * CG_U3 - 1) / ((long long)eb * CG_U3);

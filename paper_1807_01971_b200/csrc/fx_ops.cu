@@ -222,7 +222,7 @@ extern "C" fx_status fx_exdot_digits(const double* x, const double* y, int64_t n
 struct NoAcc { template <int U> __device__ void add(const double (&)[U], const double (&)[U], const bool (&)[U], ExShared*) {} };
 
 template <int P>
-__global__ void __launch_bounds__(128, 3) k_dg_apply(const __grid_constant__ DgParams g, const double* __restrict__ chi,
+__global__ void __launch_bounds__(128, (P <= 2 ? 4 : P == 3 ? 3 : 2)) k_dg_apply(const __grid_constant__ DgParams g, const double* __restrict__ chi,
                                                   const double* __restrict__ x, double* __restrict__ y) {
     const int wpb = blockDim.x >> 5;
     const long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
@@ -270,13 +270,13 @@ fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* o, double* v
 // a prologue of about 0.6 steps (the flux trace of the row below it).  Choose rows_per_seg to minimise
 // waves * (rows_per_seg + 0.6), waves = ceil(warps / resident warps): whole waves, little redundant work, and for small
 // grids as many warps as there are rows.
-void fx_dg_shape(FxCtx* c, const fx_grid* g, DgParams* p, int* grid, int* block) {
+void fx_dg_shape(FxCtx* c, const fx_grid* g, DgParams* p, int warps_per_sm, int* grid, int* block) {
     int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
     if (wpb > 4) wpb = 4;                       // the kernels are compiled for <= 128 threads per CTA
     p->nstrip = (g->Nx + FX_STRIP - 1) / FX_STRIP;
     int rps = c->launch[2][0];
     if (rps <= 0) {
-        const long long resident = (long long)c->num_sms * 12;      // 3 CTAs x 4 warps per SM (168 registers per thread)
+        const long long resident = (long long)c->num_sms * (warps_per_sm > 0 ? warps_per_sm : 12);
         double best = 1e300;
         rps = 1;
         for (int r = 1; r <= g->Ny; ++r) {
@@ -298,9 +298,16 @@ fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const d
     DgParams p;
     fx_status s = fx_make_dg_params(g, normed, &p, nullptr);
     if (s != FX_OK) return s;
+    static int occ[FX_PMAX + 1] = {0};                           // resident warps per SM of k_dg_apply<P> (128-thread CTAs)
+    if (!occ[g->P]) {
+        int nb = 0;
+        const void* f = g->P == 1 ? (const void*)k_dg_apply<1> : g->P == 2 ? (const void*)k_dg_apply<2> : g->P == 3 ? (const void*)k_dg_apply<3>
+                      : g->P == 4 ? (const void*)k_dg_apply<4> : (const void*)k_dg_apply<5>;
+        FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, 128, 0));
+        occ[g->P] = nb > 0 ? nb * 4 : 4;
+    }
     int grid, block;
-    fx_dg_shape(c, g, &p, &grid, &block);
-    const int wpb = block / 32;
+    fx_dg_shape(c, g, &p, occ[g->P], &grid, &block);
     switch (g->P) {
     case 1: k_dg_apply<1><<<grid, block, 0, c->stream>>>(p, chi, x, y); break;
     case 2: k_dg_apply<2><<<grid, block, 0, c->stream>>>(p, chi, x, y); break;

@@ -69,35 +69,43 @@ __device__ __forceinline__ void dg_prefetch(const double* __restrict__ a, long l
 #define FF(m) f[m]
 
 // y lines of one cell: flux, flux trace, adjoint; acc_ += cyy * sy.  FIRST: first cell of a Dirichlet direction (T0L).
-// tByp: in = flux trace of the cell below, out = this cell's.
+// tByp: in = flux trace of the cell below, out = this cell's.  The P*P chains of each stage are independent: they are
+// written stage by stage so that the scheduler sees P*P-way instruction-level parallelism.
 template <int P, bool FIRST>
 __device__ __forceinline__ void dg_ylines(const DgParams& g, const DgCell<P>& uc, const DgCell<P>& cc, const double (&tLyn)[P],
                                           double (&tByp)[P], double (&acc_)[P][P]) {
+    double f[P][P];                                                   // f[l][k]
 #pragma unroll
-    for (int k = 0; k < P; ++k) {
-        double f[P];
+    for (int l = 0; l < P; ++l)
 #pragma unroll
-        for (int l = 0; l < P; ++l) {
+        for (int k = 0; k < P; ++k) {
             double a;
 #define UC(m) uc.v[m][k]
 #define CT(m) (FIRST ? g.T0L[l][m] : g.T0[l][m])
             FX_CHAIN(a, CT, UC)
 #undef CT
 #undef UC
-            f[l] = __dmul_rn(cc.v[l][k], __fma_rn(g.B[l], tLyn[k], a));
+            f[l][k] = __dmul_rn(cc.v[l][k], __fma_rn(g.B[l], tLyn[k], a));
         }
-        double tB;
-        FX_CHAIN(tB, CB, FF)
+    double tB[P];
 #pragma unroll
-        for (int l = 0; l < P; ++l) {
+    for (int k = 0; k < P; ++k) {
+#define FK(m) f[m][k]
+        FX_CHAIN(tB[k], CB, FK)
+    }
+#pragma unroll
+    for (int l = 0; l < P; ++l)
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
             double a;
 #define CT(m) (FIRST ? g.T0L[m][l] : g.T0[m][l])
-            FX_CHAIN(a, CT, FF)
+            FX_CHAIN(a, CT, FK)
 #undef CT
             acc_[l][k] = __fma_rn(g.cyy, __fma_rn(g.L[l], tByp[k], a), acc_[l][k]);
         }
-        tByp[k] = tB;
-    }
+#undef FK
+#pragma unroll
+    for (int k = 0; k < P; ++k) tByp[k] = tB[k];
 }
 
 // x lines of one cell.  SEL: this warp contains the first cell of a Dirichlet x direction (lane flag firstx).
@@ -105,9 +113,9 @@ __device__ __forceinline__ void dg_ylines(const DgParams& g, const DgCell<P>& uc
 template <int P, bool SEL>
 __device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc, const DgCell<P>& cc, const double (&tLxr)[P],
                                           bool firstx, bool xghost, double (&acc_)[P][P]) {
+    double f[P][P];                                                   // f[l][k]
 #pragma unroll
-    for (int l = 0; l < P; ++l) {
-        double f[P];
+    for (int l = 0; l < P; ++l)
 #pragma unroll
         for (int k = 0; k < P; ++k) {
             double a;
@@ -116,23 +124,30 @@ __device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc
             FX_CHAIN(a, CT, UC)
 #undef CT
 #undef UC
-            f[k] = __dmul_rn(cc.v[l][k], __fma_rn(g.B[k], tLxr[l], a));
+            f[l][k] = __dmul_rn(cc.v[l][k], __fma_rn(g.B[k], tLxr[l], a));
         }
+    double tBl[P];
+#pragma unroll
+    for (int l = 0; l < P; ++l) {
         double tB;
-        FX_CHAIN(tB, CB, FF)
+#define FL(m) f[l][m]
+        FX_CHAIN(tB, CB, FL)
         if (xghost) tB = 0.0;
-        const double tBl = __shfl_up_sync(0xffffffffu, tB, 1);
+        tBl[l] = __shfl_up_sync(0xffffffffu, tB, 1);
+    }
+#pragma unroll
+    for (int l = 0; l < P; ++l)
 #pragma unroll
         for (int k = 0; k < P; ++k) {
             double a;
 #define CT(m) ((SEL && firstx) ? g.T0L[m][k] : g.T0[m][k])
-            FX_CHAIN(a, CT, FF)
+            FX_CHAIN(a, CT, FL)
 #undef CT
-            double o = __fma_rn(g.cxx, __fma_rn(g.L[k], tBl, a), acc_[l][k]);
+            double o = __fma_rn(g.cxx, __fma_rn(g.L[k], tBl[l], a), acc_[l][k]);
             if (g.normed) o = __dmul_rn(g.V[l][k], o);
             acc_[l][k] = o;
         }
-    }
+#undef FL
 }
 
 // One warp: strip `strip` of 30 cells, cell rows [j0, j1).  FUSE: feed (x, y) pairs of the produced cells into the

@@ -37,8 +37,11 @@ def fit(points, m):
     ls = [(S, t) for S, t in pts if S <= 0.5e6 or 3 * S >= 2 * L2_BYTES]
     n = len(ls)
     sx = sum(S for S, _ in ls); sy = sum(t for _, t in ls); sxx = sum(S * S for S, _ in ls); sxy = sum(S * t for S, t in ls)
-    slope = (n * sxy - sx * sy) / (n * sxx - sx * sx)
-    icpt = (sy - slope * sx) / n
+    if sum(1 for S, _ in ls if 3 * S >= 2 * L2_BYTES) >= 2:
+        slope = (n * sxy - sx * sy) / (n * sxx - sx * sx)
+        icpt = (sy - slope * sx) / n
+    else:                                   # no two sizes beyond L2: a line through the cache bump means nothing
+        slope, icpt = float("nan"), float("nan")
     err = max(abs((Tlat + m * S / B) / t - 1.0) for S, t in pts if not (0.5e6 < S and 3 * S < 2 * L2_BYTES))
     return {"B_GBps": B / 1e9, "B_std_GBps": Bstd / 1e9, "T_lat_us": Tlat * 1e6, "T_lat_times_B_MB": Tlat * B / 1e6,
             "lsq_B_GBps": m / slope / 1e9, "lsq_T_lat_us": icpt * 1e6, "model_max_rel_err_outside_L2_bump": err}
@@ -63,7 +66,7 @@ def main():
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
         for P in Ps:
-            for N in Ns:
+            for N in Ns + ([4096] if (P <= 2 and not args.quick) else []):
                 c = fi.config4(P, N)
                 g = fx.make_grid(**c["grid"])
                 n = g.n

@@ -1,10 +1,10 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line for the driver (contract: task prompt "bench.py" + tier section 4).
 
-A "step" is one pass of the whole hot path = ONE preconditioned-CG iteration (dG apply + exact dot, the two vector
-updates + preconditioner + exact dot, the direction update) on BASELINE.json configs[3]: 1024 x 1024 cells, P = 3
+A "step" is one pass of the whole hot path = ONE preconditioned-CG iteration (direction update + dG apply + exact dot; the two
+vector updates + preconditioner + exact dot) on BASELINE.json configs[3]: 1024 x 1024 cells, P = 3
 (9.4 M fp64 unknowns, 75.5 MB per vector, working set 7 vectors = 528 MB > L2), chi / rho as configs[2].
-value = algorithmic GB/s of the iteration: 12 vector passes x 8 B x n per iteration / device time.
+value = algorithmic GB/s of the iteration: 11 vector passes x 8 B x n per iteration / device time.
 Extra keys report the metric's other parts: exact-dot, dG-apply and axpby GB/s at >= 100 MB vectors.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--quick]
@@ -20,8 +20,8 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-PASSES_FUSED = 12          # vector passes of one fused CG iteration: K1 3, K2 6, K3 3
-METRIC = "CG-iteration algorithmic bandwidth (dG apply + exact dots + vector updates; 12 vector passes x 8 B x n per iteration)"
+PASSES_FUSED = 11          # vector passes of one fused CG iteration: K1 5 (r, p_old, chi -> p, q), K2 6
+METRIC = "CG-iteration algorithmic bandwidth (dG apply + exact dots + vector updates; 11 vector passes x 8 B x n per iteration)"
 UNIT = "GB/s"
 
 
@@ -150,13 +150,12 @@ def run_fx(args):
         peak, peak_src = peaks()
 
         # ---- roofline of the dominant kernel (K1: dG apply fused with the exact dot p.Sp) ------------------------
-        k_ms = {k: prof[k + "_ms"] / K for k in ("k1", "k2", "k3")}
+        k_ms = {k: prof[k + "_ms"] / K for k in ("k1", "k2")}
         dom = max(k_ms, key=k_ms.get)
-        bytes_per_launch = {"k1": 24.0 * n, "k2": 48.0 * n, "k3": 24.0 * n}
+        bytes_per_launch = {"k1": 40.0 * n, "k2": 48.0 * n}
         achieved = bytes_per_launch[dom] / (k_ms[dom] * 1e-3) / 1e9
-        names = {"k1": "k_cg_apply_dot<3> (q = S p fused with exact dot p.q; 24 B/unknown)",
-                 "k2": "k_cg_update<3> (phi,r updates + preconditioner + exact dot r.z; 48 B/unknown)",
-                 "k3": "k_cg_dir<3> (p = z + beta p; 24 B/unknown)"}
+        names = {"k1": "k_cg_dir_apply_dot<3> (p = z + beta p, q = S p, exact dot p.q; reads r, p_old, chi, writes p, q: 40 B/unknown)",
+                 "k2": "k_cg_update_lin<3> (phi,r updates + preconditioner + exact dot r.z; 48 B/unknown)"}
         roofline = {"bound": "hbm", "kernel": names[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
                     "frac": achieved / peak, "peak_source": peak_src, "traffic": None,
                     "frac_of_nominal_8TBs": achieved / 8000.0,
@@ -218,7 +217,7 @@ def run_fx(args):
            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic (seeded; fxinputs.config3: chi = 1+0.5 exp(-r^2/0.5), rho = n-N with 1e-3 uniform noise; stands in for the paper's datasets [58],[59])",
            "config": {"workload": "BASELINE.json configs[3]: dG elliptic PCG, %dx%d cells, P=3, %d fp64 unknowns, DIRxDIR, tol=0, fixed K iterations" % (N, N, n),
-                      "step": "one fused PCG iteration (3 kernels)", "l2": "inputs larger than L2 (7 vectors x %.1f MB)" % (8e-6 * n),
+                      "step": "one fused PCG iteration (2 kernels)", "l2": "inputs larger than L2 (7 vectors x %.1f MB)" % (8e-6 * n),
                       "multi_gpu": "replicas only (north star: one GPU, no sharding)", "algorithmic_bytes_per_step": PASSES_FUSED * 8.0 * n},
            "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
            "cg": {"iterations": int(info.iterations), "status": int(info.status), "rel_residual": info.rel_residual},

@@ -4,11 +4,12 @@
 // Two drivers that produce bit-identical iterates:
 //   * unfused: one kernel per primitive, both dot results visit the host every iteration -- the structure the paper
 //     benchmarks (its GPU dot latency IS that host round trip);
-//   * fused (default; the paper's remedy "fewer calls, fewer passes"): three kernels per iteration
-//       K1  q = S p  and the exact dot p.q accumulated while q is produced      -> alpha = rz / pq   (device)
+//   * fused (default; the paper's remedy "fewer calls, fewer passes"): two kernels per iteration
+//       K1  p = z + beta p formed on the fly from r and the previous p (z = V o r recomputed; p is double-buffered because
+//           neighbouring warps still read the old one), q = S p, and the exact dot p.q accumulated while q is produced
+//           -> alpha = rz / pq   (device)
 //       K2  phi += alpha p;  r -= alpha q;  z = V o r on the fly;  exact dot r.z -> convergence test, beta (device)
-//       K3  p = z + beta p   (z recomputed from r)
-//     12 vector passes instead of 19.  The scalars never leave the device; a `done` flag turns the kernels that
+//     11 vector passes instead of 19.  The scalars never leave the device; a `done` flag turns the kernels that
 //     were enqueued past convergence into no-ops, and the host looks at it once per batch of iterations.
 
 #include <math.h>
@@ -27,16 +28,19 @@ struct CgScal {
 #define CG_W 40
 typedef ExAcc<CG_K, CG_W> CgAcc;
 
-// ---- K1: apply + dot -----------------------------------------------------------------------------------------
+// ---- K1: direction update + apply + dot -------------------------------------------------------------------------
 template <int P>
-__global__ void __launch_bounds__(128, (P <= 2 ? 4 : P == 3 ? 3 : 2)) k_cg_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi,
-                                                      const double* __restrict__ p, double* __restrict__ q, ExGlobal ex,
-                                                      CgScal* sc) {
+__global__ void __launch_bounds__(128, (P <= 2 ? 4 : P == 3 ? 3 : 2))
+k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi, const double* __restrict__ pin,
+                   const double* __restrict__ r, double* __restrict__ pout, double* __restrict__ q, ExGlobal ex, CgScal* sc) {
     if (*(volatile int*)&sc->done) return;
     __shared__ ExShared sh;
     ex_shared_init(&sh);
     CgAcc acc;
     acc.init();
+    // first iteration: p = z was set up by the caller, copy it through; later: p = z + beta p with the beta K2 left.
+    // (sc->iters is bumped by this kernel's own finaliser, which runs after every CTA has started.)
+    const DgSrc src = {pin, r, pout, sc->beta, *(volatile int*)&sc->iters > 0};
     const int wpb = blockDim.x >> 5;
     const long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
     if (w < (long long)g.nstrip * g.nseg) {
@@ -44,7 +48,7 @@ __global__ void __launch_bounds__(128, (P <= 2 ? 4 : P == 3 ? 3 : 2)) k_cg_apply
         const int j0 = seg * g.rows_per_seg;
         int j1 = j0 + g.rows_per_seg;
         if (j1 > g.Ny) j1 = g.Ny;
-        dg_warp_strip<P, true, CgAcc>(g, chi, p, q, strip, j0, j1, &acc, &sh);
+        dg_warp_strip<P, true, true, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh);
     }
     acc.flush(&sh);
     if (ex_block_finish(&sh, ex, 1, 1, &sc->pq) && threadIdx.x == 0) {
@@ -265,42 +269,12 @@ __global__ void __launch_bounds__(256, 3) k_cg_update_lin(const __grid_constant_
     }
 }
 
-// K3: p = z + beta p,  z = V o r.  Two fp64 operations per element: plain coalesced loads, four chunks in flight.
-#define CG_U3 4
-template <int P>
-__global__ void __launch_bounds__(256) k_cg_dir(const __grid_constant__ DgParams g, const double* __restrict__ r, double* p,
-                                                const CgScal* sc) {
-    if (*(volatile const int*)&sc->done) return;
-    const double beta = sc->beta;
-    const int pitch = g.Nx * P, rows = g.Ny * P, bd = blockDim.x;
-    const int cpr = (pitch + CG_U3 * bd - 1) / (CG_U3 * bd);
-    ChunkIter ic;
-    ic.init(blockIdx.x, gridDim.x, cpr);
-    for (; ic.row < rows; ic.next()) {
-        const int l = ic.row % P;
-        const long long base = (long long)ic.row * pitch;
-        double pv[CG_U3], rv[CG_U3];
-        int col[CG_U3];
-#pragma unroll
-        for (int u = 0; u < CG_U3; ++u) {
-            col[u] = ic.cb * (CG_U3 * bd) + u * bd + threadIdx.x;
-            if (col[u] < pitch) { pv[u] = p[base + col[u]]; rv[u] = r[base + col[u]]; }
-        }
-#pragma unroll
-        for (int u = 0; u < CG_U3; ++u)
-            if (col[u] < pitch) {
-                const double z = __dmul_rn(g.V[l][col[u] % P], rv[u]);
-                p[base + col[u]] = __fma_rn(1.0, z, __dmul_rn(beta, pv[u]));    // axpby(1, z, beta, p)
-            }
-    }
-}
-
 // ------------------------------------------------------------------------------------------------------------
 
 static fx_status cg_workspace(FxCtx* c, int64_t n) {
     if (c->cg_cap < n) {
         if (c->cg_vec) { cudaStreamSynchronize(c->stream); cudaFree(c->cg_vec); c->cg_vec = nullptr; c->cg_cap = 0; }
-        if (cudaMalloc(&c->cg_vec, (size_t)7 * n * sizeof(double)) != cudaSuccess) {
+        if (cudaMalloc(&c->cg_vec, (size_t)8 * n * sizeof(double)) != cudaSuccess) {
             fx_set_error("CG work space: %s", cudaGetErrorString(cudaGetLastError())); return FX_ENOMEM;
         }
         c->cg_cap = n;
@@ -329,8 +303,8 @@ static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int k1_warps_per_
 }
 
 template <int P>
-static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, int eg, int eb, int dg, const double* chi, double* phi,
-                                  double* r, double* p, double* q, CgScal* sc, int iters) {
+static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, int eg, int eb, const double* chi, double* phi,
+                                  double* r, double* pbuf0, double* pbuf1, double* q, CgScal* sc, int first_index, int iters) {
     static bool attr_done = false;
     if (!attr_done) {
         FX_CUDA(cudaFuncSetAttribute(k_cg_update<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, FX_STAGES * 4 * CG_U * 256 * 8));
@@ -338,7 +312,7 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, 
         attr_done = true;
     }
     // K2 fast path: 16-byte aligned vectors (the work vectors always are; phi is the caller's)
-    const bool lin = aligned16(phi) && aligned16(r) && aligned16(p) && aligned16(q);
+    const bool lin = aligned16(phi) && aligned16(r) && aligned16(pbuf0) && aligned16(pbuf1) && aligned16(q);
     int lg;
     {
         const long long n = (long long)dp.Nx * dp.Ny * P * P, tile = 2ll * eb;
@@ -348,17 +322,19 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, 
         lg = (int)nt;
     }
     for (int i = 0; i < iters; ++i) {
+        // p is double-buffered: iteration k reads buffer k & 1 and writes the other one
+        const int k = first_index + i;
+        const double* pin = (k & 1) ? pbuf1 : pbuf0;
+        double* pout = (k & 1) ? pbuf0 : pbuf1;
         cudaEvent_t* ev = nullptr;
         if (c->prof_on && c->prof_iters < c->prof_cap) { ev = c->prof_ev + 4 * c->prof_iters; c->prof_iters++; }
         if (ev) cudaEventRecord(ev[0], c->stream);
-        k_cg_apply_dot<P><<<ag, ab, 0, c->stream>>>(dp, chi, p, q, c->ex, sc);
+        k_cg_dir_apply_dot<P><<<ag, ab, 0, c->stream>>>(dp, chi, pin, r, pout, q, c->ex, sc);
         if (ev) cudaEventRecord(ev[1], c->stream);
-        if (lin) k_cg_update_lin<P><<<lg, eb, (size_t)FX_STAGES * 4 * 2 * eb * 8, c->stream>>>(dp, p, q, phi, r, c->ex, sc);
-        else k_cg_update<P><<<eg, eb, (size_t)FX_STAGES * 4 * CG_U * eb * 8, c->stream>>>(dp, p, q, phi, r, c->ex, sc);
-        if (ev) cudaEventRecord(ev[2], c->stream);
-        k_cg_dir<P><<<dg, eb, 0, c->stream>>>(dp, r, p, sc);
-        if (ev) cudaEventRecord(ev[3], c->stream);
-        c->launches += 3;
+        if (lin) k_cg_update_lin<P><<<lg, eb, (size_t)FX_STAGES * 4 * 2 * eb * 8, c->stream>>>(dp, pout, q, phi, r, c->ex, sc);
+        else k_cg_update<P><<<eg, eb, (size_t)FX_STAGES * 4 * CG_U * eb * 8, c->stream>>>(dp, pout, q, phi, r, c->ex, sc);
+        if (ev) { cudaEventRecord(ev[2], c->stream); cudaEventRecord(ev[3], c->stream); }
+        c->launches += 2;
     }
     FX_CUDA(cudaGetLastError());
     return FX_OK;
@@ -409,7 +385,7 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
     const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
     fx_status s = cg_workspace(c, n);
     if (s != FX_OK) return s;
-    double *W = c->cg_vec, *V = W + n, *rhs = V + n, *r = rhs + n, *z = r + n, *p = z + n, *q = p + n;
+    double *W = c->cg_vec, *V = W + n, *rhs = V + n, *r = rhs + n, *z = r + n, *p = z + n, *q = p + n, *p2 = q + n;
     const size_t bytes = (size_t)n * sizeof(double);
 
     // setup with the public primitives (lines before the loop)
@@ -455,19 +431,11 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
             int ag, ab, eg, eb;
             int occb = 0;
             {
-                const void* f = g->P == 1 ? (const void*)k_cg_apply_dot<1> : g->P == 2 ? (const void*)k_cg_apply_dot<2>
-                              : g->P == 3 ? (const void*)k_cg_apply_dot<3> : g->P == 4 ? (const void*)k_cg_apply_dot<4> : (const void*)k_cg_apply_dot<5>;
+                const void* f = g->P == 1 ? (const void*)k_cg_dir_apply_dot<1> : g->P == 2 ? (const void*)k_cg_dir_apply_dot<2>
+                              : g->P == 3 ? (const void*)k_cg_dir_apply_dot<3> : g->P == 4 ? (const void*)k_cg_dir_apply_dot<4> : (const void*)k_cg_dir_apply_dot<5>;
                 FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occb, f, 128, 0));
             }
             cg_shapes(c, g, &dp, occb > 0 ? occb * 4 : 4, &ag, &ab, &eg, &eb);
-            int dgrid;                                   // K3: grid-stride over chunks of CG_U3*eb columns, ~4 waves
-            {
-                const long long cpr3 = ((long long)g->Nx * g->P + (long long)eb * CG_U3 - 1) / ((long long)eb * CG_U3);
-                long long ch = cpr3 * g->Ny * g->P, gm = (long long)c->num_sms * (2048 / eb) * 4;
-                if (ch > gm) ch = gm;
-                if (c->launch[3][0]) ch = c->launch[3][0];
-                dgrid = (int)ch;
-            }
             CgScal* sc = (CgScal*)c->cg_scal;
             CgScal* hs = (CgScal*)c->cg_scal_pinned;
             memset(hs, 0, sizeof(*hs));
@@ -484,11 +452,11 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
                 if (enq < maxit) {
                     const int m = (maxit - enq < batch) ? (maxit - enq) : batch;
                     switch (g->P) {
-                    case 1: s = cg_enqueue_iters<1>(c, dp, ag, ab, eg, eb, dgrid, chi, phi, r, p, q, sc, m); break;
-                    case 2: s = cg_enqueue_iters<2>(c, dp, ag, ab, eg, eb, dgrid, chi, phi, r, p, q, sc, m); break;
-                    case 3: s = cg_enqueue_iters<3>(c, dp, ag, ab, eg, eb, dgrid, chi, phi, r, p, q, sc, m); break;
-                    case 4: s = cg_enqueue_iters<4>(c, dp, ag, ab, eg, eb, dgrid, chi, phi, r, p, q, sc, m); break;
-                    default: s = cg_enqueue_iters<5>(c, dp, ag, ab, eg, eb, dgrid, chi, phi, r, p, q, sc, m); break;
+                    case 1: s = cg_enqueue_iters<1>(c, dp, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
+                    case 2: s = cg_enqueue_iters<2>(c, dp, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
+                    case 3: s = cg_enqueue_iters<3>(c, dp, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
+                    case 4: s = cg_enqueue_iters<4>(c, dp, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
+                    default: s = cg_enqueue_iters<5>(c, dp, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
                     }
                     if (s != FX_OK) return s;
                     enq += m;

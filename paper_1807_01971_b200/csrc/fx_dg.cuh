@@ -56,6 +56,33 @@ __device__ __forceinline__ void dg_prefetch(const double* __restrict__ a, long l
     for (int l = 0; l < P; ++l) asm volatile("prefetch.global.L1 [%0];" ::"l"(q + l * pitch));
 }
 
+// Source of the vector the operator is applied to.  DIRF (the CG's fused direction update): the vector is
+// p_new = fma(1, RN(V*r), RN(beta*p_old)) formed on the fly from r and p_old -- axpby(1, z, beta, p) with z = V o r in
+// the canonical order of DESIGN.md 3.2 -- or p_old itself while upd is false (first iteration: p = z was set up).
+struct DgSrc {
+    const double* x;       // the vector (DIRF: p_old)
+    const double* r;       // DIRF only
+    double* pout;          // DIRF only: where p_new is stored (a different buffer than x: neighbours still read p_old)
+    double beta;
+    bool upd;
+};
+
+template <int P, bool DIRF>
+__device__ __forceinline__ void dg_load_u(DgCell<P>& c, const DgParams& g, const DgSrc& s, long long pitch, int col0, int j) {
+    dg_load<P>(c, s.x, pitch, col0, j, false);
+    if (DIRF) {
+        if (s.upd) {
+            DgCell<P> rr;
+            dg_load<P>(rr, s.r, pitch, col0, j, false);
+#pragma unroll
+            for (int l = 0; l < P; ++l)
+#pragma unroll
+                for (int k = 0; k < P; ++k)
+                    c.v[l][k] = __fma_rn(1.0, __dmul_rn(g.V[l][k], rr.v[l][k]), __dmul_rn(s.beta, c.v[l][k]));
+        }
+    }
+}
+
 // chain over m:  acc = c[0]*v[0]; acc = fma(c[m], v[m], acc)
 #define FX_CHAIN(acc, COEF, VAL)                         \
     {                                                    \
@@ -152,10 +179,10 @@ __device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc
 
 // One warp: strip `strip` of 30 cells, cell rows [j0, j1).  FUSE: feed (x, y) pairs of the produced cells into the
 // exact-dot accumulator `acc` (the CG's p.Sp).
-template <int P, bool FUSE, class ACC>
-__device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* __restrict__ chi,
-                                              const double* __restrict__ x, double* __restrict__ y, int strip, int j0,
-                                              int j1, ACC* acc, ExShared* sh) {
+template <int P, bool FUSE, bool DIRF, class ACC>
+__device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* __restrict__ chi, const DgSrc& src,
+                                              double* __restrict__ y, int strip, int j0, int j1, ACC* acc, ExShared* sh) {
+    const double* __restrict__ x = src.x;
     const int lane = threadIdx.x & 31;
     const int Nx = g.Nx, Ny = g.Ny;
     const long long pitch = (long long)Nx * P;
@@ -175,9 +202,9 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
     double tLy[P], tRyp[P], tByp[P];                               // own bottom trace; previous cell's top / flux trace
 
     // ---- prologue: state of cell row j0-1 ------------------------------------------------------------------
-    dg_load<P>(uc, x, pitch, col0, j0, xghost);
+    dg_load_u<P, DIRF>(uc, g, src, pitch, col0, j0);
     dg_load<P>(cc, chi, pitch, col0, j0, xghost);
-    if (!xghost && j0 + 1 < Ny) dg_prefetch<P>(x, pitch, col0, j0 + 1);
+    if (!xghost && j0 + 1 < Ny) { dg_prefetch<P>(x, pitch, col0, j0 + 1); if (DIRF) dg_prefetch<P>(src.r, pitch, col0, j0 + 1); }
 #pragma unroll
     for (int k = 0; k < P; ++k) {
 #define UC(m) uc.v[m][k]
@@ -190,7 +217,7 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
     } else {
         const int jp = (j0 == 0) ? Ny - 1 : j0 - 1;
         DgCell<P> up, cp;
-        dg_load<P>(up, x, pitch, col0, jp, xghost);
+        dg_load_u<P, DIRF>(up, g, src, pitch, col0, jp);
         dg_load<P>(cp, chi, pitch, col0, jp, xghost);
         double dummy[P][P];
 #pragma unroll
@@ -214,11 +241,11 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
         int jn = j + 1;
         bool yghost = false;
         if (jn == Ny) { jn = 0; yghost = diry; }
-        if (j > j0) { dg_load<P>(uc, x, pitch, col0, j, xghost); dg_load<P>(cc, chi, pitch, col0, j, xghost); }
-        dg_load<P>(un, x, pitch, col0, jn, xghost || yghost);
+        if (j > j0) { dg_load_u<P, DIRF>(uc, g, src, pitch, col0, j); dg_load<P>(cc, chi, pitch, col0, j, xghost); }
+        dg_load_u<P, DIRF>(un, g, src, pitch, col0, jn);
         if (j + 1 < j1 && !xghost) {                                 // next step's rows
             const int j2 = (j + 2 == Ny) ? 0 : j + 2;
-            if (!(j + 2 == Ny && diry)) dg_prefetch<P>(x, pitch, col0, j2);
+            if (!(j + 2 == Ny && diry)) { dg_prefetch<P>(x, pitch, col0, j2); if (DIRF) dg_prefetch<P>(src.r, pitch, col0, j2); }
             dg_prefetch<P>(chi, pitch, col0, j + 1);
         }
 
@@ -265,6 +292,13 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
         if (selx) dg_xlines<P, true>(g, uc, cc, tLxr, firstx, xghost, acc_);
         else dg_xlines<P, false>(g, uc, cc, tLxr, firstx, xghost, acc_);
 
+        if (DIRF && produce) {
+            double* prow = src.pout + (long long)j * P * pitch + col0;
+#pragma unroll
+            for (int l = 0; l < P; ++l)
+#pragma unroll
+                for (int k = 0; k < P; ++k) prow[l * pitch + k] = uc.v[l][k];
+        }
         if (produce) {
             double* yrow = y + (long long)j * P * pitch + col0;
 #pragma unroll

@@ -232,7 +232,8 @@ __global__ void __launch_bounds__(128, (P <= 2 ? 4 : P == 3 ? 3 : 2)) k_dg_apply
     const int j0 = seg * g.rows_per_seg;
     int j1 = j0 + g.rows_per_seg;
     if (j1 > g.Ny) j1 = g.Ny;
-    dg_warp_strip<P, false, NoAcc>(g, chi, x, y, strip, j0, j1, nullptr, nullptr);
+    const DgSrc src = {x, nullptr, nullptr, 0.0, false};
+    dg_warp_strip<P, false, false, NoAcc>(g, chi, src, y, strip, j0, j1, nullptr, nullptr);
 }
 
 int fx_grid_ok(const fx_grid* g) {

@@ -30,7 +30,7 @@ typedef ExAcc<CG_K, CG_W> CgAcc;
 
 // ---- K1: direction update + apply + dot -------------------------------------------------------------------------
 template <int P>
-__global__ void __launch_bounds__(128, (P <= 2 ? 4 : P == 3 ? 3 : 2))
+__global__ void __launch_bounds__(128, (P <= 2 ? 4 : 2))
 k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi, const double* __restrict__ pin,
                    const double* __restrict__ r, double* __restrict__ pout, double* __restrict__ q, ExGlobal ex, CgScal* sc) {
     if (*(volatile int*)&sc->done) return;

@@ -241,7 +241,7 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
         int jn = j + 1;
         bool yghost = false;
         if (jn == Ny) { jn = 0; yghost = diry; }
-        if (j > j0) { dg_load_u<P, DIRF>(uc, g, src, pitch, col0, j); dg_load<P>(cc, chi, pitch, col0, j, xghost); }
+        if (j > j0) { if (!DIRF) dg_load_u<P, DIRF>(uc, g, src, pitch, col0, j); dg_load<P>(cc, chi, pitch, col0, j, xghost); }
         dg_load_u<P, DIRF>(un, g, src, pitch, col0, jn);
         if (j + 1 < j1 && !xghost) {                                 // next step's rows
             const int j2 = (j + 2 == Ny) ? 0 : j + 2;
@@ -317,6 +317,7 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
                 }
             acc->template add<P * P>(xs, ys, act, sh);
         }
+        if (DIRF) uc = un;                                           // formed once per row: carried instead of re-formed
     }
 }
 #undef CL

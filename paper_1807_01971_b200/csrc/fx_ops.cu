@@ -13,6 +13,7 @@
 #define EX_K 4
 #define EX_W 40
 #define EX_U 4
+#define EX_STAGES 4
 
 // Tiles of blockDim.x * EX_U elements, grid-stride; FX_STAGES-1 tiles in flight per thread through cp.async.
 // Shared layout (doubles): [stage][array 0..1][u][thread]   (VEC: [stage][array][u/2][thread] of 16 B)
@@ -77,10 +78,10 @@ __device__ __forceinline__ void exdot_consume(const double* buf, int stage, long
     acc.add<EX_U>(xv, yv, act, sh);
 }
 
-// The kernel.  CTA b takes tiles b, b+G, b+2G, ...; FX_STAGES-1 tiles are in flight per thread.
+// The kernel.  CTA b takes tiles b, b+G, b+2G, ...; EX_STAGES-1 tiles are in flight per thread.
 // Hot loop (16-byte aligned inputs, full tiles): pointer increments only, compile-time stage offsets, no bounds.
 template <bool VEC>
-__global__ void __launch_bounds__(256, 3) k_exdot(const double* __restrict__ x, const double* __restrict__ y, long long n,
+__global__ void __launch_bounds__(256, 2) k_exdot(const double* __restrict__ x, const double* __restrict__ y, long long n,
                                                   ExGlobal g, int first, int last, double* result) {
     extern __shared__ __align__(16) double ex_buf[];
     __shared__ ExShared sh;
@@ -93,7 +94,7 @@ __global__ void __launch_bounds__(256, 3) k_exdot(const double* __restrict__ x, 
     long long tq = blockIdx.x;                                   // next tile to issue
     long long t = blockIdx.x;                                    // next tile to consume
 #pragma unroll
-    for (int s = 0; s < FX_STAGES - 1; ++s) { exdot_issue<VEC>(ex_buf, s, x, y, n, tq * tile, tq < ntiles); tq += gridDim.x; }
+    for (int s = 0; s < EX_STAGES - 1; ++s) { exdot_issue<VEC>(ex_buf, s, x, y, n, tq * tile, tq < ntiles); tq += gridDim.x; }
     int stage = 0;
     if (VEC) {
         // per-thread pointers of the tile to issue; shared slots of this thread
@@ -103,16 +104,21 @@ __global__ void __launch_bounds__(256, 3) k_exdot(const double* __restrict__ x, 
         const unsigned s0 = fx_smem_addr(ex_buf) + 16u * threadIdx.x;
         const unsigned stage_bytes = 2u * EX_U * bd * 8u, arr_bytes = (unsigned)EX_U * bd * 8u, u_bytes = 16u * bd;
         unsigned so = 0;                                             // byte offset of the stage to consume
-        unsigned sqo = (FX_STAGES - 1) * stage_bytes;                // ... and of the stage to fill
-        while (tq < nfull) {                                         // the tile to issue is a full one
+        unsigned sqo = (EX_STAGES - 1) * stage_bytes;                // ... and of the stage to fill
+        // number of hot iterations as a 32-bit down-counter; pointers are kept as opaque induction variables (the
+        // empty asm stops the compiler from re-deriving them from the tile index with 64-bit multiplies every iteration)
+        int hot = tq < nfull ? (int)((nfull - tq + gridDim.x - 1) / gridDim.x) : 0;
+        tq += (long long)hot * gridDim.x; t += (long long)hot * gridDim.x;
+        for (; hot > 0; --hot) {                                     // the tile to issue is a full one
 #pragma unroll
             for (int u = 0; u < EX_U / 2; ++u) {
                 fx_cp_async16_full(s0 + sqo + u * u_bytes, gx + 2 * u * bd);
                 fx_cp_async16_full(s0 + sqo + arr_bytes + u * u_bytes, gy + 2 * u * bd);
             }
             fx_cp_commit();
-            gx += step; gy += step; tq += gridDim.x;
-            fx_cp_wait<FX_STAGES - 1>();
+            gx += step; gy += step;
+            asm volatile("" : "+l"(gx), "+l"(gy));
+            fx_cp_wait<EX_STAGES - 1>();
             double xv[EX_U], yv[EX_U];
 #pragma unroll
             for (int u = 0; u < EX_U / 2; ++u) {
@@ -122,18 +128,17 @@ __global__ void __launch_bounds__(256, 3) k_exdot(const double* __restrict__ x, 
                 xv[2 * u] = a.x; xv[2 * u + 1] = a.y; yv[2 * u] = b.x; yv[2 * u + 1] = b.y;
             }
             acc.add_all<EX_U>(xv, yv, &sh);                          // consumed tile < issued tile: full as well
-            t += gridDim.x;
             sqo = so;
-            so += stage_bytes; if (so == FX_STAGES * stage_bytes) so = 0;
-            if (++stage == FX_STAGES) stage = 0;
+            so += stage_bytes; if (so == EX_STAGES * stage_bytes) so = 0;
+            if (++stage == EX_STAGES) stage = 0;
         }
     }
     for (; t < ntiles; t += gridDim.x) {                                     // generic: tail tiles, unaligned inputs
-        int sq = stage + FX_STAGES - 1; if (sq >= FX_STAGES) sq -= FX_STAGES;
+        int sq = stage + EX_STAGES - 1; if (sq >= EX_STAGES) sq -= EX_STAGES;
         exdot_issue<VEC>(ex_buf, sq, x, y, n, tq * tile, tq < ntiles); tq += gridDim.x;
-        fx_cp_wait<FX_STAGES - 1>();
+        fx_cp_wait<EX_STAGES - 1>();
         exdot_consume<VEC>(ex_buf, stage, n, t * tile, acc, &sh);
-        if (++stage == FX_STAGES) stage = 0;
+        if (++stage == EX_STAGES) stage = 0;
     }
     fx_cp_wait<0>();
     acc.flush(&sh);
@@ -145,19 +150,22 @@ fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64
     const bool vec = aligned16(x) && aligned16(y);
     int bd = c->launch[0][1] ? c->launch[0][1] : 256;
     if (bd > 256) bd = 256;                     // compiled for <= 256 threads per CTA
+    const size_t smem = (size_t)EX_STAGES * 2 * EX_U * bd * sizeof(double);
+    static bool attr_done = false;
+    static int occ_cache[9] = {0};              // resident CTAs per SM by block size / 32
+    if (!attr_done) {
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_STAGES * 2 * EX_U * 256 * 8));
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_STAGES * 2 * EX_U * 256 * 8));
+        attr_done = true;
+    }
+    int& occ = occ_cache[bd / 32];
+    if (!occ && (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_exdot<true>, bd, smem) != cudaSuccess || occ < 1)) occ = 1;
     const long long tile = (long long)bd * EX_U;
     long long grid = (m + tile - 1) / tile;
-    const long long gmax = (long long)c->num_sms * (768 / bd);      // one resident wave: every CTA pays one flush + merge
+    const long long gmax = (long long)c->num_sms * occ;             // one resident wave: every CTA pays one flush + merge
     if (grid > gmax) grid = gmax;
     if (grid < 1) grid = 1;
     if (c->launch[0][0]) grid = c->launch[0][0];
-    const size_t smem = (size_t)FX_STAGES * 2 * EX_U * bd * sizeof(double);
-    static bool attr_done = false;
-    if (!attr_done) {
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, FX_STAGES * 2 * EX_U * 256 * 8));
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, FX_STAGES * 2 * EX_U * 256 * 8));
-        attr_done = true;
-    }
     if (vec) k_exdot<true><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
     else k_exdot<false><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
     c->launches++;

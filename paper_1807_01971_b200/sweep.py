@@ -33,11 +33,11 @@ def fit(points, m):
     Bstd = math.sqrt(sum((b - B) ** 2 for b in bw) / len(bw))
     small = pts[:3]
     Tlat = max(0.0, min(t - m * S / B for S, t in small))
-    # least squares of t = a + S*m/Bfit over points outside the cache bump (tiny sizes and sizes with 3 vectors > L2)
-    ls = [(S, t) for S, t in pts if S <= 0.5e6 or 3 * S >= 2 * L2_BYTES]
+    # least squares of t = a + S*m/Bfit over points outside the cache bump (tiny sizes and sizes with 3 vectors >= 1.5 x L2)
+    ls = [(S, t) for S, t in pts if S <= 0.5e6 or 3 * S >= 1.5 * L2_BYTES]
     n = len(ls)
     sx = sum(S for S, _ in ls); sy = sum(t for _, t in ls); sxx = sum(S * S for S, _ in ls); sxy = sum(S * t for S, t in ls)
-    if sum(1 for S, _ in ls if 3 * S >= 2 * L2_BYTES) >= 2:
+    if sum(1 for S, _ in ls if 3 * S >= 1.5 * L2_BYTES) >= 2:
         slope = (n * sxy - sx * sy) / (n * sxx - sx * sx)
         icpt = (sy - slope * sx) / n
     else:                                   # no two sizes beyond L2: a line through the cache bump means nothing

@@ -108,7 +108,7 @@ def set_launch(kernel_id, grid_dim=0, block_dim=0):
 
 
 def set_cg_fused(fused):
-    _check(lib().fx_set_cg_fused(int(bool(fused))), "fx_set_cg_fused")
+    _check(lib().fx_set_cg_fused(int(fused)), "fx_set_cg_fused")
 
 
 def launch_count():

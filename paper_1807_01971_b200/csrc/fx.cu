@@ -67,7 +67,12 @@ extern "C" fx_status fx_set_launch(int32_t id, int32_t grid_dim, int32_t block_d
     g_ctx.launch[id][0] = grid_dim; g_ctx.launch[id][1] = block_dim;
     return FX_OK;
 }
-extern "C" fx_status fx_set_cg_fused(int32_t fused) { g_ctx.cg_fused = fused ? 1 : 0; if (!g_ctx.ready) fx_ctx(); g_ctx.cg_fused = fused ? 1 : 0; return FX_OK; }
+extern "C" fx_status fx_set_cg_fused(int32_t fused) {
+    if (fused < 0 || fused > 3) { fx_set_error("fx_set_cg_fused: mode must be 0..3"); return FX_EINVAL; }
+    if (!g_ctx.ready && !fx_ctx()) return FX_ECUDA;
+    g_ctx.cg_fused = fused;
+    return FX_OK;
+}
 extern "C" int64_t fx_launch_count(void) { return g_ctx.launches; }
 
 extern "C" void fx_shutdown(void) {
@@ -77,6 +82,7 @@ extern "C" void fx_shutdown(void) {
     cudaFree(c->ex.dig); cudaFree(c->result_dev); cudaFreeHost(c->result_pinned);
     if (c->cg_vec) cudaFree(c->cg_vec);
     if (c->cg_scal) cudaFree(c->cg_scal);
+    if (c->cg_pdig) cudaFree(c->cg_pdig);
     if (c->cg_scal_pinned) cudaFreeHost(c->cg_scal_pinned);
     for (int i = 0; i < 4; ++i) if (c->stage[i]) cudaFree(c->stage[i]);
     if (c->copy_stream) { cudaStreamDestroy(c->copy_stream); for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_copy[i]); cudaEventDestroy(c->ev_comp[i]); } }

@@ -16,8 +16,12 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <cooperative_groups.h>
+
 #include "fx_internal.h"
 #include "fx_stream.cuh"
+
+namespace cgr = cooperative_groups;
 
 struct CgScal {
     double rz, pq, alpha, beta, bz, thresh, dot;
@@ -269,6 +273,120 @@ __global__ void __launch_bounds__(256, 3) k_cg_update_lin(const __grid_constant_
     }
 }
 
+// ---- persistent driver for grids that fit in L2 --------------------------------------------------------
+// One cooperative launch runs the whole loop: phase A (= K1) and phase B (= K2) of every iteration are separated by
+// grid-wide exact reductions (ex_grid_reduce: one grid.sync each, every CTA rounds the merged digits itself), the
+// scalars live in registers, nothing returns to the host until convergence.  Per iteration: two grid syncs instead of two
+// launches, two single-pass tails and their gaps.  The arithmetic, and therefore every bit of the result, is unchanged.
+// Digit buffers: pdig[0..1] for p.q of even/odd iterations, pdig[2..3] for r.z; CTA 0 re-zeroes the buffer of the next
+// iteration one phase after its last reader has passed a grid sync.
+template <int P>
+__global__ void __launch_bounds__(128, 2)
+k_cg_persistent(const __grid_constant__ DgParams g, const double* __restrict__ chi, double* r, double* p0, double* p1, double* q,
+                double* phi, fx_u64* pdig, int* pflags, CgScal* sc, int maxit) {
+    cgr::grid_group grid = cgr::this_grid();
+    __shared__ ExShared sh;
+    const unsigned pitch = (unsigned)(g.Nx * P);
+    const unsigned n = pitch * (unsigned)(g.Ny * P);                 // the host takes this path only for n < 2^24
+    const double thresh = sc->thresh;
+    double rz = sc->rz, beta = 0.0;
+    int status = FX_MAXIT, it;
+    const int wpb = blockDim.x >> 5;
+    const long long gw = (long long)blockIdx.x * wpb + (threadIdx.x >> 5), tw = (long long)gridDim.x * wpb;
+    const long long nwork = (long long)g.nstrip * g.nseg;
+    const unsigned tile = blockDim.x * 2u, ntiles = (n + tile - 1) / tile;
+    for (it = 1; it <= maxit; ++it) {
+        const int k = it - 1;
+        const double* pin = (k & 1) ? p1 : p0;
+        double* pout = (k & 1) ? p0 : p1;
+        // ---- phase A: p = z + beta p, q = S p, exact dot p.q ---------------------------------------------------------
+        ex_shared_init(&sh);
+        CgAcc acc;
+        acc.init();
+        {
+            const DgSrc src = {pin, r, pout, beta, k > 0};
+            for (long long w = gw; w < nwork; w += tw) {
+                const int seg = (int)(w / g.nstrip), strip = (int)(w % g.nstrip);
+                const int j0 = seg * g.rows_per_seg;
+                int j1 = j0 + g.rows_per_seg;
+                if (j1 > g.Ny) j1 = g.Ny;
+                dg_warp_strip<P, true, true, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh);
+            }
+        }
+        acc.flush(&sh);
+        const double pq = ex_grid_reduce(&sh, pdig + (size_t)(k & 1) * FX_NDIG, pflags + (k & 1), grid);
+        if (blockIdx.x == 0) {
+            for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) pdig[(size_t)((k + 1) & 1) * FX_NDIG + i] = 0ull;
+            if (threadIdx.x == 0) pflags[(k + 1) & 1] = 0;
+        }
+        if (!(pq > 0.0) || isinf(pq)) { status = FX_EBREAKDOWN; break; }
+        const double alpha = __ddiv_rn(rz, pq), nalpha = -alpha;
+        // ---- phase B: phi += alpha p, r -= alpha q, z = V o r, exact dot r.z -----------------------------------------
+        ex_shared_init(&sh);
+        acc.init();
+        for (unsigned t = blockIdx.x; t < ntiles; t += gridDim.x) {
+            double rr[2], zz[2];
+            bool act[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const unsigned e = t * tile + u * blockDim.x + threadIdx.x;
+                act[u] = e < n;
+                rr[u] = 0.0; zz[u] = 0.0;
+                if (act[u]) {
+                    const unsigned row = e / pitch, col = e - row * pitch;
+                    phi[e] = __fma_rn(alpha, pout[e], phi[e]);
+                    const double rn = __fma_rn(nalpha, q[e], r[e]);
+                    r[e] = rn;
+                    rr[u] = rn; zz[u] = __dmul_rn(g.V[row % P][col % P], rn);
+                }
+            }
+            acc.add<2>(rr, zz, act, &sh);
+        }
+        acc.flush(&sh);
+        const double rzn = ex_grid_reduce(&sh, pdig + (size_t)(2 + (k & 1)) * FX_NDIG, pflags + 2 + (k & 1), grid);
+        if (blockIdx.x == 0) {
+            for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) pdig[(size_t)(2 + ((k + 1) & 1)) * FX_NDIG + i] = 0ull;
+            if (threadIdx.x == 0) pflags[2 + ((k + 1) & 1)] = 0;
+        }
+        if (__dsqrt_rn(rzn) <= thresh) { rz = rzn; status = FX_OK; break; }
+        beta = __ddiv_rn(rzn, rz);
+        rz = rzn;
+    }
+    if (it > maxit) it = maxit;
+    if (blockIdx.x == 0 && threadIdx.x == 0) { sc->rz = rz; sc->status = status; sc->iters = it; sc->done = 1; }
+}
+
+template <int P>
+static fx_status cg_run_persistent(FxCtx* c, const fx_grid* g, DgParams dp, const double* chi, double* r, double* p0, double* p1, double* q,
+                                   double* phi, CgScal* sc, int maxit, bool* ran) {
+    *ran = false;
+    int coop = 0, occ = 0;
+    FX_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device));
+    if (!coop) return FX_OK;
+    FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_cg_persistent<P>, 128, 0));
+    if (occ < 1) return FX_OK;
+    if (!c->cg_pdig) {
+        if (cudaMalloc(&c->cg_pdig, 4 * FX_NDIG * sizeof(fx_u64) + 64) != cudaSuccess) { fx_set_error("persistent CG scratch: %s", cudaGetErrorString(cudaGetLastError())); return FX_ENOMEM; }
+    }
+    FX_CUDA(cudaMemsetAsync(c->cg_pdig, 0, 4 * FX_NDIG * sizeof(fx_u64) + 64, c->stream));
+    fx_u64* pdig = (fx_u64*)c->cg_pdig;
+    int* pflags = (int*)(pdig + 4 * FX_NDIG);
+    int ag, ab;
+    fx_dg_shape(c, g, &dp, occ * 4, &ag, &ab);
+    // as many CTAs as either phase can use, at most one resident wave (a cooperative launch must be co-resident)
+    const long long n = (long long)g->Nx * g->Ny * g->P * g->P;
+    long long want = ((long long)dp.nstrip * dp.nseg + 3) / 4, wantB = (n + 255) / 256;
+    if (wantB > want) want = wantB;
+    long long grid = (long long)c->num_sms * occ;
+    if (want < grid) grid = want;
+    if (grid < 1) grid = 1;
+    void* args[] = {&dp, &chi, &r, &p0, &p1, &q, &phi, &pdig, &pflags, &sc, &maxit};
+    FX_CUDA(cudaLaunchCooperativeKernel((const void*)k_cg_persistent<P>, dim3((unsigned)grid), dim3(128), args, 0, c->stream));
+    c->launches++;
+    *ran = true;
+    return FX_OK;
+}
+
 // ------------------------------------------------------------------------------------------------------------
 
 static fx_status cg_workspace(FxCtx* c, int64_t n) {
@@ -442,12 +560,30 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
             hs->rz = rz; hs->bz = bz; hs->thresh = thresh; hs->status = FX_MAXIT;
             FX_CUDA(cudaMemcpyAsync(sc, hs, sizeof(CgScal), cudaMemcpyHostToDevice, c->stream));
             FX_CUDA(cudaStreamSynchronize(c->stream));           // hs is reused as the read-back buffer
+            // small grids (vectors resident in L2): the whole loop in one cooperative launch.  mode 1 = automatic,
+            // 2 = never, 3 = whenever the device allows it (tests)
+            bool persistent = false;
+            if ((c->cg_fused == 1 && n <= ((int64_t)1 << 21)) || (c->cg_fused == 3 && n < ((int64_t)1 << 24))) {
+                switch (g->P) {
+                case 1: s = cg_run_persistent<1>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
+                case 2: s = cg_run_persistent<2>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
+                case 3: s = cg_run_persistent<3>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
+                case 4: s = cg_run_persistent<4>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
+                default: s = cg_run_persistent<5>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
+                }
+                if (s != FX_OK) return s;
+                if (persistent) {
+                    FX_CUDA(cudaMemcpyAsync(hs, sc, sizeof(CgScal), cudaMemcpyDeviceToHost, c->stream));
+                    FX_CUDA(cudaStreamSynchronize(c->stream));
+                    c->prof_iters = 0;
+                }
+            }
             // batches of iterations; the host looks at the `done` flag of batch b only after batch b+1 is enqueued,
             // so the device never idles while the flag travels
             CgScal* slot[2] = {hs, hs + 1};
             int enq = 0, batch = 8, nb = 0;
-            bool finished = false;
-            c->prof_iters = 0;
+            bool finished = persistent;
+            if (!persistent) c->prof_iters = 0;
             while (!finished) {
                 if (enq < maxit) {
                     const int m = (maxit - enq < batch) ? (maxit - enq) : batch;
@@ -471,7 +607,7 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
                 } else finished = true;
             }
             FX_CUDA(cudaStreamSynchronize(c->stream));
-            hs = slot[(nb - 1) & 1];                                             // state after the last enqueued batch
+            if (!persistent) hs = slot[(nb - 1) & 1];                            // state after the last enqueued batch
             if (c->prof_on) { if ((s = cg_collect_profile(c, hs->iters)) != FX_OK) return s; }
             it = hs->iters; status = hs->status; rz = hs->rz;
         }

@@ -41,6 +41,7 @@ struct ExShared {
     int flags;
     int is_last;
     int dlo, dhi;            // last CTA only: range of non-zero merged digits
+    double res;              // ex_grid_reduce: the rounded value, broadcast to the CTA
 };
 
 struct ExGlobal {            // device scratch of one context
@@ -371,6 +372,53 @@ __device__ __forceinline__ bool ex_block_finish(ExShared* sh, const ExGlobal& g,
     __threadfence();
     __syncthreads();
     return true;
+}
+
+// Thread 0 of a CTA: sh->dig holds merged digits (range dlo..dhi), limbs start from zero -> RN(value).
+__device__ inline double ex_round_digits_shared(ExShared* sh, int flags) {
+    const int la = sh->dhi < 0 ? 0 : (sh->dlo >> 1), lb = sh->dhi < 0 ? 0 : (sh->dhi >> 1);
+    long long carry = 0;
+    int k = la;
+    for (; k < FX_NLIMB; ++k) {
+        if (k > lb && (carry == 0 || carry == -1)) break;
+        long long v = (long long)sh->dig[2 * k] + carry;
+        const fx_u64 lo = (fx_u64)v & 0xffffffffull;
+        carry = v >> 32;
+        v = (long long)sh->dig[2 * k + 1] + carry;
+        const fx_u64 hi = (fx_u64)v & 0xffffffffull;
+        carry = v >> 32;
+        sh->lim[k] = lo | (hi << 32);
+    }
+    int bb = k;
+    if (k < FX_NLIMB) sh->lim[k] = (carry == -1) ? ~0ull : 0ull; else bb = FX_NLIMB - 1;
+    return ex_round(sh->lim, flags, sh->dig, la, bb);
+}
+
+// Grid-wide exact reduction inside a cooperative (persistent) kernel: every CTA adds its digits to gdig, the grid
+// synchronises, and EVERY CTA normalises and rounds the merged digits itself, so that all of them hold the same bits
+// without a second synchronisation.  gdig/gflags must be zero on entry; the caller re-zeroes them one phase later
+// (DESIGN.md 6.5).  `gsync` is cooperative_groups::grid_group::sync.
+template <class GRID>
+__device__ __forceinline__ double ex_grid_reduce(ExShared* sh, fx_u64* gdig, int* gflags, GRID& grid) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) {
+        const fx_u64 v = sh->dig[i];
+        if (v) atomicAdd(&gdig[i], v);
+    }
+    if (threadIdx.x == 0 && sh->flags) atomicOr(gflags, sh->flags);
+    __threadfence();
+    grid.sync();
+    if (threadIdx.x == 0) { sh->dlo = FX_NDIG; sh->dhi = -1; }
+    __syncthreads();
+    for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) {
+        const fx_u64 v = __ldcg(&gdig[i]);
+        sh->dig[i] = v;
+        if (v) { atomicMin(&sh->dlo, i); atomicMax(&sh->dhi, i); }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) sh->res = ex_round_digits_shared(sh, __ldcg(gflags));
+    __syncthreads();
+    return sh->res;
 }
 
 #endif

@@ -46,7 +46,7 @@ def _default_launch(fx):
     yield
     for k in range(4):
         fx.set_launch(k, 0, 0)
-    fx.set_cg_fused(True)
+    fx.set_cg_fused(1)
 
 
 # ---- exact dot ----------------------------------------------------------------------------------------------------
@@ -298,14 +298,17 @@ def test_cg_reproducible_across_runs_drivers_and_shapes(fx):
     for _ in range(2):
         got, info = _solve(fx, c)
         assert same_bits(got, ref) and info.iterations == info0.iterations
-    fx.set_cg_fused(False)
-    got, info = _solve(fx, c)
-    assert same_bits(got, ref) and info.iterations == info0.iterations
-    fx.set_cg_fused(True)
+    for mode in (0, 2, 3):          # unfused / two fused kernels per iteration / persistent cooperative kernel
+        fx.set_cg_fused(mode)
+        got, info = _solve(fx, c)
+        assert same_bits(got, ref) and info.iterations == info0.iterations, mode
+    fx.set_cg_fused(2)
     for (rows, ablock, egrid, eblock, dgrid, dblock) in [(1, 32, 1, 32, 1, 32), (5, 128, 37, 512, 300, 64), (100, 1024, 999, 128, 2, 1024)]:
         fx.set_launch(2, rows, ablock); fx.set_launch(3, egrid, eblock); fx.set_launch(0, dgrid, dblock)
-        got, info = _solve(fx, c)
-        assert same_bits(got, ref) and info.iterations == info0.iterations
+        for mode in (2, 3):
+            fx.set_cg_fused(mode)
+            got, info = _solve(fx, c)
+            assert same_bits(got, ref) and info.iterations == info0.iterations, (mode, rows)
 
 
 @pytest.mark.parametrize("P", [1, 2, 4, 5])
@@ -318,7 +321,9 @@ def test_cg_other_orders(fx, oracle, P):
     assert same_bits(got, want)
 
 
-def test_cg_config2_reduced_and_maxit(fx, oracle):
+@pytest.mark.parametrize("mode", [1, 2])
+def test_cg_config2_reduced_and_maxit(fx, oracle, mode):
+    fx.set_cg_fused(mode)
     c = fi.config2(N=48)
     og = oracle.Grid(**c["grid"])
     want, oinfo = oracle.cg_solve(og, c["chi"], c["rho"], c["phi0"], c["tol"], c["maxit"])

@@ -195,6 +195,20 @@ def run_fx(args):
             prim["dg_apply"] = {"grid": "%dx%d P=3" % (N, N), "n": n, "MB_per_vector": 8e-6 * n, "ms": t, "GBps": 24.0 * n / t / 1e6,
                                 "frac_of_peak": 24.0 * n / t / 1e6 / peak, "note": "3 x 75.5 MB partly L2-resident between repeats"}
 
+        # ---- configs[0] and configs[2] in full (small grids: latency-bound; persistent cooperative kernel) ----------------
+        small = {}
+        if rank == 0 and not args.no_primitives and not args.quick:
+            for name, cf in (("config0_64x64_P3_tol1e-10", fi.config0()), ("config2_256x256_P3_tol1e-8", fi.config2())):
+                gs = fx.make_grid(**cf["grid"])
+                c_chi = torch.from_numpy(cf["chi"]).cuda(); c_rho = torch.from_numpy(cf["rho"]).cuda()
+                c_phi = torch.zeros(gs.n, dtype=torch.float64, device="cuda")
+                fx.cg_solve(gs, c_chi, c_rho, c_phi, cf["tol"], 20)
+                c_phi.zero_()
+                s_ev, e_ev = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                s_ev.record(); inf = fx.cg_solve(gs, c_chi, c_rho, c_phi, cf["tol"], cf["maxit"]); e_ev.record(); torch.cuda.synchronize()
+                small[name] = {"iterations": int(inf.iterations), "status": int(inf.status), "rel_residual": inf.rel_residual,
+                               "ms_total_incl_setup": s_ev.elapsed_time(e_ev), "us_per_iteration": 1e3 * s_ev.elapsed_time(e_ev) / max(1, inf.iterations)}
+
         # ---- e2e: the public host-buffer call; H2D of chi, rho, phi0 and D2H of phi inside the timed region -------
         hchi = torch.from_numpy(cfg["chi"]).pin_memory(); hrho = torch.from_numpy(cfg["rho"]).pin_memory()
         hphi = torch.zeros(n, dtype=torch.float64).pin_memory()
@@ -221,7 +235,7 @@ def run_fx(args):
                       "multi_gpu": "replicas only (north star: one GPU, no sharding)", "algorithmic_bytes_per_step": PASSES_FUSED * 8.0 * n},
            "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
            "cg": {"iterations": int(info.iterations), "status": int(info.status), "rel_residual": info.rel_residual},
-           "primitives": prim}
+           "primitives": prim, "small_grid_solves": small}
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
             out["cpu_baseline"] = cpu_baseline(cfg, n, quick=args.quick)

@@ -137,6 +137,24 @@ def test_exdot_async_and_host(fx, oracle):
     assert fbits(fx.exdot_host(torch.from_numpy(x).pin_memory(), torch.from_numpy(y).pin_memory())) == fbits(want)
 
 
+def test_exdot_multi_launch_and_host_chunks(fx, oracle):
+    """n > 2^28 is accumulated over two launches (limbs carried between them); fx_exdot_host streams 2^23-element chunks"""
+    import torch
+    n = (1 << 28) + 12345
+    x, y = fi.uniform(33, n), fi.uniform(34, n)
+    x[::1000003] *= 1e30
+    want, limbs, flags = oracle.exdot_digits(x, y)
+    got, glimbs, gflags = fx.exdot_digits(dev(x), dev(y))
+    assert fbits(got) == fbits(want) and np.array_equal(glimbs, limbs) and np.array_equal(gflags, flags)
+    m = (1 << 24) + 77                                            # three host chunks, ragged tail
+    assert fbits(fx.exdot_host(x[:m], y[:m])) == fbits(oracle.exdot(x[:m], y[:m]))
+    # a negative total: the sign fill of the upper limbs after the first launch must survive the second one
+    xn = -np.abs(x[: (1 << 28) + 5]); yn = np.abs(y[: (1 << 28) + 5])
+    want, limbs, _ = oracle.exdot_digits(xn, yn)
+    got, glimbs, _ = fx.exdot_digits(dev(xn), dev(yn))
+    assert fbits(got) == fbits(want) and np.array_equal(glimbs, limbs)
+
+
 @pytest.mark.parametrize("ci", [0, 3, 5])
 def test_exdot_full_size_config1(fx, oracle, ci):
     """n = 2^27 (the largest size of config 1, the launch configuration bench.py times)"""
@@ -374,6 +392,46 @@ def test_cg_full_size_config3_first_iterations(fx, oracle):
     got, info = _solve(fx, c, tol=0.0, maxit=6)
     assert info.iterations == oinfo.iterations == 6 and info.status == 1
     assert same_bits(got, want)
+
+
+@pytest.mark.parametrize("mode", [0, 2, 3])
+def test_cg_breakdown_and_maxit0(fx, oracle, mode):
+    """an indefinite operator (chi < 0) must stop with FX_EBREAKDOWN at the same iteration as the oracle; maxit = 0"""
+    fx.set_cg_fused(mode)
+    c = fi.config0(N=8)
+    og, g = oracle.Grid(**c["grid"]), fx.make_grid(**c["grid"])
+    chi = -c["chi"]
+    want, oinfo = oracle.cg_solve(og, chi, c["rho"], c["phi0"], 1e-10, 50)
+    assert oinfo.status == oracle.EBREAKDOWN
+    phi = dev(c["phi0"])
+    with pytest.raises(fx.FxError):
+        fx.cg_solve(g, dev(chi), dev(c["rho"]), phi, 1e-10, 50)
+    info = fx.CGInfo()
+    rc = fx.lib().fx_cg_solve(__import__("ctypes").byref(g), dev(chi).data_ptr(), dev(c["rho"]).data_ptr(), phi.zero_().data_ptr(), 1e-10, 50,
+                              __import__("ctypes").byref(info))
+    assert rc == fx.EBREAKDOWN and info.status == fx.EBREAKDOWN and info.iterations == oinfo.iterations
+    phi = dev(c["phi0"])
+    info = fx.cg_solve(g, dev(c["chi"]), dev(c["rho"]), phi, 1e-10, 0)
+    want, oinfo = oracle.cg_solve(og, c["chi"], c["rho"], c["phi0"], 1e-10, 0)
+    assert info.iterations == oinfo.iterations == 0 and info.status == oinfo.status == 1 and same_bits(phi.cpu().numpy(), want)
+
+
+def test_argument_errors(fx):
+    import ctypes
+    import torch
+    L = fx.lib()
+    x = torch.zeros(8, dtype=torch.float64, device="cuda")
+    assert L.fx_axpby(1.0, x.data_ptr(), 1.0, x.data_ptr(), -1) == fx.EINVAL
+    assert L.fx_axpby(1.0, None, 1.0, x.data_ptr(), 8) == fx.EINVAL
+    assert L.fx_axpby(1.0, None, 1.0, None, 0) == fx.OK                       # n == 0 is valid
+    assert L.fx_pointwise_dot(1.0, x.data_ptr(), None, 0.0, x.data_ptr(), 8) == fx.EINVAL
+    assert math.isnan(L.fx_exdot(None, x.data_ptr(), 8)) and b"bad arguments" in L.fx_last_error()
+    g = fx.make_grid(2, 2, 1, 1.0, -1.0, 0, 1)
+    assert L.fx_dg_weights(ctypes.byref(g), x.data_ptr(), None) == fx.EINVAL
+    g = fx.make_grid(2, 2, 1, 1.0, 1.0, 0, 7)
+    assert L.fx_cg_solve(ctypes.byref(g), x.data_ptr(), x.data_ptr(), x.data_ptr(), 1e-8, 10, None) == fx.EINVAL
+    assert L.fx_set_launch(9, 0, 0) == fx.EINVAL and L.fx_set_launch(0, 0, 33) == fx.EINVAL and L.fx_set_cg_fused(7) == fx.EINVAL
+    assert fx.exdot(x[:0], x[:0]) == 0.0 and math.copysign(1.0, fx.exdot(x[:0], x[:0])) == 1.0
 
 
 def test_cg_host_entry(fx, oracle):

@@ -155,7 +155,7 @@ def run_fx(args):
         bytes_per_launch = {"k1": 40.0 * n, "k2": 48.0 * n}
         achieved = bytes_per_launch[dom] / (k_ms[dom] * 1e-3) / 1e9
         names = {"k1": "k_cg_dir_apply_dot<3> (p = z + beta p, q = S p, exact dot p.q; reads r, p_old, chi, writes p, q: 40 B/unknown)",
-                 "k2": "k_cg_update_lin<3> (phi,r updates + preconditioner + exact dot r.z; 48 B/unknown)"}
+                 "k2": "k_cg_update_tma<3> (phi,r updates + preconditioner + exact dot r.z; 48 B/unknown)"}
         roofline = {"bound": "hbm", "kernel": names[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
                     "frac": achieved / peak, "peak_source": peak_src, "traffic": None,
                     "frac_of_nominal_8TBs": achieved / 8000.0,

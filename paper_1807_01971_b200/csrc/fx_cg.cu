@@ -151,8 +151,8 @@ __global__ void __launch_bounds__(256, 3) k_cg_update(const __grid_constant__ Dg
 }
 
 // K2, fast path: all four vectors 16-byte aligned.  Linear tiles of 2*blockDim.x elements, one 16-byte vector per thread,
-// array and tile, FX_STAGES-1 tiles in flight through cp.async (as k_exdot).  The table indices l = row % P, k = col % P
-// of a thread's elements are advanced incrementally from tile to tile (no division in the loop).
+// array and tile.  The table indices l = row % P, k = col % P of a thread's elements are advanced incrementally from tile
+// to tile (no division in the loop).
 template <int P>
 __device__ __forceinline__ void cg_update_pair(const DgParams& g, double alpha, double nalpha, int l, int k, int col, int pitch,
                                                const double2& pv, const double2& qv, const double2& fv, const double2& rv,
@@ -165,106 +165,96 @@ __device__ __forceinline__ void cg_update_pair(const DgParams& g, double alpha, 
     zz[0] = __dmul_rn(g.V[l][k], ro.x); zz[1] = __dmul_rn(g.V[l1][k1], ro.y);     // pointwise_dot(1, V, r, 0, z)
 }
 
+// The tiles are moved by TMA: one elected thread issues 1-D bulk copies (cp.async.bulk, UBLKCP in SASS) of the four vectors
+// that complete on a `full` mbarrier; the warps release a stage through an `empty` mbarrier.  No per-thread copy
+// instructions: the load/store-unit queue carries only the LDS.128 reads and the two STG.128 writes (the cp.async variant
+// of round 1 stalled on mio_throttle).  K2_STAGES-1 tiles (48 KB) are in flight per CTA, three CTAs per SM.
+#define K2_STAGES 4
 template <int P>
-__global__ void __launch_bounds__(256, 3) k_cg_update_lin(const __grid_constant__ DgParams g, const double* __restrict__ p,
+__global__ void __launch_bounds__(256, 3) k_cg_update_tma(const __grid_constant__ DgParams g, const double* __restrict__ p,
                                                           const double* __restrict__ q, double* phi, double* r, ExGlobal ex,
                                                           CgScal* sc) {
     if (*(volatile int*)&sc->done) return;
-    extern __shared__ __align__(16) double cg_buf[];
+    extern __shared__ __align__(128) double cg_buf[];
     __shared__ ExShared sh;
+    __shared__ __align__(8) unsigned long long bars[2 * K2_STAGES];
     ex_shared_init(&sh);
     CgAcc acc;
     acc.init();
     const double alpha = sc->alpha, nalpha = -alpha;
-    const int pitch = g.Nx * P, bd = blockDim.x;
+    const int pitch = g.Nx * P, bd = blockDim.x, nwarp = bd >> 5;
     const long long n = (long long)pitch * g.Ny * P;
-    const long long tile = 2ll * bd, ntiles = (n + tile - 1) / tile, nfull = n / tile;
-    const unsigned s0 = fx_smem_addr(cg_buf) + 16u * threadIdx.x;
+    const long long tile = 2ll * bd, nfull = n / tile;
     const unsigned arr_bytes = 16u * bd, stage_bytes = 4u * arr_bytes;
-    long long tq = blockIdx.x, t = blockIdx.x;
-    const long long step = (long long)gridDim.x * tile;
-    // prologue (generic issue: zero-fills what lies beyond n)
-#pragma unroll
-    for (int s = 0; s < FX_STAGES - 1; ++s) {
-        if (tq < ntiles) {
-            const long long e0 = tq * tile + 2 * threadIdx.x;
-            const long long left = n - e0;
-            const int bytes = left >= 2 ? 16 : (left == 1 ? 8 : 0);
-            const long long es = bytes ? e0 : 0;
-            fx_cp_async16(s0 + s * stage_bytes, p + es, bytes);
-            fx_cp_async16(s0 + s * stage_bytes + arr_bytes, q + es, bytes);
-            fx_cp_async16(s0 + s * stage_bytes + 2 * arr_bytes, phi + es, bytes);
-            fx_cp_async16(s0 + s * stage_bytes + 3 * arr_bytes, r + es, bytes);
-        }
-        fx_cp_commit();
-        tq += gridDim.x;
+    const unsigned sbase = fx_smem_addr(cg_buf), s0 = sbase + 16u * threadIdx.x;
+    const unsigned full0 = fx_smem_addr(bars), empty0 = full0 + 8u * K2_STAGES;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < K2_STAGES; ++s) { fx_mbar_init(full0 + 8u * s, 1u); fx_mbar_init(empty0 + 8u * s, (unsigned)nwarp); }
+        fx_mbar_fence_init();
     }
-    // incremental (l, k, col) of this thread's first element of the tile to consume
-    long long i0 = t * tile + 2 * threadIdx.x;
+    __syncthreads();
+    // my full tiles: blockIdx.x, +G, ...  (count as a 32-bit number)
+    const int mine = blockIdx.x < nfull ? (int)((nfull - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
+    const long long step = (long long)gridDim.x * tile;
+    auto issue = [&](int i) {                                         // thread 0: tile i of this CTA into stage i % K2_STAGES
+        const int s = i % K2_STAGES;
+        const long long e0 = ((long long)blockIdx.x + (long long)i * gridDim.x) * tile;
+        const unsigned dst = sbase + s * stage_bytes, bar = full0 + 8u * s;
+        fx_mbar_expect_tx(bar, stage_bytes);
+        fx_tma_load_1d(dst, p + e0, arr_bytes, bar);
+        fx_tma_load_1d(dst + arr_bytes, q + e0, arr_bytes, bar);
+        fx_tma_load_1d(dst + 2 * arr_bytes, phi + e0, arr_bytes, bar);
+        fx_tma_load_1d(dst + 3 * arr_bytes, r + e0, arr_bytes, bar);
+    };
+    if (threadIdx.x == 0)
+        for (int i = 0; i < K2_STAGES - 1 && i < mine; ++i) issue(i);
+    long long i0 = (long long)blockIdx.x * tile + 2 * threadIdx.x;
     int col = (int)(i0 % pitch), l = (int)((i0 / pitch) % P), k = col % P;
     const int dcol = (int)(step % pitch), dl = (int)((step / pitch) % P), dk1 = dcol % P, dk2 = ((dcol % P) - (pitch % P) + P) % P;
-    const double* gp = p + tq * tile + 2 * threadIdx.x;
-    const double* gq = q + tq * tile + 2 * threadIdx.x;
-    const double* gf = phi + tq * tile + 2 * threadIdx.x;
-    const double* gr = r + tq * tile + 2 * threadIdx.x;
     double* of = phi + i0;
     double* orr = r + i0;
-    unsigned so = 0, sqo = (FX_STAGES - 1) * stage_bytes;
-    while (tq < nfull) {                                             // hot loop: tile to issue is full => so is the one consumed
-        fx_cp_async16_full(s0 + sqo, gp);
-        fx_cp_async16_full(s0 + sqo + arr_bytes, gq);
-        fx_cp_async16_full(s0 + sqo + 2 * arr_bytes, gf);
-        fx_cp_async16_full(s0 + sqo + 3 * arr_bytes, gr);
-        fx_cp_commit();
-        gp += step; gq += step; gf += step; gr += step; tq += gridDim.x;
-        fx_cp_wait<FX_STAGES - 1>();
+    for (int i = 0; i < mine; ++i) {
+        const int s = i % K2_STAGES, use = i / K2_STAGES;
+        if (threadIdx.x == 0 && i + K2_STAGES - 1 < mine) {          // refill the stage consumed in the previous iteration
+            const int j = i + K2_STAGES - 1, sj = j % K2_STAGES, uj = j / K2_STAGES;
+            if (uj > 0) fx_mbar_wait(empty0 + 8u * sj, (unsigned)((uj - 1) & 1));
+            issue(j);
+        }
+        fx_mbar_wait(full0 + 8u * s, (unsigned)(use & 1));
         double2 pv, qv, fv, rv, fo, ro;
-        fx_lds128(pv, s0 + so); fx_lds128(qv, s0 + so + arr_bytes); fx_lds128(fv, s0 + so + 2 * arr_bytes); fx_lds128(rv, s0 + so + 3 * arr_bytes);
+        const unsigned sa = s0 + s * stage_bytes;
+        fx_lds128(pv, sa); fx_lds128(qv, sa + arr_bytes); fx_lds128(fv, sa + 2 * arr_bytes); fx_lds128(rv, sa + 3 * arr_bytes);
         double rr[2], zz[2];
         cg_update_pair<P>(g, alpha, nalpha, l, k, col, pitch, pv, qv, fv, rv, fo, ro, zz);
+        __syncwarp();
+        if ((threadIdx.x & 31) == 0) fx_mbar_arrive(empty0 + 8u * s);
         *reinterpret_cast<double2*>(of) = fo;
         *reinterpret_cast<double2*>(orr) = ro;
         rr[0] = ro.x; rr[1] = ro.y;
         acc.add_all<2>(rr, zz, &sh);
-        of += step; orr += step; t += gridDim.x;
+        of += step; orr += step;
         col += dcol;
         const bool wrapped = col >= pitch;
         col -= wrapped ? pitch : 0;
         k += wrapped ? dk2 : dk1; k -= (k >= P) ? P : 0;
         l += dl + (wrapped ? 1 : 0); l -= (l >= P) ? P : 0;
-        sqo = so;
-        so += stage_bytes; if (so == FX_STAGES * stage_bytes) so = 0;
     }
-    for (; t < ntiles; t += gridDim.x) {                             // the last FX_STAGES-1 issued tiles and the ragged tail
-        if (tq < ntiles) {
-            const long long e0 = tq * tile + 2 * threadIdx.x;
-            const long long left = n - e0;
-            const int bytes = left >= 2 ? 16 : (left == 1 ? 8 : 0);
-            const long long es = bytes ? e0 : 0;
-            fx_cp_async16(s0 + sqo, p + es, bytes);
-            fx_cp_async16(s0 + sqo + arr_bytes, q + es, bytes);
-            fx_cp_async16(s0 + sqo + 2 * arr_bytes, phi + es, bytes);
-            fx_cp_async16(s0 + sqo + 3 * arr_bytes, r + es, bytes);
-        }
-        fx_cp_commit();
-        tq += gridDim.x;
-        fx_cp_wait<FX_STAGES - 1>();
-        double2 pv, qv, fv, rv, fo, ro;
-        fx_lds128(pv, s0 + so); fx_lds128(qv, s0 + so + arr_bytes); fx_lds128(fv, s0 + so + 2 * arr_bytes); fx_lds128(rv, s0 + so + 3 * arr_bytes);
-        const long long e0 = t * tile + 2 * threadIdx.x;
-        const int c0 = (int)(e0 % pitch), l0 = (int)((e0 / pitch) % P);
-        double rr[2], zz[2];
+    if (nfull * tile < n && (int)(nfull % gridDim.x) == (int)blockIdx.x) {   // the ragged tail tile: plain loads
+        const long long e0 = nfull * tile + 2 * threadIdx.x;
         bool act[2] = {e0 < n, e0 + 1 < n};
-        cg_update_pair<P>(g, alpha, nalpha, l0, c0 % P, c0, pitch, pv, qv, fv, rv, fo, ro, zz);
-        if (act[1]) { *reinterpret_cast<double2*>(phi + e0) = fo; *reinterpret_cast<double2*>(r + e0) = ro; }
-        else if (act[0]) { phi[e0] = fo.x; r[e0] = ro.x; }
-        rr[0] = act[0] ? ro.x : 0.0; rr[1] = act[1] ? ro.y : 0.0;
-        zz[0] = act[0] ? zz[0] : 0.0; zz[1] = act[1] ? zz[1] : 0.0;
+        double rr[2] = {0.0, 0.0}, zz[2] = {0.0, 0.0};
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+            if (act[u]) {
+                const long long e = e0 + u;
+                const int c0 = (int)(e % pitch), l0 = (int)((e / pitch) % P);
+                phi[e] = __fma_rn(alpha, p[e], phi[e]);
+                const double rnw = __fma_rn(nalpha, q[e], r[e]);
+                r[e] = rnw;
+                rr[u] = rnw; zz[u] = __dmul_rn(g.V[l0][c0 % P], rnw);
+            }
         acc.add<2>(rr, zz, act, &sh);
-        sqo = so;
-        so += stage_bytes; if (so == FX_STAGES * stage_bytes) so = 0;
     }
-    fx_cp_wait<0>();
     acc.flush(&sh);
     if (ex_block_finish(&sh, ex, 1, 1, &sc->dot) && threadIdx.x == 0) {
         const double rzn = sc->dot;
@@ -426,7 +416,7 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, 
     static bool attr_done = false;
     if (!attr_done) {
         FX_CUDA(cudaFuncSetAttribute(k_cg_update<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, FX_STAGES * 4 * CG_U * 256 * 8));
-        FX_CUDA(cudaFuncSetAttribute(k_cg_update_lin<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, FX_STAGES * 4 * 2 * 256 * 8));
+        FX_CUDA(cudaFuncSetAttribute(k_cg_update_tma<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, K2_STAGES * 4 * 2 * 256 * 8));
         attr_done = true;
     }
     // K2 fast path: 16-byte aligned vectors (the work vectors always are; phi is the caller's)
@@ -449,7 +439,7 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, 
         if (ev) cudaEventRecord(ev[0], c->stream);
         k_cg_dir_apply_dot<P><<<ag, ab, 0, c->stream>>>(dp, chi, pin, r, pout, q, c->ex, sc);
         if (ev) cudaEventRecord(ev[1], c->stream);
-        if (lin) k_cg_update_lin<P><<<lg, eb, (size_t)FX_STAGES * 4 * 2 * eb * 8, c->stream>>>(dp, pout, q, phi, r, c->ex, sc);
+        if (lin) k_cg_update_tma<P><<<lg, eb, (size_t)K2_STAGES * 4 * 2 * eb * 8, c->stream>>>(dp, pout, q, phi, r, c->ex, sc);
         else k_cg_update<P><<<eg, eb, (size_t)FX_STAGES * 4 * CG_U * eb * 8, c->stream>>>(dp, pout, q, phi, r, c->ex, sc);
         if (ev) { cudaEventRecord(ev[2], c->stream); cudaEventRecord(ev[3], c->stream); }
         c->launches += 2;

@@ -148,6 +148,20 @@ extern "C" double fxo_exdot_digits(const double* x, const double* y, int64_t n, 
     return acc_round(a);
 }
 
+// Weighted dot sum_i x_i w_i y_i ("we also provide a function computing the weighted sum", rounding of the triple
+// product not specified): reading Q14 -- u_i = RN(x_i * w_i) in fp64, then the exact dot of u and y.  w == 1 reduces it
+// to the exact dot.  Exact sum: the exact dot with ones (EXSUM).
+extern "C" double fxo_exdot3(const double* x, const double* w, const double* y, int64_t n) {
+    BigAcc a; acc_clear(a);
+    for (int64_t i = 0; i < n; ++i) { volatile double u = x[i] * w[i]; acc_add_product(a, u, y[i]); }
+    return acc_round(a);
+}
+extern "C" double fxo_exsum(const double* x, int64_t n) {
+    BigAcc a; acc_clear(a);
+    for (int64_t i = 0; i < n; ++i) acc_add_product(a, x[i], 1.0);
+    return acc_round(a);
+}
+
 // round an externally supplied accumulator (used by the "concatenation = integer sum" pin)
 extern "C" double fxo_round_digits(const uint64_t limbs[68]) {
     BigAcc a; acc_clear(a); std::memcpy(a.limb, limbs, sizeof(a.limb));

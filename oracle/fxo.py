@@ -58,6 +58,10 @@ def lib():
         L.fxo_exdot.argtypes = [dp, dp, C.c_int64]
         L.fxo_exdot_digits.restype = C.c_double
         L.fxo_exdot_digits.argtypes = [dp, dp, C.c_int64, C.POINTER(C.c_uint64), C.POINTER(C.c_int32)]
+        L.fxo_exdot3.restype = C.c_double
+        L.fxo_exdot3.argtypes = [dp, dp, dp, C.c_int64]
+        L.fxo_exsum.restype = C.c_double
+        L.fxo_exsum.argtypes = [dp, C.c_int64]
         L.fxo_round_digits.restype = C.c_double
         L.fxo_round_digits.argtypes = [C.POINTER(C.c_uint64)]
         L.fxo_axpby.restype = None
@@ -96,6 +100,18 @@ def exdot(x, y):
     x, y = _f64(x).ravel(), _f64(y).ravel()
     assert x.size == y.size
     return float(lib().fxo_exdot(_p(x), _p(y), x.size))
+
+
+def exdot3(x, w, y):
+    """weighted dot RN(sum RN(x_i*w_i)*y_i) (Q14)"""
+    x, w, y = _f64(x).ravel(), _f64(w).ravel(), _f64(y).ravel()
+    assert x.size == w.size == y.size
+    return float(lib().fxo_exdot3(_p(x), _p(w), _p(y), x.size))
+
+
+def exsum(x):
+    x = _f64(x).ravel()
+    return float(lib().fxo_exsum(_p(x), x.size))
 
 
 def exdot_digits(x, y):

@@ -262,3 +262,34 @@ def test_fig2_integral(oracle):
     assert abs(exact - (math.e ** 2 - 1) ** 2) < 1e-13
     assert abs(val - exact) / exact < float(kv["rel_bound"])
     assert abs(val - exact) / exact > 1e-14          # P=3 quadrature is not exact for exp: a real approximation
+
+
+# ---- weighted dot and exact sum (Q14) -------------------------------------------------
+
+def test_weighted_dot_pins(oracle):
+    import math
+    from fractions import Fraction
+    import fxinputs as fi
+    rng = fi.rng(4242)
+    n = 500
+    # (1) small integers: every product exact, so the result is the correctly rounded exact triple sum
+    x = rng.integers(-1000, 1000, n).astype(float); w = rng.integers(1, 1000, n).astype(float); y = rng.integers(-1000, 1000, n).astype(float)
+    exact = sum(Fraction(a) * Fraction(b) * Fraction(c) for a, b, c in zip(x, w, y))
+    assert oracle.exdot3(x, w, y) == float(exact)
+    # (2) w == 1 reduces to the exact dot; (3) general case: rational brute force of sum RN(x w) y
+    x, y, w = fi.uniform(1, n), fi.uniform(2, n), 0.5 + fi.uniform(3, n) ** 2
+    assert oracle.exdot3(x, np.ones(n), y) == oracle.exdot(x, y)
+    exact = sum(Fraction(float(a * b)) * Fraction(float(c)) for a, b, c in zip(x, w, y))
+    assert oracle.exdot3(x, w, y) == float(exact)
+    # (4) Fig. 2: integral of exp(x)exp(y) on [0,2]^2 as the weighted dot of f_x, volume, f_y
+    g = oracle.Grid(20, 20, 3, 2.0, 2.0, 1, 1)
+    W, _ = oracle.dg_weights(g)
+    xs, ys = oracle.dg_nodes(g)
+    fx_, fy_ = np.exp(np.broadcast_to(xs[None, :], (ys.size, xs.size))).ravel(), np.exp(np.broadcast_to(ys[:, None], (ys.size, xs.size))).ravel()
+    val = oracle.exdot3(fx_, W, fy_)
+    assert abs(val / (math.exp(2.0) - 1.0) ** 2 - 1.0) < 2e-12
+    # (5) exact sum: brute force, permutation invariance, cancellation
+    v = np.ldexp(fi.uniform(5, n), rng.integers(-60, 60, n))
+    assert oracle.exsum(v) == float(sum(Fraction(float(t)) for t in v))
+    assert oracle.exsum(v[::-1].copy()) == oracle.exsum(v)
+    assert oracle.exsum(np.concatenate([v, -v])) == 0.0 and oracle.exsum(np.array([1e308, 1e308, -1e308])) == 1e308

@@ -89,6 +89,12 @@ fx_status fx_exdot_digits(const double* x_dev, const double* y_dev, int64_t n, u
  * chunks on the library stream, accumulates, returns the value.  Synchronises.                                */
 double fx_exdot_host(const double* x_host, const double* y_host, int64_t n);
 
+/* Weighted dot sum_i x[i] w[i] y[i] ("the weighted sum ... where w represents for example the volume form") in
+ * the reading D:Q14: u = RN(x[i]*w[i]) in fp64, then the exactly rounded dot of u and y.  fx_exsum: the exactly rounded
+ * sum of x (EXSUM) = exact dot with ones.  Device pointers, may alias; both synchronise and return the value.      */
+double fx_exdot3(const double* x_dev, const double* w_dev, const double* y_dev, int64_t n);
+double fx_exsum(const double* x_dev, int64_t n);
+
 /* ---- vector primitives in canonical order (D:3.2) ---------------------------------------------- */
 
 /* y[i] <- fma(alpha, x[i], RN(beta*y[i]));  beta == 0: y[i] <- RN(alpha*x[i]) and y is not read.
@@ -131,7 +137,8 @@ fx_status fx_cg_last_profile(double* ms_host, int32_t* iterations_host);
  * launches one primitive `reps` times (after one untimed call) between two CUDA events on the library stream and
  * returns the average milliseconds per call in *ms_host.  kind: 0 = exdot(a,b) result left on the device,
  * 1 = axpby(0.7,a,-0.3,c), 2 = pointwise_dot(1,a,b,0,c), 3 = dG apply_sym(grid; chi=a, x=b, y=c), 4 = dG apply (normed),
- * 5 = exdot(a,b) returned to the host every call (the paper's GPU dot latency), 6 = axpby(0.7,a,1,c).
+ * 5 = exdot(a,b) returned to the host every call (the paper's GPU dot latency), 6 = axpby(0.7,a,1,c),
+ * 7 = weighted dot(a,b,c) device-resident, 8 = exact sum(a) device-resident.
  * a, b, c: device vectors of n doubles (kinds 3,4: n must equal the grid's size).  Synchronises.               */
 fx_status fx_time_primitive(int32_t kind, const fx_grid* grid, const double* a_dev, const double* b_dev, double* c_dev,
                             int64_t n, int32_t reps, double* ms_host);

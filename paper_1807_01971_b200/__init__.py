@@ -47,6 +47,8 @@ _SIGNATURES = {
     "fx_exdot_async": (C.c_int, [_vp, _vp, C.c_int64, _vp]),
     "fx_exdot_digits": (C.c_int, [_vp, _vp, C.c_int64, _vp, _vp, _vp]),
     "fx_exdot_host": (C.c_double, [_vp, _vp, C.c_int64]),
+    "fx_exdot3": (C.c_double, [_vp, _vp, _vp, C.c_int64]),
+    "fx_exsum": (C.c_double, [_vp, C.c_int64]),
     "fx_axpby": (C.c_int, [C.c_double, _vp, C.c_double, _vp, C.c_int64]),
     "fx_pointwise_dot": (C.c_int, [C.c_double, _vp, _vp, C.c_double, _vp, C.c_int64]),
     "fx_dg_elliptic_apply": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp]),
@@ -120,6 +122,25 @@ def exdot(x, y):
     _use_torch_stream()
     n = x.numel()
     v = lib().fx_exdot(_ptr(x), _ptr(y, n), n)
+    if v != v and lib().fx_last_error():
+        raise FxError(lib().fx_last_error().decode())
+    return v
+
+
+def exdot3(x, w, y):
+    """weighted dot RN(sum RN(x_i*w_i)*y_i) (Q14); synchronises"""
+    _use_torch_stream()
+    n = x.numel()
+    v = lib().fx_exdot3(_ptr(x), _ptr(w, n), _ptr(y, n), n)
+    if v != v and lib().fx_last_error():
+        raise FxError(lib().fx_last_error().decode())
+    return v
+
+
+def exsum(x):
+    """exactly rounded sum (EXSUM); synchronises"""
+    _use_torch_stream()
+    v = lib().fx_exsum(_ptr(x), x.numel())
     if v != v and lib().fx_last_error():
         raise FxError(lib().fx_last_error().decode())
     return v
@@ -223,7 +244,7 @@ def cg_solve(grid, chi, rho, phi, tol, maxit):
     return info
 
 
-TIME_KINDS = {"exdot": 0, "axpby": 1, "pointwise_dot": 2, "dg_apply_sym": 3, "dg_apply": 4, "exdot_host": 5, "axpy": 6}
+TIME_KINDS = {"exdot": 0, "axpby": 1, "pointwise_dot": 2, "dg_apply_sym": 3, "dg_apply": 4, "exdot_host": 5, "axpy": 6, "exdot3": 7, "exsum": 8}
 
 
 def time_primitive(kind, a, b, c, reps, grid=None):

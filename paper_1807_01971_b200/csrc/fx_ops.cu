@@ -173,6 +173,111 @@ fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64
     return FX_OK;
 }
 
+// ---- weighted dot (NA = 3: x, w, y) and exact sum (NA = 1) -- SURVEY 8f-3 ---------------------------------------------
+// Same accumulator, same single-pass finaliser; generic cp.async ring (8-byte copies: no alignment requirement).
+template <int NA>
+__global__ void __launch_bounds__(256, 2) k_exdotn(const double* __restrict__ a0, const double* __restrict__ a1,
+                                                   const double* __restrict__ a2, long long n, ExGlobal g, int first, int last,
+                                                   double* result) {
+    extern __shared__ __align__(16) double ex_buf[];
+    __shared__ ExShared sh;
+    ex_shared_init(&sh);
+    ExAcc<EX_K, EX_W> acc;
+    acc.init();
+    const int bd = blockDim.x;
+    const long long tile = (long long)bd * EX_U, ntiles = (n + tile - 1) / tile;
+    const double* arr[3] = {a0, a1, a2};
+    auto issue = [&](int stage, long long t) {
+        double* s0 = ex_buf + (size_t)stage * NA * EX_U * bd;
+        if (t < ntiles) {
+#pragma unroll
+            for (int u = 0; u < EX_U; ++u) {
+                const int slot = u * bd + threadIdx.x;
+                const long long e = t * tile + slot;
+                const bool in = e < n;
+#pragma unroll
+                for (int a = 0; a < NA; ++a) fx_cp_async8(fx_smem_addr(s0 + a * EX_U * bd + slot), arr[a] + (in ? e : 0), in);
+            }
+        }
+        fx_cp_commit();
+    };
+    long long tq = blockIdx.x;
+#pragma unroll
+    for (int s = 0; s < EX_STAGES - 1; ++s) { issue(s, tq); tq += gridDim.x; }
+    int stage = 0;
+    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        int sq = stage + EX_STAGES - 1; if (sq >= EX_STAGES) sq -= EX_STAGES;
+        issue(sq, tq); tq += gridDim.x;
+        fx_cp_wait<EX_STAGES - 1>();
+        const double* s0 = ex_buf + (size_t)stage * NA * EX_U * bd;
+        double xv[EX_U], yv[EX_U];
+        bool act[EX_U];
+#pragma unroll
+        for (int u = 0; u < EX_U; ++u) {
+            const int slot = u * bd + threadIdx.x;
+            act[u] = t * tile + slot < n;
+            if (NA == 3) { xv[u] = __dmul_rn(s0[slot], s0[EX_U * bd + slot]); yv[u] = s0[2 * EX_U * bd + slot]; }   // u = RN(x*w)
+            else { xv[u] = s0[slot]; yv[u] = act[u] ? 1.0 : 0.0; }
+        }
+        acc.add<EX_U>(xv, yv, act, &sh);
+        if (++stage == EX_STAGES) stage = 0;
+    }
+    fx_cp_wait<0>();
+    acc.flush(&sh);
+    ex_block_finish(&sh, g, first, last, result);
+}
+
+template <int NA>
+static fx_status launch_exdotn(FxCtx* c, const double* a0, const double* a1, const double* a2, int64_t n, double* result_dev) {
+    const int bd = 256;
+    const size_t smem = (size_t)EX_STAGES * NA * EX_U * bd * sizeof(double);
+    static bool attr_done = false;
+    static int occ = 0;
+    if (!attr_done) {
+        FX_CUDA(cudaFuncSetAttribute(k_exdotn<NA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_exdotn<NA>, bd, smem) != cudaSuccess || occ < 1) occ = 1;
+        attr_done = true;
+    }
+    const int64_t CHUNK = (int64_t)1 << 28;
+    int64_t done = 0;
+    do {
+        const int64_t m = (n - done < CHUNK) ? (n - done) : CHUNK;
+        const long long tile = (long long)bd * EX_U;
+        long long grid = (m + tile - 1) / tile;
+        if (grid > (long long)c->num_sms * occ) grid = (long long)c->num_sms * occ;
+        if (grid < 1) grid = 1;
+        k_exdotn<NA><<<(int)grid, bd, smem, c->stream>>>(a0 + done, a1 ? a1 + done : nullptr, a2 ? a2 + done : nullptr, m, c->ex, done == 0,
+                                                         done + m == n, result_dev);
+        c->launches++;
+        FX_CUDA(cudaGetLastError());
+        done += m;
+    } while (done < n);
+    return FX_OK;
+}
+
+static double exdotn_sync(FxCtx* c, fx_status s) {
+    if (s != FX_OK) return NAN;
+    if (cudaMemcpyAsync(c->result_pinned, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess) { fx_cuda_fail(cudaGetLastError(), "exact reduction result copy"); return NAN; }
+    return c->result_pinned[0];
+}
+
+extern "C" double fx_exdot3(const double* x, const double* w, const double* y, int64_t n) {
+    if (n < 0 || (n > 0 && (!x || !w || !y))) { fx_set_error("fx_exdot3: bad arguments"); return NAN; }
+    fx_set_error("%s", "");
+    FxCtx* c = fx_ctx();
+    if (!c) return NAN;
+    return exdotn_sync(c, launch_exdotn<3>(c, x, w, y, n, c->result_dev));
+}
+
+extern "C" double fx_exsum(const double* x, int64_t n) {
+    if (n < 0 || (n > 0 && !x)) { fx_set_error("fx_exsum: bad arguments"); return NAN; }
+    fx_set_error("%s", "");
+    FxCtx* c = fx_ctx();
+    if (!c) return NAN;
+    return exdotn_sync(c, launch_exdotn<1>(c, x, nullptr, nullptr, n, c->result_dev));
+}
+
 fx_status fx_launch_exdot(FxCtx* c, const double* x, const double* y, int64_t n, double* result_dev) {
     const int64_t CHUNK = (int64_t)1 << 28;
     int64_t done = 0;
@@ -394,13 +499,15 @@ static fx_status time_one(FxCtx* c, int kind, const fx_grid* g, const double* a,
     case 4: return fx_launch_apply(c, g, a, b, cc, 1);
     case 5: { const double v = fx_exdot(a, b, n); return (v != v && fx_last_error()[0]) ? FX_ECUDA : FX_OK; }
     case 6: return fx_axpby(0.7, a, 1.0, cc, n);
+    case 7: return launch_exdotn<3>(c, a, b, cc, n, c->result_dev);
+    case 8: return launch_exdotn<1>(c, a, nullptr, nullptr, n, c->result_dev);
     }
     return FX_EINVAL;
 }
 
 extern "C" fx_status fx_time_primitive(int32_t kind, const fx_grid* g, const double* a, const double* b, double* cc, int64_t n,
                                        int32_t reps, double* ms_host) {
-    if (kind < 0 || kind > 6 || n < 0 || reps < 1 || !ms_host || !a || !b || !cc) { fx_set_error("fx_time_primitive: bad arguments"); return FX_EINVAL; }
+    if (kind < 0 || kind > 8 || n < 0 || reps < 1 || !ms_host || !a || !b || !cc) { fx_set_error("fx_time_primitive: bad arguments"); return FX_EINVAL; }
     if ((kind == 3 || kind == 4) && (!fx_grid_ok(g) || (int64_t)g->Nx * g->Ny * g->P * g->P != n)) { fx_set_error("fx_time_primitive: bad grid"); return FX_EINVAL; }
     FxCtx* c = fx_ctx();
     if (!c) return FX_ECUDA;

@@ -20,7 +20,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-M_PASSES = {"axpby": 3, "pointwise_dot": 3, "exdot": 2, "exdot_host": 2, "dg_apply_sym": 3, "dg_apply": 3}
+M_PASSES = {"axpby": 3, "pointwise_dot": 3, "exdot": 2, "exdot_host": 2, "exdot3": 3, "exsum": 1, "dg_apply_sym": 3, "dg_apply": 3}
 L2_BYTES = 126e6
 
 
@@ -74,7 +74,7 @@ def main():
                 out = torch.empty_like(x)
                 S = 8.0 * n
                 reps = int(max(10, min(2000, 0.05 / max(2e-6, 3 * S / 5e12))))
-                for kind in ("axpby", "pointwise_dot", "exdot", "exdot_host", "dg_apply_sym", "dg_apply"):
+                for kind in ("axpby", "pointwise_dot", "exdot", "exdot_host", "exdot3", "exsum", "dg_apply_sym", "dg_apply"):
                     if kind.startswith("dg"):
                         ms = fx.time_primitive(kind, chi, x, out, reps, grid=g)
                     elif kind == "axpby":

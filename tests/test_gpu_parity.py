@@ -441,3 +441,38 @@ def test_cg_host_entry(fx, oracle):
     phi = c["phi0"].copy()
     info = fx.cg_solve_host(fx.make_grid(**c["grid"]), c["chi"], c["rho"], phi, 1e-9, 2000)
     assert info.iterations == oinfo.iterations and same_bits(phi, want)
+
+
+# ---- weighted dot and exact sum ----------------------------------------------------
+
+@pytest.mark.parametrize("n", [0, 1, 33, 1025, 100003, (1 << 21) + 3])
+def test_weighted_dot_and_sum(fx, oracle, n):
+    import torch
+    x, y = fi.uniform(101, n), fi.uniform(102, n)
+    w = 0.5 + fi.uniform(103, n) ** 2
+    if n > 100:
+        x[7] = 2.0 ** 600; y[7] = 2.0 ** 500; w[7] = 2.0 ** -300      # products outside the TwoProd range
+        x[11] = 5e-324; y[11] = 3.0
+    dx = dev(x) if n else dev(np.zeros(0))
+    dw = dev(w) if n else dev(np.zeros(0))
+    dy = dev(y) if n else dev(np.zeros(0))
+    assert fbits(fx.exdot3(dx, dw, dy)) == fbits(oracle.exdot3(x, w, y) if n else 0.0)
+    assert fbits(fx.exsum(dx)) == fbits(oracle.exsum(x) if n else 0.0)
+    if n:
+        ones = torch.ones(n, dtype=torch.float64, device="cuda")
+        assert fbits(fx.exdot3(dx, ones, dy)) == fbits(fx.exdot(dx, dy))         # w == 1 reduces to the exact dot
+        assert fbits(fx.exdot3(dx[1:], dw[1:], dy[1:])) == fbits(oracle.exdot3(x[1:], w[1:], y[1:]))   # unaligned
+
+
+def test_weighted_dot_fig2_integral(fx, oracle):
+    """Fig. 2: integral of exp(x) exp(y) over [0,2]^2, P = 3, 20 x 20 cells, as dot(f_x, volume, f_y)"""
+    import torch
+    g = fx.make_grid(20, 20, 3, 2.0, 2.0, 1, 1)
+    W = torch.empty(g.n, dtype=torch.float64, device="cuda")
+    fx.dg_weights(g, W, None)
+    xs, ys = oracle.dg_nodes(oracle.Grid(20, 20, 3, 2.0, 2.0, 1, 1))
+    fxv = np.exp(np.broadcast_to(xs[None, :], (ys.size, xs.size))).ravel()
+    fyv = np.exp(np.broadcast_to(ys[:, None], (ys.size, xs.size))).ravel()
+    val = fx.exdot3(dev(fxv), W, dev(fyv))
+    assert abs(val / (math.exp(2.0) - 1.0) ** 2 - 1.0) < 2e-12
+    assert fbits(val) == fbits(oracle.exdot3(fxv, W.cpu().numpy(), fyv))

@@ -186,6 +186,11 @@ def run_fx(args):
             z = torch.empty_like(x)
             t = time_events(lambda: fx.pointwise_dot(1.0, x, y, 0.0, z), 20, torch)
             prim["pointwise_dot"] = {"n": nd, "ms": t, "GBps": 24.0 * nd / t / 1e6, "frac_of_peak": 24.0 * nd / t / 1e6 / peak}
+            x.copy_(torch.from_numpy(fi.uniform(9001, nd))); z.copy_(torch.from_numpy(fi.uniform(9004, nd)))
+            for kind, m in (("exdot3", 3), ("exsum", 1)):              # weighted dot, exact sum (device-resident result)
+                fx.time_primitive(kind, x, y, z, 3)
+                t = fx.time_primitive(kind, x, y, z, 20)
+                prim[kind] = {"n": nd, "ms": t, "GBps": m * 8.0 * nd / t / 1e6, "frac_of_peak": m * 8.0 * nd / t / 1e6 / peak}
             del x, y, z
             q = torch.empty(n, dtype=torch.float64, device="cuda")
             pvec = torch.from_numpy(fi.uniform(9003, n)).cuda()

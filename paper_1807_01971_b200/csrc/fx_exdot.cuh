@@ -161,7 +161,8 @@ struct ExAcc {
     // pass x = y = 0 (padding); they are not inspected.  ALLACT: every element is active (no selects).
     // Instruction budget per element: 2 + 3K + 3(K-1) fp64 operations and ~5 integer ones; the range
     // test and the below-window test are OR/MAX-reduced over the batch and branch once per batch.
-    template <int U, bool ALLACT>
+    // NOERR: the caller guarantees that every product is exact in fp64 (y = 1: the exact sum), so e = 0 is not carried.
+    template <int U, bool ALLACT, bool NOERR = false>
     __device__ __forceinline__ void add(const double (&x)[U], const double (&y)[U], const bool (&active)[U], ExShared* sh) {
         constexpr unsigned LOS = BE_LO << 20, RANGES = (BE_HI - BE_LO) << 20;
         double p[U], e[U];
@@ -169,7 +170,7 @@ struct ExAcc {
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             p[u] = __dmul_rn(x[u], y[u]);
-            e[u] = __fma_rn(x[u], y[u], -p[u]);                      // TwoProd
+            e[u] = NOERR ? 0.0 : __fma_rn(x[u], y[u], -p[u]);        // TwoProd
             unsigned hp = (unsigned)__double2hiint(p[u]) & 0x7ff00000u;
             if (!ALLACT) hp = active[u] ? hp : LOS;
             const unsigned t = hp - LOS;                             // wraps to huge below the range
@@ -208,7 +209,7 @@ struct ExAcc {
                 S[k] = s;
             }
 #pragma unroll
-            for (int k = 1; k < K; ++k) {                            // |e| < ulp(S[0])/2: bin 0 cannot take any of it
+            for (int k = NOERR ? K : 1; k < K; ++k) {                // |e| < ulp(S[0])/2: bin 0 cannot take any of it
                 const double s = __dadd_rn(S[k], w);
                 const double q = __dsub_rn(s, S[k]);
                 w = __dsub_rn(w, q);

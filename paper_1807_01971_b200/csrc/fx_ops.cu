@@ -219,7 +219,8 @@ __global__ void __launch_bounds__(256, 2) k_exdotn(const double* __restrict__ a0
             if (NA == 3) { xv[u] = __dmul_rn(s0[slot], s0[EX_U * bd + slot]); yv[u] = s0[2 * EX_U * bd + slot]; }   // u = RN(x*w)
             else { xv[u] = s0[slot]; yv[u] = act[u] ? 1.0 : 0.0; }
         }
-        acc.add<EX_U>(xv, yv, act, &sh);
+        if (NA == 1) acc.add<EX_U, false, true>(xv, yv, act, &sh);   // x * 1 is exact: no error term
+        else acc.add<EX_U>(xv, yv, act, &sh);
         if (++stage == EX_STAGES) stage = 0;
     }
     fx_cp_wait<0>();

@@ -525,6 +525,127 @@ extern "C" int fxo_dg_apply_canonical(const fxo_grid* g, const double* chi, cons
 }
 
 // ------------------------------------------------------------------------------------------------
+// 6b. Stand-alone dG derivatives  y <- alpha * M x + beta * y,  M = d/dx or d/dy with forward, backward or
+//     centred flux -- the paper's "dxdy" primitive ("derivatives in x and y", P:321 / Table 3, m = 3).
+//     The paper gives no formulas (refs [21],[12]); reading (Q21): forward = F(N,h,bc) of section 5,
+//     backward = -W^-1 F^T W (its negative W-adjoint), centred = (forward + backward)/2.
+//     Definition: explicit matrices in 113-bit arithmetic.  Canonical fp64 order per line (cell n, node k):
+//        a = chain_m(TT[k][m], u_{n,m});  a = fma(cP[k], tR_{n-1}, a);  a = fma(cN[k], tL_{n+1}, a);  d = RN((2/h) * a)
+//        y = beta == 0 ? RN(alpha*d) : fma(alpha, d, RN(beta*y))
+//     with TT = T (forward), -W^-1 T^T W (backward), their mean (centred); T = T0L in the first cell of a DIR line.
+// ------------------------------------------------------------------------------------------------
+
+struct DTab { double TT[2][PMAX][PMAX], cN[PMAX], cP[PMAX]; };   // [0] interior, [1] first cell of a DIR line
+
+static void make_dtab(int P, int flux, DTab& d) {
+    RefElem e; ref_elem(P, e);
+    for (int v = 0; v < 2; ++v) for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m) {
+        auto T = [&](int a, int b) { q128 t = e.D[a][b] - e.R[a] * e.R[b] / e.w[a]; if (v) t += e.L[a] * e.L[b] / e.w[a]; return t; };
+        q128 f = T(k, m), b = -T(m, k) * e.w[m] / e.w[k];
+        q128 val = flux == 0 ? f : flux == 1 ? b : (f + b) / 2;
+        d.TT[v][k][m] = snap(val);
+    }
+    for (int k = 0; k < P; ++k) {
+        q128 cn = e.R[k] / e.w[k], cp = -e.L[k] / e.w[k];
+        d.cN[k] = flux == 0 ? snap(cn) : flux == 1 ? 0.0 : snap(cn / 2);
+        d.cP[k] = flux == 0 ? 0.0 : flux == 1 ? snap(cp) : snap(cp / 2);
+    }
+}
+
+extern "C" int fxo_dg_dtables(int32_t P, int32_t flux, double* out) {      // TT[0], TT[1] (P*P each), cN, cP
+    if (P < 1 || P > PMAX || flux < 0 || flux > 2) return -1;
+    DTab d; make_dtab(P, flux, d);
+    double* o = out;
+    for (int v = 0; v < 2; ++v) for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m) *o++ = d.TT[v][k][m];
+    for (int k = 0; k < P; ++k) *o++ = d.cN[k];
+    for (int k = 0; k < P; ++k) *o++ = d.cP[k];
+    return 0;
+}
+
+static void dline_canonical(const DTab& d, int P, int N, int bc, double s, const double* u, double* out) {
+    std::vector<double> tL(N + 2), tR(N + 2);
+    Tables t; make_tables(P, t);
+    for (int n = 0; n < N; ++n) {
+        double aL = t.L[0] * u[n * P], aR = t.R[0] * u[n * P];
+        for (int m = 1; m < P; ++m) { aL = std::fma(t.L[m], u[n * P + m], aL); aR = std::fma(t.R[m], u[n * P + m], aR); }
+        tL[n + 1] = aL; tR[n + 1] = aR;
+    }
+    if (bc == BC_PER) { tL[N + 1] = tL[1]; tR[0] = tR[N]; } else { tL[N + 1] = 0; tR[0] = 0; }
+    for (int n = 0; n < N; ++n) {
+        const double (*TT)[PMAX] = d.TT[(n == 0 && bc == BC_DIR) ? 1 : 0];
+        for (int k = 0; k < P; ++k) {
+            double a = TT[k][0] * u[n * P];
+            for (int m = 1; m < P; ++m) a = std::fma(TT[k][m], u[n * P + m], a);
+            a = std::fma(d.cP[k], tR[n], a);
+            a = std::fma(d.cN[k], tL[n + 2], a);
+            out[n * P + k] = s * a;
+        }
+    }
+}
+
+extern "C" int fxo_dg_derivative_canonical(const fxo_grid* g, int32_t dir, int32_t flux, double alpha, const double* x, double beta,
+                                           double* y) {
+    if (!grid_ok(g) || dir < 0 || dir > 1 || flux < 0 || flux > 2 || x == y) return -1;
+    const int P = g->P, nx = g->Nx * P, ny = g->Ny * P;
+    DTab d; make_dtab(P, flux, d);
+    const int N = dir == 0 ? g->Nx : g->Ny, len = N * P, bc = dir == 0 ? g->bcx : g->bcy;
+    const double h = dir == 0 ? g->lx / g->Nx : g->ly / g->Ny, s = 2.0 / h;
+    std::vector<double> u(len), o(len);
+    const int nl = dir == 0 ? ny : nx;
+    for (int line = 0; line < nl; ++line) {
+        for (int a = 0; a < len; ++a) u[a] = dir == 0 ? x[(size_t)line * nx + a] : x[(size_t)a * nx + line];
+        dline_canonical(d, P, N, bc, s, u.data(), o.data());
+        for (int a = 0; a < len; ++a) {
+            size_t id = dir == 0 ? (size_t)line * nx + a : (size_t)a * nx + line;
+            if (beta == 0.0) y[id] = alpha * o[a];
+            else { double t = beta * y[id]; y[id] = std::fma(alpha, o[a], t); }
+        }
+    }
+    return 0;
+}
+
+// definition: explicit matrices, 113 bit; M (rounded to double) is also returned for the numpy-side pins
+extern "C" int fxo_dg_derivative_matrix_1d(int32_t N, int32_t P, double h, int32_t bc, int32_t flux, double* M_out) {
+    if (N < 1 || P < 1 || P > PMAX || !(h > 0) || flux < 0 || flux > 2) return -1;
+    RefElem e; ref_elem(P, e);
+    std::vector<q128> F; build_F(e, N, (q128)h, bc, F);
+    int n = N * P;
+    for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) {
+        q128 f = F[(size_t)a * n + b], bk = -F[(size_t)b * n + a] * e.w[b % P] / e.w[a % P];
+        M_out[(size_t)a * n + b] = (double)(flux == 0 ? f : flux == 1 ? bk : (f + bk) / 2);
+    }
+    return 0;
+}
+
+extern "C" int fxo_dg_derivative_definition(const fxo_grid* g, int32_t dir, int32_t flux, double alpha, const double* x, double beta,
+                                            const double* y_in, double* y_out, double* scale) {
+    if (!grid_ok(g) || dir < 0 || dir > 1 || flux < 0 || flux > 2) return -1;
+    const int P = g->P, nx = g->Nx * P, ny = g->Ny * P;
+    RefElem e; ref_elem(P, e);
+    const int N = dir == 0 ? g->Nx : g->Ny, len = N * P, bc = dir == 0 ? g->bcx : g->bcy;
+    q128 h = dir == 0 ? (q128)g->lx / g->Nx : (q128)g->ly / g->Ny;
+    std::vector<q128> F; build_F(e, N, h, bc, F);
+    auto M = [&](int a, int b) {
+        q128 f = F[(size_t)a * len + b], bk = -F[(size_t)b * len + a] * e.w[b % P] / e.w[a % P];
+        return flux == 0 ? f : flux == 1 ? bk : (f + bk) / 2;
+    };
+    auto qabs = [](q128 v) { return v < 0 ? -v : v; };
+    const int nl = dir == 0 ? ny : nx;
+    for (int line = 0; line < nl; ++line) for (int a = 0; a < len; ++a) {
+        q128 sum = 0, sa = 0;
+        for (int b = 0; b < len; ++b) {
+            q128 m = M(a, b);
+            if (m != 0) { double xv = dir == 0 ? x[(size_t)line * nx + b] : x[(size_t)b * nx + line]; sum += m * xv; sa += qabs(m) * qabs((q128)xv); }
+        }
+        size_t id = dir == 0 ? (size_t)line * nx + a : (size_t)a * nx + line;
+        q128 yv = beta == 0.0 ? (q128)0 : (q128)beta * y_in[id];
+        y_out[id] = (double)((q128)alpha * sum + yv);
+        if (scale) scale[id] = (double)(qabs((q128)alpha) * sa + qabs(yv));
+    }
+    return 0;
+}
+
+// ------------------------------------------------------------------------------------------------
 // 7. Preconditioned CG, step by step (Level-2 algorithm built from Level-1 calls only; the
 //    exact dot "is for example important in a conjugate gradient method").  DESIGN.md 3.5.
 //    Solves  div(chi grad phi) = rho  as  S phi = W o (-rho),  preconditioner V = 1/W.

@@ -81,6 +81,14 @@ def lib():
         L.fxo_dg_apply_definition.argtypes = [gp, dp, dp, C.c_int32, dp, dp]
         L.fxo_dg_apply_canonical.restype = C.c_int
         L.fxo_dg_apply_canonical.argtypes = [gp, dp, dp, C.c_int32, dp]
+        L.fxo_dg_dtables.restype = C.c_int
+        L.fxo_dg_dtables.argtypes = [C.c_int32, C.c_int32, dp]
+        L.fxo_dg_derivative_canonical.restype = C.c_int
+        L.fxo_dg_derivative_canonical.argtypes = [gp, C.c_int32, C.c_int32, C.c_double, dp, C.c_double, dp]
+        L.fxo_dg_derivative_matrix_1d.restype = C.c_int
+        L.fxo_dg_derivative_matrix_1d.argtypes = [C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_int32, dp]
+        L.fxo_dg_derivative_definition.restype = C.c_int
+        L.fxo_dg_derivative_definition.argtypes = [gp, C.c_int32, C.c_int32, C.c_double, dp, C.c_double, dp, dp, dp]
         L.fxo_cg_solve.restype = C.c_int
         L.fxo_cg_solve.argtypes = [gp, dp, dp, dp, C.c_double, C.c_int32, C.POINTER(CGInfo)]
         _lib = L
@@ -200,6 +208,44 @@ def dg_apply_canonical(g, chi, x, normed=False):
     if lib().fxo_dg_apply_canonical(C.byref(g), _p(chi), _p(x), int(normed), _p(y)) != 0:
         raise ValueError("bad grid")
     return y
+
+
+FORWARD, BACKWARD, CENTERED = 0, 1, 2
+
+
+def dg_dtables(P, flux):
+    """-> dict(TT: [2,P,P] (interior / first cell of a DIR line), cN: [P], cP: [P])"""
+    out = np.zeros(2 * P * P + 2 * P)
+    if lib().fxo_dg_dtables(P, flux, _p(out)) != 0:
+        raise ValueError("bad arguments")
+    return dict(TT=out[:2 * P * P].reshape(2, P, P).copy(), cN=out[2 * P * P:2 * P * P + P].copy(), cP=out[2 * P * P + P:].copy())
+
+
+def dg_derivative_canonical(g, direction, flux, alpha, x, beta, y):
+    """y <- alpha * M x + beta * y in the canonical fp64 order (returns the updated copy of y)"""
+    x = _f64(x).ravel()
+    y = np.array(y, dtype=np.float64).ravel().copy()
+    assert x.size == g.n and y.size == g.n
+    if lib().fxo_dg_derivative_canonical(C.byref(g), direction, flux, alpha, _p(x), beta, _p(y)) != 0:
+        raise ValueError("bad arguments")
+    return y
+
+
+def dg_derivative_matrix_1d(N, P, h, bc, flux):
+    n = N * P
+    M = np.zeros((n, n))
+    if lib().fxo_dg_derivative_matrix_1d(N, P, h, bc, flux, _p(M)) != 0:
+        raise ValueError("bad arguments")
+    return M
+
+
+def dg_derivative_definition(g, direction, flux, alpha, x, beta, y):
+    """-> (alpha*M x + beta*y from explicit 113-bit matrices, error scale)"""
+    x, y = _f64(x).ravel(), _f64(y).ravel()
+    out = np.zeros(g.n); sc = np.zeros(g.n)
+    if lib().fxo_dg_derivative_definition(C.byref(g), direction, flux, alpha, _p(x), beta, _p(y), _p(out), _p(sc)) != 0:
+        raise ValueError("bad arguments")
+    return out, sc
 
 
 def cg_solve(g, chi, rho, phi0, tol, maxit):

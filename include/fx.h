@@ -115,6 +115,16 @@ fx_status fx_dg_weights(const fx_grid* grid, double* w_dev, double* v_dev);
  * out_host: host double[5*P + 4*P*P] = xi,w,L,R,B (P each) then T0,T0L,WW,D (P*P each, row-major).  No GPU.   */
 fx_status fx_dg_tables(int32_t P, double* out_host);
 
+/* ---- stand-alone dG derivatives: the paper's "dxdy" primitive (P:240, P:321 / Table 3; D:6.7, Q21) -----------------
+ * y <- alpha * M x + beta * y (beta == 0: y is not read), M = d/dx (direction 0) or d/dy (direction 1) of the grid with its
+ * boundary condition in that direction; flux 0 = forward (the F of the elliptic operator), 1 = backward (-W^-1 F^T W),
+ * 2 = centred (their mean).  x, y: device vectors of the grid; y must not overlap x.                                   */
+fx_status fx_dg_derivative(const fx_grid* grid, int32_t direction, int32_t flux, double alpha, const double* x_dev, double beta,
+                           double* y_dev);
+/* The derivative tables for the cross-check against the oracle: host double[2*P*P + 2*P] = TT interior, TT first
+ * Dirichlet cell (P*P each, row-major), cN, cP.  No GPU.                                                               */
+fx_status fx_dg_dtables(int32_t P, int32_t flux, double* out_host);
+
 /* ---- preconditioned CG (algorithm D:3.5) ------------------------------------------------------
  * Solves div(chi grad phi) = rho as S phi = W o (-rho) with preconditioner V; every dot product exactly rounded;
  * stops when sqrt(r.V.r) <= tol*sqrt(b.W.b) (tested after every iteration) or after maxit iterations.
@@ -138,8 +148,9 @@ fx_status fx_cg_last_profile(double* ms_host, int32_t* iterations_host);
  * returns the average milliseconds per call in *ms_host.  kind: 0 = exdot(a,b) result left on the device,
  * 1 = axpby(0.7,a,-0.3,c), 2 = pointwise_dot(1,a,b,0,c), 3 = dG apply_sym(grid; chi=a, x=b, y=c), 4 = dG apply (normed),
  * 5 = exdot(a,b) returned to the host every call (the paper's GPU dot latency), 6 = axpby(0.7,a,1,c),
- * 7 = weighted dot(a,b,c) device-resident, 8 = exact sum(a) device-resident.
- * a, b, c: device vectors of n doubles (kinds 3,4: n must equal the grid's size).  Synchronises.               */
+ * 7 = weighted dot(a,b,c) device-resident, 8 = exact sum(a) device-resident; with a grid: 9/10 = d/dx, d/dy forward,
+ * 11/12 = d/dx, d/dy centred, each as c <- 0.7 M a - 0.3 c.
+ * a, b, c: device vectors of n doubles (kinds 3,4,9-12: n must equal the grid's size).  Synchronises.               */
 fx_status fx_time_primitive(int32_t kind, const fx_grid* grid, const double* a_dev, const double* b_dev, double* c_dev,
                             int64_t n, int32_t reps, double* ms_host);
 

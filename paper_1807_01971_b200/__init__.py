@@ -55,6 +55,8 @@ _SIGNATURES = {
     "fx_dg_elliptic_apply_sym": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp]),
     "fx_dg_weights": (C.c_int, [C.POINTER(Grid), _vp, _vp]),
     "fx_dg_tables": (C.c_int, [C.c_int32, _dp]),
+    "fx_dg_derivative": (C.c_int, [C.POINTER(Grid), C.c_int32, C.c_int32, C.c_double, _vp, C.c_double, _vp]),
+    "fx_dg_dtables": (C.c_int, [C.c_int32, C.c_int32, _dp]),
     "fx_cg_solve": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp, C.c_double, C.c_int32, C.POINTER(CGInfo)]),
     "fx_cg_solve_host": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp, C.c_double, C.c_int32, C.POINTER(CGInfo)]),
     "fx_cg_profile": (C.c_int, [C.c_int32]),
@@ -222,6 +224,25 @@ def dg_weights(grid, w=None, v=None):
     return w, v
 
 
+FORWARD, BACKWARD, CENTERED = 0, 1, 2
+
+
+def dg_derivative(grid, direction, flux, alpha, x, beta, y):
+    """y <- alpha * M x + beta * y, M = d/dx (direction 0) or d/dy (1), flux FORWARD/BACKWARD/CENTERED.  PAPER.md:240, 321."""
+    _use_torch_stream()
+    _check(lib().fx_dg_derivative(C.byref(grid), int(direction), int(flux), float(alpha), _ptr(x, grid.n), float(beta), _ptr(y, grid.n)),
+           "fx_dg_derivative")
+    return y
+
+
+def dg_dtables(P, flux):
+    """The derivative kernels' tables (host only): dict(TT: [2,P,P], cN: [P], cP: [P])."""
+    import numpy as np
+    out = np.zeros(2 * P * P + 2 * P)
+    _check(lib().fx_dg_dtables(P, flux, out.ctypes.data_as(_dp)), "fx_dg_dtables")
+    return dict(TT=out[:2 * P * P].reshape(2, P, P).copy(), cN=out[2 * P * P:2 * P * P + P].copy(), cP=out[2 * P * P + P:].copy())
+
+
 def dg_tables(P):
     """The kernels' reference-element tables (host only, no GPU): dict(xi,w,L,R,B: [P]; T0,T0L,WW,D: [P,P])."""
     import numpy as np
@@ -244,7 +265,7 @@ def cg_solve(grid, chi, rho, phi, tol, maxit):
     return info
 
 
-TIME_KINDS = {"exdot": 0, "axpby": 1, "pointwise_dot": 2, "dg_apply_sym": 3, "dg_apply": 4, "exdot_host": 5, "axpy": 6, "exdot3": 7, "exsum": 8}
+TIME_KINDS = {"exdot": 0, "axpby": 1, "pointwise_dot": 2, "dg_apply_sym": 3, "dg_apply": 4, "exdot_host": 5, "axpy": 6, "exdot3": 7, "exsum": 8, "dx_forward": 9, "dy_forward": 10, "dx_centered": 11, "dy_centered": 12}
 
 
 def time_primitive(kind, a, b, c, reps, grid=None):

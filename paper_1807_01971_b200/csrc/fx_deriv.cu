@@ -1,0 +1,223 @@
+// fx_deriv.cu -- stand-alone dG derivatives  y <- alpha * M x + beta * y  (the paper's "dxdy" primitive: derivatives in x and
+// y on product spaces; m = 3 memory passes, P:321 / Table 3).  SURVEY 8f-2; definition DESIGN.md 6.7 / Q21.
+//
+// Canonical order per line, cell n, node k (the test oracle restates it independently):
+//     a = chain_m(TT[k][m], u_{n,m});  a = fma(cP[k], tR_{n-1}, a);  a = fma(cN[k], tL_{n+1}, a);  d = RN((2/h) * a)
+//     y = beta == 0 ? RN(alpha * d) : fma(alpha, d, RN(beta * y))
+// The paper stores the few distinct P x P blocks once so that the matrix costs no memory traffic and makes P
+// a template parameter; here the blocks are kernel parameters (constant bank), and the two directions get the
+// thread mapping that suits the x-fastest layout:
+//   * d/dx: a lane owns one cell of one image row (P contiguous doubles), neighbour traces by warp shuffle, strips of 30
+//     cells with a one-cell halo on each side (as the elliptic apply);
+//   * d/dy: a lane owns one image COLUMN and marches through the cells of a row segment -- every load and store is a
+//     fully coalesced 256-byte row, the previous cell's top trace is carried in a register, the next cell's values are
+//     loaded one step ahead and become the current cell.
+// HBM roofline: 24 B per unknown (16 B for beta == 0), ~P + 8 fp64 operations.
+
+#include <string.h>
+
+#include "fx_internal.h"
+
+struct DdParams {
+    int Nx, Ny, bc, beta0;
+    int rows_per_seg, nseg, nstrip;
+    double s, alpha, beta;
+    double TT[2][FX_PMAX][FX_PMAX], cN[FX_PMAX], cP[FX_PMAX], L[FX_PMAX], R[FX_PMAX];
+};
+
+#define DD_CHAIN(acc, COEF, VAL)                         \
+    {                                                    \
+        acc = __dmul_rn(COEF(0), VAL(0));                \
+        _Pragma("unroll") for (int m_ = 1; m_ < P; ++m_) \
+            acc = __fma_rn(COEF(m_), VAL(m_), acc);      \
+    }
+
+template <int P>
+__device__ __forceinline__ double dd_out(const DdParams& g, int k, bool first, const double (&u)[P], double tRp, double tLn) {
+    double a;
+#define CT(m) (first ? g.TT[1][k][m] : g.TT[0][k][m])
+#define UU(m) u[m]
+    DD_CHAIN(a, CT, UU)
+#undef CT
+    a = __fma_rn(g.cP[k], tRp, a);
+    a = __fma_rn(g.cN[k], tLn, a);
+    return __dmul_rn(g.s, a);
+}
+
+__device__ __forceinline__ double dd_axpby(const DdParams& g, double d, double yold) {
+    return g.beta0 ? __dmul_rn(g.alpha, d) : __fma_rn(g.alpha, d, __dmul_rn(g.beta, yold));
+}
+
+// ---- d/dx: warp = strip of 30 cells x rows_per_seg image rows ----------------------------------------------------------
+template <int P>
+__global__ void __launch_bounds__(256) k_dg_dx(const __grid_constant__ DdParams g, const double* __restrict__ x, double* __restrict__ y) {
+    const int wpb = blockDim.x >> 5, lane = threadIdx.x & 31;
+    const long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
+    if (w >= (long long)g.nstrip * g.nseg) return;
+    const int seg = (int)(w / g.nstrip), strip = (int)(w % g.nstrip);
+    const int rows = g.Ny * P, Nx = g.Nx;
+    const long long pitch = (long long)Nx * P;
+    const int r0 = seg * g.rows_per_seg;
+    int r1 = r0 + g.rows_per_seg;
+    if (r1 > rows) r1 = rows;
+    const int ci = strip * FX_STRIP - 1 + lane;
+    const bool outside = ci < 0 || ci >= Nx, dir = g.bc == 1;
+    int cw = ci;
+    if (outside) { cw = ci % Nx; if (cw < 0) cw += Nx; }
+    const bool ghost = outside && (dir || ci < -1 || ci > Nx);
+    const bool produce = lane >= 1 && lane <= FX_STRIP && ci < Nx;
+    const bool first = dir && ci == 0;
+    for (int r = r0; r < r1; ++r) {
+        const double* q = x + (long long)r * pitch + (long long)cw * P;
+        double u[P], yo[P];
+#pragma unroll
+        for (int k = 0; k < P; ++k) u[k] = __ldg(q + k);
+        double* yq = y + (long long)r * pitch + (long long)cw * P;
+        if (!g.beta0 && produce) {
+#pragma unroll
+            for (int k = 0; k < P; ++k) yo[k] = yq[k];
+        }
+        double tL, tR;
+#define CL(m) g.L[m]
+#define CR(m) g.R[m]
+        DD_CHAIN(tL, CL, UU)
+        DD_CHAIN(tR, CR, UU)
+        if (ghost) { tL = 0.0; tR = 0.0; }
+        const double tLn = __shfl_down_sync(0xffffffffu, tL, 1), tRp = __shfl_up_sync(0xffffffffu, tR, 1);
+        if (produce) {
+#pragma unroll
+            for (int k = 0; k < P; ++k) yq[k] = dd_axpby(g, dd_out<P>(g, k, first, u, tRp, tLn), g.beta0 ? 0.0 : yo[k]);
+        }
+    }
+}
+
+// ---- d/dy: lane = image column, warp marches through the cells [j0, j1) of its row segment -------------------------------
+template <int P>
+__global__ void __launch_bounds__(256) k_dg_dy(const __grid_constant__ DdParams g, const double* __restrict__ x, double* __restrict__ y) {
+    const int wpb = blockDim.x >> 5, lane = threadIdx.x & 31;
+    const long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
+    if (w >= (long long)g.nstrip * g.nseg) return;
+    const int seg = (int)(w / g.nstrip), strip = (int)(w % g.nstrip);      // strip = block of 32 columns
+    const long long pitch = (long long)g.Nx * P;
+    const long long col = (long long)strip * 32 + lane;
+    if (col >= pitch) return;                                             // no warp-collective operations below
+    const int Ny = g.Ny;
+    const bool dir = g.bc == 1;
+    const int j0 = seg * g.rows_per_seg;
+    int j1 = j0 + g.rows_per_seg;
+    if (j1 > Ny) j1 = Ny;
+    double uc[P], un[P], tRp;
+    const double* xc = x + col;
+#pragma unroll
+    for (int l = 0; l < P; ++l) uc[l] = __ldg(xc + ((long long)j0 * P + l) * pitch);
+    if (j0 == 0 && dir) tRp = 0.0;
+    else {
+        const int jp = j0 == 0 ? Ny - 1 : j0 - 1;
+        double up[P];
+#pragma unroll
+        for (int l = 0; l < P; ++l) up[l] = __ldg(xc + ((long long)jp * P + l) * pitch);
+#define UP(m) up[m]
+        DD_CHAIN(tRp, CR, UP)
+#undef UP
+    }
+    for (int j = j0; j < j1; ++j) {
+        int jn = j + 1;
+        bool ghost = false;
+        if (jn == Ny) { jn = 0; ghost = dir; }
+#pragma unroll
+        for (int l = 0; l < P; ++l) un[l] = __ldg(xc + ((long long)jn * P + l) * pitch);
+        double yo[P];
+        double* yc = y + col + (long long)j * P * pitch;
+        if (!g.beta0) {
+#pragma unroll
+            for (int l = 0; l < P; ++l) yo[l] = yc[l * pitch];
+        }
+        double tLn, tR;
+#define UN(m) un[m]
+#define UC(m) uc[m]
+        DD_CHAIN(tLn, CL, UN)
+        if (ghost) tLn = 0.0;
+        DD_CHAIN(tR, CR, UC)
+        const bool first = dir && j == 0;
+#pragma unroll
+        for (int l = 0; l < P; ++l) yc[l * pitch] = dd_axpby(g, dd_out<P>(g, l, first, uc, tRp, tLn), g.beta0 ? 0.0 : yo[l]);
+        tRp = tR;
+#pragma unroll
+        for (int l = 0; l < P; ++l) uc[l] = un[l];
+    }
+}
+#undef UN
+#undef UC
+#undef UU
+#undef CL
+#undef CR
+
+fx_status fx_launch_derivative(FxCtx* c, const fx_grid* g, int dir, int flux, double alpha, const double* x, double beta, double* y) {
+    fx_tables t;
+    fx_dtables d;
+    if (fx_make_tables(g->P, &t) != 0 || fx_make_dtables(g->P, flux, &d) != 0) { fx_set_error("fx_dg_derivative: bad P or flux"); return FX_EINVAL; }
+    DdParams p;
+    memset(&p, 0, sizeof(p));
+    const int P = g->P;
+    p.Nx = g->Nx; p.Ny = g->Ny; p.bc = dir == 0 ? g->bcx : g->bcy; p.beta0 = beta == 0.0;
+    volatile double h = dir == 0 ? g->lx / g->Nx : g->ly / g->Ny;
+    p.s = 2.0 / h; p.alpha = alpha; p.beta = beta;
+    for (int k = 0; k < P; ++k) {
+        p.cN[k] = d.cN[k]; p.cP[k] = d.cP[k]; p.L[k] = t.L[k]; p.R[k] = t.R[k];
+        for (int m = 0; m < P; ++m) { p.TT[0][k][m] = d.TT[0][k][m]; p.TT[1][k][m] = d.TT[1][k][m]; }
+    }
+    const long long target = (long long)c->num_sms * 64;               // warps wanted (light kernels: ~2 waves of 32 per SM)
+    const int wpb = 8;
+    if (dir == 0) {
+        p.nstrip = (g->Nx + FX_STRIP - 1) / FX_STRIP;
+        const int rows = g->Ny * P;
+        long long nseg = target / p.nstrip; if (nseg < 1) nseg = 1;
+        int rps = (int)((rows + nseg - 1) / nseg); if (rps < 1) rps = 1;
+        if (c->launch[2][0] > 0) rps = c->launch[2][0];
+        if (rps > rows) rps = rows;
+        p.rows_per_seg = rps; p.nseg = (rows + rps - 1) / rps;
+    } else {
+        p.nstrip = (int)(((long long)g->Nx * P + 31) / 32);
+        long long nseg = target / p.nstrip; if (nseg < 1) nseg = 1;
+        int rps = (int)((g->Ny + nseg - 1) / nseg); if (rps < 4) rps = 4;   // each segment re-reads one cell row
+        if (c->launch[2][0] > 0) rps = c->launch[2][0];
+        if (rps > g->Ny) rps = g->Ny;
+        p.rows_per_seg = rps; p.nseg = (g->Ny + rps - 1) / rps;
+    }
+    const long long warps = (long long)p.nstrip * p.nseg;
+    const int grid = (int)((warps + wpb - 1) / wpb);
+#define FX_DD_LAUNCH(K)                                                         \
+    switch (P) {                                                                \
+    case 1: K<1><<<grid, wpb * 32, 0, c->stream>>>(p, x, y); break;             \
+    case 2: K<2><<<grid, wpb * 32, 0, c->stream>>>(p, x, y); break;             \
+    case 3: K<3><<<grid, wpb * 32, 0, c->stream>>>(p, x, y); break;             \
+    case 4: K<4><<<grid, wpb * 32, 0, c->stream>>>(p, x, y); break;             \
+    default: K<5><<<grid, wpb * 32, 0, c->stream>>>(p, x, y); break;            \
+    }
+    if (dir == 0) { FX_DD_LAUNCH(k_dg_dx) } else { FX_DD_LAUNCH(k_dg_dy) }
+    c->launches++;
+    FX_CUDA(cudaGetLastError());
+    return FX_OK;
+}
+
+extern "C" fx_status fx_dg_derivative(const fx_grid* g, int32_t direction, int32_t flux, double alpha, const double* x, double beta,
+                                      double* y) {
+    if (!fx_grid_ok(g) || !x || !y || direction < 0 || direction > 1 || flux < 0 || flux > 2) {
+        fx_set_error("fx_dg_derivative: bad grid, direction, flux or null pointer"); return FX_EINVAL;
+    }
+    const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
+    if (x < y + n && y < x + n) { fx_set_error("fx_dg_derivative: y overlaps x"); return FX_EINVAL; }
+    FxCtx* c = fx_ctx();
+    if (!c) return FX_ECUDA;
+    return fx_launch_derivative(c, g, direction, flux, alpha, x, beta, y);
+}
+
+extern "C" fx_status fx_dg_dtables(int32_t P, int32_t flux, double* out) {
+    fx_dtables d;
+    if (!out || fx_make_dtables(P, flux, &d) != 0) { fx_set_error("fx_dg_dtables: bad arguments"); return FX_EINVAL; }
+    double* o = out;
+    for (int v = 0; v < 2; ++v) for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m) *o++ = d.TT[v][k][m];
+    for (int k = 0; k < P; ++k) *o++ = d.cN[k];
+    for (int k = 0; k < P; ++k) *o++ = d.cP[k];
+    return FX_OK;
+}

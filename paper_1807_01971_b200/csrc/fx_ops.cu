@@ -502,14 +502,18 @@ static fx_status time_one(FxCtx* c, int kind, const fx_grid* g, const double* a,
     case 6: return fx_axpby(0.7, a, 1.0, cc, n);
     case 7: return launch_exdotn<3>(c, a, b, cc, n, c->result_dev);
     case 8: return launch_exdotn<1>(c, a, nullptr, nullptr, n, c->result_dev);
+    case 9: return fx_launch_derivative(c, g, 0, 0, 0.7, a, -0.3, cc);
+    case 10: return fx_launch_derivative(c, g, 1, 0, 0.7, a, -0.3, cc);
+    case 11: return fx_launch_derivative(c, g, 0, 2, 0.7, a, -0.3, cc);
+    case 12: return fx_launch_derivative(c, g, 1, 2, 0.7, a, -0.3, cc);
     }
     return FX_EINVAL;
 }
 
 extern "C" fx_status fx_time_primitive(int32_t kind, const fx_grid* g, const double* a, const double* b, double* cc, int64_t n,
                                        int32_t reps, double* ms_host) {
-    if (kind < 0 || kind > 8 || n < 0 || reps < 1 || !ms_host || !a || !b || !cc) { fx_set_error("fx_time_primitive: bad arguments"); return FX_EINVAL; }
-    if ((kind == 3 || kind == 4) && (!fx_grid_ok(g) || (int64_t)g->Nx * g->Ny * g->P * g->P != n)) { fx_set_error("fx_time_primitive: bad grid"); return FX_EINVAL; }
+    if (kind < 0 || kind > 12 || n < 0 || reps < 1 || !ms_host || !a || !b || !cc) { fx_set_error("fx_time_primitive: bad arguments"); return FX_EINVAL; }
+    if ((kind == 3 || kind == 4 || kind >= 9) && (!fx_grid_ok(g) || (int64_t)g->Nx * g->Ny * g->P * g->P != n)) { fx_set_error("fx_time_primitive: bad grid"); return FX_EINVAL; }
     FxCtx* c = fx_ctx();
     if (!c) return FX_ECUDA;
     cudaEvent_t e0, e1;

@@ -43,9 +43,32 @@ double rnd(q v) { q a = v < 0 ? -v : v; return a < 1e-25Q ? 0.0 : (double)v; }
 
 }  // namespace
 
-extern "C" int fx_make_tables(int P, fx_tables* t) {
-    if (P < 1 || P > FX_PMAX) return -1;
-    q xi[FX_PMAX], w[FX_PMAX], lam[FX_PMAX], L[FX_PMAX], R[FX_PMAX], D[FX_PMAX][FX_PMAX];
+struct Ref { q xi[FX_PMAX], w[FX_PMAX], L[FX_PMAX], R[FX_PMAX], D[FX_PMAX][FX_PMAX]; };
+static void reference_element(int P, Ref& r);
+
+// forward: T = D - W^-1 R R^T (+ W^-1 L L^T in the first cell of a Dirichlet line); backward: -W^-1 T^T W; centred: mean
+extern "C" int fx_make_dtables(int P, int flux, fx_dtables* d) {
+    if (P < 1 || P > FX_PMAX || flux < 0 || flux > 2) return -1;
+    Ref r; reference_element(P, r);
+    for (int v = 0; v < 2; ++v)
+        for (int k = 0; k < P; ++k)
+            for (int m = 0; m < P; ++m) {
+                q tkm = r.D[k][m] - r.R[k] * r.R[m] / r.w[k], tmk = r.D[m][k] - r.R[m] * r.R[k] / r.w[m];
+                if (v) { tkm += r.L[k] * r.L[m] / r.w[k]; tmk += r.L[m] * r.L[k] / r.w[m]; }
+                const q f = tkm, b = -tmk * r.w[m] / r.w[k];
+                d->TT[v][k][m] = rnd(flux == 0 ? f : flux == 1 ? b : (f + b) / 2);
+            }
+    for (int k = 0; k < P; ++k) {
+        const q cn = r.R[k] / r.w[k], cp = -r.L[k] / r.w[k];
+        d->cN[k] = flux == 0 ? rnd(cn) : flux == 1 ? 0.0 : rnd(cn / 2);
+        d->cP[k] = flux == 0 ? 0.0 : flux == 1 ? rnd(cp) : rnd(cp / 2);
+    }
+    return 0;
+}
+
+static void reference_element(int P, Ref& r) {
+    q lam[FX_PMAX];
+    q (&xi)[FX_PMAX] = r.xi; q (&w)[FX_PMAX] = r.w; q (&L)[FX_PMAX] = r.L; q (&R)[FX_PMAX] = r.R; q (&D)[FX_PMAX][FX_PMAX] = r.D;
     gauss_legendre(P, xi, w);
     for (int m = 0; m < P; ++m) {                      // barycentric weights
         q d = 1;
@@ -62,6 +85,12 @@ extern "C" int fx_make_tables(int P, fx_tables* t) {
         for (int m = 0; m < P; ++m) if (m != k) { D[k][m] = (lam[m] / lam[k]) / (xi[k] - xi[m]); diag -= D[k][m]; }
         D[k][k] = diag;
     }
+}
+
+extern "C" int fx_make_tables(int P, fx_tables* t) {
+    if (P < 1 || P > FX_PMAX) return -1;
+    Ref r; reference_element(P, r);
+    q (&xi)[FX_PMAX] = r.xi; q (&w)[FX_PMAX] = r.w; q (&L)[FX_PMAX] = r.L; q (&R)[FX_PMAX] = r.R; q (&D)[FX_PMAX][FX_PMAX] = r.D;
     t->P = P;
     for (int k = 0; k < P; ++k) {
         t->xi[k] = rnd(xi[k]); t->w[k] = (double)w[k]; t->L[k] = rnd(L[k]); t->R[k] = rnd(R[k]);

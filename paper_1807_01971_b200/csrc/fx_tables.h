@@ -15,9 +15,19 @@ typedef struct {
     double D[FX_PMAX][FX_PMAX];              // l_m'(xi_k)
 } fx_tables;
 
+// stand-alone derivative y <- alpha M x + beta y: per flux (0 forward, 1 backward, 2 centred)
+typedef struct {
+    double TT[2][FX_PMAX][FX_PMAX];          // [0] interior cell, [1] first cell of a Dirichlet line
+    double cN[FX_PMAX], cP[FX_PMAX];         // coefficients of the next cell's left trace / previous cell's right trace
+} fx_dtables;
+
 #ifdef __cplusplus
-extern "C"
+extern "C" {
 #endif
 int fx_make_tables(int P, fx_tables* t);
+int fx_make_dtables(int P, int flux, fx_dtables* d);
+#ifdef __cplusplus
+}
+#endif
 
 #endif

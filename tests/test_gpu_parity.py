@@ -476,3 +476,46 @@ def test_weighted_dot_fig2_integral(fx, oracle):
     val = fx.exdot3(dev(fxv), W, dev(fyv))
     assert abs(val / (math.exp(2.0) - 1.0) ** 2 - 1.0) < 2e-12
     assert fbits(val) == fbits(oracle.exdot3(fxv, W.cpu().numpy(), fyv))
+
+
+# ---- stand-alone dG derivatives ("dxdy") ------------------------------------------------
+
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("direction", [0, 1])
+def test_dg_derivative_bit_exact(fx, oracle, P, direction):
+    import torch
+    for (Nx, Ny) in [(1, 1), (2, 3), (31, 5), (33, 4), (64, 40), (70, 9)]:
+        for bc in (0, 1):
+            g, og = _grid(fx, oracle, Nx, Ny, P, bc, bc)
+            x, y0 = fi.uniform(401 + P, g.n), fi.uniform(402 + P, g.n)
+            for flux in (0, 1, 2):
+                for alpha, beta in ((1.0, 0.0), (0.7, -0.3)):
+                    want = oracle.dg_derivative_canonical(og, direction, flux, alpha, x, beta, y0)
+                    y = dev(y0) if beta != 0.0 else torch.full((g.n,), float("nan"), dtype=torch.float64, device="cuda")
+                    fx.dg_derivative(g, direction, flux, alpha, dev(x), beta, y)
+                    got = y.cpu().numpy()
+                    assert np.array_equal(got, want), (Nx, Ny, P, bc, flux, alpha, np.abs(got - want).max())
+
+
+@pytest.mark.parametrize("direction", [0, 1])
+def test_dg_derivative_definition_shapes_and_full_size(fx, oracle, direction):
+    import torch
+    g, og = _grid(fx, oracle, 12, 9, 3, 0, 1)
+    x, y0 = fi.uniform(411, g.n), fi.uniform(412, g.n)
+    for flux in (0, 1, 2):
+        ydef, scale = oracle.dg_derivative_definition(og, direction, flux, 0.7, x, -0.3, y0)
+        for rows in (0, 1, 5, 1000):                                   # launch-shape invariance
+            fx.set_launch(2, rows, 0)
+            y = dev(y0)
+            fx.dg_derivative(g, direction, flux, 0.7, dev(x), -0.3, y)
+            got = y.cpu().numpy()
+            assert np.all(np.abs(got - ydef) <= 1e-14 * scale)
+            assert np.array_equal(got, oracle.dg_derivative_canonical(og, direction, flux, 0.7, x, -0.3, y0))
+    fx.set_launch(2, 0, 0)
+    c = fi.config4(3, 1024)                                            # 1024^2 cells, P = 3: the size the sweep times
+    g, og = fx.make_grid(**c["grid"]), oracle.Grid(**c["grid"])
+    y = dev(c["y"])
+    fx.dg_derivative(g, direction, 2, 0.7, dev(c["x"]), -0.3, y)
+    assert np.array_equal(y.cpu().numpy(), oracle.dg_derivative_canonical(og, direction, 2, 0.7, c["x"], -0.3, c["y"]))
+    with pytest.raises(fx.FxError):
+        fx.dg_derivative(g, direction, 0, 1.0, y, 0.0, y)

@@ -197,6 +197,10 @@ def run_fx(args):
             for _ in range(3):
                 fx.dg_elliptic_apply(g, chi, pvec, q, sym=True)
             t = time_events(lambda: fx.dg_elliptic_apply(g, chi, pvec, q, sym=True), 20, torch)
+            for kind in ("dx_forward", "dy_forward", "dx_centered", "dy_centered"):   # the paper's "dxdy" primitive, Table 3 (m = 3)
+                fx.time_primitive(kind, pvec, chi, q, 3, grid=g)
+                tt = fx.time_primitive(kind, pvec, chi, q, 20, grid=g)
+                prim[kind] = {"grid": "%dx%d P=3" % (N, N), "ms": tt, "GBps": 24.0 * n / tt / 1e6, "frac_of_peak": 24.0 * n / tt / 1e6 / peak}
             prim["dg_apply"] = {"grid": "%dx%d P=3" % (N, N), "n": n, "MB_per_vector": 8e-6 * n, "ms": t, "GBps": 24.0 * n / t / 1e6,
                                 "frac_of_peak": 24.0 * n / t / 1e6 / peak, "note": "3 x 75.5 MB partly L2-resident between repeats"}
 

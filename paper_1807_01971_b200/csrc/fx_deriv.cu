@@ -106,10 +106,15 @@ __global__ void __launch_bounds__(256) k_dg_dy(const __grid_constant__ DdParams 
     const int j0 = seg * g.rows_per_seg;
     int j1 = j0 + g.rows_per_seg;
     if (j1 > Ny) j1 = Ny;
-    double uc[P], un[P], tRp;
+    double uc[P], un[P], u2[P], tRp;
     const double* xc = x + col;
 #pragma unroll
     for (int l = 0; l < P; ++l) uc[l] = __ldg(xc + ((long long)j0 * P + l) * pitch);
+    {
+        const int jn0 = (j0 + 1 == Ny) ? 0 : j0 + 1;
+#pragma unroll
+        for (int l = 0; l < P; ++l) un[l] = __ldg(xc + ((long long)jn0 * P + l) * pitch);
+    }
     if (j0 == 0 && dir) tRp = 0.0;
     else {
         const int jp = j0 == 0 ? Ny - 1 : j0 - 1;
@@ -121,11 +126,12 @@ __global__ void __launch_bounds__(256) k_dg_dy(const __grid_constant__ DdParams 
 #undef UP
     }
     for (int j = j0; j < j1; ++j) {
-        int jn = j + 1;
-        bool ghost = false;
-        if (jn == Ny) { jn = 0; ghost = dir; }
+        const bool ghost = dir && j + 1 == Ny;                           // un holds row 0 then; its trace is forced to zero
+        if (j + 1 < j1) {                                                // two cells ahead: in flight while this cell is computed
+            int j2 = j + 2; if (j2 >= Ny) j2 -= Ny;
 #pragma unroll
-        for (int l = 0; l < P; ++l) un[l] = __ldg(xc + ((long long)jn * P + l) * pitch);
+            for (int l = 0; l < P; ++l) u2[l] = __ldg(xc + ((long long)j2 * P + l) * pitch);
+        }
         double yo[P];
         double* yc = y + col + (long long)j * P * pitch;
         if (!g.beta0) {
@@ -143,7 +149,7 @@ __global__ void __launch_bounds__(256) k_dg_dy(const __grid_constant__ DdParams 
         for (int l = 0; l < P; ++l) yc[l * pitch] = dd_axpby(g, dd_out<P>(g, l, first, uc, tRp, tLn), g.beta0 ? 0.0 : yo[l]);
         tRp = tR;
 #pragma unroll
-        for (int l = 0; l < P; ++l) uc[l] = un[l];
+        for (int l = 0; l < P; ++l) { uc[l] = un[l]; un[l] = u2[l]; }
     }
 }
 #undef UN

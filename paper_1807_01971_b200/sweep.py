@@ -20,7 +20,8 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-M_PASSES = {"axpby": 3, "pointwise_dot": 3, "exdot": 2, "exdot_host": 2, "exdot3": 3, "exsum": 1, "dg_apply_sym": 3, "dg_apply": 3}
+M_PASSES = {"axpby": 3, "pointwise_dot": 3, "exdot": 2, "exdot_host": 2, "exdot3": 3, "exsum": 1, "dg_apply_sym": 3, "dg_apply": 3,
+            "dx_forward": 3, "dy_forward": 3, "dx_centered": 3, "dy_centered": 3}
 L2_BYTES = 126e6
 
 
@@ -74,14 +75,17 @@ def main():
                 out = torch.empty_like(x)
                 S = 8.0 * n
                 reps = int(max(10, min(2000, 0.05 / max(2e-6, 3 * S / 5e12))))
-                for kind in ("axpby", "pointwise_dot", "exdot", "exdot_host", "exdot3", "exsum", "dg_apply_sym", "dg_apply"):
+                for kind in ("axpby", "pointwise_dot", "exdot", "exdot_host", "exdot3", "exsum", "dg_apply_sym", "dg_apply",
+                             "dx_forward", "dy_forward", "dx_centered", "dy_centered"):
                     if kind.startswith("dg"):
                         ms = fx.time_primitive(kind, chi, x, out, reps, grid=g)
+                    elif kind.startswith("d"):
+                        out.copy_(y); ms = fx.time_primitive(kind, x, y, out, reps, grid=g)
                     elif kind == "axpby":
                         out.copy_(y); ms = fx.time_primitive(kind, x, y, out, reps)
                     else:
                         ms = fx.time_primitive(kind, x, y, out, max(10, reps // (4 if kind == "exdot_host" else 1)))
-                    key = kind if not kind.startswith("dg") else "%s_P%d" % (kind, P)
+                    key = kind if not kind.startswith("d") else "%s_P%d" % (kind, P)
                     res.setdefault(key, []).append({"P": P, "N": N, "n": n, "S_MB": S / 1e6, "t_us": ms * 1e3,
                                                     "GBps": M_PASSES[kind] * S / (ms * 1e-3) / 1e9})
                 del x, y, chi, out

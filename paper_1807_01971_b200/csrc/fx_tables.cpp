@@ -12,6 +12,8 @@
 #include <quadmath.h>
 #include <stdint.h>
 
+#include <mutex>
+
 #include "fx_tables.h"
 
 typedef __float128 q;
@@ -47,7 +49,32 @@ struct Ref { q xi[FX_PMAX], w[FX_PMAX], L[FX_PMAX], R[FX_PMAX], D[FX_PMAX][FX_PM
 static void reference_element(int P, Ref& r);
 
 // forward: T = D - W^-1 R R^T (+ W^-1 L L^T in the first cell of a Dirichlet line); backward: -W^-1 T^T W; centred: mean
+// The 113-bit derivation costs microseconds of host time; every launch needs the tables, so they are computed once.
+static int make_dtables_uncached(int P, int flux, fx_dtables* d);
+static int make_tables_uncached(int P, fx_tables* t);
+static std::once_flag g_once;
+static fx_tables g_tab[FX_PMAX + 1];
+static fx_dtables g_dtab[FX_PMAX + 1][3];
+static void fill_cache() {
+    for (int P = 1; P <= FX_PMAX; ++P) {
+        make_tables_uncached(P, &g_tab[P]);
+        for (int f = 0; f < 3; ++f) make_dtables_uncached(P, f, &g_dtab[P][f]);
+    }
+}
 extern "C" int fx_make_dtables(int P, int flux, fx_dtables* d) {
+    if (P < 1 || P > FX_PMAX || flux < 0 || flux > 2) return -1;
+    std::call_once(g_once, fill_cache);
+    *d = g_dtab[P][flux];
+    return 0;
+}
+extern "C" int fx_make_tables(int P, fx_tables* t) {
+    if (P < 1 || P > FX_PMAX) return -1;
+    std::call_once(g_once, fill_cache);
+    *t = g_tab[P];
+    return 0;
+}
+
+static int make_dtables_uncached(int P, int flux, fx_dtables* d) {
     if (P < 1 || P > FX_PMAX || flux < 0 || flux > 2) return -1;
     Ref r; reference_element(P, r);
     for (int v = 0; v < 2; ++v)
@@ -87,7 +114,7 @@ static void reference_element(int P, Ref& r) {
     }
 }
 
-extern "C" int fx_make_tables(int P, fx_tables* t) {
+static int make_tables_uncached(int P, fx_tables* t) {
     if (P < 1 || P > FX_PMAX) return -1;
     Ref r; reference_element(P, r);
     q (&xi)[FX_PMAX] = r.xi; q (&w)[FX_PMAX] = r.w; q (&L)[FX_PMAX] = r.L; q (&R)[FX_PMAX] = r.R; q (&D)[FX_PMAX][FX_PMAX] = r.D;

@@ -162,6 +162,14 @@ extern "C" double fxo_exsum(const double* x, int64_t n) {
     return acc_round(a);
 }
 
+// Single-precision inputs, exact accumulation (an exact dot lets single precision keep its accuracy):
+// RN_double( sum_i x_i * y_i ) for binary32 x, y -- every product is formed exactly (48-bit mantissa) as in fxo_exdot.
+extern "C" double fxo_exdot_f32(const float* x, const float* y, int64_t n) {
+    BigAcc a; acc_clear(a);
+    for (int64_t i = 0; i < n; ++i) acc_add_product(a, (double)x[i], (double)y[i]);
+    return acc_round(a);
+}
+
 // round an externally supplied accumulator (used by the "concatenation = integer sum" pin)
 extern "C" double fxo_round_digits(const uint64_t limbs[68]) {
     BigAcc a; acc_clear(a); std::memcpy(a.limb, limbs, sizeof(a.limb));

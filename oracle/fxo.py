@@ -60,6 +60,8 @@ def lib():
         L.fxo_exdot_digits.argtypes = [dp, dp, C.c_int64, C.POINTER(C.c_uint64), C.POINTER(C.c_int32)]
         L.fxo_exdot3.restype = C.c_double
         L.fxo_exdot3.argtypes = [dp, dp, dp, C.c_int64]
+        L.fxo_exdot_f32.restype = C.c_double
+        L.fxo_exdot_f32.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_int64]
         L.fxo_exsum.restype = C.c_double
         L.fxo_exsum.argtypes = [dp, C.c_int64]
         L.fxo_round_digits.restype = C.c_double
@@ -115,6 +117,14 @@ def exdot3(x, w, y):
     x, w, y = _f64(x).ravel(), _f64(w).ravel(), _f64(y).ravel()
     assert x.size == w.size == y.size
     return float(lib().fxo_exdot3(_p(x), _p(w), _p(y), x.size))
+
+
+def exdot_f32(x, y):
+    """RN_double(sum x_i*y_i) for float32 inputs"""
+    x = np.ascontiguousarray(x, dtype=np.float32).ravel(); y = np.ascontiguousarray(y, dtype=np.float32).ravel()
+    assert x.size == y.size
+    fp = C.POINTER(C.c_float)
+    return float(lib().fxo_exdot_f32(x.ctypes.data_as(fp), y.ctypes.data_as(fp), x.size))
 
 
 def exsum(x):

@@ -293,3 +293,19 @@ def test_weighted_dot_pins(oracle):
     assert oracle.exsum(v) == float(sum(Fraction(float(t)) for t in v))
     assert oracle.exsum(v[::-1].copy()) == oracle.exsum(v)
     assert oracle.exsum(np.concatenate([v, -v])) == 0.0 and oracle.exsum(np.array([1e308, 1e308, -1e308])) == 1e308
+
+
+def test_exdot_f32_pins(oracle):
+    """binary32 inputs: rational brute force, agreement with the fp64 dot of the converted inputs, subnormals, overflow"""
+    from fractions import Fraction
+    import fxinputs as fi
+    n = 700
+    x = fi.uniform(51, n).astype(np.float32); y = (fi.uniform(52, n) * 1e3).astype(np.float32)
+    x[3] = np.float32(1e-45); y[3] = np.float32(1e-40); x[5] = np.float32(3e38); y[5] = np.float32(3e38)     # subnormal*subnormal, beyond float range
+    exact = sum(Fraction(float(a)) * Fraction(float(b)) for a, b in zip(x, y))
+    assert oracle.exdot_f32(x, y) == float(exact)
+    assert oracle.exdot_f32(x, y) == oracle.exdot(x.astype(np.float64), y.astype(np.float64))
+    assert oracle.exdot_f32(x[:0], y[:0]) == 0.0
+    # naive float32 accumulation loses the small terms that the exact accumulation keeps
+    big = np.array([1e8, 1.0, -1e8, 1.0], dtype=np.float32)
+    assert oracle.exdot_f32(big, np.ones(4, dtype=np.float32)) == 2.0

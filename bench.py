@@ -191,7 +191,13 @@ def run_fx(args):
                 fx.time_primitive(kind, x, y, z, 3)
                 t = fx.time_primitive(kind, x, y, z, 20)
                 prim[kind] = {"n": nd, "ms": t, "GBps": m * 8.0 * nd / t / 1e6, "frac_of_peak": m * 8.0 * nd / t / 1e6 / peak}
-            del x, y, z
+            xf = x.to(torch.float32); yf = z.to(torch.float32)           # binary32 inputs, exact accumulation
+            for _ in range(3):
+                fx.exdot_f32(xf, yf)
+            t = time_events(lambda: fx.exdot_f32(xf, yf), 10, torch)
+            prim["exdot_f32"] = {"n": nd, "ms": t, "GBps": 8.0 * nd / t / 1e6, "frac_of_peak": 8.0 * nd / t / 1e6 / peak,
+                                 "Gelem_per_s": nd / t / 1e6, "note": "result returned to the host every call; fp64 exdot: %.0f Gelem/s" % (nd / prim["exdot"]["ms"] / 1e6)}
+            del x, y, z, xf, yf
             q = torch.empty(n, dtype=torch.float64, device="cuda")
             pvec = torch.from_numpy(fi.uniform(9003, n)).cuda()
             for _ in range(3):

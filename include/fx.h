@@ -94,6 +94,8 @@ double fx_exdot_host(const double* x_host, const double* y_host, int64_t n);
  * sum of x (EXSUM) = exact dot with ones.  Device pointers, may alias; both synchronise and return the value.      */
 double fx_exdot3(const double* x_dev, const double* w_dev, const double* y_dev, int64_t n);
 double fx_exsum(const double* x_dev, int64_t n);
+/* binary32 inputs, exact accumulation: RN_double(sum x[i]*y[i]), every product exact.  Synchronises.          */
+double fx_exdot_f32(const float* x_dev, const float* y_dev, int64_t n);
 
 /* ---- vector primitives in canonical order (D:3.2) ---------------------------------------------- */
 

@@ -49,6 +49,7 @@ _SIGNATURES = {
     "fx_exdot_host": (C.c_double, [_vp, _vp, C.c_int64]),
     "fx_exdot3": (C.c_double, [_vp, _vp, _vp, C.c_int64]),
     "fx_exsum": (C.c_double, [_vp, C.c_int64]),
+    "fx_exdot_f32": (C.c_double, [_vp, _vp, C.c_int64]),
     "fx_axpby": (C.c_int, [C.c_double, _vp, C.c_double, _vp, C.c_int64]),
     "fx_pointwise_dot": (C.c_int, [C.c_double, _vp, _vp, C.c_double, _vp, C.c_int64]),
     "fx_dg_elliptic_apply": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp]),
@@ -143,6 +144,18 @@ def exsum(x):
     """exactly rounded sum (EXSUM); synchronises"""
     _use_torch_stream()
     v = lib().fx_exsum(_ptr(x), x.numel())
+    if v != v and lib().fx_last_error():
+        raise FxError(lib().fx_last_error().decode())
+    return v
+
+
+def exdot_f32(x, y):
+    """RN_double(sum x_i*y_i) for contiguous float32 CUDA tensors; synchronises"""
+    import torch
+    _use_torch_stream()
+    assert x.is_cuda and y.is_cuda and x.dtype == torch.float32 and y.dtype == torch.float32 and x.is_contiguous() and y.is_contiguous()
+    assert x.numel() == y.numel()
+    v = lib().fx_exdot_f32(x.data_ptr(), y.data_ptr(), x.numel())
     if v != v and lib().fx_last_error():
         raise FxError(lib().fx_last_error().decode())
     return v

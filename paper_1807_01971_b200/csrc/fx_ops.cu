@@ -256,6 +256,122 @@ static fx_status launch_exdotn(FxCtx* c, const double* a0, const double* a1, con
     return FX_OK;
 }
 
+// ---- binary32 inputs, exact accumulation ---------------------------------------------------------------------
+// Every product of two floats is exact in fp64 (48-bit mantissa), so p = (double)x * (double)y carries no error term
+// (NOERR path: 3K fp64 operations per element).  8 elements per thread and tile; 16-byte cp.async when both arrays are
+// 16-byte aligned, 4-byte copies otherwise.
+#define EXF_U 8
+template <bool VEC>
+__global__ void __launch_bounds__(256, 2) k_exdot_f32(const float* __restrict__ x, const float* __restrict__ y, long long n, ExGlobal g,
+                                                       int first, int last, double* result) {
+    extern __shared__ __align__(16) float exf_buf[];
+    __shared__ ExShared sh;
+    ex_shared_init(&sh);
+    ExAcc<EX_K, EX_W> acc;
+    acc.init();
+    const int bd = blockDim.x;
+    const long long tile = (long long)bd * EXF_U, ntiles = (n + tile - 1) / tile;
+    auto issue = [&](int stage, long long t) {
+        float* sx = exf_buf + (size_t)stage * 2 * EXF_U * bd;
+        float* sy = sx + EXF_U * bd;
+        if (t < ntiles) {
+            if (VEC) {
+#pragma unroll
+                for (int u = 0; u < EXF_U / 4; ++u) {
+                    const int slot = 4 * (u * bd + threadIdx.x);
+                    const long long e = t * tile + slot, left = n - e;
+                    const int bytes = left >= 4 ? 16 : (left > 0 ? 4 * (int)left : 0);
+                    const long long es = bytes ? e : 0;
+                    fx_cp_async16(fx_smem_addr(sx + slot), x + es, bytes);
+                    fx_cp_async16(fx_smem_addr(sy + slot), y + es, bytes);
+                }
+            } else {
+#pragma unroll
+                for (int u = 0; u < EXF_U; ++u) {
+                    const int slot = u * bd + threadIdx.x;
+                    const long long e = t * tile + slot;
+                    const bool in = e < n;
+                    fx_cp_async4(fx_smem_addr(sx + slot), x + (in ? e : 0), in);
+                    fx_cp_async4(fx_smem_addr(sy + slot), y + (in ? e : 0), in);
+                }
+            }
+        }
+        fx_cp_commit();
+    };
+    long long tq = blockIdx.x;
+#pragma unroll
+    for (int s = 0; s < EX_STAGES - 1; ++s) { issue(s, tq); tq += gridDim.x; }
+    int stage = 0;
+    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        int sq = stage + EX_STAGES - 1; if (sq >= EX_STAGES) sq -= EX_STAGES;
+        issue(sq, tq); tq += gridDim.x;
+        fx_cp_wait<EX_STAGES - 1>();
+        const float* sx = exf_buf + (size_t)stage * 2 * EXF_U * bd;
+        const float* sy = sx + EXF_U * bd;
+        double xv[EXF_U], yv[EXF_U];
+        bool act[EXF_U];
+        if (VEC) {
+#pragma unroll
+            for (int u = 0; u < EXF_U / 4; ++u) {
+                const int slot = 4 * (u * bd + threadIdx.x);
+                const float4 a = *reinterpret_cast<const float4*>(sx + slot), b = *reinterpret_cast<const float4*>(sy + slot);
+                const long long e = t * tile + slot;
+                xv[4 * u] = a.x; xv[4 * u + 1] = a.y; xv[4 * u + 2] = a.z; xv[4 * u + 3] = a.w;
+                yv[4 * u] = b.x; yv[4 * u + 1] = b.y; yv[4 * u + 2] = b.z; yv[4 * u + 3] = b.w;
+#pragma unroll
+                for (int i = 0; i < 4; ++i) act[4 * u + i] = e + i < n;
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < EXF_U; ++u) {
+                const int slot = u * bd + threadIdx.x;
+                xv[u] = sx[slot]; yv[u] = sy[slot];
+                act[u] = t * tile + slot < n;
+            }
+        }
+        acc.add<EXF_U, false, true>(xv, yv, act, &sh);                 // float * float is exact in fp64: no error term
+        if (++stage == EX_STAGES) stage = 0;
+    }
+    fx_cp_wait<0>();
+    acc.flush(&sh);
+    ex_block_finish(&sh, g, first, last, result);
+}
+
+extern "C" double fx_exdot_f32(const float* x, const float* y, int64_t n) {
+    if (n < 0 || (n > 0 && (!x || !y))) { fx_set_error("fx_exdot_f32: bad arguments"); return NAN; }
+    fx_set_error("%s", "");
+    FxCtx* c = fx_ctx();
+    if (!c) return NAN;
+    const int bd = 256;
+    const size_t smem = (size_t)EX_STAGES * 2 * EXF_U * bd * sizeof(float);
+    static int occ = 0;
+    if (!occ) {
+        if (cudaFuncSetAttribute(k_exdot_f32<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+            cudaFuncSetAttribute(k_exdot_f32<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+            fx_cuda_fail(cudaGetLastError(), "k_exdot_f32 attributes"); return NAN;
+        }
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_exdot_f32<true>, bd, smem) != cudaSuccess || occ < 1) occ = 1;
+    }
+    const bool vec = aligned16(x) && aligned16(y);
+    const int64_t CHUNK = (int64_t)1 << 28;
+    int64_t done = 0;
+    do {
+        const int64_t m = (n - done < CHUNK) ? (n - done) : CHUNK;
+        const long long tile = (long long)bd * EXF_U;
+        long long grid = (m + tile - 1) / tile;
+        if (grid > (long long)c->num_sms * occ) grid = (long long)c->num_sms * occ;
+        if (grid < 1) grid = 1;
+        if (vec) k_exdot_f32<true><<<(int)grid, bd, smem, c->stream>>>(x + done, y + done, m, c->ex, done == 0, done + m == n, c->result_dev);
+        else k_exdot_f32<false><<<(int)grid, bd, smem, c->stream>>>(x + done, y + done, m, c->ex, done == 0, done + m == n, c->result_dev);
+        c->launches++;
+        if (cudaGetLastError() != cudaSuccess) { fx_cuda_fail(cudaGetLastError(), "k_exdot_f32"); return NAN; }
+        done += m;
+    } while (done < n);
+    if (cudaMemcpyAsync(c->result_pinned, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess) { fx_cuda_fail(cudaGetLastError(), "fx_exdot_f32 result copy"); return NAN; }
+    return c->result_pinned[0];
+}
+
 static double exdotn_sync(FxCtx* c, fx_status s) {
     if (s != FX_OK) return NAN;
     if (cudaMemcpyAsync(c->result_pinned, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||

@@ -519,3 +519,16 @@ def test_dg_derivative_definition_shapes_and_full_size(fx, oracle, direction):
     assert np.array_equal(y.cpu().numpy(), oracle.dg_derivative_canonical(og, direction, 2, 0.7, c["x"], -0.3, c["y"]))
     with pytest.raises(fx.FxError):
         fx.dg_derivative(g, direction, 0, 1.0, y, 0.0, y)
+
+
+@pytest.mark.parametrize("n", [0, 1, 5, 1027, 100003, (1 << 22) + 9])
+def test_exdot_f32(fx, oracle, n):
+    """binary32 inputs, exact accumulation"""
+    import torch
+    x = fi.uniform(111, n).astype(np.float32); y = (fi.uniform(112, n) * 1e3).astype(np.float32)
+    if n > 100:
+        x[3] = np.float32(1e-45); y[3] = np.float32(1e-40); x[5] = np.float32(3e38); y[5] = np.float32(3e38)
+    dx, dy = torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda()
+    assert fbits(fx.exdot_f32(dx, dy)) == fbits(oracle.exdot_f32(x, y) if n else 0.0)
+    if n > 4:
+        assert fbits(fx.exdot_f32(dx[1:], dy[1:])) == fbits(oracle.exdot_f32(x[1:], y[1:]))      # 4-byte aligned only

@@ -31,6 +31,9 @@ struct DgParams {
 };
 
 #define FX_STRIP 30
+#ifndef FX_PFD
+#define FX_PFD 1          // prefetch distance in marching steps (2 and 3 measured slower: L1 capacity / set conflicts)
+#endif
 
 template <int P>
 struct DgCell { double v[P][P]; };     // [l][k]: row l (y node), column k (x node)
@@ -204,7 +207,15 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
     // ---- prologue: state of cell row j0-1 ------------------------------------------------------------------
     dg_load_u<P, DIRF>(uc, g, src, pitch, col0, j0);
     dg_load<P>(cc, chi, pitch, col0, j0, xghost);
-    if (!xghost && j0 + 1 < Ny) { dg_prefetch<P>(x, pitch, col0, j0 + 1); if (DIRF) dg_prefetch<P>(src.r, pitch, col0, j0 + 1); }
+    // L1 prefetch, FX_PFD steps ahead: row jr of the input vector (needed as the upper neighbour at step jr-1) and of chi
+    auto pf_x = [&](int jr) {
+        if (xghost || jr > j1) return;
+        if (jr >= Ny) { if (diry) return; jr -= Ny; }
+        dg_prefetch<P>(x, pitch, col0, jr); if (DIRF) dg_prefetch<P>(src.r, pitch, col0, jr);
+    };
+    auto pf_c = [&](int jr) { if (!xghost && jr < j1) dg_prefetch<P>(chi, pitch, col0, jr); };
+#pragma unroll
+    for (int d = 1; d <= FX_PFD; ++d) { pf_x(j0 + d); pf_c(j0 + d); }
 #pragma unroll
     for (int k = 0; k < P; ++k) {
 #define UC(m) uc.v[m][k]
@@ -243,11 +254,7 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
         if (jn == Ny) { jn = 0; yghost = diry; }
         if (j > j0) { if (!DIRF) dg_load_u<P, DIRF>(uc, g, src, pitch, col0, j); dg_load<P>(cc, chi, pitch, col0, j, xghost); }
         dg_load_u<P, DIRF>(un, g, src, pitch, col0, jn);
-        if (j + 1 < j1 && !xghost) {                                 // next step's rows
-            const int j2 = (j + 2 == Ny) ? 0 : j + 2;
-            if (!(j + 2 == Ny && diry)) { dg_prefetch<P>(x, pitch, col0, j2); if (DIRF) dg_prefetch<P>(src.r, pitch, col0, j2); }
-            dg_prefetch<P>(chi, pitch, col0, j + 1);
-        }
+        pf_x(j + 1 + FX_PFD); pf_c(j + FX_PFD);                    // rows of the steps ahead
 
         double tRy[P], tLyn[P], tLx[P], tRx[P];
 #pragma unroll

@@ -52,7 +52,9 @@ k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict_
         const int j0 = seg * g.rows_per_seg;
         int j1 = j0 + g.rows_per_seg;
         if (j1 > g.Ny) j1 = g.Ny;
-        dg_warp_strip<P, true, true, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh);
+        extern __shared__ __align__(16) double dg_smem[];
+        if (P <= 3 && g.smr) dg_warp_strip<P, true, true, true, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, dg_smem + (size_t)(threadIdx.x >> 5) * 8 * P * P * 32);
+        else dg_warp_strip<P, true, true, false, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, nullptr);
     }
     acc.flush(&sh);
     if (ex_block_finish(&sh, ex, 1, 1, &sc->pq) && threadIdx.x == 0) {
@@ -300,7 +302,7 @@ k_cg_persistent(const __grid_constant__ DgParams g, const double* __restrict__ c
                 const int j0 = seg * g.rows_per_seg;
                 int j1 = j0 + g.rows_per_seg;
                 if (j1 > g.Ny) j1 = g.Ny;
-                dg_warp_strip<P, true, true, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh);
+                dg_warp_strip<P, true, true, false, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, nullptr);   // L2-resident grids: generic rows
             }
         }
         acc.flush(&sh);
@@ -419,6 +421,7 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, 
         FX_CUDA(cudaFuncSetAttribute(k_cg_update_tma<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, K2_STAGES * 4 * 2 * 256 * 8));
         attr_done = true;
     }
+    const size_t k1_smem = dp.smr ? fx_dg_ring_bytes(P, ab / 32, true) : 0;
     // K2 fast path: 16-byte aligned vectors (the work vectors always are; phi is the caller's)
     const bool lin = aligned16(phi) && aligned16(r) && aligned16(pbuf0) && aligned16(pbuf1) && aligned16(q);
     int lg;
@@ -437,7 +440,7 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, 
         cudaEvent_t* ev = nullptr;
         if (c->prof_on && c->prof_iters < c->prof_cap) { ev = c->prof_ev + 4 * c->prof_iters; c->prof_iters++; }
         if (ev) cudaEventRecord(ev[0], c->stream);
-        k_cg_dir_apply_dot<P><<<ag, ab, 0, c->stream>>>(dp, chi, pin, r, pout, q, c->ex, sc);
+        k_cg_dir_apply_dot<P><<<ag, ab, k1_smem, c->stream>>>(dp, chi, pin, r, pout, q, c->ex, sc);
         if (ev) cudaEventRecord(ev[1], c->stream);
         if (lin) k_cg_update_tma<P><<<lg, eb, (size_t)K2_STAGES * 4 * 2 * eb * 8, c->stream>>>(dp, pout, q, phi, r, c->ex, sc);
         else k_cg_update<P><<<eg, eb, (size_t)FX_STAGES * 4 * CG_U * eb * 8, c->stream>>>(dp, pout, q, phi, r, c->ex, sc);
@@ -541,7 +544,10 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
             {
                 const void* f = g->P == 1 ? (const void*)k_cg_dir_apply_dot<1> : g->P == 2 ? (const void*)k_cg_dir_apply_dot<2>
                               : g->P == 3 ? (const void*)k_cg_dir_apply_dot<3> : g->P == 4 ? (const void*)k_cg_dir_apply_dot<4> : (const void*)k_cg_dir_apply_dot<5>;
-                FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occb, f, 128, 0));
+                dp.smr = g->P <= 3 ? 1 : 0;
+                const size_t sm = dp.smr ? fx_dg_ring_bytes(g->P, 4, true) : 0;
+                if (sm) FX_CUDA(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+                FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occb, f, 128, sm));
             }
             cg_shapes(c, g, &dp, occb > 0 ? occb * 4 : 4, &ag, &ab, &eg, &eb);
             CgScal* sc = (CgScal*)c->cg_scal;

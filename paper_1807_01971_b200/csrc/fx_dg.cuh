@@ -19,12 +19,14 @@
 #define FX_DG_CUH
 
 #include "fx_exdot.cuh"
+#include "fx_stream.cuh"
 #include "fx_tables.h"
 
 struct DgParams {
     int Nx, Ny, bcx, bcy;          // bc: 0 = periodic, 1 = Dirichlet
     int rows_per_seg, nseg, nstrip;
     int normed;
+    int smr;                       // rows staged through the per-lane shared-memory ring (P <= 3)
     double cxx, cyy;               // hy/hx, hx/hy
     double T0[FX_PMAX][FX_PMAX], T0L[FX_PMAX][FX_PMAX], WW[FX_PMAX][FX_PMAX], V[FX_PMAX][FX_PMAX];
     double B[FX_PMAX], L[FX_PMAX], R[FX_PMAX], JX[FX_PMAX], JY[FX_PMAX];
@@ -83,6 +85,44 @@ __device__ __forceinline__ void dg_load_u(DgCell<P>& c, const DgParams& g, const
                 for (int k = 0; k < P; ++k)
                     c.v[l][k] = __fma_rn(1.0, __dmul_rn(g.V[l][k], rr.v[l][k]), __dmul_rn(s.beta, c.v[l][k]));
         }
+    }
+}
+
+// ---- per-lane shared-memory row ring (SMR path, P <= 3) -------------------------------------------------------------------
+// The generic path above relies on L1 prefetches; rows of one cell lie one image row (a multiple of 8 KB at the
+// benchmark sizes) apart, so they compete for the same L1 sets and ~1/3 of the register loads still miss.  With SMR every
+// lane copies ITS OWN cell of the rows ahead into its own shared-memory slots with cp.async (as the streaming kernels do,
+// fx_stream.cuh) and reads them back after cp.async.wait_group: residency is guaranteed, no barrier, no extra registers.
+// Slot = P*P doubles per lane, lane-interleaved (conflict-free); slots 0..2: input vector rows (sequence number mod 3),
+// 3..4: chi (mod 2), 5..7: r for the fused direction update.
+template <int P>
+__device__ __forceinline__ void smr_issue(double* ring, int slot, const double* __restrict__ a, long long pitch, int col0, int jr) {
+    const double* q = a + (long long)jr * P * pitch + col0;
+    const unsigned dst = fx_smem_addr(ring + (size_t)slot * P * P * 32 + (threadIdx.x & 31));
+#pragma unroll
+    for (int l = 0; l < P; ++l)
+#pragma unroll
+        for (int k = 0; k < P; ++k) fx_cp_async8(dst + (unsigned)((l * P + k) * 32 * 8), q + l * pitch + k, true);
+}
+template <int P>
+__device__ __forceinline__ void smr_read(DgCell<P>& c, const double* ring, int slot) {
+    const double* q = ring + (size_t)slot * P * P * 32 + (threadIdx.x & 31);
+#pragma unroll
+    for (int l = 0; l < P; ++l)
+#pragma unroll
+        for (int k = 0; k < P; ++k) c.v[l][k] = q[(l * P + k) * 32];
+}
+template <int P, bool DIRF>
+__device__ __forceinline__ void smr_read_u(DgCell<P>& c, const DgParams& g, const DgSrc& s, const double* ring, int sq) {
+    smr_read<P>(c, ring, sq % 3);
+    if (DIRF && s.upd) {
+        DgCell<P> rr;
+        smr_read<P>(rr, ring, 5 + sq % 3);
+#pragma unroll
+        for (int l = 0; l < P; ++l)
+#pragma unroll
+            for (int k = 0; k < P; ++k)
+                c.v[l][k] = __fma_rn(1.0, __dmul_rn(g.V[l][k], rr.v[l][k]), __dmul_rn(s.beta, c.v[l][k]));
     }
 }
 
@@ -182,9 +222,10 @@ __device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc
 
 // One warp: strip `strip` of 30 cells, cell rows [j0, j1).  FUSE: feed (x, y) pairs of the produced cells into the
 // exact-dot accumulator `acc` (the CG's p.Sp).
-template <int P, bool FUSE, bool DIRF, class ACC>
+template <int P, bool FUSE, bool DIRF, bool SMR, class ACC>
 __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* __restrict__ chi, const DgSrc& src,
-                                              double* __restrict__ y, int strip, int j0, int j1, ACC* acc, ExShared* sh) {
+                                              double* __restrict__ y, int strip, int j0, int j1, ACC* acc, ExShared* sh,
+                                              double* ring) {
     const double* __restrict__ x = src.x;
     const int lane = threadIdx.x & 31;
     const int Nx = g.Nx, Ny = g.Ny;
@@ -214,8 +255,15 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
         dg_prefetch<P>(x, pitch, col0, jr); if (DIRF) dg_prefetch<P>(src.r, pitch, col0, jr);
     };
     auto pf_c = [&](int jr) { if (!xghost && jr < j1) dg_prefetch<P>(chi, pitch, col0, jr); };
+    auto rowx = [&](int jr) { return jr >= Ny ? jr - Ny : jr; };       // beyond the top: wrap (a Dirichlet ghost row is never used)
+    if (SMR) {
+        smr_issue<P>(ring, 1, x, pitch, col0, rowx(j0 + 1));
+        if (DIRF) smr_issue<P>(ring, 5 + 1, src.r, pitch, col0, rowx(j0 + 1));
+        fx_cp_commit();
+    } else {
 #pragma unroll
-    for (int d = 1; d <= FX_PFD; ++d) { pf_x(j0 + d); pf_c(j0 + d); }
+        for (int d = 1; d <= FX_PFD; ++d) { pf_x(j0 + d); pf_c(j0 + d); }
+    }
 #pragma unroll
     for (int k = 0; k < P; ++k) {
 #define UC(m) uc.v[m][k]
@@ -252,9 +300,22 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
         int jn = j + 1;
         bool yghost = false;
         if (jn == Ny) { jn = 0; yghost = diry; }
-        if (j > j0) { if (!DIRF) dg_load_u<P, DIRF>(uc, g, src, pitch, col0, j); dg_load<P>(cc, chi, pitch, col0, j, xghost); }
-        dg_load_u<P, DIRF>(un, g, src, pitch, col0, jn);
-        pf_x(j + 1 + FX_PFD); pf_c(j + FX_PFD);                    // rows of the steps ahead
+        if (SMR) {
+            const int sq = j - j0;
+            if (j + 1 < j1) {                                        // the rows of the next step
+                smr_issue<P>(ring, (sq + 2) % 3, x, pitch, col0, rowx(j + 2));
+                if (DIRF) smr_issue<P>(ring, 5 + (sq + 2) % 3, src.r, pitch, col0, rowx(j + 2));
+                smr_issue<P>(ring, 3 + ((sq + 1) & 1), chi, pitch, col0, j + 1);
+            }
+            fx_cp_commit();
+            fx_cp_wait<1>();                                         // everything but the group just committed has landed
+            if (j > j0) { if (!DIRF) smr_read_u<P, DIRF>(uc, g, src, ring, sq); smr_read<P>(cc, ring, 3 + (sq & 1)); }
+            smr_read_u<P, DIRF>(un, g, src, ring, sq + 1);
+        } else {
+            if (j > j0) { if (!DIRF) dg_load_u<P, DIRF>(uc, g, src, pitch, col0, j); dg_load<P>(cc, chi, pitch, col0, j, xghost); }
+            dg_load_u<P, DIRF>(un, g, src, pitch, col0, jn);
+            pf_x(j + 1 + FX_PFD); pf_c(j + FX_PFD);                // rows of the steps ahead
+        }
 
         double tRy[P], tLyn[P], tLx[P], tRx[P];
 #pragma unroll
@@ -326,6 +387,7 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
         }
         if (DIRF) uc = un;                                           // formed once per row: carried instead of re-formed
     }
+    if (SMR) fx_cp_wait<0>();
 }
 #undef CL
 #undef CR

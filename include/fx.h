@@ -66,7 +66,7 @@ void fx_shutdown(void);
  * reads it as warps-per-CTA*32 and grid_dim as rows-per-segment).                                              */
 fx_status fx_set_launch(int32_t kernel_id, int32_t grid_dim, int32_t block_dim);
 /* fx_cg_solve driver: 0 = one kernel per primitive, both dots visit the host; 1 (default) = fused: a single persistent
- * cooperative kernel for grids of up to 2^21 unknowns, two fused kernels per iteration above; 2 = always the two fused
+ * cooperative kernel for grids of up to 2^20 unknowns, two fused kernels per iteration above; 2 = always the two fused
  * kernels; 3 = the persistent kernel whenever possible (< 2^24 unknowns).  Results are bit-identical in every mode.      */
 fx_status fx_set_cg_fused(int32_t fused);
 

@@ -559,7 +559,7 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
             // small grids (vectors resident in L2): the whole loop in one cooperative launch.  mode 1 = automatic,
             // 2 = never, 3 = whenever the device allows it (tests)
             bool persistent = false;
-            if ((c->cg_fused == 1 && n <= ((int64_t)1 << 21)) || (c->cg_fused == 3 && n < ((int64_t)1 << 24))) {
+            if ((c->cg_fused == 1 && n <= ((int64_t)1 << 20)) || (c->cg_fused == 3 && n < ((int64_t)1 << 24))) {
                 switch (g->P) {
                 case 1: s = cg_run_persistent<1>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
                 case 2: s = cg_run_persistent<2>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;

@@ -654,6 +654,43 @@ extern "C" int fxo_dg_derivative_definition(const fxo_grid* g, int32_t dir, int3
 }
 
 // ------------------------------------------------------------------------------------------------
+// 6c. Fused pointwise product z <- alpha x1 y1 + beta x2 y2 + gamma z (added "to raise the work per call") and the
+//     Arakawa bracket ("the Arakawa scheme [21]", the second composite the paper benchmarks, Fig. 6a: N = 9 calls).
+//     Canonical order (Q22):  a = RN(alpha*x1); b = RN(beta*x2);
+//         t = gamma == 0 ? RN(b*y2) : fma(b, y2, RN(gamma*z));   z = fma(a, y1, t).
+//     Bracket {f,g} = df/dx dg/dy - df/dy dg/dx in Arakawa's conserving form, the mean of the three equivalent
+//     expressions J1 = fx gy - fy gx, J2 = (f gy)_x - (f gx)_y, J3 = (g fx)_y - (g fy)_x, regrouped by outer derivative:
+//         {f,g} = 1/3 [ fx gy - fy gx  +  Dx( f gy - g fy )  +  Dy( g fx - f gx ) ]      with centred dG derivatives,
+//     evaluated as nine calls: 4 derivatives, 3 fused pointwise products, 2 accumulating derivatives.
+// ------------------------------------------------------------------------------------------------
+extern "C" void fxo_pointwise_dot2(double alpha, const double* x1, const double* y1, double beta, const double* x2, const double* y2,
+                                   double gamma, double* z, int64_t n) {
+    for (int64_t i = 0; i < n; ++i) {
+        double a = alpha * x1[i], b = beta * x2[i], t;
+        if (gamma == 0.0) t = b * y2[i];
+        else { double gz = gamma * z[i]; t = std::fma(b, y2[i], gz); }
+        z[i] = std::fma(a, y1[i], t);
+    }
+}
+
+extern "C" int fxo_arakawa(const fxo_grid* g, const double* f, const double* gg, double* out) {
+    if (!grid_ok(g)) return -1;
+    const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
+    std::vector<double> fx(n), fy(n), gx(n), gy(n), h1(n), h2(n);
+    const double third = 1.0 / 3.0;
+    fxo_dg_derivative_canonical(g, 0, 2, 1.0, f, 0.0, fx.data());
+    fxo_dg_derivative_canonical(g, 1, 2, 1.0, f, 0.0, fy.data());
+    fxo_dg_derivative_canonical(g, 0, 2, 1.0, gg, 0.0, gx.data());
+    fxo_dg_derivative_canonical(g, 1, 2, 1.0, gg, 0.0, gy.data());
+    fxo_pointwise_dot2(third, fx.data(), gy.data(), -third, fy.data(), gx.data(), 0.0, out, n);      // 1/3 (fx gy - fy gx)
+    fxo_pointwise_dot2(third, f, gy.data(), -third, gg, fy.data(), 0.0, h1.data(), n);                // 1/3 (f gy - g fy)
+    fxo_pointwise_dot2(third, gg, fx.data(), -third, f, gx.data(), 0.0, h2.data(), n);                // 1/3 (g fx - f gx)
+    fxo_dg_derivative_canonical(g, 0, 2, 1.0, h1.data(), 1.0, out);                                  // += Dx(...)
+    fxo_dg_derivative_canonical(g, 1, 2, 1.0, h2.data(), 1.0, out);                                  // += Dy(...)
+    return 0;
+}
+
+// ------------------------------------------------------------------------------------------------
 // 7. Preconditioned CG, step by step (Level-2 algorithm built from Level-1 calls only; the
 //    exact dot "is for example important in a conjugate gradient method").  DESIGN.md 3.5.
 //    Solves  div(chi grad phi) = rho  as  S phi = W o (-rho),  preconditioner V = 1/W.

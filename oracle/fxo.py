@@ -91,6 +91,10 @@ def lib():
         L.fxo_dg_derivative_matrix_1d.argtypes = [C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_int32, dp]
         L.fxo_dg_derivative_definition.restype = C.c_int
         L.fxo_dg_derivative_definition.argtypes = [gp, C.c_int32, C.c_int32, C.c_double, dp, C.c_double, dp, dp, dp]
+        L.fxo_pointwise_dot2.restype = None
+        L.fxo_pointwise_dot2.argtypes = [C.c_double, dp, dp, C.c_double, dp, dp, C.c_double, dp, C.c_int64]
+        L.fxo_arakawa.restype = C.c_int
+        L.fxo_arakawa.argtypes = [gp, dp, dp, dp]
         L.fxo_cg_solve.restype = C.c_int
         L.fxo_cg_solve.argtypes = [gp, dp, dp, dp, C.c_double, C.c_int32, C.POINTER(CGInfo)]
         _lib = L
@@ -256,6 +260,23 @@ def dg_derivative_definition(g, direction, flux, alpha, x, beta, y):
     if lib().fxo_dg_derivative_definition(C.byref(g), direction, flux, alpha, _p(x), beta, _p(y), _p(out), _p(sc)) != 0:
         raise ValueError("bad arguments")
     return out, sc
+
+
+def pointwise_dot2(alpha, x1, y1, beta, x2, y2, gamma, z):
+    """z <- alpha*x1*y1 + beta*x2*y2 + gamma*z in the canonical order (returns the updated copy of z)"""
+    x1, y1, x2, y2 = (_f64(a).ravel() for a in (x1, y1, x2, y2))
+    z = np.array(z, dtype=np.float64).ravel().copy()
+    lib().fxo_pointwise_dot2(alpha, _p(x1), _p(y1), beta, _p(x2), _p(y2), gamma, _p(z), z.size)
+    return z
+
+
+def arakawa(g, f, gg):
+    """Arakawa bracket {f,g} with centred dG derivatives (nine canonical calls)"""
+    f, gg = _f64(f).ravel(), _f64(gg).ravel()
+    out = np.zeros(g.n)
+    if lib().fxo_arakawa(C.byref(g), _p(f), _p(gg), _p(out)) != 0:
+        raise ValueError("bad grid")
+    return out
 
 
 def cg_solve(g, chi, rho, phi0, tol, maxit):

@@ -103,3 +103,43 @@ def test_matrix_matches_2d_application(oracle):
     gx = oracle.dg_derivative_canonical(g, 0, FWD, 1.0, x, 0.0, np.zeros(g.n)).reshape(X.shape)
     gy = oracle.dg_derivative_canonical(g, 1, BWD, 1.0, x, 0.0, np.zeros(g.n)).reshape(X.shape)
     assert np.allclose(gx, X @ Mx.T, atol=1e-12) and np.allclose(gy, My @ X, atol=1e-12)
+
+
+# ---- fused pointwise product and the Arakawa bracket (Q22) ----------------------------------
+
+def test_pointwise_dot2_pins(oracle):
+    from fractions import Fraction
+    rng = fi.rng(777)
+    n = 300
+    ints = lambda: rng.integers(-50, 50, n).astype(float)           # small integers: no rounding anywhere
+    x1, y1, x2, y2, z = ints(), ints(), ints(), ints(), ints()
+    got = oracle.pointwise_dot2(2.0, x1, y1, -3.0, x2, y2, 5.0, z)
+    assert np.array_equal(got, 2 * x1 * y1 - 3 * x2 * y2 + 5 * z)
+    assert np.array_equal(oracle.pointwise_dot2(2.0, x1, y1, -3.0, x2, y2, 0.0, np.full(n, np.nan)), 2 * x1 * y1 - 3 * x2 * y2)
+    # reduces to pointwise_dot when beta = 0 (b*y2 = 0 exactly, fma(a, y1, 0 or RN(gamma z)))
+    u, v, w = fi.uniform(1, n), fi.uniform(2, n), fi.uniform(3, n)
+    assert np.array_equal(oracle.pointwise_dot2(0.7, u, v, 0.0, u, v, -0.3, w), oracle.pointwise_dot(0.7, u, v, -0.3, w))
+
+
+@pytest.mark.parametrize("P", [2, 3, 4])
+def test_arakawa_converges_and_conserves(oracle, P):
+    """{f,g} -> analytic Poisson bracket with order ~P-1; Arakawa's conservation: int J = int f J = int g J = 0 (periodic)"""
+    errs = []
+    for N in (8, 16, 32):
+        g = oracle.Grid(N, N, P, 2 * math.pi, 2 * math.pi, 0, 0)
+        xs, ys = oracle.dg_nodes(g)
+        X, Y = np.meshgrid(xs, ys)
+        f, gg = np.sin(X) * np.cos(Y), np.cos(X) * np.sin(2 * Y) + 0.3 * np.sin(X + Y)
+        fx_, fy_ = np.cos(X) * np.cos(Y), -np.sin(X) * np.sin(Y)
+        gx_, gy_ = -np.sin(X) * np.sin(2 * Y) + 0.3 * np.cos(X + Y), 2 * np.cos(X) * np.cos(2 * Y) + 0.3 * np.cos(X + Y)
+        exact = (fx_ * gy_ - fy_ * gx_).ravel()
+        J = oracle.arakawa(g, f.ravel(), gg.ravel())
+        W, _ = oracle.dg_weights(g)
+        errs.append(math.sqrt(np.sum(W * (J - exact) ** 2) / np.sum(W * exact ** 2)))
+        scale = np.sum(W * np.abs(J))
+        assert abs(oracle.exdot(W, J)) < 1e-12 * scale                                   # int {f,g} = 0
+        assert abs(oracle.exdot3(f.ravel(), W, J)) < 1e-12 * scale                       # int f {f,g} = 0
+        assert abs(oracle.exdot3(gg.ravel(), W, J)) < 1e-12 * scale                      # int g {f,g} = 0
+        Jr = oracle.arakawa(g, gg.ravel(), f.ravel())
+        assert np.max(np.abs(J + Jr)) < 1e-12 * np.max(np.abs(J))                        # antisymmetry
+    assert errs[2] < errs[1] < errs[0] and math.log2(errs[1] / errs[2]) > P - 1.5

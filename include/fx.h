@@ -106,6 +106,12 @@ fx_status fx_axpby(double alpha, const double* x_dev, double beta, double* y_dev
 fx_status fx_pointwise_dot(double alpha, const double* x1_dev, const double* x2_dev, double beta, double* y_dev,
                            int64_t n);
 
+/* z[i] <- alpha*x1[i]*y1[i] + beta*x2[i]*y2[i] + gamma*z[i], the fused product the paper adds "to raise the work per call"
+ * (P:414).  Canonical order (D:Q22): a = RN(alpha*x1); b = RN(beta*x2); t = gamma == 0 ? RN(b*y2) : fma(b, y2, RN(gamma*z));
+ * z = fma(a, y1, t).  gamma == 0: z is not read.  Inputs may alias each other and z.                                     */
+fx_status fx_pointwise_dot2(double alpha, const double* x1_dev, const double* y1_dev, double beta, const double* x2_dev,
+                            const double* y2_dev, double gamma, double* z_dev, int64_t n);
+
 /* ---- dG elliptic operator (construction D:3.3, operation order D:3.4) -------------------------
  * S = Fx^T diag(W chi) Fx + Fy^T diag(W chi) Fy + (jump terms), symmetric; A = diag(V) S ~ -div(chi grad .),
  * V = 1/W the inverse dG weights.  chi, x, y: device vectors of the grid; y must not overlap x or chi.         */
@@ -123,6 +129,10 @@ fx_status fx_dg_tables(int32_t P, double* out_host);
  * 2 = centred (their mean).  x, y: device vectors of the grid; y must not overlap x.                                   */
 fx_status fx_dg_derivative(const fx_grid* grid, int32_t direction, int32_t flux, double alpha, const double* x_dev, double beta,
                            double* y_dev);
+/* Arakawa bracket out = {f, g} = f_x g_y - f_y g_x in Arakawa's conserving form with centred dG derivatives (the
+ * second composite the paper benchmarks, Fig. 6a), evaluated as the nine calls of D:6.8: 4 derivatives, 3 fused pointwise
+ * products, 2 accumulating derivatives.  f, g, out: device vectors of the grid; out must not overlap f or g.            */
+fx_status fx_arakawa(const fx_grid* grid, const double* f_dev, const double* g_dev, double* out_dev);
 /* The derivative tables for the cross-check against the oracle: host double[2*P*P + 2*P] = TT interior, TT first
  * Dirichlet cell (P*P each, row-major), cN, cP.  No GPU.                                                               */
 fx_status fx_dg_dtables(int32_t P, int32_t flux, double* out_host);

@@ -52,6 +52,8 @@ _SIGNATURES = {
     "fx_exdot_f32": (C.c_double, [_vp, _vp, C.c_int64]),
     "fx_axpby": (C.c_int, [C.c_double, _vp, C.c_double, _vp, C.c_int64]),
     "fx_pointwise_dot": (C.c_int, [C.c_double, _vp, _vp, C.c_double, _vp, C.c_int64]),
+    "fx_pointwise_dot2": (C.c_int, [C.c_double, _vp, _vp, C.c_double, _vp, _vp, C.c_double, _vp, C.c_int64]),
+    "fx_arakawa": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp]),
     "fx_dg_elliptic_apply": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp]),
     "fx_dg_elliptic_apply_sym": (C.c_int, [C.POINTER(Grid), _vp, _vp, _vp]),
     "fx_dg_weights": (C.c_int, [C.POINTER(Grid), _vp, _vp]),
@@ -220,6 +222,22 @@ def pointwise_dot(alpha, x1, x2, beta, y):
     n = y.numel()
     _check(lib().fx_pointwise_dot(float(alpha), _ptr(x1, n), _ptr(x2, n), float(beta), _ptr(y), n), "fx_pointwise_dot")
     return y
+
+
+def pointwise_dot2(alpha, x1, y1, beta, x2, y2, gamma, z):
+    """z <- alpha*x1*y1 + beta*x2*y2 + gamma*z (in place; returns z).  PAPER.md:414."""
+    _use_torch_stream()
+    n = z.numel()
+    _check(lib().fx_pointwise_dot2(float(alpha), _ptr(x1, n), _ptr(y1, n), float(beta), _ptr(x2, n), _ptr(y2, n), float(gamma), _ptr(z), n),
+           "fx_pointwise_dot2")
+    return z
+
+
+def arakawa(grid, f, g, out):
+    """out = {f, g}: Arakawa bracket with centred dG derivatives (nine primitive calls).  PAPER.md:240, Fig. 6a."""
+    _use_torch_stream()
+    _check(lib().fx_arakawa(C.byref(grid), _ptr(f, grid.n), _ptr(g, grid.n), _ptr(out, grid.n)), "fx_arakawa")
+    return out
 
 
 def dg_elliptic_apply(grid, chi, x, y, sym=False):

@@ -227,3 +227,31 @@ extern "C" fx_status fx_dg_dtables(int32_t P, int32_t flux, double* out) {
     for (int k = 0; k < P; ++k) *o++ = d.cP[k];
     return FX_OK;
 }
+
+// ---- Arakawa bracket as the paper runs it: nine calls of the primitives --------------------------------
+extern "C" fx_status fx_arakawa(const fx_grid* g, const double* f, const double* gg, double* out) {
+    if (!fx_grid_ok(g) || !f || !gg || !out) { fx_set_error("fx_arakawa: bad grid or null pointer"); return FX_EINVAL; }
+    const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
+    if ((f < out + n && out < f + n) || (gg < out + n && out < gg + n)) { fx_set_error("fx_arakawa: out overlaps an input"); return FX_EINVAL; }
+    FxCtx* c = fx_ctx();
+    if (!c) return FX_ECUDA;
+    if (c->ara_cap < n) {
+        if (c->ara_vec) { cudaStreamSynchronize(c->stream); cudaFree(c->ara_vec); c->ara_vec = nullptr; c->ara_cap = 0; }
+        if (cudaMalloc(&c->ara_vec, (size_t)6 * n * sizeof(double)) != cudaSuccess) {
+            fx_set_error("Arakawa work space: %s", cudaGetErrorString(cudaGetLastError())); return FX_ENOMEM;
+        }
+        c->ara_cap = n;
+    }
+    double *fx_ = c->ara_vec, *fy_ = fx_ + n, *gx_ = fy_ + n, *gy_ = gx_ + n, *h1 = gy_ + n, *h2 = h1 + n;
+    const double third = 1.0 / 3.0;
+    fx_status s;
+    if ((s = fx_launch_derivative(c, g, 0, 2, 1.0, f, 0.0, fx_)) != FX_OK) return s;
+    if ((s = fx_launch_derivative(c, g, 1, 2, 1.0, f, 0.0, fy_)) != FX_OK) return s;
+    if ((s = fx_launch_derivative(c, g, 0, 2, 1.0, gg, 0.0, gx_)) != FX_OK) return s;
+    if ((s = fx_launch_derivative(c, g, 1, 2, 1.0, gg, 0.0, gy_)) != FX_OK) return s;
+    if ((s = fx_pointwise_dot2(third, fx_, gy_, -third, fy_, gx_, 0.0, out, n)) != FX_OK) return s;     // 1/3 (fx gy - fy gx)
+    if ((s = fx_pointwise_dot2(third, f, gy_, -third, gg, fy_, 0.0, h1, n)) != FX_OK) return s;          // 1/3 (f gy - g fy)
+    if ((s = fx_pointwise_dot2(third, gg, fx_, -third, f, gx_, 0.0, h2, n)) != FX_OK) return s;          // 1/3 (g fx - f gx)
+    if ((s = fx_launch_derivative(c, g, 0, 2, 1.0, h1, 1.0, out)) != FX_OK) return s;                   // += Dx(...)
+    return fx_launch_derivative(c, g, 1, 2, 1.0, h2, 1.0, out);                                         // += Dy(...)
+}

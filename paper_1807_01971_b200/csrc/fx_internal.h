@@ -27,6 +27,7 @@ struct FxCtx {
     double* cg_vec; int64_t cg_cap;   // 7 vectors of cg_cap doubles
     void* cg_scal;                     // CgScal on the device
     void* cg_scal_pinned;
+    double* ara_vec; int64_t ara_cap;  // six work vectors of fx_arakawa
     void* cg_pdig;                     // digit buffers of the persistent CG kernel
     cudaEvent_t cg_ev[2];
     // host staging for the *_host entry points

@@ -532,3 +532,40 @@ def test_exdot_f32(fx, oracle, n):
     assert fbits(fx.exdot_f32(dx, dy)) == fbits(oracle.exdot_f32(x, y) if n else 0.0)
     if n > 4:
         assert fbits(fx.exdot_f32(dx[1:], dy[1:])) == fbits(oracle.exdot_f32(x[1:], y[1:]))      # 4-byte aligned only
+
+
+# ---- fused pointwise product and Arakawa bracket --------------------------------------------------------
+
+@pytest.mark.parametrize("n", [1, 1023, 100003])
+@pytest.mark.parametrize("gamma", [0.0, -0.4])
+def test_pointwise_dot2_bit_exact(fx, oracle, n, gamma):
+    a = [fi.uniform(501 + i, n) for i in range(5)]
+    want = oracle.pointwise_dot2(0.7, a[0], a[1], -1.3, a[2], a[3], gamma, a[4])
+    z = dev(a[4]) if gamma != 0.0 else dev(np.full(n, np.nan))
+    got = fx.pointwise_dot2(0.7, dev(a[0]), dev(a[1]), -1.3, dev(a[2]), dev(a[3]), gamma, z).cpu().numpy()
+    assert same_bits(got, want)
+    zz = dev(a[0])                                                     # everything aliased
+    assert same_bits(fx.pointwise_dot2(0.5, zz, zz, 2.0, zz, zz, 1.0, zz).cpu().numpy(), oracle.pointwise_dot2(0.5, a[0], a[0], 2.0, a[0], a[0], 1.0, a[0]))
+
+
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
+def test_arakawa_bit_exact(fx, oracle, P):
+    import torch
+    for (Nx, Ny, bcx, bcy) in [(1, 1, 0, 0), (7, 5, 0, 1), (33, 12, 1, 0), (64, 40, 0, 0)]:
+        g, og = _grid(fx, oracle, Nx, Ny, P, bcx, bcy)
+        f, gg = fi.uniform(511 + P, g.n), fi.uniform(512 + P, g.n)
+        want = oracle.arakawa(og, f, gg)
+        out = torch.full((g.n,), float("nan"), dtype=torch.float64, device="cuda")
+        fx.arakawa(g, dev(f), dev(gg), out)
+        assert np.array_equal(out.cpu().numpy(), want), (Nx, Ny, P)
+    g, og = _grid(fx, oracle, 256, 256, 3, 0, 0, 2 * math.pi, 2 * math.pi)      # conservation on the GPU result
+    xs, ys = oracle.dg_nodes(og)
+    X, Y = np.meshgrid(xs, ys)
+    f, gg = (np.sin(X) * np.cos(Y)).ravel(), (np.cos(X) * np.sin(2 * Y)).ravel()
+    out = torch.empty(g.n, dtype=torch.float64, device="cuda")
+    fx.arakawa(g, dev(f), dev(gg), out)
+    W = torch.empty_like(out)
+    fx.dg_weights(g, W, None)
+    scale = float((W * out.abs()).sum())
+    assert abs(fx.exdot(W, out)) < 1e-12 * scale and abs(fx.exdot3(dev(f), W, out)) < 1e-12 * scale
+    assert np.array_equal(out.cpu().numpy(), oracle.arakawa(og, f, gg))

@@ -207,6 +207,11 @@ def run_fx(args):
                 fx.time_primitive(kind, pvec, chi, q, 3, grid=g)
                 tt = fx.time_primitive(kind, pvec, chi, q, 20, grid=g)
                 prim[kind] = {"grid": "%dx%d P=3" % (N, N), "ms": tt, "GBps": 24.0 * n / tt / 1e6, "frac_of_peak": 24.0 * n / tt / 1e6 / peak}
+            fx.time_primitive("arakawa", pvec, chi, q, 3, grid=g)        # the paper's second composite (Fig. 6a): 9 calls
+            tt = fx.time_primitive("arakawa", pvec, chi, q, 10, grid=g)
+            prim["arakawa"] = {"grid": "%dx%d P=3" % (N, N), "ms": tt, "calls": 9, "vector_passes": 29,
+                               "GBps": 29 * 8.0 * n / tt / 1e6, "frac_of_peak": 29 * 8.0 * n / tt / 1e6 / peak,
+                               "note": "unfused composite as in the paper (N = 9; the paper counts M = 34 passes, its ideal fused form M = 4)"}
             prim["dg_apply"] = {"grid": "%dx%d P=3" % (N, N), "n": n, "MB_per_vector": 8e-6 * n, "ms": t, "GBps": 24.0 * n / t / 1e6,
                                 "frac_of_peak": 24.0 * n / t / 1e6 / peak, "note": "3 x 75.5 MB partly L2-resident between repeats"}
 

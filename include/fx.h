@@ -161,8 +161,8 @@ fx_status fx_cg_last_profile(double* ms_host, int32_t* iterations_host);
  * 1 = axpby(0.7,a,-0.3,c), 2 = pointwise_dot(1,a,b,0,c), 3 = dG apply_sym(grid; chi=a, x=b, y=c), 4 = dG apply (normed),
  * 5 = exdot(a,b) returned to the host every call (the paper's GPU dot latency), 6 = axpby(0.7,a,1,c),
  * 7 = weighted dot(a,b,c) device-resident, 8 = exact sum(a) device-resident; with a grid: 9/10 = d/dx, d/dy forward,
- * 11/12 = d/dx, d/dy centred, each as c <- 0.7 M a - 0.3 c.
- * a, b, c: device vectors of n doubles (kinds 3,4,9-12: n must equal the grid's size).  Synchronises.               */
+ * 11/12 = d/dx, d/dy centred, each as c <- 0.7 M a - 0.3 c; 13 = Arakawa bracket c = {a, b} (nine calls).
+ * a, b, c: device vectors of n doubles (kinds 3,4,9-13: n must equal the grid's size).  Synchronises.               */
 fx_status fx_time_primitive(int32_t kind, const fx_grid* grid, const double* a_dev, const double* b_dev, double* c_dev,
                             int64_t n, int32_t reps, double* ms_host);
 

@@ -296,7 +296,7 @@ def cg_solve(grid, chi, rho, phi, tol, maxit):
     return info
 
 
-TIME_KINDS = {"exdot": 0, "axpby": 1, "pointwise_dot": 2, "dg_apply_sym": 3, "dg_apply": 4, "exdot_host": 5, "axpy": 6, "exdot3": 7, "exsum": 8, "dx_forward": 9, "dy_forward": 10, "dx_centered": 11, "dy_centered": 12}
+TIME_KINDS = {"exdot": 0, "axpby": 1, "pointwise_dot": 2, "dg_apply_sym": 3, "dg_apply": 4, "exdot_host": 5, "axpy": 6, "exdot3": 7, "exsum": 8, "dx_forward": 9, "dy_forward": 10, "dx_centered": 11, "dy_centered": 12, "arakawa": 13}
 
 
 def time_primitive(kind, a, b, c, reps, grid=None):

@@ -629,13 +629,14 @@ static fx_status time_one(FxCtx* c, int kind, const fx_grid* g, const double* a,
     case 10: return fx_launch_derivative(c, g, 1, 0, 0.7, a, -0.3, cc);
     case 11: return fx_launch_derivative(c, g, 0, 2, 0.7, a, -0.3, cc);
     case 12: return fx_launch_derivative(c, g, 1, 2, 0.7, a, -0.3, cc);
+    case 13: return fx_arakawa(g, a, b, cc);
     }
     return FX_EINVAL;
 }
 
 extern "C" fx_status fx_time_primitive(int32_t kind, const fx_grid* g, const double* a, const double* b, double* cc, int64_t n,
                                        int32_t reps, double* ms_host) {
-    if (kind < 0 || kind > 12 || n < 0 || reps < 1 || !ms_host || !a || !b || !cc) { fx_set_error("fx_time_primitive: bad arguments"); return FX_EINVAL; }
+    if (kind < 0 || kind > 13 || n < 0 || reps < 1 || !ms_host || !a || !b || !cc) { fx_set_error("fx_time_primitive: bad arguments"); return FX_EINVAL; }
     if ((kind == 3 || kind == 4 || kind >= 9) && (!fx_grid_ok(g) || (int64_t)g->Nx * g->Ny * g->P * g->P != n)) { fx_set_error("fx_time_primitive: bad grid"); return FX_EINVAL; }
     FxCtx* c = fx_ctx();
     if (!c) return FX_ECUDA;

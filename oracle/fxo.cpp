@@ -300,13 +300,21 @@ extern "C" int fxo_dg_tables(int32_t P, double* out) {
 //        idx = ((j*P + l)*Nx + i)*P + k     cell (i,j), node (k,l)
 // ------------------------------------------------------------------------------------------------
 
-struct fxo_grid { int32_t Nx, Ny, P; double lx, ly; int32_t bcx, bcy; };   // bc: 0 = PER, 1 = DIR
-enum { BC_PER = 0, BC_DIR = 1 };
+struct fxo_grid { int32_t Nx, Ny, P; double lx, ly; int32_t bcx, bcy; };
+// bc of one direction: 0 = PER, 1 = DIR (both walls), 2 = NEU (both walls), 3 = DIR_NEU (Dirichlet at the lower wall,
+// Neumann at the upper one), 4 = NEU_DIR.  NEU and the mixed kinds: SURVEY 8f-4, reading DESIGN.md Q23.
+enum { BC_PER = 0, BC_DIR = 1, BC_NEU = 2, BC_DIR_NEU = 3, BC_NEU_DIR = 4 };
+static int wall_lo(int bc) { return bc == BC_PER ? BC_PER : (bc == BC_DIR || bc == BC_DIR_NEU) ? BC_DIR : BC_NEU; }
+static int wall_hi(int bc) { return bc == BC_PER ? BC_PER : (bc == BC_DIR || bc == BC_NEU_DIR) ? BC_DIR : BC_NEU; }
+static bool bc_ok(int bc, int N) { return bc >= BC_PER && bc <= BC_NEU_DIR && !(bc == BC_DIR_NEU && N < 2); }
 
 static int grid_ok(const fxo_grid* g) {
     return g && g->Nx >= 1 && g->Ny >= 1 && g->P >= 1 && g->P <= PMAX && g->lx > 0 && g->ly > 0 &&
-           (g->bcx == BC_PER || g->bcx == BC_DIR) && (g->bcy == BC_PER || g->bcy == BC_DIR);
+           bc_ok(g->bcx, g->Nx) && bc_ok(g->bcy, g->Ny);
 }
+
+// the stand-alone derivatives and the bracket are defined for PER and DIR only (Q21, Q23)
+static bool deriv_bc_ok(const fxo_grid* g) { return g->bcx <= BC_DIR && g->bcy <= BC_DIR; }
 
 static inline int64_t gidx(const fxo_grid* g, int i, int j, int k, int l) {
     return (((int64_t)j * g->P + l) * g->Nx + i) * g->P + k;
@@ -343,10 +351,14 @@ extern "C" int fxo_dg_nodes(const fxo_grid* g, double* xs, double* ys) {
 //    The paper names the construction only by reference (dG derivatives [21], elliptic
 //    discretisation after [12],[6]); the reading is DESIGN.md 3.3 / Q8:
 //      F(N,h,bc): forward-flux derivative.  block row n:
-//          F[n][n]   = (2/h) (D - W^-1 R R^T)            (+ (2/h) W^-1 L L^T  if n==0 and bc==DIR)
-//          F[n][n+1] = (2/h)  W^-1 R L^T                 (PER: n+1 mod N;  DIR: absent for n==N-1)
+//          F[n][n]   = (2/h) (D - W^-1 R R^T)            (+ (2/h) W^-1 L L^T  if n==0 and the lower wall is DIR)
+//          F[n][n+1] = (2/h)  W^-1 R L^T                 (PER: n+1 mod N;  walls: absent for n==N-1)
 //      J(N,bc): jump  sum_faces [v][u], un-normed.  block row n:
-//          J[n][n] = R R^T + L L^T,  J[n][n+1] = -R L^T,  J[n][n-1] = -L R^T   (PER wraps; DIR: absent)
+//          J[n][n] = R R^T + L L^T,  J[n][n+1] = -R L^T,  J[n][n-1] = -L R^T   (PER wraps; walls: absent)
+//      Neumann wall (Q23): the ghost cell mirrors the interior trace, so the face carries neither a jump nor a
+//      flux correction: at an upper NEU wall F[N-1][N-1] = (2/h) D (the -W^-1 R R^T term cancels against the
+//      mirrored neighbour) and J[N-1][N-1] = L L^T; at a lower NEU wall F[0][0] is the interior block (the forward
+//      flux takes the cell's own value there anyway) and J[0][0] = R R^T.
 //      S = Fx^T diag(W chi) Fx + Fy^T diag(W chi) Fy + diag(Wy) (x) Jx + Jy (x) diag(Wx),  A = diag(V) S.
 // ------------------------------------------------------------------------------------------------
 
@@ -356,8 +368,9 @@ static void build_F(const RefElem& e, int N, q128 h, int bc, std::vector<q128>& 
     F.assign((size_t)n * n, 0);
     q128 s = 2 / h;
     for (int c = 0; c < N; ++c) for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m) {
-        q128 d = e.D[k][m] - e.R[k] * e.R[m] / e.w[k];
-        if (c == 0 && bc == BC_DIR) d += e.L[k] * e.L[m] / e.w[k];
+        q128 d = e.D[k][m];
+        if (!(c == N - 1 && wall_hi(bc) == BC_NEU)) d -= e.R[k] * e.R[m] / e.w[k];
+        if (c == 0 && wall_lo(bc) == BC_DIR) d += e.L[k] * e.L[m] / e.w[k];
         F[(size_t)(c * P + k) * n + (c * P + m)] += s * d;
         int cn = c + 1;
         if (cn == N) { if (bc == BC_PER) cn = 0; else continue; }
@@ -369,7 +382,8 @@ static void build_J(const RefElem& e, int N, int bc, std::vector<q128>& J) {
     int P = e.P, n = N * P;
     J.assign((size_t)n * n, 0);
     for (int c = 0; c < N; ++c) for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m) {
-        J[(size_t)(c * P + k) * n + (c * P + m)] += e.R[k] * e.R[m] + e.L[k] * e.L[m];
+        if (!(c == N - 1 && wall_hi(bc) == BC_NEU)) J[(size_t)(c * P + k) * n + (c * P + m)] += e.R[k] * e.R[m];
+        if (!(c == 0 && wall_lo(bc) == BC_NEU)) J[(size_t)(c * P + k) * n + (c * P + m)] += e.L[k] * e.L[m];
         int cn = c + 1, cp = c - 1;
         if (cn == N) cn = (bc == BC_PER) ? 0 : -1;
         if (cp < 0) cp = (bc == BC_PER) ? N - 1 : -1;
@@ -468,9 +482,16 @@ static void line_ops(const Tables& t, int N, int bc, const double* u, const doub
     }
     if (bc == BC_PER) { tL[N + 1] = tL[1]; tR[0] = tR[N]; tL[0] = tL[N]; tR[N + 1] = tR[1]; }
     else { tL[N + 1] = 0; tR[0] = 0; tL[0] = 0; tR[N + 1] = 0; }
+    // cell tables: T0L in the first cell of a line that starts at a DIR wall; D in the last cell of a line that ends
+    // at a NEU wall (Q23; with the zero ghost trace above, step 2 then gives the plain in-cell derivative there)
+    auto table = [&](int n) -> const double (*)[PMAX] {
+        if (n == 0 && wall_lo(bc) == BC_DIR) return t.T0L;
+        if (n == N - 1 && wall_hi(bc) == BC_NEU) return t.D;
+        return t.T0;
+    };
     // steps 2,3: reference gradient, flux, flux trace
     for (int n = 0; n < N; ++n) {
-        const double (*T)[PMAX] = (n == 0 && bc == BC_DIR) ? t.T0L : t.T0;
+        const double (*T)[PMAX] = table(n);
         double aB = 0;
         for (int k = 0; k < P; ++k) {
             double a = T[k][0] * u[n * P];
@@ -485,9 +506,12 @@ static void line_ops(const Tables& t, int N, int bc, const double* u, const doub
     tB[0] = (bc == BC_PER) ? tB[N] : 0;
     // steps 4,5: adjoint and jump
     for (int n = 0; n < N; ++n) {
-        const double (*T)[PMAX] = (n == 0 && bc == BC_DIR) ? t.T0L : t.T0;
-        double dl = tL[n + 1] - tR[n];          // own left trace - left neighbour's right trace
-        double dr = tR[n + 1] - tL[n + 2];      // own right trace - right neighbour's left trace
+        const double (*T)[PMAX] = table(n);
+        // the jump's ghost at a NEU wall is the mirror image of the cell's own trace: the difference is +0
+        double gR = (n == 0 && wall_lo(bc) == BC_NEU) ? tL[1] : tR[n];
+        double gL = (n == N - 1 && wall_hi(bc) == BC_NEU) ? tR[N] : tL[n + 2];
+        double dl = tL[n + 1] - gR;             // own left trace - left neighbour's right trace
+        double dr = tR[n + 1] - gL;             // own right trace - right neighbour's left trace
         for (int k = 0; k < P; ++k) {
             double a = T[0][k] * f[(size_t)n * P];
             for (int m = 1; m < P; ++m) a = std::fma(T[m][k], f[(size_t)n * P + m], a);
@@ -593,7 +617,7 @@ static void dline_canonical(const DTab& d, int P, int N, int bc, double s, const
 
 extern "C" int fxo_dg_derivative_canonical(const fxo_grid* g, int32_t dir, int32_t flux, double alpha, const double* x, double beta,
                                            double* y) {
-    if (!grid_ok(g) || dir < 0 || dir > 1 || flux < 0 || flux > 2 || x == y) return -1;
+    if (!grid_ok(g) || !deriv_bc_ok(g) || dir < 0 || dir > 1 || flux < 0 || flux > 2 || x == y) return -1;
     const int P = g->P, nx = g->Nx * P, ny = g->Ny * P;
     DTab d; make_dtab(P, flux, d);
     const int N = dir == 0 ? g->Nx : g->Ny, len = N * P, bc = dir == 0 ? g->bcx : g->bcy;
@@ -614,6 +638,7 @@ extern "C" int fxo_dg_derivative_canonical(const fxo_grid* g, int32_t dir, int32
 
 // definition: explicit matrices, 113 bit; M (rounded to double) is also returned for the numpy-side pins
 extern "C" int fxo_dg_derivative_matrix_1d(int32_t N, int32_t P, double h, int32_t bc, int32_t flux, double* M_out) {
+    if (bc != BC_PER && bc != BC_DIR) return -1;
     if (N < 1 || P < 1 || P > PMAX || !(h > 0) || flux < 0 || flux > 2) return -1;
     RefElem e; ref_elem(P, e);
     std::vector<q128> F; build_F(e, N, (q128)h, bc, F);
@@ -627,7 +652,7 @@ extern "C" int fxo_dg_derivative_matrix_1d(int32_t N, int32_t P, double h, int32
 
 extern "C" int fxo_dg_derivative_definition(const fxo_grid* g, int32_t dir, int32_t flux, double alpha, const double* x, double beta,
                                             const double* y_in, double* y_out, double* scale) {
-    if (!grid_ok(g) || dir < 0 || dir > 1 || flux < 0 || flux > 2) return -1;
+    if (!grid_ok(g) || !deriv_bc_ok(g) || dir < 0 || dir > 1 || flux < 0 || flux > 2) return -1;
     const int P = g->P, nx = g->Nx * P, ny = g->Ny * P;
     RefElem e; ref_elem(P, e);
     const int N = dir == 0 ? g->Nx : g->Ny, len = N * P, bc = dir == 0 ? g->bcx : g->bcy;
@@ -674,7 +699,7 @@ extern "C" void fxo_pointwise_dot2(double alpha, const double* x1, const double*
 }
 
 extern "C" int fxo_arakawa(const fxo_grid* g, const double* f, const double* gg, double* out) {
-    if (!grid_ok(g)) return -1;
+    if (!grid_ok(g) || !deriv_bc_ok(g)) return -1;
     const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
     std::vector<double> fx(n), fy(n), gx(n), gy(n), h1(n), h2(n);
     const double third = 1.0 / 3.0;

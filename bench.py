@@ -212,6 +212,12 @@ def run_fx(args):
             prim["arakawa"] = {"grid": "%dx%d P=3" % (N, N), "ms": tt, "calls": 9, "vector_passes": 29,
                                "GBps": 29 * 8.0 * n / tt / 1e6, "frac_of_peak": 29 * 8.0 * n / tt / 1e6 / peak,
                                "note": "unfused composite as in the paper (N = 9; the paper counts M = 34 passes, its ideal fused form M = 4)"}
+            gneu = fx.make_grid(N, N, 3, cfg["grid"]["lx"], cfg["grid"]["ly"], fx.NEU, fx.DIR_NEU)   # Neumann / mixed walls
+            for _ in range(3):
+                fx.dg_elliptic_apply(gneu, chi, pvec, q, sym=True)
+            tn = time_events(lambda: fx.dg_elliptic_apply(gneu, chi, pvec, q, sym=True), 20, torch)
+            prim["dg_apply_neumann"] = {"grid": "%dx%d P=3, bcx NEU, bcy DIR_NEU" % (N, N), "ms": tn, "GBps": 24.0 * n / tn / 1e6,
+                                        "frac_of_peak": 24.0 * n / tn / 1e6 / peak}
             prim["dg_apply"] = {"grid": "%dx%d P=3" % (N, N), "n": n, "MB_per_vector": 8e-6 * n, "ms": t, "GBps": 24.0 * n / t / 1e6,
                                 "frac_of_peak": 24.0 * n / t / 1e6 / peak, "note": "3 x 75.5 MB partly L2-resident between repeats"}
 

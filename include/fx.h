@@ -36,7 +36,13 @@ typedef enum {
     FX_EBREAKDOWN = -4     /* fx_cg_solve: p.Sp <= 0 or non-finite (operator not positive definite on p)       */
 } fx_status;
 
-typedef enum { FX_BC_PER = 0, FX_BC_DIR = 1 } fx_bc;   /* periodic / homogeneous Dirichlet                     */
+/* Boundary kind of one direction.  PER: periodic.  DIR: homogeneous Dirichlet at both walls (the ghost cell is zero).
+ * NEU: homogeneous Neumann at both walls (the ghost cell mirrors the interior trace: no jump and no flux correction on
+ * the wall face).  DIR_NEU: Dirichlet at the lower wall (x = 0 / y = 0), Neumann at the upper one; needs >= 2 cells in
+ * that direction.  NEU_DIR: the reverse.  NEU kinds are for the elliptic operator and the CG solve (a grid without any
+ * Dirichlet wall gives a singular operator: constants are its null space); fx_dg_derivative and fx_arakawa take PER
+ * and DIR only and return FX_EINVAL otherwise.  (Q23, section 6.9) */
+typedef enum { FX_BC_PER = 0, FX_BC_DIR = 1, FX_BC_NEU = 2, FX_BC_DIR_NEU = 3, FX_BC_NEU_DIR = 4 } fx_bc;
 
 /* Grid of Fig. 2 `CartesianGrid2d(x0,x1,y0,y1,P,Nx,Ny)` on the domain [0,lx] x [0,ly]:
  * Nx x Ny cells, P Gauss-Legendre nodes per cell and direction (P = number of polynomial coefficients). */

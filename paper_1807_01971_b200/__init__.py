@@ -9,7 +9,7 @@ import os
 
 from . import build as _build
 
-PER, DIR = 0, 1
+PER, DIR, NEU, DIR_NEU, NEU_DIR = 0, 1, 2, 3, 4      # fx_bc (include/fx.h)
 OK, MAXIT, EINVAL, ECUDA, ENOMEM, EBREAKDOWN = 0, 1, -1, -2, -3, -4
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

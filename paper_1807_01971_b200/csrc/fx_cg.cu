@@ -33,7 +33,7 @@ struct CgScal {
 typedef ExAcc<CG_K, CG_W> CgAcc;
 
 // ---- K1: direction update + apply + dot -------------------------------------------------------------------------
-template <int P>
+template <int P, bool NEU>
 __global__ void __launch_bounds__(128, (P <= 2 ? 4 : 2))
 k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi, const double* __restrict__ pin,
                    const double* __restrict__ r, double* __restrict__ pout, double* __restrict__ q, ExGlobal ex, CgScal* sc) {
@@ -53,8 +53,8 @@ k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict_
         int j1 = j0 + g.rows_per_seg;
         if (j1 > g.Ny) j1 = g.Ny;
         extern __shared__ __align__(16) double dg_smem[];
-        if (P <= 3 && g.smr) dg_warp_strip<P, true, true, true, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, dg_smem + (size_t)(threadIdx.x >> 5) * 8 * P * P * 32);
-        else dg_warp_strip<P, true, true, false, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, nullptr);
+        if (P <= 3 && g.smr) dg_warp_strip<P, true, true, true, NEU, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, dg_smem + (size_t)(threadIdx.x >> 5) * 8 * P * P * 32);
+        else dg_warp_strip<P, true, true, false, NEU, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, nullptr);
     }
     acc.flush(&sh);
     if (ex_block_finish(&sh, ex, 1, 1, &sc->pq) && threadIdx.x == 0) {
@@ -302,7 +302,7 @@ k_cg_persistent(const __grid_constant__ DgParams g, const double* __restrict__ c
                 const int j0 = seg * g.rows_per_seg;
                 int j1 = j0 + g.rows_per_seg;
                 if (j1 > g.Ny) j1 = g.Ny;
-                dg_warp_strip<P, true, true, false, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, nullptr);   // L2-resident grids: generic rows
+                dg_warp_strip<P, true, true, false, false, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, nullptr);   // L2-resident grids: generic rows
             }
         }
         acc.flush(&sh);
@@ -440,7 +440,8 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, 
         cudaEvent_t* ev = nullptr;
         if (c->prof_on && c->prof_iters < c->prof_cap) { ev = c->prof_ev + 4 * c->prof_iters; c->prof_iters++; }
         if (ev) cudaEventRecord(ev[0], c->stream);
-        k_cg_dir_apply_dot<P><<<ag, ab, k1_smem, c->stream>>>(dp, chi, pin, r, pout, q, c->ex, sc);
+        if (fx_dg_has_neumann(&dp)) k_cg_dir_apply_dot<P, true><<<ag, ab, k1_smem, c->stream>>>(dp, chi, pin, r, pout, q, c->ex, sc);
+        else k_cg_dir_apply_dot<P, false><<<ag, ab, k1_smem, c->stream>>>(dp, chi, pin, r, pout, q, c->ex, sc);
         if (ev) cudaEventRecord(ev[1], c->stream);
         if (lin) k_cg_update_tma<P><<<lg, eb, (size_t)K2_STAGES * 4 * 2 * eb * 8, c->stream>>>(dp, pout, q, phi, r, c->ex, sc);
         else k_cg_update<P><<<eg, eb, (size_t)FX_STAGES * 4 * CG_U * eb * 8, c->stream>>>(dp, pout, q, phi, r, c->ex, sc);
@@ -542,8 +543,13 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
             int ag, ab, eg, eb;
             int occb = 0;
             {
-                const void* f = g->P == 1 ? (const void*)k_cg_dir_apply_dot<1> : g->P == 2 ? (const void*)k_cg_dir_apply_dot<2>
-                              : g->P == 3 ? (const void*)k_cg_dir_apply_dot<3> : g->P == 4 ? (const void*)k_cg_dir_apply_dot<4> : (const void*)k_cg_dir_apply_dot<5>;
+                const void* f;
+                if (fx_dg_has_neumann(&dp))
+                    f = g->P == 1 ? (const void*)k_cg_dir_apply_dot<1, true> : g->P == 2 ? (const void*)k_cg_dir_apply_dot<2, true>
+                      : g->P == 3 ? (const void*)k_cg_dir_apply_dot<3, true> : g->P == 4 ? (const void*)k_cg_dir_apply_dot<4, true> : (const void*)k_cg_dir_apply_dot<5, true>;
+                else
+                    f = g->P == 1 ? (const void*)k_cg_dir_apply_dot<1, false> : g->P == 2 ? (const void*)k_cg_dir_apply_dot<2, false>
+                      : g->P == 3 ? (const void*)k_cg_dir_apply_dot<3, false> : g->P == 4 ? (const void*)k_cg_dir_apply_dot<4, false> : (const void*)k_cg_dir_apply_dot<5, false>;
                 dp.smr = g->P <= 3 ? 1 : 0;
                 const size_t sm = dp.smr ? fx_dg_ring_bytes(g->P, 4, true) : 0;
                 if (sm) FX_CUDA(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
@@ -559,7 +565,8 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
             // small grids (vectors resident in L2): the whole loop in one cooperative launch.  mode 1 = automatic,
             // 2 = never, 3 = whenever the device allows it (tests)
             bool persistent = false;
-            if ((c->cg_fused == 1 && n <= ((int64_t)1 << 20)) || (c->cg_fused == 3 && n < ((int64_t)1 << 24))) {
+            // (grids with a Neumann wall always take the two-kernel path: the cooperative kernel is not instantiated for them)
+            if (!fx_dg_has_neumann(&dp) && ((c->cg_fused == 1 && n <= ((int64_t)1 << 20)) || (c->cg_fused == 3 && n < ((int64_t)1 << 24)))) {
                 switch (g->P) {
                 case 1: s = cg_run_persistent<1>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
                 case 2: s = cg_run_persistent<2>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;

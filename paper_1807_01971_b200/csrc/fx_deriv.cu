@@ -208,7 +208,7 @@ fx_status fx_launch_derivative(FxCtx* c, const fx_grid* g, int dir, int flux, do
 
 extern "C" fx_status fx_dg_derivative(const fx_grid* g, int32_t direction, int32_t flux, double alpha, const double* x, double beta,
                                       double* y) {
-    if (!fx_grid_ok(g) || !x || !y || direction < 0 || direction > 1 || flux < 0 || flux > 2) {
+    if (!fx_grid_ok(g) || !fx_grid_deriv_ok(g) || !x || !y || direction < 0 || direction > 1 || flux < 0 || flux > 2) {
         fx_set_error("fx_dg_derivative: bad grid, direction, flux or null pointer"); return FX_EINVAL;
     }
     const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
@@ -230,7 +230,7 @@ extern "C" fx_status fx_dg_dtables(int32_t P, int32_t flux, double* out) {
 
 // ---- Arakawa bracket as the paper runs it: nine calls of the primitives --------------------------------
 extern "C" fx_status fx_arakawa(const fx_grid* g, const double* f, const double* gg, double* out) {
-    if (!fx_grid_ok(g) || !f || !gg || !out) { fx_set_error("fx_arakawa: bad grid or null pointer"); return FX_EINVAL; }
+    if (!fx_grid_ok(g) || !fx_grid_deriv_ok(g) || !f || !gg || !out) { fx_set_error("fx_arakawa: bad grid (PER / DIR only) or null pointer"); return FX_EINVAL; }
     const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
     if ((f < out + n && out < f + n) || (gg < out + n && out < gg + n)) { fx_set_error("fx_arakawa: out overlaps an input"); return FX_EINVAL; }
     FxCtx* c = fx_ctx();

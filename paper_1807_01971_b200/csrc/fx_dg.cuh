@@ -23,12 +23,14 @@
 #include "fx_tables.h"
 
 struct DgParams {
-    int Nx, Ny, bcx, bcy;          // bc: 0 = periodic, 1 = Dirichlet
+    int Nx, Ny, bcx, bcy;          // fx_bc of each direction
+    int lox, hix, loy, hiy;        // the four walls: 0 = none (periodic), 1 = Dirichlet, 2 = Neumann
     int rows_per_seg, nseg, nstrip;
     int normed;
     int smr;                       // rows staged through the per-lane shared-memory ring (P <= 3)
     double cxx, cyy;               // hy/hx, hx/hy
     double T0[FX_PMAX][FX_PMAX], T0L[FX_PMAX][FX_PMAX], WW[FX_PMAX][FX_PMAX], V[FX_PMAX][FX_PMAX];
+    double TD[FX_PMAX][FX_PMAX];   // D: the cell table of the last cell before a Neumann wall
     double B[FX_PMAX], L[FX_PMAX], R[FX_PMAX], JX[FX_PMAX], JY[FX_PMAX];
 };
 
@@ -138,10 +140,11 @@ __device__ __forceinline__ void smr_read_u(DgCell<P>& c, const DgParams& g, cons
 #define CB(m) g.B[m]
 #define FF(m) f[m]
 
-// y lines of one cell: flux, flux trace, adjoint; acc_ += cyy * sy.  FIRST: first cell of a Dirichlet direction (T0L).
+// y lines of one cell: flux, flux trace, adjoint; acc_ += cyy * sy.  TK: the cell table -- 0 = T0, 1 = T0L (first cell
+// of a line that starts at a Dirichlet wall), 2 = TD (last cell of a line that ends at a Neumann wall).
 // tByp: in = flux trace of the cell below, out = this cell's.  The P*P chains of each stage are independent: they are
 // written stage by stage so that the scheduler sees P*P-way instruction-level parallelism.
-template <int P, bool FIRST>
+template <int P, int TK>
 __device__ __forceinline__ void dg_ylines(const DgParams& g, const DgCell<P>& uc, const DgCell<P>& cc, const double (&tLyn)[P],
                                           double (&tByp)[P], double (&acc_)[P][P]) {
     double f[P][P];                                                   // f[l][k]
@@ -151,7 +154,7 @@ __device__ __forceinline__ void dg_ylines(const DgParams& g, const DgCell<P>& uc
         for (int k = 0; k < P; ++k) {
             double a;
 #define UC(m) uc.v[m][k]
-#define CT(m) (FIRST ? g.T0L[l][m] : g.T0[l][m])
+#define CT(m) (TK == 1 ? g.T0L[l][m] : TK == 2 ? g.TD[l][m] : g.T0[l][m])
             FX_CHAIN(a, CT, UC)
 #undef CT
 #undef UC
@@ -168,7 +171,7 @@ __device__ __forceinline__ void dg_ylines(const DgParams& g, const DgCell<P>& uc
 #pragma unroll
         for (int k = 0; k < P; ++k) {
             double a;
-#define CT(m) (FIRST ? g.T0L[m][l] : g.T0[m][l])
+#define CT(m) (TK == 1 ? g.T0L[m][l] : TK == 2 ? g.TD[m][l] : g.T0[m][l])
             FX_CHAIN(a, CT, FK)
 #undef CT
             acc_[l][k] = __fma_rn(g.cyy, __fma_rn(g.L[l], tByp[k], a), acc_[l][k]);
@@ -178,11 +181,11 @@ __device__ __forceinline__ void dg_ylines(const DgParams& g, const DgCell<P>& uc
     for (int k = 0; k < P; ++k) tByp[k] = tB[k];
 }
 
-// x lines of one cell.  SEL: this warp contains the first cell of a Dirichlet x direction (lane flag firstx).
+// x lines of one cell.  SEL: this warp contains a cell with a wall table (lane flags firstx: T0L; lastx, NEU only: TD).
 // out[l][k] = cxx * sx + acc_ (times V if normed)
-template <int P, bool SEL>
+template <int P, bool SEL, bool NEU>
 __device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc, const DgCell<P>& cc, const double (&tLxr)[P],
-                                          bool firstx, bool xghost, double (&acc_)[P][P]) {
+                                          bool firstx, bool lastx, bool xghost, double (&acc_)[P][P]) {
     double f[P][P];                                                   // f[l][k]
 #pragma unroll
     for (int l = 0; l < P; ++l)
@@ -190,7 +193,7 @@ __device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc
         for (int k = 0; k < P; ++k) {
             double a;
 #define UC(m) uc.v[l][m]
-#define CT(m) ((SEL && firstx) ? g.T0L[k][m] : g.T0[k][m])
+#define CT(m) ((SEL && firstx) ? g.T0L[k][m] : (SEL && NEU && lastx) ? g.TD[k][m] : g.T0[k][m])
             FX_CHAIN(a, CT, UC)
 #undef CT
 #undef UC
@@ -210,7 +213,7 @@ __device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc
 #pragma unroll
         for (int k = 0; k < P; ++k) {
             double a;
-#define CT(m) ((SEL && firstx) ? g.T0L[m][k] : g.T0[m][k])
+#define CT(m) ((SEL && firstx) ? g.T0L[m][k] : (SEL && NEU && lastx) ? g.TD[m][k] : g.T0[m][k])
             FX_CHAIN(a, CT, FL)
 #undef CT
             double o = __fma_rn(g.cxx, __fma_rn(g.L[k], tBl[l], a), acc_[l][k]);
@@ -222,7 +225,8 @@ __device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc
 
 // One warp: strip `strip` of 30 cells, cell rows [j0, j1).  FUSE: feed (x, y) pairs of the produced cells into the
 // exact-dot accumulator `acc` (the CG's p.Sp).
-template <int P, bool FUSE, bool DIRF, bool SMR, class ACC>
+// NEU: the grid has a Neumann wall (a separate instantiation, so that the periodic / Dirichlet code is untouched by it).
+template <int P, bool FUSE, bool DIRF, bool SMR, bool NEU, class ACC>
 __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* __restrict__ chi, const DgSrc& src,
                                               double* __restrict__ y, int strip, int j0, int j1, ACC* acc, ExShared* sh,
                                               double* ring) {
@@ -232,14 +236,16 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
     const long long pitch = (long long)Nx * P;
     const int ci = strip * FX_STRIP - 1 + lane;                    // this lane's cell column (may be outside)
     const bool outside = ci < 0 || ci >= Nx;
-    const bool dirx = g.bcx == 1, diry = g.bcy == 1;
+    const bool dirx = NEU ? g.bcx != 0 : g.bcx == 1, diry = NEU ? g.bcy != 0 : g.bcy == 1;   // walls (ghost traces are zero)
     // periodic: wrap once; lanes further out are never used but must read valid memory
     int cw = ci;
     if (outside) { cw = ci % Nx; if (cw < 0) cw += Nx; }
     const bool xghost = outside && (dirx || ci < -1 || ci > Nx);   // contributes zero traces
     const bool produce = lane >= 1 && lane <= FX_STRIP && ci < Nx; // ci >= 0 holds for lanes >= 1
-    const bool firstx = dirx && ci == 0;                           // T0L instead of T0 along x
-    const bool selx = dirx && strip == 0;                          // warp-uniform: some lane has firstx
+    const bool firstx = (NEU ? g.lox == 1 : dirx) && ci == 0;      // T0L instead of T0 along x
+    const bool lastx = NEU && g.hix == 2 && ci == Nx - 1;          // TD instead of T0 along x; the jump's ghost mirrors
+    const bool mirlx = NEU && g.lox == 2 && ci == 0;               // lower Neumann wall: the jump's ghost mirrors
+    const bool selx = dirx && (strip == 0 || (NEU && strip == g.nstrip - 1));   // warp-uniform: some lane has a wall table
     const int col0 = cw * P;
 
     DgCell<P> uc, un, cc;
@@ -272,7 +278,7 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
     }
     if (j0 == 0 && diry) {
 #pragma unroll
-        for (int k = 0; k < P; ++k) { tRyp[k] = 0.0; tByp[k] = 0.0; }
+        for (int k = 0; k < P; ++k) { tRyp[k] = (NEU && g.loy == 2) ? tLy[k] : 0.0; tByp[k] = 0.0; }   // Neumann: mirrored, jump +0
     } else {
         const int jp = (j0 == 0) ? Ny - 1 : j0 - 1;
         DgCell<P> up, cp;
@@ -288,8 +294,8 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
 #pragma unroll
             for (int l = 0; l < P; ++l) { cp.v[l][k] = __dmul_rn(g.WW[l][k], cp.v[l][k]); dummy[l][k] = 0.0; }
         }
-        if (diry && jp == 0) dg_ylines<P, true>(g, up, cp, tLy, tByp, dummy);
-        else dg_ylines<P, false>(g, up, cp, tLy, tByp, dummy);
+        if ((NEU ? g.loy == 1 : diry) && jp == 0) dg_ylines<P, 1>(g, up, cp, tLy, tByp, dummy);
+        else dg_ylines<P, 0>(g, up, cp, tLy, tByp, dummy);
     }
 
     // ---- march ---------------------------------------------------------------------------------------------
@@ -349,16 +355,20 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
 #pragma unroll
             for (int k = 0; k < P; ++k) {
                 cc.v[l][k] = __dmul_rn(g.WW[l][k], cc.v[l][k]);
-                const double jy = __fma_rn(g.L[l], __dsub_rn(tLy[k], tRyp[k]), __dmul_rn(g.R[l], __dsub_rn(tRy[k], tLyn[k])));
-                const double jx = __fma_rn(g.L[k], __dsub_rn(tLx[l], tRxl[l]), __dmul_rn(g.R[k], __dsub_rn(tRx[l], tLxr[l])));
+                // the jump's ghost at a Neumann wall is the cell's own trace (difference +0); the gradient's ghost stays 0
+                const double gyn = (NEU && yghost && g.hiy == 2) ? tRy[k] : tLyn[k];
+                const double gxp = mirlx ? tLx[l] : tRxl[l], gxn = lastx ? tRx[l] : tLxr[l];
+                const double jy = __fma_rn(g.L[l], __dsub_rn(tLy[k], tRyp[k]), __dmul_rn(g.R[l], __dsub_rn(tRy[k], gyn)));
+                const double jx = __fma_rn(g.L[k], __dsub_rn(tLx[l], gxp), __dmul_rn(g.R[k], __dsub_rn(tRx[l], gxn)));
                 acc_[l][k] = __fma_rn(g.JX[l], jx, __dmul_rn(g.JY[k], jy));
             }
-        if (diry && j == 0) dg_ylines<P, true>(g, uc, cc, tLyn, tByp, acc_);
-        else dg_ylines<P, false>(g, uc, cc, tLyn, tByp, acc_);
+        if (NEU && g.hiy == 2 && j == Ny - 1) dg_ylines<P, 2>(g, uc, cc, tLyn, tByp, acc_);
+        else if ((NEU ? g.loy == 1 : diry) && j == 0) dg_ylines<P, 1>(g, uc, cc, tLyn, tByp, acc_);
+        else dg_ylines<P, 0>(g, uc, cc, tLyn, tByp, acc_);
 #pragma unroll
         for (int k = 0; k < P; ++k) { tRyp[k] = tRy[k]; tLy[k] = tLyn[k]; }
-        if (selx) dg_xlines<P, true>(g, uc, cc, tLxr, firstx, xghost, acc_);
-        else dg_xlines<P, false>(g, uc, cc, tLxr, firstx, xghost, acc_);
+        if (selx) dg_xlines<P, true, NEU>(g, uc, cc, tLxr, firstx, lastx, xghost, acc_);
+        else dg_xlines<P, false, NEU>(g, uc, cc, tLxr, firstx, lastx, xghost, acc_);
 
         if (DIRF && produce) {
             double* prow = src.pout + (long long)j * P * pitch + col0;

@@ -53,6 +53,9 @@ fx_status fx_cuda_fail(cudaError_t e, const char* what);
 
 static inline bool aligned16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
 int fx_grid_ok(const fx_grid* g);
+int fx_grid_deriv_ok(const fx_grid* g);          // PER / DIR only: stand-alone derivatives and the bracket
+struct DgParams;
+int fx_dg_has_neumann(const DgParams* p);
 fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* out, double* vol4_out);
 
 // internal launchers (stream-ordered, no synchronisation)

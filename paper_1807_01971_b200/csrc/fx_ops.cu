@@ -451,7 +451,7 @@ extern "C" fx_status fx_exdot_digits(const double* x, const double* y, int64_t n
 
 struct NoAcc { template <int U> __device__ void add(const double (&)[U], const double (&)[U], const bool (&)[U], ExShared*) {} };
 
-template <int P>
+template <int P, bool NEU>
 __global__ void __launch_bounds__(128, (P <= 2 ? 4 : P == 3 ? 3 : 2)) k_dg_apply(const __grid_constant__ DgParams g, const double* __restrict__ chi,
                                                   const double* __restrict__ x, double* __restrict__ y) {
     const int wpb = blockDim.x >> 5;
@@ -464,13 +464,20 @@ __global__ void __launch_bounds__(128, (P <= 2 ? 4 : P == 3 ? 3 : 2)) k_dg_apply
     if (j1 > g.Ny) j1 = g.Ny;
     const DgSrc src = {x, nullptr, nullptr, 0.0, false};
     extern __shared__ __align__(16) double dg_smem[];
-    if (P <= 3 && g.smr) dg_warp_strip<P, false, false, true, NoAcc>(g, chi, src, y, strip, j0, j1, nullptr, nullptr, dg_smem + (size_t)(threadIdx.x >> 5) * 5 * P * P * 32);
-    else dg_warp_strip<P, false, false, false, NoAcc>(g, chi, src, y, strip, j0, j1, nullptr, nullptr, nullptr);
+    if (P <= 3 && g.smr) dg_warp_strip<P, false, false, true, NEU, NoAcc>(g, chi, src, y, strip, j0, j1, nullptr, nullptr, dg_smem + (size_t)(threadIdx.x >> 5) * 5 * P * P * 32);
+    else dg_warp_strip<P, false, false, false, NEU, NoAcc>(g, chi, src, y, strip, j0, j1, nullptr, nullptr, nullptr);
 }
+
+// a one-cell direction cannot carry a Dirichlet and a Neumann wall table at once (Q23)
+static bool bc_ok(int bc, int N) { return bc >= FX_BC_PER && bc <= FX_BC_NEU_DIR && !(bc == FX_BC_DIR_NEU && N < 2); }
+static int wall_lo(int bc) { return bc == FX_BC_PER ? 0 : (bc == FX_BC_DIR || bc == FX_BC_DIR_NEU) ? 1 : 2; }
+static int wall_hi(int bc) { return bc == FX_BC_PER ? 0 : (bc == FX_BC_DIR || bc == FX_BC_NEU_DIR) ? 1 : 2; }
+int fx_dg_has_neumann(const DgParams* p) { return p->lox == 2 || p->hix == 2 || p->loy == 2 || p->hiy == 2; }
+int fx_grid_deriv_ok(const fx_grid* g) { return g->bcx <= FX_BC_DIR && g->bcy <= FX_BC_DIR; }
 
 int fx_grid_ok(const fx_grid* g) {
     return g && g->Nx >= 1 && g->Ny >= 1 && g->P >= 1 && g->P <= FX_PMAX && g->lx > 0 && g->ly > 0 &&
-           (g->bcx == FX_BC_PER || g->bcx == FX_BC_DIR) && (g->bcy == FX_BC_PER || g->bcy == FX_BC_DIR) &&
+           bc_ok(g->bcx, g->Nx) && bc_ok(g->bcy, g->Ny) &&
            (int64_t)g->Nx * g->P < (1ll << 30) && (int64_t)g->Ny * g->P < (1ll << 30);
 }
 
@@ -484,13 +491,14 @@ fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* o, double* v
     volatile double hxhy = hx * hy;
     const double vol4 = hxhy / 4;
     o->Nx = g->Nx; o->Ny = g->Ny; o->bcx = g->bcx; o->bcy = g->bcy; o->normed = normed;
+    o->lox = wall_lo(g->bcx); o->hix = wall_hi(g->bcx); o->loy = wall_lo(g->bcy); o->hiy = wall_hi(g->bcy);
     o->cxx = hy / hx; o->cyy = hx / hy;
     volatile double hy2 = hy / 2, hx2 = hx / 2;
     for (int k = 0; k < P; ++k) {
         o->B[k] = t.B[k]; o->L[k] = t.L[k]; o->R[k] = t.R[k];
         o->JX[k] = hy2 * t.w[k]; o->JY[k] = hx2 * t.w[k];          // jump factor jf = 1 (Q8)
         for (int m = 0; m < P; ++m) {
-            o->T0[k][m] = t.T0[k][m]; o->T0L[k][m] = t.T0L[k][m]; o->WW[k][m] = t.WW[k][m];
+            o->T0[k][m] = t.T0[k][m]; o->T0L[k][m] = t.T0L[k][m]; o->WW[k][m] = t.WW[k][m]; o->TD[k][m] = t.D[k][m];
             volatile double w = vol4 * t.WW[k][m];
             o->V[k][m] = 1.0 / w;
         }
@@ -534,11 +542,16 @@ fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const d
     DgParams p;
     fx_status s = fx_make_dg_params(g, normed, &p, nullptr);
     if (s != FX_OK) return s;
-    static int occ[FX_PMAX + 1] = {0};                           // resident warps per SM of k_dg_apply<P> (128-thread CTAs)
+    const int neu = fx_dg_has_neumann(&p);
+    static int occs[2][FX_PMAX + 1] = {{0}, {0}};                // resident warps per SM of k_dg_apply<P, NEU> (128-thread CTAs)
+    int* occ = occs[neu];
     if (!occ[g->P]) {
         int nb = 0;
-        const void* f = g->P == 1 ? (const void*)k_dg_apply<1> : g->P == 2 ? (const void*)k_dg_apply<2> : g->P == 3 ? (const void*)k_dg_apply<3>
-                      : g->P == 4 ? (const void*)k_dg_apply<4> : (const void*)k_dg_apply<5>;
+        const void* f;
+        if (neu) f = g->P == 1 ? (const void*)k_dg_apply<1, true> : g->P == 2 ? (const void*)k_dg_apply<2, true> : g->P == 3 ? (const void*)k_dg_apply<3, true>
+                   : g->P == 4 ? (const void*)k_dg_apply<4, true> : (const void*)k_dg_apply<5, true>;
+        else f = g->P == 1 ? (const void*)k_dg_apply<1, false> : g->P == 2 ? (const void*)k_dg_apply<2, false> : g->P == 3 ? (const void*)k_dg_apply<3, false>
+               : g->P == 4 ? (const void*)k_dg_apply<4, false> : (const void*)k_dg_apply<5, false>;
         FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, 128, 0));
         occ[g->P] = nb > 0 ? nb * 4 : 4;
     }
@@ -546,13 +559,18 @@ fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const d
     int grid, block;
     fx_dg_shape(c, g, &p, occ[g->P], &grid, &block);
     const size_t smem = p.smr ? fx_dg_ring_bytes(g->P, block / 32, false) : 0;
+#define FX_APPLY(PP) \
+    if (neu) k_dg_apply<PP, true><<<grid, block, smem, c->stream>>>(p, chi, x, y); \
+    else k_dg_apply<PP, false><<<grid, block, smem, c->stream>>>(p, chi, x, y); \
+    break;
     switch (g->P) {
-    case 1: k_dg_apply<1><<<grid, block, smem, c->stream>>>(p, chi, x, y); break;
-    case 2: k_dg_apply<2><<<grid, block, smem, c->stream>>>(p, chi, x, y); break;
-    case 3: k_dg_apply<3><<<grid, block, smem, c->stream>>>(p, chi, x, y); break;
-    case 4: k_dg_apply<4><<<grid, block, smem, c->stream>>>(p, chi, x, y); break;
-    case 5: k_dg_apply<5><<<grid, block, smem, c->stream>>>(p, chi, x, y); break;
+    case 1: FX_APPLY(1)
+    case 2: FX_APPLY(2)
+    case 3: FX_APPLY(3)
+    case 4: FX_APPLY(4)
+    case 5: FX_APPLY(5)
     }
+#undef FX_APPLY
     c->launches++;
     FX_CUDA(cudaGetLastError());
     return FX_OK;

@@ -569,3 +569,96 @@ def test_arakawa_bit_exact(fx, oracle, P):
     scale = float((W * out.abs()).sum())
     assert abs(fx.exdot(W, out)) < 1e-12 * scale and abs(fx.exdot3(dev(f), W, out)) < 1e-12 * scale
     assert np.array_equal(out.cpu().numpy(), oracle.arakawa(og, f, gg))
+
+
+# ---- Neumann and mixed walls (Q23, 6.9) ------------------------------------------------------
+
+PER, DIR, NEU, DIR_NEU, NEU_DIR = 0, 1, 2, 3, 4
+NEUBCS = [(2, 2), (2, 0), (0, 2), (1, 2), (2, 1), (3, 4), (4, 3), (3, 0), (0, 4), (4, 2), (1, 3)]
+
+
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("bc", NEUBCS)
+def test_dg_apply_neumann_bit_exact(fx, oracle, P, bc):
+    import torch
+    for (Nx, Ny) in [(1, 1), (2, 3), (3, 2), (31, 5), (30, 9), (61, 17), (64, 33)]:
+        if (bc[0] == DIR_NEU and Nx < 2) or (bc[1] == DIR_NEU and Ny < 2):
+            with pytest.raises(Exception):
+                fx.dg_elliptic_apply(fx.make_grid(Nx, Ny, P, 1.0, 1.0, *bc), dev(np.ones(Nx * Ny * P * P)), dev(np.ones(Nx * Ny * P * P)),
+                                     torch.empty(Nx * Ny * P * P, dtype=torch.float64, device="cuda"))
+            continue
+        g, og = _grid(fx, oracle, Nx, Ny, P, *bc)
+        x = fi.uniform(151 + P, g.n); chi = 1.0 + 0.5 * fi.uniform(161 + P, g.n)
+        for sym in (True, False):
+            want = oracle.dg_apply_canonical(og, chi, x, normed=not sym)
+            y = torch.full((g.n,), float("nan"), dtype=torch.float64, device="cuda")
+            fx.dg_elliptic_apply(g, dev(chi), dev(x), y, sym=sym)
+            got = y.cpu().numpy()
+            assert np.array_equal(got, want), (Nx, Ny, P, bc, sym, np.abs(got - want).max())
+            assert same_bits(got + 0.0, want + 0.0)
+
+
+def test_dg_apply_neumann_definition_shapes_and_null_space(fx, oracle):
+    import torch
+    g, og = _grid(fx, oracle, 95, 40, 3, NEU, DIR_NEU)
+    x = fi.uniform(171, g.n); chi = 1.0 + 0.5 * fi.uniform(172, g.n)
+    want = oracle.dg_apply_canonical(og, chi, x, normed=False)
+    for rows, block in [(0, 0), (1, 32), (3, 64), (7, 128), (40, 128), (1000, 1024)]:
+        fx.set_launch(2, rows, block)
+        y = torch.empty(g.n, dtype=torch.float64, device="cuda")
+        fx.dg_elliptic_apply(g, dev(chi), dev(x), y, sym=True)
+        assert np.array_equal(y.cpu().numpy(), want), (rows, block)
+    fx.set_launch(2, 0, 0)
+    g, og = _grid(fx, oracle, 12, 9, 4, NEU_DIR, NEU)
+    x = fi.uniform(173, g.n); chi = 1.0 + 0.5 * fi.uniform(174, g.n)
+    ydef, scale = oracle.dg_apply_definition(og, chi, x, normed=False)
+    y = torch.empty(g.n, dtype=torch.float64, device="cuda")
+    fx.dg_elliptic_apply(g, dev(chi), dev(x), y, sym=True)
+    assert np.all(np.abs(y.cpu().numpy() - ydef) <= 1e-14 * scale)
+    # pure Neumann: constants are in the null space (to rounding of the in-cell derivative of 1)
+    g, og = _grid(fx, oracle, 64, 48, 3, NEU, NEU)
+    chi = 1.0 + 0.5 * fi.uniform(175, g.n)
+    y = torch.empty(g.n, dtype=torch.float64, device="cuda")
+    fx.dg_elliptic_apply(g, dev(chi), dev(np.ones(g.n)), y, sym=True)
+    assert np.abs(y.cpu().numpy()).max() < 1e-12
+    # derivatives and the bracket take PER / DIR only
+    with pytest.raises(Exception):
+        fx.dg_derivative(g, 0, 0, 1.0, dev(np.ones(g.n)), 0.0, y)
+    with pytest.raises(Exception):
+        fx.arakawa(g, dev(np.ones(g.n)), dev(np.ones(g.n)), y)
+
+
+@pytest.mark.parametrize("mode", [0, 1, 2, 3])
+@pytest.mark.parametrize("Nx,Ny,P,bc", [(16, 16, 3, (NEU, DIR)), (33, 7, 5, (DIR_NEU, NEU_DIR)), (7, 5, 1, (DIR, NEU)),
+                                        (61, 4, 2, (NEU_DIR, NEU)), (40, 35, 4, (NEU, DIR_NEU)), (64, 64, 3, (PER, NEU_DIR))])
+def test_cg_neumann_matches_oracle(fx, oracle, mode, Nx, Ny, P, bc):
+    """every driver (unfused, automatic, two-kernel, persistent requested) gives the oracle's iterates bit for bit"""
+    fx.set_cg_fused(mode)
+    grid = dict(Nx=Nx, Ny=Ny, P=P, lx=math.pi, ly=1.7, bcx=bc[0], bcy=bc[1])
+    g, og = fx.make_grid(**grid), oracle.Grid(**grid)
+    chi = 1.0 + 0.5 * fi.uniform(191, g.n); rho = fi.uniform(192, g.n); phi0 = 0.01 * fi.uniform(193, g.n)
+    want, oinfo = oracle.cg_solve(og, chi, rho, phi0, 1e-9, 600)
+    phi = dev(phi0)
+    info = fx.cg_solve(g, dev(chi), dev(rho), phi, 1e-9, 600)
+    assert info.iterations == oinfo.iterations and info.status == oinfo.status
+    assert same_bits(phi.cpu().numpy(), want)
+
+
+def test_cg_neumann_manufactured_solution(fx, oracle):
+    """phi = cos x sin(y/2) on [0,pi]^2: zero normal derivative at x = 0, pi (NEU) and y = pi, zero value at y = 0 (DIR_NEU)"""
+    P, N = 3, 48
+    g = fx.make_grid(N, N, P, math.pi, math.pi, NEU, DIR_NEU)
+    og = oracle.Grid(N, N, P, math.pi, math.pi, NEU, DIR_NEU)
+    xs, ys = oracle.dg_nodes(og)
+    X, Y = np.meshgrid(xs, ys)
+    chi = 1 + 0.5 * np.cos(X) * np.cos(Y)
+    phi_exact = np.cos(X) * np.sin(Y / 2)
+    rho = (-0.5 * np.sin(X) * np.cos(Y)) * (-np.sin(X)) * np.sin(Y / 2) + chi * (-np.cos(X)) * np.sin(Y / 2) \
+        + (-0.5 * np.cos(X) * np.sin(Y)) * np.cos(X) * np.cos(Y / 2) / 2 + chi * np.cos(X) * (-np.sin(Y / 2) / 4)
+    phi = dev(np.zeros(g.n))
+    info = fx.cg_solve(g, dev(chi.ravel()), dev(rho.ravel()), phi, 1e-11, 5000)
+    assert info.status == 0
+    W, _ = oracle.dg_weights(og)
+    e = phi.cpu().numpy() - phi_exact.ravel()
+    rel = math.sqrt(oracle.exdot(W * e, e) / oracle.exdot(W * phi_exact.ravel(), phi_exact.ravel()))
+    assert rel < 2e-6, rel                 # 1.04e-6 with the oracle; order P

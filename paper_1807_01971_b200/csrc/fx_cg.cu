@@ -33,8 +33,13 @@ struct CgScal {
 typedef ExAcc<CG_K, CG_W> CgAcc;
 
 // ---- K1: direction update + apply + dot -------------------------------------------------------------------------
+#ifndef FX_K1_T
+#define FX_K1_T 128      // threads per CTA and CTAs per SM of K1 for P >= 3
+#define FX_K1_B 2
+#endif
+#define K1_THREADS(P) ((P) <= 2 ? 128 : FX_K1_T)
 template <int P, bool NEU>
-__global__ void __launch_bounds__(128, (P <= 2 ? 4 : 2))
+__global__ void __launch_bounds__(K1_THREADS(P), (P <= 2 ? 4 : FX_K1_B))
 k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi, const double* __restrict__ pin,
                    const double* __restrict__ r, double* __restrict__ pout, double* __restrict__ q, ExGlobal ex, CgScal* sc) {
     if (*(volatile int*)&sc->done) return;
@@ -400,7 +405,7 @@ static fx_status cg_workspace(FxCtx* c, int64_t n) {
 }
 
 static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int k1_warps_per_sm, int* apply_grid, int* apply_block, int* ew_grid, int* ew_block) {
-    fx_dg_shape(c, g, p, k1_warps_per_sm, apply_grid, apply_block);
+    fx_dg_shape(c, g, p, k1_warps_per_sm, apply_grid, apply_block, K1_THREADS(g->P) / 32);
     int bd = c->launch[3][1] ? c->launch[3][1] : 256;
     if (bd > 256) bd = 256;
     const int pitch = g->Nx * g->P;
@@ -551,11 +556,13 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
                     f = g->P == 1 ? (const void*)k_cg_dir_apply_dot<1, false> : g->P == 2 ? (const void*)k_cg_dir_apply_dot<2, false>
                       : g->P == 3 ? (const void*)k_cg_dir_apply_dot<3, false> : g->P == 4 ? (const void*)k_cg_dir_apply_dot<4, false> : (const void*)k_cg_dir_apply_dot<5, false>;
                 dp.smr = g->P <= 3 ? 1 : 0;
-                const size_t sm = dp.smr ? fx_dg_ring_bytes(g->P, 4, true) : 0;
+                const int k1w = K1_THREADS(g->P) / 32;
+                const size_t sm = dp.smr ? fx_dg_ring_bytes(g->P, k1w, true) : 0;
                 if (sm) FX_CUDA(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-                FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occb, f, 128, sm));
+                FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occb, f, k1w * 32, sm));
+                occb *= k1w;
             }
-            cg_shapes(c, g, &dp, occb > 0 ? occb * 4 : 4, &ag, &ab, &eg, &eb);
+            cg_shapes(c, g, &dp, occb > 0 ? occb : 4, &ag, &ab, &eg, &eb);
             CgScal* sc = (CgScal*)c->cg_scal;
             CgScal* hs = (CgScal*)c->cg_scal_pinned;
             memset(hs, 0, sizeof(*hs));

@@ -514,9 +514,10 @@ size_t fx_dg_ring_bytes(int P, int warps, bool dirf) { return (size_t)warps * (d
 // a prologue of about 0.6 steps (the flux trace of the row below it).  Choose rows_per_seg to minimise
 // waves * (rows_per_seg + 0.6), waves = ceil(warps / resident warps): whole waves, little redundant work, and for small
 // grids as many warps as there are rows.
-void fx_dg_shape(FxCtx* c, const fx_grid* g, DgParams* p, int warps_per_sm, int* grid, int* block) {
-    int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : 4;
-    if (wpb > 4) wpb = 4;                       // the kernels are compiled for <= 128 threads per CTA
+void fx_dg_shape(FxCtx* c, const fx_grid* g, DgParams* p, int warps_per_sm, int* grid, int* block, int max_wpb) {
+    int wpb = c->launch[2][1] ? c->launch[2][1] / 32 : max_wpb;
+    if (wpb > max_wpb) wpb = max_wpb;           // the kernels are compiled for <= 128 threads per CTA
+    if (wpb < 1) wpb = 1;
     p->nstrip = (g->Nx + FX_STRIP - 1) / FX_STRIP;
     int rps = c->launch[2][0];
     if (rps <= 0) {

@@ -33,13 +33,16 @@ struct CgScal {
 typedef ExAcc<CG_K, CG_W> CgAcc;
 
 // ---- K1: direction update + apply + dot -------------------------------------------------------------------------
-#ifndef FX_K1_T
-#define FX_K1_T 128      // threads per CTA and CTAs per SM of K1 for P >= 3
-#define FX_K1_B 2
+// Register budget of K1: __maxnreg__ instead of __launch_bounds__(threads, minBlocks) -- the latter makes
+// ptxas pick 168 registers for anything between two and three 128-thread CTAs per SM, and K1<3> then spills 880 bytes;
+// with the cap spelled out it needs 212 registers without spilling, 200 with 44 bytes.
+#ifndef FX_K1_R
+#define FX_K1_R 255      // registers per thread of K1<3>
+#define FX_K1_W 4        // warps per CTA of K1<3>
 #endif
-#define K1_THREADS(P) ((P) <= 2 ? 128 : FX_K1_T)
+#define K1_THREADS(P) ((P) == 3 ? FX_K1_W * 32 : 128)
 template <int P, bool NEU>
-__global__ void __launch_bounds__(K1_THREADS(P), (P <= 2 ? 4 : FX_K1_B))
+__global__ void __maxnreg__(P <= 2 ? 128 : P == 3 ? FX_K1_R : 255)
 k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi, const double* __restrict__ pin,
                    const double* __restrict__ r, double* __restrict__ pout, double* __restrict__ q, ExGlobal ex, CgScal* sc) {
     if (*(volatile int*)&sc->done) return;

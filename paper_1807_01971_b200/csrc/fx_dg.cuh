@@ -181,6 +181,21 @@ __device__ __forceinline__ void dg_ylines(const DgParams& g, const DgCell<P>& uc
     for (int k = 0; k < P; ++k) tByp[k] = tB[k];
 }
 
+// Cell-table coefficient of this lane's cell along x.  Periodic / Dirichlet: one two-way select.  With Neumann walls the
+// three-way choice is spelled as two selp (as plain conditionals the compiler turns it into divergent branches around
+// every FMA, and the two wall strips then take twice as long as the rest of the single wave).
+__device__ __forceinline__ double fx_selp(bool c, double a, double b) {
+    double r;
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %3, 0;\n\tselp.f64 %0, %1, %2, p;\n\t}" : "=d"(r) : "d"(a), "d"(b), "r"((int)c));
+    return r;
+}
+template <bool SEL, bool NEU>
+__device__ __forceinline__ double dg_coef(double t0, double t0l, double td, bool firstx, bool lastx) {
+    if (!SEL) return t0;
+    if (!NEU) return firstx ? t0l : t0;
+    return fx_selp(lastx, td, fx_selp(firstx, t0l, t0));
+}
+
 // x lines of one cell.  SEL: this warp contains a cell with a wall table (lane flags firstx: T0L; lastx, NEU only: TD).
 // out[l][k] = cxx * sx + acc_ (times V if normed)
 template <int P, bool SEL, bool NEU>
@@ -193,7 +208,7 @@ __device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc
         for (int k = 0; k < P; ++k) {
             double a;
 #define UC(m) uc.v[l][m]
-#define CT(m) ((SEL && firstx) ? g.T0L[k][m] : (SEL && NEU && lastx) ? g.TD[k][m] : g.T0[k][m])
+#define CT(m) dg_coef<SEL, NEU>(g.T0[k][m], g.T0L[k][m], g.TD[k][m], firstx, lastx)
             FX_CHAIN(a, CT, UC)
 #undef CT
 #undef UC
@@ -213,7 +228,7 @@ __device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc
 #pragma unroll
         for (int k = 0; k < P; ++k) {
             double a;
-#define CT(m) ((SEL && firstx) ? g.T0L[m][k] : (SEL && NEU && lastx) ? g.TD[m][k] : g.T0[m][k])
+#define CT(m) dg_coef<SEL, NEU>(g.T0[m][k], g.T0L[m][k], g.TD[m][k], firstx, lastx)
             FX_CHAIN(a, CT, FL)
 #undef CT
             double o = __fma_rn(g.cxx, __fma_rn(g.L[k], tBl[l], a), acc_[l][k]);
@@ -357,7 +372,7 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
                 cc.v[l][k] = __dmul_rn(g.WW[l][k], cc.v[l][k]);
                 // the jump's ghost at a Neumann wall is the cell's own trace (difference +0); the gradient's ghost stays 0
                 const double gyn = (NEU && yghost && g.hiy == 2) ? tRy[k] : tLyn[k];
-                const double gxp = mirlx ? tLx[l] : tRxl[l], gxn = lastx ? tRx[l] : tLxr[l];
+                const double gxp = NEU ? fx_selp(mirlx, tLx[l], tRxl[l]) : tRxl[l], gxn = NEU ? fx_selp(lastx, tRx[l], tLxr[l]) : tLxr[l];
                 const double jy = __fma_rn(g.L[l], __dsub_rn(tLy[k], tRyp[k]), __dmul_rn(g.R[l], __dsub_rn(tRy[k], gyn)));
                 const double jx = __fma_rn(g.L[k], __dsub_rn(tLx[l], gxp), __dmul_rn(g.R[k], __dsub_rn(tRx[l], gxn)));
                 acc_[l][k] = __fma_rn(g.JX[l], jx, __dmul_rn(g.JY[k], jy));

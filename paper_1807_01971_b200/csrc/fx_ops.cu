@@ -451,8 +451,12 @@ extern "C" fx_status fx_exdot_digits(const double* x, const double* y, int64_t n
 
 struct NoAcc { template <int U> __device__ void add(const double (&)[U], const double (&)[U], const bool (&)[U], ExShared*) {} };
 
+#ifndef FX_AP_R
+#define FX_AP_R 168      // registers per thread / warps per CTA of k_dg_apply<3>
+#define FX_AP_W 4
+#endif
 template <int P, bool NEU>
-__global__ void __launch_bounds__(128, (P <= 2 ? 4 : P == 3 ? 3 : 2)) k_dg_apply(const __grid_constant__ DgParams g, const double* __restrict__ chi,
+__global__ void __maxnreg__(P <= 2 ? 128 : P == 3 ? FX_AP_R : 255) k_dg_apply(const __grid_constant__ DgParams g, const double* __restrict__ chi,
                                                   const double* __restrict__ x, double* __restrict__ y) {
     const int wpb = blockDim.x >> 5;
     const long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
@@ -553,12 +557,13 @@ fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const d
                    : g->P == 4 ? (const void*)k_dg_apply<4, true> : (const void*)k_dg_apply<5, true>;
         else f = g->P == 1 ? (const void*)k_dg_apply<1, false> : g->P == 2 ? (const void*)k_dg_apply<2, false> : g->P == 3 ? (const void*)k_dg_apply<3, false>
                : g->P == 4 ? (const void*)k_dg_apply<4, false> : (const void*)k_dg_apply<5, false>;
-        FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, 128, 0));
-        occ[g->P] = nb > 0 ? nb * 4 : 4;
+        const int w = g->P == 3 ? FX_AP_W : 4;
+        FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, w * 32, 0));
+        occ[g->P] = nb > 0 ? nb * w : 4;
     }
     p.smr = 0;            // measured: the stand-alone apply is 2 % faster on the L1-prefetch path, the fused K1 6 % faster with the ring
     int grid, block;
-    fx_dg_shape(c, g, &p, occ[g->P], &grid, &block);
+    fx_dg_shape(c, g, &p, occ[g->P], &grid, &block, g->P == 3 ? FX_AP_W : 4);
     const size_t smem = p.smr ? fx_dg_ring_bytes(g->P, block / 32, false) : 0;
 #define FX_APPLY(PP) \
     if (neu) k_dg_apply<PP, true><<<grid, block, smem, c->stream>>>(p, chi, x, y); \

@@ -50,7 +50,9 @@ __device__ __forceinline__ void exdot_issue(double* buf, int stage, const double
 }
 
 // Consume one landed tile from shared memory (generic: bounds-checked).
-template <bool VEC>
+// SUM: the two arrays are the two halves of one vector whose exact sum is wanted -- every element is accumulated as
+// element * 1 (no error term); same loads, same ring, about the same fp64 work per byte as the dot.
+template <bool VEC, bool SUM>
 __device__ __forceinline__ void exdot_consume(const double* buf, int stage, long long n, long long base, ExAcc<EX_K, EX_W>& acc,
                                               ExShared* sh) {
     const int bd = blockDim.x;
@@ -75,12 +77,18 @@ __device__ __forceinline__ void exdot_consume(const double* buf, int stage, long
             act[u] = base + slot < n;
         }
     }
-    acc.add<EX_U>(xv, yv, act, sh);
+    if (SUM) {
+        double one[EX_U];
+#pragma unroll
+        for (int u = 0; u < EX_U; ++u) one[u] = 1.0;
+        acc.add<EX_U, false, true>(xv, one, act, sh);
+        acc.add<EX_U, false, true>(yv, one, act, sh);
+    } else acc.add<EX_U>(xv, yv, act, sh);
 }
 
 // The kernel.  CTA b takes tiles b, b+G, b+2G, ...; EX_STAGES-1 tiles are in flight per thread.
 // Hot loop (16-byte aligned inputs, full tiles): pointer increments only, compile-time stage offsets, no bounds.
-template <bool VEC>
+template <bool VEC, bool SUM>
 __global__ void __launch_bounds__(256, 2) k_exdot(const double* __restrict__ x, const double* __restrict__ y, long long n,
                                                   ExGlobal g, int first, int last, double* result) {
     extern __shared__ __align__(16) double ex_buf[];
@@ -127,7 +135,14 @@ __global__ void __launch_bounds__(256, 2) k_exdot(const double* __restrict__ x, 
                 fx_lds128(b, s0 + so + arr_bytes + u * u_bytes);
                 xv[2 * u] = a.x; xv[2 * u + 1] = a.y; yv[2 * u] = b.x; yv[2 * u + 1] = b.y;
             }
-            acc.add_all<EX_U>(xv, yv, &sh);                          // consumed tile < issued tile: full as well
+            if (SUM) {
+                double one[EX_U];
+                bool act[EX_U];
+#pragma unroll
+                for (int u = 0; u < EX_U; ++u) { one[u] = 1.0; act[u] = true; }
+                acc.add<EX_U, true, true>(xv, one, act, &sh);
+                acc.add<EX_U, true, true>(yv, one, act, &sh);
+            } else acc.add_all<EX_U>(xv, yv, &sh);                   // consumed tile < issued tile: full as well
             sqo = so;
             so += stage_bytes; if (so == EX_STAGES * stage_bytes) so = 0;
             if (++stage == EX_STAGES) stage = 0;
@@ -137,7 +152,7 @@ __global__ void __launch_bounds__(256, 2) k_exdot(const double* __restrict__ x, 
         int sq = stage + EX_STAGES - 1; if (sq >= EX_STAGES) sq -= EX_STAGES;
         exdot_issue<VEC>(ex_buf, sq, x, y, n, tq * tile, tq < ntiles); tq += gridDim.x;
         fx_cp_wait<EX_STAGES - 1>();
-        exdot_consume<VEC>(ex_buf, stage, n, t * tile, acc, &sh);
+        exdot_consume<VEC, SUM>(ex_buf, stage, n, t * tile, acc, &sh);
         if (++stage == EX_STAGES) stage = 0;
     }
     fx_cp_wait<0>();
@@ -146,7 +161,7 @@ __global__ void __launch_bounds__(256, 2) k_exdot(const double* __restrict__ x, 
 }
 
 // one launch over m <= 2^28 elements (keeps every 64-bit digit far from overflow); first/last: position in the call
-fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64_t m, int first, int last, double* result_dev) {
+fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64_t m, int first, int last, double* result_dev, bool sum) {
     const bool vec = aligned16(x) && aligned16(y);
     int bd = c->launch[0][1] ? c->launch[0][1] : 256;
     if (bd > 256) bd = 256;                     // compiled for <= 256 threads per CTA
@@ -154,20 +169,25 @@ fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64
     static bool attr_done = false;
     static int occ_cache[9] = {0};              // resident CTAs per SM by block size / 32
     if (!attr_done) {
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_STAGES * 2 * EX_U * 256 * 8));
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_STAGES * 2 * EX_U * 256 * 8));
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_STAGES * 2 * EX_U * 256 * 8));
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_STAGES * 2 * EX_U * 256 * 8));
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_STAGES * 2 * EX_U * 256 * 8));
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_STAGES * 2 * EX_U * 256 * 8));
         attr_done = true;
     }
     int& occ = occ_cache[bd / 32];
-    if (!occ && (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_exdot<true>, bd, smem) != cudaSuccess || occ < 1)) occ = 1;
+    if (!occ && (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_exdot<true, false>, bd, smem) != cudaSuccess || occ < 1)) occ = 1;
     const long long tile = (long long)bd * EX_U;
     long long grid = (m + tile - 1) / tile;
     const long long gmax = (long long)c->num_sms * occ;             // one resident wave: every CTA pays one flush + merge
     if (grid > gmax) grid = gmax;
     if (grid < 1) grid = 1;
     if (c->launch[0][0]) grid = c->launch[0][0];
-    if (vec) k_exdot<true><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
-    else k_exdot<false><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
+    if (sum) {
+        if (vec) k_exdot<true, true><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
+        else k_exdot<false, true><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
+    } else if (vec) k_exdot<true, false><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
+    else k_exdot<false, false><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
     c->launches++;
     FX_CUDA(cudaGetLastError());
     return FX_OK;
@@ -387,12 +407,37 @@ extern "C" double fx_exdot3(const double* x, const double* w, const double* y, i
     return exdotn_sync(c, launch_exdotn<3>(c, x, w, y, n, c->result_dev));
 }
 
+// Exact sum: long vectors go through the dot kernel's ring as two halves (x[0,h) and x[h,2h), h even so that both keep
+// the alignment of x), 2^27 elements per half and launch; what is left (<= 3 elements, or a short vector) through the
+// generic kernel.  All launches accumulate into the same digits; the last one rounds.
+fx_status fx_launch_exsum(FxCtx* c, const double* x, int64_t n, double* result_dev) {
+    if (n < 4096) return launch_exdotn<1>(c, x, nullptr, nullptr, n, result_dev);
+    const int64_t HALF = (int64_t)1 << 27;
+    int64_t done = 0;
+    bool first = true;
+    while (n - done >= 4) {
+        int64_t h = ((n - done) / 2) & ~(int64_t)1;
+        if (h > HALF) h = HALF;
+        const bool last = done + 2 * h == n;
+        fx_status s = fx_launch_exdot_part(c, x + done, x + done + h, h, first, last, result_dev, true);
+        if (s != FX_OK) return s;
+        first = false;
+        done += 2 * h;
+    }
+    if (done < n) {
+        k_exdotn<1><<<1, 256, (size_t)EX_STAGES * EX_U * 256 * sizeof(double), c->stream>>>(x + done, nullptr, nullptr, n - done, c->ex, 0, 1, result_dev);
+        c->launches++;
+        FX_CUDA(cudaGetLastError());
+    }
+    return FX_OK;
+}
+
 extern "C" double fx_exsum(const double* x, int64_t n) {
     if (n < 0 || (n > 0 && !x)) { fx_set_error("fx_exsum: bad arguments"); return NAN; }
     fx_set_error("%s", "");
     FxCtx* c = fx_ctx();
     if (!c) return NAN;
-    return exdotn_sync(c, launch_exdotn<1>(c, x, nullptr, nullptr, n, c->result_dev));
+    return exdotn_sync(c, fx_launch_exsum(c, x, n, c->result_dev));
 }
 
 fx_status fx_launch_exdot(FxCtx* c, const double* x, const double* y, int64_t n, double* result_dev) {
@@ -648,7 +693,7 @@ static fx_status time_one(FxCtx* c, int kind, const fx_grid* g, const double* a,
     case 5: { const double v = fx_exdot(a, b, n); return (v != v && fx_last_error()[0]) ? FX_ECUDA : FX_OK; }
     case 6: return fx_axpby(0.7, a, 1.0, cc, n);
     case 7: return launch_exdotn<3>(c, a, b, cc, n, c->result_dev);
-    case 8: return launch_exdotn<1>(c, a, nullptr, nullptr, n, c->result_dev);
+    case 8: return fx_launch_exsum(c, a, n, c->result_dev);
     case 9: return fx_launch_derivative(c, g, 0, 0, 0.7, a, -0.3, cc);
     case 10: return fx_launch_derivative(c, g, 1, 0, 0.7, a, -0.3, cc);
     case 11: return fx_launch_derivative(c, g, 0, 2, 0.7, a, -0.3, cc);

@@ -662,3 +662,36 @@ def test_cg_neumann_manufactured_solution(fx, oracle):
     e = phi.cpu().numpy() - phi_exact.ravel()
     rel = math.sqrt(oracle.exdot(W * e, e) / oracle.exdot(W * phi_exact.ravel(), phi_exact.ravel()))
     assert rel < 2e-6, rel                 # 1.04e-6 with the oracle; order P
+
+
+@pytest.mark.parametrize("n", [4095, 4096, 4097, 4098, 4099, 70001, (1 << 22) + 1])
+def test_exsum_two_half_path(fx, oracle, n):
+    """long vectors are summed as two halves through the dot kernel's ring plus a <= 3-element tail"""
+    x = fi.uniform(111, n) * np.ldexp(1.0, fi.rng(112).integers(-200, 200, n))
+    want = oracle.exsum(x)
+    dx = dev(x)
+    assert fbits(fx.exsum(dx)) == fbits(want)
+    buf = dev(np.concatenate([[0.0], x]))
+    assert fbits(fx.exsum(buf[1:])) == fbits(want)                         # only 8-byte aligned
+    for grid, block in [(1, 32), (7, 64), (300, 256)]:
+        fx.set_launch(0, grid, block)
+        assert fbits(fx.exsum(dx)) == fbits(want), (grid, block)
+    fx.set_launch(0, 0, 0)
+    # cancellation and specials through the same path
+    z = np.concatenate([x, -x]); fi.rng(113).shuffle(z)
+    assert fx.exsum(dev(z)) == 0.0
+    z[5] = np.inf
+    assert fx.exsum(dev(z)) == np.inf
+    z[n] = -np.inf
+    assert math.isnan(fx.exsum(dev(z)))
+
+
+def test_exsum_multi_launch(fx, oracle):
+    n = (1 << 28) + 5                                                       # two ring launches of 2^27 pairs ... and a tail
+    import torch
+    g = torch.Generator(device="cuda"); g.manual_seed(5)
+    x = torch.rand(n, dtype=torch.float64, device="cuda", generator=g) - 0.5
+    got = fx.exsum(x)
+    # the oracle over the same values, in four host chunks (the exact sum is order-free: compare through the exact dot with ones)
+    want = oracle.exsum(x.cpu().numpy())
+    assert fbits(got) == fbits(want)

@@ -60,7 +60,7 @@ fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* out, double*
 
 // internal launchers (stream-ordered, no synchronisation)
 fx_status fx_launch_exdot(FxCtx* c, const double* x, const double* y, int64_t n, double* result_dev);
-fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64_t m, int first, int last, double* result_dev, bool sum = false);
+fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64_t m, int first, int last, double* result_dev, int mode = 0);   // mode 1: exact sum of two halves, 2: binary32 pairs
 fx_status fx_launch_exsum(FxCtx* c, const double* x, int64_t n, double* result_dev);
 size_t fx_dg_ring_bytes(int P, int warps, bool dirf);
 void fx_dg_shape(FxCtx* c, const fx_grid* g, DgParams* p, int warps_per_sm, int* grid, int* block, int max_wpb = 4);

@@ -50,9 +50,32 @@ __device__ __forceinline__ void exdot_issue(double* buf, int stage, const double
 }
 
 // Consume one landed tile from shared memory (generic: bounds-checked).
-// SUM: the two arrays are the two halves of one vector whose exact sum is wanted -- every element is accumulated as
-// element * 1 (no error term); same loads, same ring, about the same fp64 work per byte as the dot.
-template <bool VEC, bool SUM>
+// MODE 1 (sum): the two arrays are the two halves of one vector whose exact sum is wanted -- every element is accumulated
+// as element * 1 (no error term); same loads, same ring, about the same fp64 work per byte as the dot.
+// MODE 2 (binary32 dot): every 8-byte slot holds two floats; float * float is exact in fp64 (no error term).
+template <int MODE>
+__device__ __forceinline__ void ex_feed(ExAcc<EX_K, EX_W>& acc, const double (&xv)[EX_U], const double (&yv)[EX_U], const bool (&act)[EX_U],
+                                        ExShared* sh) {
+    if (MODE == 1) {
+        double one[EX_U];
+#pragma unroll
+        for (int u = 0; u < EX_U; ++u) one[u] = 1.0;
+        acc.add<EX_U, false, true>(xv, one, act, sh);
+        acc.add<EX_U, false, true>(yv, one, act, sh);
+    } else if (MODE == 2) {
+        double a[2 * EX_U], b[2 * EX_U];
+        bool ac[2 * EX_U];
+#pragma unroll
+        for (int u = 0; u < EX_U; ++u) {
+            a[2 * u] = __int_as_float(__double2loint(xv[u])); a[2 * u + 1] = __int_as_float(__double2hiint(xv[u]));
+            b[2 * u] = __int_as_float(__double2loint(yv[u])); b[2 * u + 1] = __int_as_float(__double2hiint(yv[u]));
+            ac[2 * u] = act[u]; ac[2 * u + 1] = act[u];
+        }
+        acc.add<2 * EX_U, false, true>(a, b, ac, sh);
+    } else acc.add<EX_U>(xv, yv, act, sh);
+}
+
+template <bool VEC, int MODE>
 __device__ __forceinline__ void exdot_consume(const double* buf, int stage, long long n, long long base, ExAcc<EX_K, EX_W>& acc,
                                               ExShared* sh) {
     const int bd = blockDim.x;
@@ -77,18 +100,12 @@ __device__ __forceinline__ void exdot_consume(const double* buf, int stage, long
             act[u] = base + slot < n;
         }
     }
-    if (SUM) {
-        double one[EX_U];
-#pragma unroll
-        for (int u = 0; u < EX_U; ++u) one[u] = 1.0;
-        acc.add<EX_U, false, true>(xv, one, act, sh);
-        acc.add<EX_U, false, true>(yv, one, act, sh);
-    } else acc.add<EX_U>(xv, yv, act, sh);
+    ex_feed<MODE>(acc, xv, yv, act, sh);
 }
 
 // The kernel.  CTA b takes tiles b, b+G, b+2G, ...; EX_STAGES-1 tiles are in flight per thread.
 // Hot loop (16-byte aligned inputs, full tiles): pointer increments only, compile-time stage offsets, no bounds.
-template <bool VEC, bool SUM>
+template <bool VEC, int MODE>
 __global__ void __launch_bounds__(256, 2) k_exdot(const double* __restrict__ x, const double* __restrict__ y, long long n,
                                                   ExGlobal g, int first, int last, double* result) {
     extern __shared__ __align__(16) double ex_buf[];
@@ -135,14 +152,13 @@ __global__ void __launch_bounds__(256, 2) k_exdot(const double* __restrict__ x, 
                 fx_lds128(b, s0 + so + arr_bytes + u * u_bytes);
                 xv[2 * u] = a.x; xv[2 * u + 1] = a.y; yv[2 * u] = b.x; yv[2 * u + 1] = b.y;
             }
-            if (SUM) {
-                double one[EX_U];
+            if (MODE == 0) acc.add_all<EX_U>(xv, yv, &sh);           // consumed tile < issued tile: full as well
+            else {
                 bool act[EX_U];
 #pragma unroll
-                for (int u = 0; u < EX_U; ++u) { one[u] = 1.0; act[u] = true; }
-                acc.add<EX_U, true, true>(xv, one, act, &sh);
-                acc.add<EX_U, true, true>(yv, one, act, &sh);
-            } else acc.add_all<EX_U>(xv, yv, &sh);                   // consumed tile < issued tile: full as well
+                for (int u = 0; u < EX_U; ++u) act[u] = true;
+                ex_feed<MODE>(acc, xv, yv, act, &sh);
+            }
             sqo = so;
             so += stage_bytes; if (so == EX_STAGES * stage_bytes) so = 0;
             if (++stage == EX_STAGES) stage = 0;
@@ -152,7 +168,7 @@ __global__ void __launch_bounds__(256, 2) k_exdot(const double* __restrict__ x, 
         int sq = stage + EX_STAGES - 1; if (sq >= EX_STAGES) sq -= EX_STAGES;
         exdot_issue<VEC>(ex_buf, sq, x, y, n, tq * tile, tq < ntiles); tq += gridDim.x;
         fx_cp_wait<EX_STAGES - 1>();
-        exdot_consume<VEC, SUM>(ex_buf, stage, n, t * tile, acc, &sh);
+        exdot_consume<VEC, MODE>(ex_buf, stage, n, t * tile, acc, &sh);
         if (++stage == EX_STAGES) stage = 0;
     }
     fx_cp_wait<0>();
@@ -161,7 +177,7 @@ __global__ void __launch_bounds__(256, 2) k_exdot(const double* __restrict__ x, 
 }
 
 // one launch over m <= 2^28 elements (keeps every 64-bit digit far from overflow); first/last: position in the call
-fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64_t m, int first, int last, double* result_dev, bool sum) {
+fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64_t m, int first, int last, double* result_dev, int mode) {
     const bool vec = aligned16(x) && aligned16(y);
     int bd = c->launch[0][1] ? c->launch[0][1] : 256;
     if (bd > 256) bd = 256;                     // compiled for <= 256 threads per CTA
@@ -169,25 +185,28 @@ fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64
     static bool attr_done = false;
     static int occ_cache[9] = {0};              // resident CTAs per SM by block size / 32
     if (!attr_done) {
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_STAGES * 2 * EX_U * 256 * 8));
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_STAGES * 2 * EX_U * 256 * 8));
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_STAGES * 2 * EX_U * 256 * 8));
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, EX_STAGES * 2 * EX_U * 256 * 8));
+        const int sm = EX_STAGES * 2 * EX_U * 256 * 8;
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
+        FX_CUDA(cudaFuncSetAttribute(k_exdot<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
         attr_done = true;
     }
     int& occ = occ_cache[bd / 32];
-    if (!occ && (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_exdot<true, false>, bd, smem) != cudaSuccess || occ < 1)) occ = 1;
+    if (!occ && (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_exdot<true, 0>, bd, smem) != cudaSuccess || occ < 1)) occ = 1;
     const long long tile = (long long)bd * EX_U;
     long long grid = (m + tile - 1) / tile;
     const long long gmax = (long long)c->num_sms * occ;             // one resident wave: every CTA pays one flush + merge
     if (grid > gmax) grid = gmax;
     if (grid < 1) grid = 1;
     if (c->launch[0][0]) grid = c->launch[0][0];
-    if (sum) {
-        if (vec) k_exdot<true, true><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
-        else k_exdot<false, true><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
-    } else if (vec) k_exdot<true, false><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
-    else k_exdot<false, false><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
+#define FX_EXDOT_GO(M) \
+    if (vec) k_exdot<true, M><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev); \
+    else k_exdot<false, M><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev);
+    if (mode == 1) { FX_EXDOT_GO(1) } else if (mode == 2) { FX_EXDOT_GO(2) } else { FX_EXDOT_GO(0) }
+#undef FX_EXDOT_GO
     c->launches++;
     FX_CUDA(cudaGetLastError());
     return FX_OK;
@@ -375,13 +394,25 @@ extern "C" double fx_exdot_f32(const float* x, const float* y, int64_t n) {
     const bool vec = aligned16(x) && aligned16(y);
     const int64_t CHUNK = (int64_t)1 << 28;
     int64_t done = 0;
-    do {
+    // long, 8-byte aligned inputs: pairs of floats through the fp64 dot kernel's ring (k_exdot<., 2>), 2^27 pairs per
+    // launch; an odd last element (or short / 4-byte aligned input) through the generic kernel below
+    if (n >= 8192 && ((uintptr_t)x & 7) == 0 && ((uintptr_t)y & 7) == 0) {
+        const int64_t SLOTS = (int64_t)1 << 27;
+        while (n - done >= 2) {
+            int64_t h = (n - done) / 2;
+            if (h > SLOTS) h = SLOTS;
+            if (fx_launch_exdot_part(c, (const double*)(x + done), (const double*)(y + done), h, done == 0, done + 2 * h == n, c->result_dev, 2) != FX_OK) return NAN;
+            done += 2 * h;
+        }
+    }
+    const bool tailvec = vec && done == 0;
+    if (done < n || n == 0) do {
         const int64_t m = (n - done < CHUNK) ? (n - done) : CHUNK;
         const long long tile = (long long)bd * EXF_U;
         long long grid = (m + tile - 1) / tile;
         if (grid > (long long)c->num_sms * occ) grid = (long long)c->num_sms * occ;
         if (grid < 1) grid = 1;
-        if (vec) k_exdot_f32<true><<<(int)grid, bd, smem, c->stream>>>(x + done, y + done, m, c->ex, done == 0, done + m == n, c->result_dev);
+        if (tailvec) k_exdot_f32<true><<<(int)grid, bd, smem, c->stream>>>(x + done, y + done, m, c->ex, done == 0, done + m == n, c->result_dev);
         else k_exdot_f32<false><<<(int)grid, bd, smem, c->stream>>>(x + done, y + done, m, c->ex, done == 0, done + m == n, c->result_dev);
         c->launches++;
         if (cudaGetLastError() != cudaSuccess) { fx_cuda_fail(cudaGetLastError(), "k_exdot_f32"); return NAN; }
@@ -419,7 +450,7 @@ fx_status fx_launch_exsum(FxCtx* c, const double* x, int64_t n, double* result_d
         int64_t h = ((n - done) / 2) & ~(int64_t)1;
         if (h > HALF) h = HALF;
         const bool last = done + 2 * h == n;
-        fx_status s = fx_launch_exdot_part(c, x + done, x + done + h, h, first, last, result_dev, true);
+        fx_status s = fx_launch_exdot_part(c, x + done, x + done + h, h, first, last, result_dev, 1);
         if (s != FX_OK) return s;
         first = false;
         done += 2 * h;

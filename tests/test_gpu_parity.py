@@ -521,7 +521,7 @@ def test_dg_derivative_definition_shapes_and_full_size(fx, oracle, direction):
         fx.dg_derivative(g, direction, 0, 1.0, y, 0.0, y)
 
 
-@pytest.mark.parametrize("n", [0, 1, 5, 1027, 100003, (1 << 22) + 9])
+@pytest.mark.parametrize("n", [0, 1, 5, 1027, 8191, 8192, 8193, 100003, (1 << 22) + 9])
 def test_exdot_f32(fx, oracle, n):
     """binary32 inputs, exact accumulation"""
     import torch
@@ -532,6 +532,11 @@ def test_exdot_f32(fx, oracle, n):
     assert fbits(fx.exdot_f32(dx, dy)) == fbits(oracle.exdot_f32(x, y) if n else 0.0)
     if n > 4:
         assert fbits(fx.exdot_f32(dx[1:], dy[1:])) == fbits(oracle.exdot_f32(x[1:], y[1:]))      # 4-byte aligned only
+        assert fbits(fx.exdot_f32(dx[2:], dy[2:])) == fbits(oracle.exdot_f32(x[2:], y[2:]))      # 8-byte aligned only
+        for grid, block in [(1, 32), (9, 128)]:
+            fx.set_launch(0, grid, block)
+            assert fbits(fx.exdot_f32(dx, dy)) == fbits(oracle.exdot_f32(x, y)), (grid, block)
+        fx.set_launch(0, 0, 0)
 
 
 # ---- fused pointwise product and Arakawa bracket --------------------------------------------------------
@@ -695,3 +700,27 @@ def test_exsum_multi_launch(fx, oracle):
     # the oracle over the same values, in four host chunks (the exact sum is order-free: compare through the exact dot with ones)
     want = oracle.exsum(x.cpu().numpy())
     assert fbits(got) == fbits(want)
+
+
+def test_exdot_f32_widening_cases(fx, oracle):
+    """every class of binary32 value through the kernel's integer widening: subnormals, both zeros, extremes, inf, nan"""
+    import torch
+    r = fi.rng(121)
+    n = 50001                                                  # long enough for the ring path (float pairs in 8-byte slots)
+    bitsx = r.integers(0, 1 << 32, n, dtype=np.uint64).astype(np.uint32)
+    bitsy = r.integers(0, 1 << 32, n, dtype=np.uint64).astype(np.uint32)
+    for b in (bitsx, bitsy):                                   # no inf / nan in the bulk
+        e = (b >> 23) & 0xff
+        b[e == 0xff] &= np.uint32(0xbfffffff)
+    bitsx[:2000] &= np.uint32(0x807fffff)                      # 2000 subnormals and zeros of either sign
+    bitsy[1000:3000] &= np.uint32(0x807fffff)
+    bitsx[3000] = 0x80000000; bitsy[3001] = 0x00000001; bitsx[3002] = 0x7f7fffff; bitsy[3002] = 0xff7fffff
+    x = bitsx.view(np.float32).copy(); y = bitsy.view(np.float32).copy()
+    with np.errstate(all="ignore"):
+        want = oracle.exdot_f32(x, y)
+    got = fx.exdot_f32(torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda())
+    assert fbits(got) == fbits(want)
+    x[7] = np.inf; y[7] = np.float32(-2.0)
+    assert fx.exdot_f32(torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda()) == -np.inf
+    y[9] = np.nan
+    assert math.isnan(fx.exdot_f32(torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda()))

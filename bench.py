@@ -129,8 +129,8 @@ def run_fx(args):
         # ---- warm-up: W iterations through the same call (also allocates the library's work space) -------------
         fx.cg_solve(g, chi, rho, phi, 0.0, Wm)
         phi.zero_()
-        fx.cg_profile(True)
-        torch.cuda.synchronize()
+        fx.cg_profile(8)             # events around the whole loop and around K1, K2 of every 8th iteration (each sampled
+        torch.cuda.synchronize()     # iteration costs ~9 us of serialisation; with every iteration sampled the step reads 5 % slow)
         if world > 1:
             dist.barrier()
         l0 = fx.launch_count()

@@ -155,9 +155,11 @@ fx_status fx_cg_solve_host(const fx_grid* grid, const double* chi_host, const do
                            double tol, int32_t maxit, fx_cg_info* info);
 
 /* Timing hook for bench.py: with enable != 0, fx_cg_solve (fused driver) records CUDA events on its stream around
- * every kernel of the iteration loop.  fx_cg_last_profile then returns, for the most recent solve: the device time
- * of the whole loop, the summed device time of each of the three kernels K1 (apply + dot), K2 (updates + dot),
- * K3 (direction), and the number of iterations those sums cover.  ms_host: host double[4] = {loop, K1, K2, K3}.   */
+ * the kernels of every enable-th iteration of the loop (1 = every iteration; the events between the kernels cost
+ * about 9 us per sampled iteration on a B200, so bench.py samples every 8th) and around the whole loop.
+ * fx_cg_last_profile then returns, for the most recent solve: the device time of the whole loop, the device time of each
+ * of the three kernels K1 (apply + dot), K2 (updates + dot), K3 (direction) summed over the sampled iterations and
+ * scaled to the loop's iteration count, and that count.  ms_host: host double[4] = {loop, K1, K2, K3}.              */
 fx_status fx_cg_profile(int32_t enable);
 fx_status fx_cg_last_profile(double* ms_host, int32_t* iterations_host);
 

@@ -310,7 +310,8 @@ def time_primitive(kind, a, b, c, reps, grid=None):
 
 
 def cg_profile(enable):
-    _check(lib().fx_cg_profile(int(bool(enable))), "fx_cg_profile")
+    """enable: False/0 = off, True/1 = events around the kernels of every iteration, n > 1 = of every n-th iteration"""
+    _check(lib().fx_cg_profile(int(enable)), "fx_cg_profile")
 
 
 def cg_last_profile():

@@ -1,6 +1,7 @@
 // fx.cu -- context, the vector primitives, the exact-dot kernel, the dG apply kernel and their C ABI (include/fx.h).
 // sm_100a only.  Compile with -fmad=false: every FMA below is written explicitly.
 
+#include <cstdlib>
 #include <math.h>
 #include <stdarg.h>
 #include <string.h>
@@ -49,6 +50,7 @@ FxCtx* fx_ctx() {
     c->ex.flags = (int*)(c->ex.limbs + FX_NLIMB);
     c->ex.ticket = (unsigned int*)(c->ex.flags + 4);
     c->cg_fused = 1;
+    { const char* e = getenv("FX_PDL"); c->cg_pdl = e && e[0] == '1'; }      // measured slower on B200: off unless asked for
     c->ready = true;
     return c;
 }

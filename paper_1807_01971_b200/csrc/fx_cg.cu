@@ -32,6 +32,24 @@ struct CgScal {
 #define CG_W 40
 typedef ExAcc<CG_K, CG_W> CgAcc;
 
+// Programmatic dependent launch (optional, FX_PDL=1): K1 and K2 of the fused loop are launched with programmatic stream
+// serialisation, so a kernel's CTAs are scheduled as soon as the previous kernel's CTAs leave the SMs, set up their
+// shared memory and wait here until the previous kernel has completed and flushed; nothing that depends on it (not even
+// the done flag) is read before, and nothing is written before.  Without the launch attribute both calls are no-ops.
+// Measured on config 3: 196 us per iteration with it, 171 us without -- off by default.
+#define FX_PDL_SYNC() do { cudaGridDependencySynchronize(); cudaTriggerProgrammaticLaunchCompletion(); } while (0)
+
+template <class... KArgs, class... Args>
+static cudaError_t cg_launch(bool pdl, void (*kern)(KArgs...), int grid, int block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 // ---- K1: direction update + apply + dot -------------------------------------------------------------------------
 // Register budget of K1: __maxnreg__ instead of __launch_bounds__(threads, minBlocks) -- the latter makes
 // ptxas pick 168 registers for anything between two and three 128-thread CTAs per SM, and K1<3> then spills 880 bytes;
@@ -45,11 +63,12 @@ template <int P, bool NEU>
 __global__ void __maxnreg__(P <= 2 ? 128 : P == 3 ? FX_K1_R : 255)
 k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi, const double* __restrict__ pin,
                    const double* __restrict__ r, double* __restrict__ pout, double* __restrict__ q, ExGlobal ex, CgScal* sc) {
-    if (*(volatile int*)&sc->done) return;
     __shared__ ExShared sh;
     ex_shared_init(&sh);
     CgAcc acc;
     acc.init();
+    FX_PDL_SYNC();                          // everything above overlaps the previous kernel's tail
+    if (*(volatile int*)&sc->done) return;
     // first iteration: p = z was set up by the caller, copy it through; later: p = z + beta p with the beta K2 left.
     // (sc->iters is bumped by this kernel's own finaliser, which runs after every CTA has started.)
     const DgSrc src = {pin, r, pout, sc->beta, *(volatile int*)&sc->iters > 0};
@@ -110,12 +129,13 @@ template <int P>
 __global__ void __launch_bounds__(256, 3) k_cg_update(const __grid_constant__ DgParams g, const double* __restrict__ p,
                                                       const double* __restrict__ q, double* phi, double* r, ExGlobal ex,
                                                       CgScal* sc) {
-    if (*(volatile int*)&sc->done) return;
     extern __shared__ __align__(16) double cg_buf[];
     __shared__ ExShared sh;
     ex_shared_init(&sh);
     CgAcc acc;
     acc.init();
+    FX_PDL_SYNC();
+    if (*(volatile int*)&sc->done) return;
     const double alpha = sc->alpha, nalpha = -alpha;
     const int pitch = g.Nx * P, rows = g.Ny * P, bd = blockDim.x;
     const int cpr = (pitch + CG_U * bd - 1) / (CG_U * bd);
@@ -184,14 +204,12 @@ template <int P>
 __global__ void __launch_bounds__(256, 3) k_cg_update_tma(const __grid_constant__ DgParams g, const double* __restrict__ p,
                                                           const double* __restrict__ q, double* phi, double* r, ExGlobal ex,
                                                           CgScal* sc) {
-    if (*(volatile int*)&sc->done) return;
     extern __shared__ __align__(128) double cg_buf[];
     __shared__ ExShared sh;
     __shared__ __align__(8) unsigned long long bars[2 * K2_STAGES];
     ex_shared_init(&sh);
     CgAcc acc;
     acc.init();
-    const double alpha = sc->alpha, nalpha = -alpha;
     const int pitch = g.Nx * P, bd = blockDim.x, nwarp = bd >> 5;
     const long long n = (long long)pitch * g.Ny * P;
     const long long tile = 2ll * bd, nfull = n / tile;
@@ -203,6 +221,9 @@ __global__ void __launch_bounds__(256, 3) k_cg_update_tma(const __grid_constant_
         fx_mbar_fence_init();
     }
     __syncthreads();
+    FX_PDL_SYNC();                          // barriers are set up while the previous kernel drains
+    if (*(volatile int*)&sc->done) return;
+    const double alpha = sc->alpha, nalpha = -alpha;
     // my full tiles: blockIdx.x, +G, ...  (count as a 32-bit number)
     const int mine = blockIdx.x < nfull ? (int)((nfull - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
     const long long step = (long long)gridDim.x * tile;
@@ -446,16 +467,19 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, 
         const double* pin = (k & 1) ? pbuf1 : pbuf0;
         double* pout = (k & 1) ? pbuf0 : pbuf1;
         cudaEvent_t* ev = nullptr;
-        if (c->prof_on && c->prof_iters < c->prof_cap) { ev = c->prof_ev + 4 * c->prof_iters; c->prof_iters++; }
+        if (c->prof_on && k == 0) cudaEventRecord(c->prof_loop[0], c->stream);
+        if (c->prof_on && k % c->prof_stride == 0 && c->prof_iters < c->prof_cap) { ev = c->prof_ev + 4 * c->prof_iters; c->prof_iters++; }
         if (ev) cudaEventRecord(ev[0], c->stream);
-        if (fx_dg_has_neumann(&dp)) k_cg_dir_apply_dot<P, true><<<ag, ab, k1_smem, c->stream>>>(dp, chi, pin, r, pout, q, c->ex, sc);
-        else k_cg_dir_apply_dot<P, false><<<ag, ab, k1_smem, c->stream>>>(dp, chi, pin, r, pout, q, c->ex, sc);
+        const bool pdl = !ev && c->cg_pdl;                        // (profiling events between the kernels: plain launches)
+        if (fx_dg_has_neumann(&dp)) cg_launch(pdl, k_cg_dir_apply_dot<P, true>, ag, ab, k1_smem, c->stream, dp, chi, pin, r, pout, q, c->ex, sc);
+        else cg_launch(pdl, k_cg_dir_apply_dot<P, false>, ag, ab, k1_smem, c->stream, dp, chi, pin, r, pout, q, c->ex, sc);
         if (ev) cudaEventRecord(ev[1], c->stream);
-        if (lin) k_cg_update_tma<P><<<lg, eb, (size_t)K2_STAGES * 4 * 2 * eb * 8, c->stream>>>(dp, pout, q, phi, r, c->ex, sc);
-        else k_cg_update<P><<<eg, eb, (size_t)FX_STAGES * 4 * CG_U * eb * 8, c->stream>>>(dp, pout, q, phi, r, c->ex, sc);
+        if (lin) cg_launch(pdl, k_cg_update_tma<P>, lg, eb, (size_t)K2_STAGES * 4 * 2 * eb * 8, c->stream, dp, (const double*)pout, (const double*)q, phi, r, c->ex, sc);
+        else cg_launch(pdl, k_cg_update<P>, eg, eb, (size_t)FX_STAGES * 4 * CG_U * eb * 8, c->stream, dp, (const double*)pout, (const double*)q, phi, r, c->ex, sc);
         if (ev) { cudaEventRecord(ev[2], c->stream); cudaEventRecord(ev[3], c->stream); }
         c->launches += 2;
     }
+    if (c->prof_on) cudaEventRecord(c->prof_loop[1], c->stream);      // re-recorded after every batch: the last one stands
     FX_CUDA(cudaGetLastError());
     return FX_OK;
 }
@@ -467,8 +491,11 @@ extern "C" fx_status fx_cg_profile(int32_t enable) {
         c->prof_cap = 1024;
         c->prof_ev = (cudaEvent_t*)calloc((size_t)4 * c->prof_cap, sizeof(cudaEvent_t));
         for (int i = 0; i < 4 * c->prof_cap; ++i) FX_CUDA(cudaEventCreate(&c->prof_ev[i]));
+        FX_CUDA(cudaEventCreate(&c->prof_loop[0]));
+        FX_CUDA(cudaEventCreate(&c->prof_loop[1]));
     }
-    c->prof_on = enable ? 1 : 0;
+    c->prof_on = enable > 0 ? 1 : 0;
+    c->prof_stride = enable > 0 ? enable : 1;
     return FX_OK;
 }
 
@@ -483,17 +510,21 @@ extern "C" fx_status fx_cg_last_profile(double* ms, int32_t* iters) {
 
 static fx_status cg_collect_profile(FxCtx* c, int iters_done) {
     for (int i = 0; i < 4; ++i) c->prof_ms[i] = 0.0;
-    int m = c->prof_iters < iters_done ? c->prof_iters : iters_done;
-    c->prof_iters = m;
+    // sampled iterations: 0, stride, 2 stride, ... below iters_done
+    int m = c->prof_iters;
+    const int valid = iters_done > 0 ? (iters_done - 1) / c->prof_stride + 1 : 0;
+    if (m > valid) m = valid;
+    c->prof_iters = iters_done;
     if (m <= 0) return FX_OK;
     float t;
-    FX_CUDA(cudaEventElapsedTime(&t, c->prof_ev[0], c->prof_ev[4 * (m - 1) + 3]));
+    FX_CUDA(cudaEventElapsedTime(&t, c->prof_loop[0], c->prof_loop[1]));
     c->prof_ms[0] = t;
     for (int i = 0; i < m; ++i)
         for (int k = 0; k < 3; ++k) {
             FX_CUDA(cudaEventElapsedTime(&t, c->prof_ev[4 * i + k], c->prof_ev[4 * i + k + 1]));
             c->prof_ms[1 + k] += t;
         }
+    for (int k = 0; k < 3; ++k) c->prof_ms[1 + k] *= (double)iters_done / m;       // scaled from the m sampled iterations to the loop
     return FX_OK;
 }
 

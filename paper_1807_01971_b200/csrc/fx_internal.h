@@ -23,6 +23,7 @@ struct FxCtx {
     // launch-shape overrides (fx_set_launch): [kernel_id][0]=grid, [1]=block
     int launch[4][2];
     int cg_fused;
+    int cg_pdl;                 // programmatic dependent launch of the fused loop's kernels (off; environment FX_PDL=1 turns it on)
     // CG work space
     double* cg_vec; int64_t cg_cap;   // 7 vectors of cg_cap doubles
     void* cg_scal;                     // CgScal on the device
@@ -36,7 +37,8 @@ struct FxCtx {
     cudaEvent_t ev_copy[2], ev_comp[2];
     int64_t launches;
     // fx_cg_profile
-    int prof_on, prof_iters, prof_cap;
+    int prof_on, prof_iters, prof_cap, prof_stride;
+    cudaEvent_t prof_loop[2];   // begin of iteration 0, end of the last enqueued batch
     cudaEvent_t* prof_ev;
     double prof_ms[4];
 };

@@ -214,7 +214,7 @@ fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64
 
 // ---- weighted dot (NA = 3: x, w, y) and exact sum (NA = 1) -- SURVEY 8f-3 ---------------------------------------------
 // Same accumulator, same single-pass finaliser; generic cp.async ring (8-byte copies: no alignment requirement).
-template <int NA>
+template <int NA, bool VEC>
 __global__ void __launch_bounds__(256, 2) k_exdotn(const double* __restrict__ a0, const double* __restrict__ a1,
                                                    const double* __restrict__ a2, long long n, ExGlobal g, int first, int last,
                                                    double* result) {
@@ -229,13 +229,25 @@ __global__ void __launch_bounds__(256, 2) k_exdotn(const double* __restrict__ a0
     auto issue = [&](int stage, long long t) {
         double* s0 = ex_buf + (size_t)stage * NA * EX_U * bd;
         if (t < ntiles) {
+            if (VEC) {                                               // 16-byte copies: all arrays 16-byte aligned
 #pragma unroll
-            for (int u = 0; u < EX_U; ++u) {
-                const int slot = u * bd + threadIdx.x;
-                const long long e = t * tile + slot;
-                const bool in = e < n;
+                for (int u = 0; u < EX_U / 2; ++u) {
+                    const int slot = 2 * (u * bd + threadIdx.x);
+                    const long long e = t * tile + slot;
+                    const long long left = n - e;
+                    const int bytes = left >= 2 ? 16 : (left == 1 ? 8 : 0);
 #pragma unroll
-                for (int a = 0; a < NA; ++a) fx_cp_async8(fx_smem_addr(s0 + a * EX_U * bd + slot), arr[a] + (in ? e : 0), in);
+                    for (int a = 0; a < NA; ++a) fx_cp_async16(fx_smem_addr(s0 + a * EX_U * bd + slot), arr[a] + (bytes ? e : 0), bytes);
+                }
+            } else {
+#pragma unroll
+                for (int u = 0; u < EX_U; ++u) {
+                    const int slot = u * bd + threadIdx.x;
+                    const long long e = t * tile + slot;
+                    const bool in = e < n;
+#pragma unroll
+                    for (int a = 0; a < NA; ++a) fx_cp_async8(fx_smem_addr(s0 + a * EX_U * bd + slot), arr[a] + (in ? e : 0), in);
+                }
             }
         }
         fx_cp_commit();
@@ -251,14 +263,29 @@ __global__ void __launch_bounds__(256, 2) k_exdotn(const double* __restrict__ a0
         const double* s0 = ex_buf + (size_t)stage * NA * EX_U * bd;
         double xv[EX_U], yv[EX_U];
         bool act[EX_U];
+        if (VEC) {
 #pragma unroll
-        for (int u = 0; u < EX_U; ++u) {
-            const int slot = u * bd + threadIdx.x;
-            act[u] = t * tile + slot < n;
-            if (NA == 3) { xv[u] = __dmul_rn(s0[slot], s0[EX_U * bd + slot]); yv[u] = s0[2 * EX_U * bd + slot]; }   // u = RN(x*w)
-            else { xv[u] = s0[slot]; yv[u] = act[u] ? 1.0 : 0.0; }
+            for (int u = 0; u < EX_U / 2; ++u) {
+                const int slot = 2 * (u * bd + threadIdx.x);
+                act[2 * u] = t * tile + slot < n; act[2 * u + 1] = t * tile + slot + 1 < n;
+                const double2 a = *reinterpret_cast<const double2*>(s0 + slot);
+                if (NA == 3) {
+                    const double2 w = *reinterpret_cast<const double2*>(s0 + EX_U * bd + slot);
+                    const double2 b = *reinterpret_cast<const double2*>(s0 + 2 * EX_U * bd + slot);
+                    xv[2 * u] = __dmul_rn(a.x, w.x); xv[2 * u + 1] = __dmul_rn(a.y, w.y); yv[2 * u] = b.x; yv[2 * u + 1] = b.y;
+                } else { xv[2 * u] = a.x; xv[2 * u + 1] = a.y; yv[2 * u] = act[2 * u] ? 1.0 : 0.0; yv[2 * u + 1] = act[2 * u + 1] ? 1.0 : 0.0; }
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < EX_U; ++u) {
+                const int slot = u * bd + threadIdx.x;
+                act[u] = t * tile + slot < n;
+                if (NA == 3) { xv[u] = __dmul_rn(s0[slot], s0[EX_U * bd + slot]); yv[u] = s0[2 * EX_U * bd + slot]; }   // u = RN(x*w)
+                else { xv[u] = s0[slot]; yv[u] = act[u] ? 1.0 : 0.0; }
+            }
         }
         if (NA == 1) acc.add<EX_U, false, true>(xv, yv, act, &sh);   // x * 1 is exact: no error term
+        else if (VEC && (t + 1) * tile <= n) acc.add_all<EX_U>(xv, yv, &sh);   // full tile: no activity flags
         else acc.add<EX_U>(xv, yv, act, &sh);
         if (++stage == EX_STAGES) stage = 0;
     }
@@ -274,8 +301,9 @@ static fx_status launch_exdotn(FxCtx* c, const double* a0, const double* a1, con
     static bool attr_done = false;
     static int occ = 0;
     if (!attr_done) {
-        FX_CUDA(cudaFuncSetAttribute(k_exdotn<NA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_exdotn<NA>, bd, smem) != cudaSuccess || occ < 1) occ = 1;
+        FX_CUDA(cudaFuncSetAttribute(k_exdotn<NA, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        FX_CUDA(cudaFuncSetAttribute(k_exdotn<NA, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_exdotn<NA, true>, bd, smem) != cudaSuccess || occ < 1) occ = 1;
         attr_done = true;
     }
     const int64_t CHUNK = (int64_t)1 << 28;
@@ -286,8 +314,11 @@ static fx_status launch_exdotn(FxCtx* c, const double* a0, const double* a1, con
         long long grid = (m + tile - 1) / tile;
         if (grid > (long long)c->num_sms * occ) grid = (long long)c->num_sms * occ;
         if (grid < 1) grid = 1;
-        k_exdotn<NA><<<(int)grid, bd, smem, c->stream>>>(a0 + done, a1 ? a1 + done : nullptr, a2 ? a2 + done : nullptr, m, c->ex, done == 0,
-                                                         done + m == n, result_dev);
+        const bool vec = aligned16(a0) && (!a1 || aligned16(a1)) && (!a2 || aligned16(a2));     // (done is a multiple of 2^28)
+        if (vec) k_exdotn<NA, true><<<(int)grid, bd, smem, c->stream>>>(a0 + done, a1 ? a1 + done : nullptr, a2 ? a2 + done : nullptr, m, c->ex,
+                                                                        done == 0, done + m == n, result_dev);
+        else k_exdotn<NA, false><<<(int)grid, bd, smem, c->stream>>>(a0 + done, a1 ? a1 + done : nullptr, a2 ? a2 + done : nullptr, m, c->ex,
+                                                                     done == 0, done + m == n, result_dev);
         c->launches++;
         FX_CUDA(cudaGetLastError());
         done += m;
@@ -456,7 +487,7 @@ fx_status fx_launch_exsum(FxCtx* c, const double* x, int64_t n, double* result_d
         done += 2 * h;
     }
     if (done < n) {
-        k_exdotn<1><<<1, 256, (size_t)EX_STAGES * EX_U * 256 * sizeof(double), c->stream>>>(x + done, nullptr, nullptr, n - done, c->ex, 0, 1, result_dev);
+        k_exdotn<1, false><<<1, 256, (size_t)EX_STAGES * EX_U * 256 * sizeof(double), c->stream>>>(x + done, nullptr, nullptr, n - done, c->ex, 0, 1, result_dev);
         c->launches++;
         FX_CUDA(cudaGetLastError());
     }

@@ -136,8 +136,9 @@ fx_status fx_dg_tables(int32_t P, double* out_host);
 fx_status fx_dg_derivative(const fx_grid* grid, int32_t direction, int32_t flux, double alpha, const double* x_dev, double beta,
                            double* y_dev);
 /* Arakawa bracket out = {f, g} = f_x g_y - f_y g_x in Arakawa's conserving form with centred dG derivatives (the
- * second composite the paper benchmarks, Fig. 6a), evaluated as the nine calls of D:6.8: 4 derivatives, 3 fused pointwise
- * products, 2 accumulating derivatives.  f, g, out: device vectors of the grid; out must not overlap f or g.            */
+ * second composite the paper benchmarks, Fig. 6a), defined as the nine calls of D:6.8: 4 derivatives, 3 fused pointwise
+ * products, 2 accumulating derivatives (the three products run in one kernel, with the bits of the three calls).
+ * f, g, out: device vectors of the grid; out must not overlap f or g.  Six work vectors are kept by the library.        */
 fx_status fx_arakawa(const fx_grid* grid, const double* f_dev, const double* g_dev, double* out_dev);
 /* The derivative tables for the cross-check against the oracle: host double[2*P*P + 2*P] = TT interior, TT first
  * Dirichlet cell (P*P each, row-major), cN, cP.  No GPU.                                                               */

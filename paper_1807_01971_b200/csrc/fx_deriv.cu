@@ -229,6 +229,21 @@ extern "C" fx_status fx_dg_dtables(int32_t P, int32_t flux, double* out) {
 }
 
 // ---- Arakawa bracket as the paper runs it: nine calls of the primitives --------------------------------
+// The three fused products of the bracket in one pass (6 vectors in, 3 out instead of 3 x (4 in, 1 out)); per element the
+// operation sequence of three fx_pointwise_dot2 calls with alpha = 1/3, beta = -1/3, gamma = 0:
+//   out = 1/3 (fx gy - fy gx),  h1 = 1/3 (f gy - g fy),  h2 = 1/3 (g fx - f gx)
+__global__ void __launch_bounds__(512) k_arakawa_products(double a, double b, const double* __restrict__ f, const double* __restrict__ g,
+                                                          const double* __restrict__ fx, const double* __restrict__ fy,
+                                                          const double* __restrict__ gx, const double* __restrict__ gy,
+                                                          double* __restrict__ out, double* __restrict__ h1, double* __restrict__ h2, long long n) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const double F = f[i], G = g[i], FX = fx[i], FY = fy[i], GX = gx[i], GY = gy[i];
+        out[i] = __fma_rn(__dmul_rn(a, FX), GY, __dmul_rn(__dmul_rn(b, FY), GX));
+        h1[i] = __fma_rn(__dmul_rn(a, F), GY, __dmul_rn(__dmul_rn(b, G), FY));
+        h2[i] = __fma_rn(__dmul_rn(a, G), FX, __dmul_rn(__dmul_rn(b, F), GX));
+    }
+}
+
 extern "C" fx_status fx_arakawa(const fx_grid* g, const double* f, const double* gg, double* out) {
     if (!fx_grid_ok(g) || !fx_grid_deriv_ok(g) || !f || !gg || !out) { fx_set_error("fx_arakawa: bad grid (PER / DIR only) or null pointer"); return FX_EINVAL; }
     const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
@@ -249,9 +264,15 @@ extern "C" fx_status fx_arakawa(const fx_grid* g, const double* f, const double*
     if ((s = fx_launch_derivative(c, g, 1, 2, 1.0, f, 0.0, fy_)) != FX_OK) return s;
     if ((s = fx_launch_derivative(c, g, 0, 2, 1.0, gg, 0.0, gx_)) != FX_OK) return s;
     if ((s = fx_launch_derivative(c, g, 1, 2, 1.0, gg, 0.0, gy_)) != FX_OK) return s;
-    if ((s = fx_pointwise_dot2(third, fx_, gy_, -third, fy_, gx_, 0.0, out, n)) != FX_OK) return s;     // 1/3 (fx gy - fy gx)
-    if ((s = fx_pointwise_dot2(third, f, gy_, -third, gg, fy_, 0.0, h1, n)) != FX_OK) return s;          // 1/3 (f gy - g fy)
-    if ((s = fx_pointwise_dot2(third, gg, fx_, -third, f, gx_, 0.0, h2, n)) != FX_OK) return s;          // 1/3 (g fx - f gx)
+    {
+        long long blocks = (n + 511) / 512;
+        const long long cap = (long long)c->num_sms * 4;
+        if (blocks > cap) blocks = cap;
+        if (blocks < 1) blocks = 1;
+        k_arakawa_products<<<(int)blocks, 512, 0, c->stream>>>(third, -third, f, gg, fx_, fy_, gx_, gy_, out, h1, h2, n);
+        c->launches++;
+        FX_CUDA(cudaGetLastError());
+    }
     if ((s = fx_launch_derivative(c, g, 0, 2, 1.0, h1, 1.0, out)) != FX_OK) return s;                   // += Dx(...)
     return fx_launch_derivative(c, g, 1, 2, 1.0, h2, 1.0, out);                                         // += Dy(...)
 }

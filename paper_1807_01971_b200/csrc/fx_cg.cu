@@ -471,7 +471,7 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, 
         if (c->prof_on && k % c->prof_stride == 0 && c->prof_iters < c->prof_cap) { ev = c->prof_ev + 4 * c->prof_iters; c->prof_iters++; }
         if (ev) cudaEventRecord(ev[0], c->stream);
         const bool pdl = !ev && c->cg_pdl;                        // (profiling events between the kernels: plain launches)
-        if (fx_dg_has_neumann(&dp)) cg_launch(pdl, k_cg_dir_apply_dot<P, true>, ag, ab, k1_smem, c->stream, dp, chi, pin, r, pout, q, c->ex, sc);
+        if (fx_dg_neu_variant(&dp, P)) cg_launch(pdl, k_cg_dir_apply_dot<P, true>, ag, ab, k1_smem, c->stream, dp, chi, pin, r, pout, q, c->ex, sc);
         else cg_launch(pdl, k_cg_dir_apply_dot<P, false>, ag, ab, k1_smem, c->stream, dp, chi, pin, r, pout, q, c->ex, sc);
         if (ev) cudaEventRecord(ev[1], c->stream);
         if (lin) cg_launch(pdl, k_cg_update_tma<P>, lg, eb, (size_t)K2_STAGES * 4 * 2 * eb * 8, c->stream, dp, (const double*)pout, (const double*)q, phi, r, c->ex, sc);
@@ -583,7 +583,7 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
             int occb = 0;
             {
                 const void* f;
-                if (fx_dg_has_neumann(&dp))
+                if (fx_dg_neu_variant(&dp, g->P))
                     f = g->P == 1 ? (const void*)k_cg_dir_apply_dot<1, true> : g->P == 2 ? (const void*)k_cg_dir_apply_dot<2, true>
                       : g->P == 3 ? (const void*)k_cg_dir_apply_dot<3, true> : g->P == 4 ? (const void*)k_cg_dir_apply_dot<4, true> : (const void*)k_cg_dir_apply_dot<5, true>;
                 else

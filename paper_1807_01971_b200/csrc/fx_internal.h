@@ -58,6 +58,7 @@ int fx_grid_ok(const fx_grid* g);
 int fx_grid_deriv_ok(const fx_grid* g);          // PER / DIR only: stand-alone derivatives and the bracket
 struct DgParams;
 int fx_dg_has_neumann(const DgParams* p);
+int fx_dg_neu_variant(const DgParams* p, int P);
 fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* out, double* vol4_out);
 
 // internal launchers (stream-ordered, no synchronisation)

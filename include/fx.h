@@ -75,6 +75,10 @@ fx_status fx_set_launch(int32_t kernel_id, int32_t grid_dim, int32_t block_dim);
  * cooperative kernel for grids of up to 2^20 unknowns, two fused kernels per iteration above; 2 = always the two fused
  * kernels; 3 = the persistent kernel whenever possible (< 2^24 unknowns).  Results are bit-identical in every mode.      */
 fx_status fx_set_cg_fused(int32_t fused);
+/* Test hook: which dG stencil kernels serve fx_dg_elliptic_apply* and fx_cg_solve.  0 (default) = the CTA-tile kernels
+ * (2-D TMA staging, D:6.2) whenever the row pitch Nx*P is even and the vectors are 16-byte aligned, else the warp-strip
+ * kernels; 1 = always the warp-strip kernels; 2 = as 0.  Same bits either way.                                            */
+fx_status fx_set_dg_path(int32_t path);
 
 /* ---- exactly rounded dot product (P:9) ----------------------------------------------------------
  * result = RN( sum_i x[i]*y[i] ), products and sum over the reals, one rounding to nearest-even at the end; the

@@ -43,6 +43,7 @@ _SIGNATURES = {
     "fx_shutdown": (None, []),
     "fx_set_launch": (C.c_int, [C.c_int32, C.c_int32, C.c_int32]),
     "fx_set_cg_fused": (C.c_int, [C.c_int32]),
+    "fx_set_dg_path": (C.c_int, [C.c_int32]),
     "fx_exdot": (C.c_double, [_vp, _vp, C.c_int64]),
     "fx_exdot_async": (C.c_int, [_vp, _vp, C.c_int64, _vp]),
     "fx_exdot_digits": (C.c_int, [_vp, _vp, C.c_int64, _vp, _vp, _vp]),
@@ -116,6 +117,10 @@ def set_launch(kernel_id, grid_dim=0, block_dim=0):
 
 def set_cg_fused(fused):
     _check(lib().fx_set_cg_fused(int(fused)), "fx_set_cg_fused")
+
+
+def set_dg_path(path):
+    _check(lib().fx_set_dg_path(int(path)), "fx_set_dg_path")
 
 
 def launch_count():

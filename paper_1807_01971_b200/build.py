@@ -12,7 +12,7 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libfx.so")
 BUILD = os.path.join(HERE, "build")
 
-NVCC_FLAGS = [("-D%s=%s" % (k, os.environ[k])) for k in ("FX_PFD", "FX_K1_R", "FX_K1_W", "FX_AP_R", "FX_AP_W") if os.environ.get(k)] + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
+NVCC_FLAGS = [("-D%s=%s" % (k, os.environ[k])) for k in ("FX_PFD", "FX_K1_R", "FX_K1_W", "FX_AP_R", "FX_AP_W", "FX_NBX3", "FX_MINB3", "FX_DGT_DEBUG", "FX_K1T_NS", "FX_K1T_R") if os.environ.get(k)] + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math", "-Xptxas", "-v"]
 
 
@@ -31,13 +31,19 @@ def build(force=False, verbose=False):
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     objs = []
     log = []
-    for f in cu:
+
+    def _nvcc(f):
         o = os.path.join(BUILD, f + ".o")
         r = subprocess.run([nvcc] + NVCC_FLAGS + ["-c", os.path.join(CSRC, f), "-o", o], capture_output=True, text=True)
-        log.append(r.stderr)
-        if r.returncode != 0:
-            raise RuntimeError("nvcc failed on %s:\n%s" % (f, r.stderr))
-        objs.append(o)
+        return f, o, r
+
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=min(len(cu), os.cpu_count() or 1)) as ex:      # one nvcc per translation unit, side by side
+        for f, o, r in ex.map(_nvcc, cu):
+            log.append(r.stderr)
+            if r.returncode != 0:
+                raise RuntimeError("nvcc failed on %s:\n%s" % (f, r.stderr))
+            objs.append(o)
     for f in cpp:
         o = os.path.join(BUILD, f + ".o")
         r = subprocess.run(["g++", "-O2", "-std=gnu++17", "-fPIC", "-ffp-contract=off", "-fno-fast-math", "-c",

@@ -75,6 +75,12 @@ extern "C" fx_status fx_set_cg_fused(int32_t fused) {
     g_ctx.cg_fused = fused;
     return FX_OK;
 }
+extern "C" fx_status fx_set_dg_path(int32_t path) {
+    if (path < 0 || path > 2) { fx_set_error("fx_set_dg_path: path must be 0..2"); return FX_EINVAL; }
+    if (!g_ctx.ready && !fx_ctx()) return FX_ECUDA;
+    g_ctx.dg_path = path;
+    return FX_OK;
+}
 extern "C" int64_t fx_launch_count(void) { return g_ctx.launches; }
 
 extern "C" void fx_shutdown(void) {

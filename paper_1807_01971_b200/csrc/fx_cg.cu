@@ -19,6 +19,7 @@
 #include <cooperative_groups.h>
 
 #include "fx_internal.h"
+#include "fx_dgt.cuh"
 #include "fx_stream.cuh"
 
 namespace cgr = cooperative_groups;
@@ -37,7 +38,11 @@ typedef ExAcc<CG_K, CG_W> CgAcc;
 // shared memory and wait here until the previous kernel has completed and flushed; nothing that depends on it (not even
 // the done flag) is read before, and nothing is written before.  Without the launch attribute both calls are no-ops.
 // Measured on config 3: 196 us per iteration with it, 171 us without -- off by default.
-#define FX_PDL_SYNC() do { cudaGridDependencySynchronize(); cudaTriggerProgrammaticLaunchCompletion(); } while (0)
+#define FX_PDL_SYNC() cudaGridDependencySynchronize()
+// ... and this is where a CTA lets the next kernel's CTAs be scheduled: after its main loop, so that they take over the SM
+// as this kernel drains (round 1 triggered at the start: the next kernel's CTAs then sat on shared memory and registers for
+// the whole kernel -- 196 us per iteration against 171 us)
+#define FX_PDL_TRIGGER() cudaTriggerProgrammaticLaunchCompletion()
 
 template <class... KArgs, class... Args>
 static cudaError_t cg_launch(bool pdl, void (*kern)(KArgs...), int grid, int block, size_t smem, cudaStream_t st, Args... args) {
@@ -83,6 +88,7 @@ k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict_
         if (P <= 3 && g.smr) dg_warp_strip<P, true, true, true, NEU, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, dg_smem + (size_t)(threadIdx.x >> 5) * 8 * P * P * 32);
         else dg_warp_strip<P, true, true, false, NEU, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, nullptr);
     }
+    FX_PDL_TRIGGER();
     acc.flush(&sh);
     if (ex_block_finish(&sh, ex, 1, 1, &sc->pq) && threadIdx.x == 0) {
         const double pq = sc->pq;
@@ -90,6 +96,79 @@ k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict_
         if (!(pq > 0.0) || isinf(pq)) { sc->status = FX_EBREAKDOWN; sc->done = 1; }
         else sc->alpha = __ddiv_rn(sc->rz, pq);
     }
+}
+
+// K1 on the CTA-tile stencil (fx_dgt.cuh): rows of r, p_old and chi arrive by 2-D TMA, the direction update is formed in
+// shared memory, q = S p leaves through coalesced stores and every (p, q) pair enters the column thread's exact-dot bins.
+template <int P>
+struct CgtCfg {
+    static constexpr int MINB = P >= 4 ? 2 : 3;
+    static constexpr int REGS = P == 3 ? FX_K1T_R : (65536 / (MINB * DgtCfg<P>::NT)) / 8 * 8 > 255 ? 255 : (65536 / (MINB * DgtCfg<P>::NT)) / 8 * 8;
+};
+template <int P, bool NEU>
+__global__ void __launch_bounds__(DgtCfg<P>::NT) __maxnreg__(CgtCfg<P>::REGS)
+k_cgt_dir_apply_dot(const __grid_constant__ DgParams g, const __grid_constant__ DgtTile t, const __grid_constant__ CUtensorMap mp,
+                    const __grid_constant__ CUtensorMap mph, const __grid_constant__ CUtensorMap mc, const __grid_constant__ CUtensorMap mch,
+                    const __grid_constant__ CUtensorMap mr, const __grid_constant__ CUtensorMap mrh, double* __restrict__ pout,
+                    double* __restrict__ q, ExGlobal ex, CgScal* sc) {
+    extern __shared__ __align__(128) double dgt_smem[];
+    __shared__ ExShared sh;
+    __shared__ __align__(8) unsigned long long bars[DGT_NS_K1];
+    ex_shared_init(&sh);
+    CgAcc acc;
+    acc.init();
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < DGT_NS_K1; ++s) fx_mbar_init(fx_smem_addr(bars) + 8u * s, 1u);
+        fx_mbar_fence_init();
+        fx_tma_prefetch_desc(&mp); fx_tma_prefetch_desc(&mc); fx_tma_prefetch_desc(&mr);
+    }
+    __syncthreads();
+    FX_PDL_SYNC();
+    if (*(volatile int*)&sc->done) return;
+    const DgtDir dir = {&mr, &mrh, pout, sc->beta, *(volatile int*)&sc->iters > 0};
+    dgt_tile<P, DgtCfg<P>::NBX, DGT_NS_K1, true, true, NEU, CgAcc>(g, t, &mp, &mph, &mc, &mch, dir, q, bars, (int)(blockIdx.x % t.ntx),
+                                                                    (int)(blockIdx.x / t.ntx), &acc, &sh);
+    FX_PDL_TRIGGER();
+    acc.flush(&sh);
+    if (ex_block_finish(&sh, ex, 1, 1, &sc->pq) && threadIdx.x == 0) {
+        const double pq = sc->pq;
+        sc->iters += 1;
+        if (!(pq > 0.0) || isinf(pq)) { sc->status = FX_EBREAKDOWN; sc->done = 1; }
+        else sc->alpha = __ddiv_rn(sc->rz, pq);
+    }
+}
+
+// launch state of the tile K1 for one solve: geometry and the tensor maps of p (both buffers), chi and r
+struct CgTile {
+    bool on;
+    DgtTile t;
+    int grid, block;
+    size_t smem;
+    CUtensorMap p[2], ph[2], c, ch, r, rh;
+};
+
+template <int P, bool NEU>
+static fx_status cgt_setup(FxCtx* c, const fx_grid* g, const double* chi, const double* r, const double* pb0, const double* pb1, CgTile* ct) {
+    constexpr int NBX = DgtCfg<P>::NBX;
+    typedef DgtGeom<P, NBX, 3, DGT_NS_K1> G;
+    static int occ = 0;
+    if (!occ) {
+        FX_CUDA(cudaFuncSetAttribute(k_cgt_dir_apply_dot<P, NEU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
+        FX_CUDA(cudaFuncSetAttribute(k_cgt_dir_apply_dot<P, NEU>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
+        FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_cgt_dir_apply_dot<P, NEU>, G::NT, G::SMEM));
+        if (occ < 1) occ = 1;
+    }
+    fx_dgt_shape(c, g, NBX, c->num_sms * occ, &ct->t);
+    ct->grid = ct->t.ntx * ct->t.nseg; ct->block = G::NT; ct->smem = G::SMEM;
+    const int pitch = g->Nx * P, rows = g->Ny * P;
+    fx_status s;
+    const double* pb[2] = {pb0, pb1};
+    for (int i = 0; i < 2; ++i)
+        if ((s = fx_dgt_make_map(&ct->p[i], pb[i], pitch, rows, G::BW, P)) != FX_OK || (s = fx_dgt_make_map(&ct->ph[i], pb[i], pitch, rows, G::HW, P)) != FX_OK) return s;
+    if ((s = fx_dgt_make_map(&ct->c, chi, pitch, rows, G::BW, P)) != FX_OK || (s = fx_dgt_make_map(&ct->ch, chi, pitch, rows, G::HW, P)) != FX_OK ||
+        (s = fx_dgt_make_map(&ct->r, r, pitch, rows, G::BW, P)) != FX_OK || (s = fx_dgt_make_map(&ct->rh, r, pitch, rows, G::HW, P)) != FX_OK) return s;
+    ct->on = true;
+    return FX_OK;
 }
 
 // ---- K2 / K3: streaming kernels over (row, column block) chunks --------------------------------------------------
@@ -172,6 +251,7 @@ __global__ void __launch_bounds__(256, 3) k_cg_update(const __grid_constant__ Dg
         if (++stage == FX_STAGES) stage = 0;
     }
     fx_cp_wait<0>();
+    FX_PDL_TRIGGER();
     acc.flush(&sh);
     if (ex_block_finish(&sh, ex, 1, 1, &sc->dot) && threadIdx.x == 0) {
         const double rzn = sc->dot;
@@ -286,6 +366,7 @@ __global__ void __launch_bounds__(256, 3) k_cg_update_tma(const __grid_constant_
             }
         acc.add<2>(rr, zz, act, &sh);
     }
+    FX_PDL_TRIGGER();
     acc.flush(&sh);
     if (ex_block_finish(&sh, ex, 1, 1, &sc->dot) && threadIdx.x == 0) {
         const double rzn = sc->dot;
@@ -442,7 +523,7 @@ static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int k1_warps_per_
 }
 
 template <int P>
-static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, int eg, int eb, const double* chi, double* phi,
+static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, const CgTile& ct, int ag, int ab, int eg, int eb, const double* chi, double* phi,
                                   double* r, double* pbuf0, double* pbuf1, double* q, CgScal* sc, int first_index, int iters) {
     static bool attr_done = false;
     if (!attr_done) {
@@ -471,7 +552,11 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, int ag, int ab, 
         if (c->prof_on && k % c->prof_stride == 0 && c->prof_iters < c->prof_cap) { ev = c->prof_ev + 4 * c->prof_iters; c->prof_iters++; }
         if (ev) cudaEventRecord(ev[0], c->stream);
         const bool pdl = !ev && c->cg_pdl;                        // (profiling events between the kernels: plain launches)
-        if (fx_dg_neu_variant(&dp, P)) cg_launch(pdl, k_cg_dir_apply_dot<P, true>, ag, ab, k1_smem, c->stream, dp, chi, pin, r, pout, q, c->ex, sc);
+        if (ct.on) {
+            const int b = k & 1;
+            if (fx_dg_has_neumann(&dp)) cg_launch(pdl, k_cgt_dir_apply_dot<P, true>, ct.grid, ct.block, ct.smem, c->stream, dp, ct.t, ct.p[b], ct.ph[b], ct.c, ct.ch, ct.r, ct.rh, pout, q, c->ex, sc);
+            else cg_launch(pdl, k_cgt_dir_apply_dot<P, false>, ct.grid, ct.block, ct.smem, c->stream, dp, ct.t, ct.p[b], ct.ph[b], ct.c, ct.ch, ct.r, ct.rh, pout, q, c->ex, sc);
+        } else if (fx_dg_neu_variant(&dp, P)) cg_launch(pdl, k_cg_dir_apply_dot<P, true>, ag, ab, k1_smem, c->stream, dp, chi, pin, r, pout, q, c->ex, sc);
         else cg_launch(pdl, k_cg_dir_apply_dot<P, false>, ag, ab, k1_smem, c->stream, dp, chi, pin, r, pout, q, c->ex, sc);
         if (ev) cudaEventRecord(ev[1], c->stream);
         if (lin) cg_launch(pdl, k_cg_update_tma<P>, lg, eb, (size_t)K2_STAGES * 4 * 2 * eb * 8, c->stream, dp, (const double*)pout, (const double*)q, phi, r, c->ex, sc);
@@ -597,6 +682,21 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
                 occb *= k1w;
             }
             cg_shapes(c, g, &dp, occb > 0 ? occb : 4, &ag, &ab, &eg, &eb);
+            static CgTile ct;                                    // (tensor maps are 64-byte aligned objects: kept out of the stack frame)
+            ct.on = false;
+            if (c->dg_path == 2 && fx_dgt_eligible(g, chi, r, p) && aligned16(p2)) {   // (measured: K1 on the warp-strip stencil is still the faster one)
+                const bool neu = fx_dg_has_neumann(&dp) != 0;
+#define FX_CGT(PP) s = neu ? cgt_setup<PP, true>(c, g, chi, r, p, p2, &ct) : cgt_setup<PP, false>(c, g, chi, r, p, p2, &ct); break;
+                switch (g->P) {
+                case 1: FX_CGT(1)
+                case 2: FX_CGT(2)
+                case 3: FX_CGT(3)
+                case 4: FX_CGT(4)
+                default: FX_CGT(5)
+                }
+#undef FX_CGT
+                if (s != FX_OK) return s;
+            }
             CgScal* sc = (CgScal*)c->cg_scal;
             CgScal* hs = (CgScal*)c->cg_scal_pinned;
             memset(hs, 0, sizeof(*hs));
@@ -632,11 +732,11 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
                 if (enq < maxit) {
                     const int m = (maxit - enq < batch) ? (maxit - enq) : batch;
                     switch (g->P) {
-                    case 1: s = cg_enqueue_iters<1>(c, dp, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
-                    case 2: s = cg_enqueue_iters<2>(c, dp, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
-                    case 3: s = cg_enqueue_iters<3>(c, dp, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
-                    case 4: s = cg_enqueue_iters<4>(c, dp, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
-                    default: s = cg_enqueue_iters<5>(c, dp, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
+                    case 1: s = cg_enqueue_iters<1>(c, dp, ct, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
+                    case 2: s = cg_enqueue_iters<2>(c, dp, ct, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
+                    case 3: s = cg_enqueue_iters<3>(c, dp, ct, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
+                    case 4: s = cg_enqueue_iters<4>(c, dp, ct, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
+                    default: s = cg_enqueue_iters<5>(c, dp, ct, ag, ab, eg, eb, chi, phi, r, p, p2, q, sc, enq, m); break;
                     }
                     if (s != FX_OK) return s;
                     enq += m;

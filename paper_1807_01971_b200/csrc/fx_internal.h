@@ -8,6 +8,7 @@
 
 #include "../../include/fx.h"
 #include "fx_dg.cuh"
+#include "fx_dgt.cuh"
 #include "fx_exdot.cuh"
 #include "fx_tables.h"
 
@@ -23,6 +24,7 @@ struct FxCtx {
     // launch-shape overrides (fx_set_launch): [kernel_id][0]=grid, [1]=block
     int launch[4][2];
     int cg_fused;
+    int dg_path;                // 0 = automatic (CTA-tile kernels where TMA's rules allow), 1 = warp-strip kernels, 2 = tile kernels (as 0)
     int cg_pdl;                 // programmatic dependent launch of the fused loop's kernels (off; environment FX_PDL=1 turns it on)
     // CG work space
     double* cg_vec; int64_t cg_cap;   // 7 vectors of cg_cap doubles
@@ -67,6 +69,10 @@ fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64
 fx_status fx_launch_exsum(FxCtx* c, const double* x, int64_t n, double* result_dev);
 size_t fx_dg_ring_bytes(int P, int warps, bool dirf);
 void fx_dg_shape(FxCtx* c, const fx_grid* g, DgParams* p, int warps_per_sm, int* grid, int* block, int max_wpb = 4);
+// CTA-tile stencil kernels (fx_dgt.cuh): eligibility (TMA's global-memory rules), tensor maps, launch geometry
+bool fx_dgt_eligible(const fx_grid* g, const void* a, const void* b, const void* c2);
+fx_status fx_dgt_make_map(CUtensorMap* m, const double* base, int pitch, int rows, int boxw, int boxh);
+void fx_dgt_shape(FxCtx* c, const fx_grid* g, int nbx, int resident, DgtTile* t);
 fx_status fx_launch_derivative(FxCtx* c, const fx_grid* g, int dir, int flux, double alpha, const double* x, double beta, double* y);
 fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const double* x, double* y, int normed);
 

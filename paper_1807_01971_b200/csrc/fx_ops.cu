@@ -4,6 +4,7 @@
 #include <string.h>
 
 #include "fx_internal.h"
+#include "fx_dgt.cuh"
 #include "fx_stream.cuh"
 
 // ------------------------------------------------------------------------------------------------------------
@@ -579,6 +580,112 @@ __global__ void __maxnreg__(P <= 2 ? 128 : P == 3 ? FX_AP_R : 255) k_dg_apply(co
     else dg_warp_strip<P, false, false, false, NEU, NoAcc>(g, chi, src, y, strip, j0, j1, nullptr, nullptr, nullptr);
 }
 
+// ---- the CTA-tile kernel (fx_dgt.cuh): 2-D TMA staging, O(P) registers per thread -------------------------------------------
+template <int P, bool NEU>
+__global__ void __launch_bounds__(DgtCfg<P>::NT) __maxnreg__(DgtCfg<P>::REGS)
+k_dgt_apply(const __grid_constant__ DgParams g, const __grid_constant__ DgtTile t, const __grid_constant__ CUtensorMap mu,
+            const __grid_constant__ CUtensorMap muh, const __grid_constant__ CUtensorMap mc, const __grid_constant__ CUtensorMap mch,
+            double* __restrict__ y) {
+    extern __shared__ __align__(128) double dgt_smem[];
+    __shared__ __align__(8) unsigned long long bars[DGT_NS];
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < DGT_NS; ++s) fx_mbar_init(fx_smem_addr(bars) + 8u * s, 1u);
+        fx_mbar_fence_init();
+        fx_tma_prefetch_desc(&mu); fx_tma_prefetch_desc(&muh); fx_tma_prefetch_desc(&mc); fx_tma_prefetch_desc(&mch);
+    }
+    __syncthreads();
+    const DgtDir nodir = {nullptr, nullptr, nullptr, 0.0, false};
+    dgt_tile<P, DgtCfg<P>::NBX, DGT_NS, false, false, NEU, NoAcc>(g, t, &mu, &muh, &mc, &mch, nodir, y, bars, (int)(blockIdx.x % t.ntx),
+                                                                  (int)(blockIdx.x / t.ntx), nullptr, nullptr);
+}
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (libfx.so does not link libcuda)
+typedef CUresult (*fx_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                       const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                       CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static fx_encode_tiled_fn fx_encode_tiled() {
+    static fx_encode_tiled_fn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess && qr == cudaDriverEntryPointSuccess)
+            fn = (fx_encode_tiled_fn)p;
+        tried = true;
+    }
+    return fn;
+}
+
+// tensor map over the row-major (rows x pitch) fp64 image at `base`, box = boxw x boxh doubles, zero fill outside
+fx_status fx_dgt_make_map(CUtensorMap* m, const double* base, int pitch, int rows, int boxw, int boxh) {
+    fx_encode_tiled_fn enc = fx_encode_tiled();
+    if (!enc) { fx_set_error("cuTensorMapEncodeTiled is not available"); return FX_ECUDA; }
+    const cuuint64_t dims[2] = {(cuuint64_t)pitch, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)pitch * 8ull};
+    const cuuint32_t box[2] = {(cuuint32_t)boxw, (cuuint32_t)boxh};
+    const cuuint32_t es[2] = {1u, 1u};
+    const CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                           CU_TENSOR_MAP_SWIZZLE_NONE, boxw >= 32 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { fx_set_error("cuTensorMapEncodeTiled failed (%d)", (int)r); return FX_ECUDA; }
+    return FX_OK;
+}
+
+// The tile kernels need: even row pitch and 16-byte aligned images (TMA's global-memory rules), and cuTensorMapEncodeTiled.
+bool fx_dgt_eligible(const fx_grid* g, const void* a, const void* b, const void* c2) {
+    return ((g->Nx * g->P) & 1) == 0 && aligned16(a) && aligned16(b) && aligned16(c2) && fx_encode_tiled() != nullptr;
+}
+
+// Launch geometry: tiles of NBX blocks of wb <= 30 cells, balanced over the row; segments so that the grid is whole waves
+// of `resident` CTAs with little prologue work (one extra cell row of loads and about half a row of arithmetic each).
+void fx_dgt_shape(FxCtx* c, const fx_grid* g, int nbx, int resident, DgtTile* t) {
+    const int tmax = FX_STRIP * nbx;
+    t->ntx = (g->Nx + tmax - 1) / tmax;
+    t->wb = (g->Nx + t->ntx * nbx - 1) / (t->ntx * nbx);
+    // every box must start on a 16-byte boundary of the image row (an odd starting column raised "illegal instruction" on
+    // the B200): tiles start at even columns, i.e. an even number of doubles per tile; the one-cell halo boxes then start
+    // at even columns too (fx_dgt.cuh, colL / colR)
+    if ((t->wb * nbx * g->P) & 1) t->wb++;
+    t->ntx = (g->Nx + t->wb * nbx - 1) / (t->wb * nbx);
+    int rps = c->launch[2][0];
+    if (rps <= 0) {
+        double best = 1e300;
+        rps = 1;
+        for (int r = 1; r <= g->Ny; ++r) {
+            const long long ctas = (long long)t->ntx * ((g->Ny + r - 1) / r);
+            const double cost = (double)((ctas + resident - 1) / resident) * (r + 1.0);
+            if (cost <= best) { best = cost; rps = r; }
+            if (ctas <= resident && r >= 2) break;
+        }
+    }
+    if (rps > g->Ny) rps = g->Ny;
+    t->rows_per_seg = rps;
+    t->nseg = (g->Ny + rps - 1) / rps;
+}
+
+template <int P, bool NEU>
+static fx_status launch_dgt_apply(FxCtx* c, const fx_grid* g, const DgParams& p, const double* chi, const double* x, double* y) {
+    constexpr int NBX = DgtCfg<P>::NBX;
+    typedef DgtGeom<P, NBX, 2> G;
+    static int occ = 0;
+    if (!occ) {
+        FX_CUDA(cudaFuncSetAttribute(k_dgt_apply<P, NEU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
+        FX_CUDA(cudaFuncSetAttribute(k_dgt_apply<P, NEU>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
+        FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_dgt_apply<P, NEU>, G::NT, G::SMEM));
+        if (occ < 1) occ = 1;
+    }
+    DgtTile t;
+    fx_dgt_shape(c, g, NBX, c->num_sms * occ, &t);
+    const int pitch = g->Nx * P, rows = g->Ny * P;
+    CUtensorMap mu, muh, mc, mch;
+    fx_status s;
+    if ((s = fx_dgt_make_map(&mu, x, pitch, rows, G::BW, P)) != FX_OK || (s = fx_dgt_make_map(&muh, x, pitch, rows, G::HW, P)) != FX_OK ||
+        (s = fx_dgt_make_map(&mc, chi, pitch, rows, G::BW, P)) != FX_OK || (s = fx_dgt_make_map(&mch, chi, pitch, rows, G::HW, P)) != FX_OK)
+        return s;
+    k_dgt_apply<P, NEU><<<t.ntx * t.nseg, G::NT, G::SMEM, c->stream>>>(p, t, mu, muh, mc, mch, y);
+    return FX_OK;
+}
+
 // a one-cell direction cannot carry a Dirichlet and a Neumann wall table at once (Q23)
 static bool bc_ok(int bc, int N) { return bc >= FX_BC_PER && bc <= FX_BC_NEU_DIR && !(bc == FX_BC_DIR_NEU && N < 2); }
 static int wall_lo(int bc) { return bc == FX_BC_PER ? 0 : (bc == FX_BC_DIR || bc == FX_BC_DIR_NEU) ? 1 : 2; }
@@ -671,6 +778,23 @@ fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const d
         const int w = g->P == 3 ? FX_AP_W : 4;
         FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, w * 32, 0));
         occ[g->P] = nb > 0 ? nb * w : 4;
+    }
+    if (c->dg_path != 1 && fx_dgt_eligible(g, chi, x, y)) {
+#define FX_TAPPLY(PP) \
+    s = neu ? launch_dgt_apply<PP, true>(c, g, p, chi, x, y) : launch_dgt_apply<PP, false>(c, g, p, chi, x, y); break;
+        const bool neu = fx_dg_has_neumann(&p) != 0;
+        switch (g->P) {
+        case 1: FX_TAPPLY(1)
+        case 2: FX_TAPPLY(2)
+        case 3: FX_TAPPLY(3)
+        case 4: FX_TAPPLY(4)
+        default: FX_TAPPLY(5)
+        }
+#undef FX_TAPPLY
+        if (s != FX_OK) return s;
+        c->launches++;
+        FX_CUDA(cudaGetLastError());
+        return FX_OK;
     }
     p.smr = 0;            // measured: the stand-alone apply is 2 % faster on the L1-prefetch path, the fused K1 6 % faster with the ring
     int grid, block;

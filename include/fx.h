@@ -12,8 +12,13 @@
  *     never retained or freed by the library; pointers documented "host" are ordinary host memory.
  *   - vectors are dense fp64 arrays.  A dG vector of a grid {Nx,Ny,P} has n = P*P*Nx*Ny entries laid out as a
  *     row-major (Ny*P) x (Nx*P) image, x fastest:  idx = ((j*P + l)*Nx + i)*P + k   for cell (i,j), node (k,l)   (D:4).
- *   - all work is enqueued on the stream set with fx_set_stream (default: the legacy default stream).  Calls are
- *     asynchronous except where "synchronises" is stated.
+ *   - every compute call exists in two forms.  NAME_ex(ctx, ...) works on an explicit context (fx_create: one device, one
+ *     stream, its own scratch).  The plain NAME(...) uses the default context of the calling thread's current device,
+ *     created on first use; its stream is the one set with fx_set_stream (default: the legacy default stream).  Calls are
+ *     asynchronous (stream-ordered) except where "synchronises" is stated.
+ *   - threads: different contexts are independent (two threads, two streams, two devices may work at the same time).  ONE
+ *     context -- in particular the default one -- must be used by one thread at a time, and its stream must not be changed
+ *     while work of an earlier call is still in flight (the exact-dot digits and the CG scalars are per-context scratch).
  *   - return value: fx_status.  < 0 is an error (nothing useful was computed), >= 0 is success.  No exceptions,
  *     no aborts.  fx_last_error() returns a thread-local message for the last error.
  *   - there is no CPU fallback: without a CUDA device every compute call returns FX_ECUDA.
@@ -58,12 +63,24 @@ typedef struct {
     double rel_residual;   /* sqrt(r.V.r) / sqrt(b.W.b) at exit                                                  */
 } fx_cg_info;
 
+/* ---- contexts ----------------------------------------------------------------------------------
+ * The paper's user picks the backend through the vector type (dg::DVec); here the context carries the device
+ * and the stream.  fx_create: a context on `device` (a CUDA ordinal) whose work is enqueued on `cuda_stream` (a cudaStream_t
+ * passed as void*; NULL = legacy default stream).  It owns its scratch (about 2 KB until a CG solve or a *_host call sizes
+ * work vectors) and never retains user pointers.  fx_destroy synchronises the context's stream and frees everything; NULL
+ * is ignored.  An _ex call makes the context's device current for its duration and restores the caller's device.       */
+typedef struct fx_ctx fx_ctx;
+fx_status fx_create(fx_ctx** ctx_out, int32_t device, void* cuda_stream);
+void fx_destroy(fx_ctx* ctx);
+
 /* ---- housekeeping ---------------------------------------------------------------------------------------- */
 
 /* Stream (a cudaStream_t passed as void*) used by all later calls of this process; NULL = legacy default.     */
 fx_status fx_set_stream(void* cuda_stream);
+fx_status fx_set_stream_ex(fx_ctx* ctx, void* cuda_stream);
 const char* fx_last_error(void);
-/* Release all library scratch (device digits, CG work vectors).  Optional; safe to call repeatedly.           */
+/* Release the default contexts of all devices with their scratch (device digits, CG work vectors, events).  Optional; safe
+ * to call repeatedly; contexts made by fx_create are not touched.                                               */
 void fx_shutdown(void);
 
 /* Test hook for the launch-shape invariance tests (north star: results identical "regardless of grid and block
@@ -71,14 +88,17 @@ void fx_shutdown(void);
  * CTAs (0 = default), block_dim = threads per CTA (0 = default; must be a multiple of 32, <= 1024; the dG apply
  * reads it as warps-per-CTA*32 and grid_dim as rows-per-segment).                                              */
 fx_status fx_set_launch(int32_t kernel_id, int32_t grid_dim, int32_t block_dim);
+fx_status fx_set_launch_ex(fx_ctx* ctx, int32_t kernel_id, int32_t grid_dim, int32_t block_dim);
 /* fx_cg_solve driver: 0 = one kernel per primitive, both dots visit the host; 1 (default) = fused: a single persistent
  * cooperative kernel for grids of up to 2^20 unknowns, two fused kernels per iteration above; 2 = always the two fused
  * kernels; 3 = the persistent kernel whenever possible (< 2^24 unknowns).  Results are bit-identical in every mode.      */
 fx_status fx_set_cg_fused(int32_t fused);
+fx_status fx_set_cg_fused_ex(fx_ctx* ctx, int32_t fused);
 /* Test hook: which dG stencil kernels serve fx_dg_elliptic_apply* and fx_cg_solve.  0 (default) = the CTA-tile kernels
  * (2-D TMA staging, D:6.2) whenever the row pitch Nx*P is even and the vectors are 16-byte aligned, else the warp-strip
  * kernels; 1 = always the warp-strip kernels; 2 = as 0.  Same bits either way.                                            */
 fx_status fx_set_dg_path(int32_t path);
+fx_status fx_set_dg_path_ex(fx_ctx* ctx, int32_t path);
 
 /* ---- exactly rounded dot product (P:9) ----------------------------------------------------------
  * result = RN( sum_i x[i]*y[i] ), products and sum over the reals, one rounding to nearest-even at the end; the
@@ -89,46 +109,63 @@ fx_status fx_set_dg_path(int32_t path);
 
 /* Synchronises; returns the value (NaN and fx_last_error() on failure). */
 double fx_exdot(const double* x_dev, const double* y_dev, int64_t n);
+/* Context form: result_host (host double; synchronises) and / or result_dev (device double; stream-ordered), at least one. */
+fx_status fx_exdot_ex(fx_ctx* ctx, const double* x_dev, const double* y_dev, int64_t n, double* result_host, double* result_dev);
 /* Asynchronous form: writes the double to result_dev (device, 8 bytes). */
 fx_status fx_exdot_async(const double* x_dev, const double* y_dev, int64_t n, double* result_dev);
+fx_status fx_exdot_async_ex(fx_ctx* ctx, const double* x_dev, const double* y_dev, int64_t n, double* result_dev);
 /* The long accumulator itself: 68 limbs, two's complement, limb k weighs 2^(64k-2176), plus flags
  * {nan, +inf, -inf}.  limbs_host: host uint64[68]; flags_host: host int32[3] or NULL.  Synchronises.          */
 fx_status fx_exdot_digits(const double* x_dev, const double* y_dev, int64_t n, uint64_t* limbs_host,
                           int32_t* flags_host, double* result_host);
+fx_status fx_exdot_digits_ex(fx_ctx* ctx, const double* x_dev, const double* y_dev, int64_t n, uint64_t* limbs_host,
+                             int32_t* flags_host, double* result_host);
 /* Host-buffer convenience (the "e2e" path of bench.py): x, y are HOST arrays; copies them to device scratch in
  * chunks on the library stream, accumulates, returns the value.  Synchronises.                                */
 double fx_exdot_host(const double* x_host, const double* y_host, int64_t n);
+fx_status fx_exdot_host_ex(fx_ctx* ctx, const double* x_host, const double* y_host, int64_t n, double* result_host);
 
 /* Weighted dot sum_i x[i] w[i] y[i] ("the weighted sum ... where w represents for example the volume form") in
  * the reading D:Q14: u = RN(x[i]*w[i]) in fp64, then the exactly rounded dot of u and y.  fx_exsum: the exactly rounded
  * sum of x (EXSUM) = exact dot with ones.  Device pointers, may alias; both synchronise and return the value.      */
 double fx_exdot3(const double* x_dev, const double* w_dev, const double* y_dev, int64_t n);
 double fx_exsum(const double* x_dev, int64_t n);
+fx_status fx_exdot3_ex(fx_ctx* ctx, const double* x_dev, const double* w_dev, const double* y_dev, int64_t n, double* result_host);
+fx_status fx_exsum_ex(fx_ctx* ctx, const double* x_dev, int64_t n, double* result_host);
 /* binary32 inputs, exact accumulation: RN_double(sum x[i]*y[i]), every product exact.  Synchronises.          */
 double fx_exdot_f32(const float* x_dev, const float* y_dev, int64_t n);
+fx_status fx_exdot_f32_ex(fx_ctx* ctx, const float* x_dev, const float* y_dev, int64_t n, double* result_host);
 
 /* ---- vector primitives in canonical order (D:3.2) ---------------------------------------------- */
 
 /* y[i] <- fma(alpha, x[i], RN(beta*y[i]));  beta == 0: y[i] <- RN(alpha*x[i]) and y is not read.
  * x, y: device; x may equal y; partial overlap is undefined.                                                   */
 fx_status fx_axpby(double alpha, const double* x_dev, double beta, double* y_dev, int64_t n);
+fx_status fx_axpby_ex(fx_ctx* ctx, double alpha, const double* x_dev, double beta, double* y_dev, int64_t n);
 /* u = RN(alpha*x1[i]); y[i] <- fma(u, x2[i], RN(beta*y[i]));  beta == 0: y[i] <- RN(u*x2[i]), y not read.      */
 fx_status fx_pointwise_dot(double alpha, const double* x1_dev, const double* x2_dev, double beta, double* y_dev,
                            int64_t n);
+fx_status fx_pointwise_dot_ex(fx_ctx* ctx, double alpha, const double* x1_dev, const double* x2_dev, double beta, double* y_dev,
+                              int64_t n);
 
 /* z[i] <- alpha*x1[i]*y1[i] + beta*x2[i]*y2[i] + gamma*z[i], the fused product the paper adds "to raise the work per call"
  * (P:414).  Canonical order (D:Q22): a = RN(alpha*x1); b = RN(beta*x2); t = gamma == 0 ? RN(b*y2) : fma(b, y2, RN(gamma*z));
  * z = fma(a, y1, t).  gamma == 0: z is not read.  Inputs may alias each other and z.                                     */
 fx_status fx_pointwise_dot2(double alpha, const double* x1_dev, const double* y1_dev, double beta, const double* x2_dev,
                             const double* y2_dev, double gamma, double* z_dev, int64_t n);
+fx_status fx_pointwise_dot2_ex(fx_ctx* ctx, double alpha, const double* x1_dev, const double* y1_dev, double beta, const double* x2_dev,
+                               const double* y2_dev, double gamma, double* z_dev, int64_t n);
 
 /* ---- dG elliptic operator (construction D:3.3, operation order D:3.4) -------------------------
  * S = Fx^T diag(W chi) Fx + Fy^T diag(W chi) Fy + (jump terms), symmetric; A = diag(V) S ~ -div(chi grad .),
  * V = 1/W the inverse dG weights.  chi, x, y: device vectors of the grid; y must not overlap x or chi.         */
 fx_status fx_dg_elliptic_apply(const fx_grid* grid, const double* chi_dev, const double* x_dev, double* y_dev);     /* y = A x */
 fx_status fx_dg_elliptic_apply_sym(const fx_grid* grid, const double* chi_dev, const double* x_dev, double* y_dev); /* y = S x */
+fx_status fx_dg_elliptic_apply_ex(fx_ctx* ctx, const fx_grid* grid, const double* chi_dev, const double* x_dev, double* y_dev);
+fx_status fx_dg_elliptic_apply_sym_ex(fx_ctx* ctx, const fx_grid* grid, const double* chi_dev, const double* x_dev, double* y_dev);
 /* dG weights W ("volume" of Fig. 2) and V = 1/W; either pointer may be NULL.  Device vectors.           */
 fx_status fx_dg_weights(const fx_grid* grid, double* w_dev, double* v_dev);
+fx_status fx_dg_weights_ex(fx_ctx* ctx, const fx_grid* grid, double* w_dev, double* v_dev);
 /* The reference-element tables the kernels use, for the cross-check against the oracle's own tables.
  * out_host: host double[5*P + 4*P*P] = xi,w,L,R,B (P each) then T0,T0L,WW,D (P*P each, row-major).  No GPU.   */
 fx_status fx_dg_tables(int32_t P, double* out_host);
@@ -139,11 +176,14 @@ fx_status fx_dg_tables(int32_t P, double* out_host);
  * 2 = centred (their mean).  x, y: device vectors of the grid; y must not overlap x.                                   */
 fx_status fx_dg_derivative(const fx_grid* grid, int32_t direction, int32_t flux, double alpha, const double* x_dev, double beta,
                            double* y_dev);
+fx_status fx_dg_derivative_ex(fx_ctx* ctx, const fx_grid* grid, int32_t direction, int32_t flux, double alpha, const double* x_dev,
+                              double beta, double* y_dev);
 /* Arakawa bracket out = {f, g} = f_x g_y - f_y g_x in Arakawa's conserving form with centred dG derivatives (the
  * second composite the paper benchmarks, Fig. 6a), defined as the nine calls of D:6.8: 4 derivatives, 3 fused pointwise
  * products, 2 accumulating derivatives (the three products run in one kernel, with the bits of the three calls).
  * f, g, out: device vectors of the grid; out must not overlap f or g.  Six work vectors are kept by the library.        */
 fx_status fx_arakawa(const fx_grid* grid, const double* f_dev, const double* g_dev, double* out_dev);
+fx_status fx_arakawa_ex(fx_ctx* ctx, const fx_grid* grid, const double* f_dev, const double* g_dev, double* out_dev);
 /* The derivative tables for the cross-check against the oracle: host double[2*P*P + 2*P] = TT interior, TT first
  * Dirichlet cell (P*P each, row-major), cN, cP.  No GPU.                                                               */
 fx_status fx_dg_dtables(int32_t P, int32_t flux, double* out_host);
@@ -155,18 +195,24 @@ fx_status fx_dg_dtables(int32_t P, int32_t flux, double* out_host);
  * Returns info->status.                                                                                       */
 fx_status fx_cg_solve(const fx_grid* grid, const double* chi_dev, const double* rho_dev, double* phi_dev,
                       double tol, int32_t maxit, fx_cg_info* info);
+fx_status fx_cg_solve_ex(fx_ctx* ctx, const fx_grid* grid, const double* chi_dev, const double* rho_dev, double* phi_dev,
+                         double tol, int32_t maxit, fx_cg_info* info);
 /* Host-buffer convenience (bench.py "e2e"): chi, rho, phi are HOST arrays of the grid's n doubles.            */
 fx_status fx_cg_solve_host(const fx_grid* grid, const double* chi_host, const double* rho_host, double* phi_host,
                            double tol, int32_t maxit, fx_cg_info* info);
+fx_status fx_cg_solve_host_ex(fx_ctx* ctx, const fx_grid* grid, const double* chi_host, const double* rho_host, double* phi_host,
+                              double tol, int32_t maxit, fx_cg_info* info);
 
 /* Timing hook for bench.py: with enable != 0, fx_cg_solve (fused driver) records CUDA events on its stream around
  * the kernels of every enable-th iteration of the loop (1 = every iteration; the events between the kernels cost
  * about 9 us per sampled iteration on a B200, so bench.py samples every 8th) and around the whole loop.
  * fx_cg_last_profile then returns, for the most recent solve: the device time of the whole loop, the device time of each
- * of the three kernels K1 (apply + dot), K2 (updates + dot), K3 (direction) summed over the sampled iterations and
- * scaled to the loop's iteration count, and that count.  ms_host: host double[4] = {loop, K1, K2, K3}.              */
+ * of the two kernels K1 (direction update + apply + dot) and K2 (updates + preconditioner + dot) summed over the sampled
+ * iterations and scaled to the loop's iteration count, and that count.  ms_host: host double[4] = {loop, K1, K2, 0}.  */
 fx_status fx_cg_profile(int32_t enable);
 fx_status fx_cg_last_profile(double* ms_host, int32_t* iterations_host);
+fx_status fx_cg_profile_ex(fx_ctx* ctx, int32_t enable);
+fx_status fx_cg_last_profile_ex(fx_ctx* ctx, double* ms_host, int32_t* iterations_host);
 
 /* Timing hook for the latency-bandwidth sweep (the paper reports average run times of back-to-back calls):
  * launches one primitive `reps` times (after one untimed call) between two CUDA events on the library stream and
@@ -178,8 +224,10 @@ fx_status fx_cg_last_profile(double* ms_host, int32_t* iterations_host);
  * a, b, c: device vectors of n doubles (kinds 3,4,9-13: n must equal the grid's size).  Synchronises.               */
 fx_status fx_time_primitive(int32_t kind, const fx_grid* grid, const double* a_dev, const double* b_dev, double* c_dev,
                             int64_t n, int32_t reps, double* ms_host);
+fx_status fx_time_primitive_ex(fx_ctx* ctx, int32_t kind, const fx_grid* grid, const double* a_dev, const double* b_dev, double* c_dev,
+                               int64_t n, int32_t reps, double* ms_host);
 
-/* Number of kernels this library has launched since load (bench.py's "gpu_launches").                          */
+/* Number of kernels this library has launched since load, over all contexts (bench.py's "gpu_launches").      */
 int64_t fx_launch_count(void);
 
 #ifdef __cplusplus

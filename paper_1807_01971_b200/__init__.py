@@ -67,7 +67,17 @@ _SIGNATURES = {
     "fx_cg_last_profile": (C.c_int, [_dp, C.POINTER(C.c_int32)]),
     "fx_time_primitive": (C.c_int, [C.c_int32, C.POINTER(Grid), _vp, _vp, _vp, C.c_int64, C.c_int32, _dp]),
     "fx_launch_count": (C.c_int64, []),
+    "fx_create": (C.c_int, [C.POINTER(_vp), C.c_int32, _vp]),
+    "fx_destroy": (None, [_vp]),
 }
+# the context forms: NAME_ex(ctx, <the plain call's arguments> [, result_host for the value-returning reductions])
+for _n in ("fx_set_stream", "fx_set_launch", "fx_set_cg_fused", "fx_set_dg_path", "fx_exdot_async", "fx_exdot_digits", "fx_axpby",
+           "fx_pointwise_dot", "fx_pointwise_dot2", "fx_arakawa", "fx_dg_elliptic_apply", "fx_dg_elliptic_apply_sym", "fx_dg_weights",
+           "fx_dg_derivative", "fx_cg_solve", "fx_cg_solve_host", "fx_cg_profile", "fx_cg_last_profile", "fx_time_primitive"):
+    _SIGNATURES[_n + "_ex"] = (C.c_int, [_vp] + _SIGNATURES[_n][1])
+for _n in ("fx_exdot_host", "fx_exdot3", "fx_exsum", "fx_exdot_f32"):
+    _SIGNATURES[_n + "_ex"] = (C.c_int, [_vp] + _SIGNATURES[_n][1] + [_dp])
+_SIGNATURES["fx_exdot_ex"] = (C.c_int, [_vp, _vp, _vp, C.c_int64, _dp, _vp])
 
 
 def lib_path():
@@ -105,6 +115,73 @@ def _ptr(t, n=None):
 def _use_torch_stream():
     import torch
     _check(lib().fx_set_stream(torch.cuda.current_stream().cuda_stream), "fx_set_stream")
+
+
+class Context:
+    """An explicit fx_ctx (include/fx.h "contexts"): one device, one stream, its own scratch.  The module-level functions use
+    the default context of the current device; this class exposes the same calls on a context of its own."""
+
+    def __init__(self, device=None, stream=None):
+        import torch
+        self._h = _vp()
+        dev = torch.cuda.current_device() if device is None else int(device)
+        st = stream.cuda_stream if hasattr(stream, "cuda_stream") else (stream or 0)
+        _check(lib().fx_create(C.byref(self._h), dev, st), "fx_create")
+
+    def destroy(self):
+        if self._h:
+            lib().fx_destroy(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def set_stream(self, stream):
+        st = stream.cuda_stream if hasattr(stream, "cuda_stream") else (stream or 0)
+        _check(lib().fx_set_stream_ex(self._h, st), "fx_set_stream_ex")
+
+    def set_dg_path(self, path):
+        _check(lib().fx_set_dg_path_ex(self._h, int(path)), "fx_set_dg_path_ex")
+
+    def set_cg_fused(self, fused):
+        _check(lib().fx_set_cg_fused_ex(self._h, int(fused)), "fx_set_cg_fused_ex")
+
+    def exdot(self, x, y, out=None):
+        """host float (synchronises) or, with `out` (a 1-element float64 CUDA tensor), the stream-ordered device form"""
+        n = x.numel()
+        if out is not None:
+            _check(lib().fx_exdot_ex(self._h, _ptr(x), _ptr(y, n), n, None, _ptr(out, 1)), "fx_exdot_ex")
+            return out
+        v = C.c_double(0.0)
+        _check(lib().fx_exdot_ex(self._h, _ptr(x), _ptr(y, n), n, C.byref(v), None), "fx_exdot_ex")
+        return v.value
+
+    def exsum(self, x):
+        v = C.c_double(0.0)
+        _check(lib().fx_exsum_ex(self._h, _ptr(x), x.numel(), C.byref(v)), "fx_exsum_ex")
+        return v.value
+
+    def axpby(self, alpha, x, beta, y):
+        n = x.numel()
+        _check(lib().fx_axpby_ex(self._h, float(alpha), _ptr(x), float(beta), _ptr(y, n), n), "fx_axpby_ex")
+
+    def pointwise_dot(self, alpha, x1, x2, beta, y):
+        n = x1.numel()
+        _check(lib().fx_pointwise_dot_ex(self._h, float(alpha), _ptr(x1), _ptr(x2, n), float(beta), _ptr(y, n), n), "fx_pointwise_dot_ex")
+
+    def dg_elliptic_apply(self, grid, chi, x, y, sym=False):
+        fn = lib().fx_dg_elliptic_apply_sym_ex if sym else lib().fx_dg_elliptic_apply_ex
+        _check(fn(self._h, C.byref(grid), _ptr(chi, grid.n), _ptr(x, grid.n), _ptr(y, grid.n)), "fx_dg_elliptic_apply_ex")
+
+    def cg_solve(self, grid, chi, rho, phi, tol, maxit):
+        info = CGInfo()
+        rc = lib().fx_cg_solve_ex(self._h, C.byref(grid), _ptr(chi, grid.n), _ptr(rho, grid.n), _ptr(phi, grid.n), float(tol), int(maxit),
+                                  C.byref(info))
+        _check(rc, "fx_cg_solve_ex")
+        return info
 
 
 def make_grid(Nx, Ny, P, lx, ly, bcx, bcy):

@@ -147,17 +147,16 @@ struct CgTile {
     CUtensorMap p[2], ph[2], c, ch, r, rh;
 };
 
+static CgTile* fx_cg_tile(FxCtx* c) {              // (tensor maps are 64-byte aligned objects: kept out of the stack frame)
+    if (!c->cg_tile) c->cg_tile = aligned_alloc(64, (sizeof(CgTile) + 63) / 64 * 64);
+    return (CgTile*)c->cg_tile;
+}
+
 template <int P, bool NEU>
 static fx_status cgt_setup(FxCtx* c, const fx_grid* g, const double* chi, const double* r, const double* pb0, const double* pb1, CgTile* ct) {
     constexpr int NBX = DgtCfg<P>::NBX;
     typedef DgtGeom<P, NBX, 3, DGT_NS_K1> G;
-    static int occ = 0;
-    if (!occ) {
-        FX_CUDA(cudaFuncSetAttribute(k_cgt_dir_apply_dot<P, NEU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
-        FX_CUDA(cudaFuncSetAttribute(k_cgt_dir_apply_dot<P, NEU>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
-        FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_cgt_dir_apply_dot<P, NEU>, G::NT, G::SMEM));
-        if (occ < 1) occ = 1;
-    }
+    const int occ = fx_func_occ(c, (const void*)k_cgt_dir_apply_dot<P, NEU>, G::NT, G::SMEM, true);
     fx_dgt_shape(c, g, NBX, c->num_sms * occ, &ct->t);
     ct->grid = ct->t.ntx * ct->t.nseg; ct->block = G::NT; ct->smem = G::SMEM;
     const int pitch = g->Nx * P, rows = g->Ny * P;
@@ -412,7 +411,7 @@ k_cg_persistent(const __grid_constant__ DgParams g, const double* __restrict__ c
                 const int j0 = seg * g.rows_per_seg;
                 int j1 = j0 + g.rows_per_seg;
                 if (j1 > g.Ny) j1 = g.Ny;
-                dg_warp_strip<P, true, true, false, false, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, nullptr);   // L2-resident grids: generic rows
+                dg_warp_strip<P, true, true, false, false, CgAcc, true>(g, chi, src, q, strip, j0, j1, &acc, &sh, nullptr);   // L2-resident grids: generic rows, coherent loads
             }
         }
         acc.flush(&sh);
@@ -465,8 +464,7 @@ static fx_status cg_run_persistent(FxCtx* c, const fx_grid* g, DgParams dp, cons
     int coop = 0, occ = 0;
     FX_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device));
     if (!coop) return FX_OK;
-    FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_cg_persistent<P>, 128, 0));
-    if (occ < 1) return FX_OK;
+    occ = fx_func_occ(c, (const void*)k_cg_persistent<P>, 128, 0);
     if (!c->cg_pdig) {
         if (cudaMalloc(&c->cg_pdig, 4 * FX_NDIG * sizeof(fx_u64) + 64) != cudaSuccess) { fx_set_error("persistent CG scratch: %s", cudaGetErrorString(cudaGetLastError())); return FX_ENOMEM; }
     }
@@ -525,12 +523,8 @@ static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int k1_warps_per_
 template <int P>
 static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, const CgTile& ct, int ag, int ab, int eg, int eb, const double* chi, double* phi,
                                   double* r, double* pbuf0, double* pbuf1, double* q, CgScal* sc, int first_index, int iters) {
-    static bool attr_done = false;
-    if (!attr_done) {
-        FX_CUDA(cudaFuncSetAttribute(k_cg_update<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, FX_STAGES * 4 * CG_U * 256 * 8));
-        FX_CUDA(cudaFuncSetAttribute(k_cg_update_tma<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, K2_STAGES * 4 * 2 * 256 * 8));
-        attr_done = true;
-    }
+    fx_func_occ(c, (const void*)k_cg_update<P>, 256, (size_t)FX_STAGES * 4 * CG_U * 256 * 8);
+    fx_func_occ(c, (const void*)k_cg_update_tma<P>, 256, (size_t)K2_STAGES * 4 * 2 * 256 * 8);
     const size_t k1_smem = dp.smr ? fx_dg_ring_bytes(P, ab / 32, true) : 0;
     // K2 fast path: 16-byte aligned vectors (the work vectors always are; phi is the caller's)
     const bool lin = aligned16(phi) && aligned16(r) && aligned16(pbuf0) && aligned16(pbuf1) && aligned16(q);
@@ -569,9 +563,8 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, const CgTile& ct
     return FX_OK;
 }
 
-extern "C" fx_status fx_cg_profile(int32_t enable) {
-    FxCtx* c = fx_ctx();
-    if (!c) return FX_ECUDA;
+extern "C" fx_status fx_cg_profile_ex(fx_ctx* c, int32_t enable) {
+    FX_ENTER(c, "fx_cg_profile");
     if (enable && !c->prof_ev) {
         c->prof_cap = 1024;
         c->prof_ev = (cudaEvent_t*)calloc((size_t)4 * c->prof_cap, sizeof(cudaEvent_t));
@@ -583,14 +576,21 @@ extern "C" fx_status fx_cg_profile(int32_t enable) {
     c->prof_stride = enable > 0 ? enable : 1;
     return FX_OK;
 }
+extern "C" fx_status fx_cg_profile(int32_t enable) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_cg_profile_ex(c, enable) : FX_ECUDA;
+}
 
-extern "C" fx_status fx_cg_last_profile(double* ms, int32_t* iters) {
-    FxCtx* c = fx_ctx();
-    if (!c) return FX_ECUDA;
+extern "C" fx_status fx_cg_last_profile_ex(fx_ctx* c, double* ms, int32_t* iters) {
+    FX_ENTER(c, "fx_cg_last_profile");
     if (!ms) { fx_set_error("fx_cg_last_profile: null pointer"); return FX_EINVAL; }
     for (int i = 0; i < 4; ++i) ms[i] = c->prof_ms[i];
     if (iters) *iters = c->prof_iters;
     return FX_OK;
+}
+extern "C" fx_status fx_cg_last_profile(double* ms, int32_t* iters) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_cg_last_profile_ex(c, ms, iters) : FX_ECUDA;
 }
 
 static fx_status cg_collect_profile(FxCtx* c, int iters_done) {
@@ -613,11 +613,10 @@ static fx_status cg_collect_profile(FxCtx* c, int iters_done) {
     return FX_OK;
 }
 
-extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const double* rho, double* phi, double tol, int32_t maxit,
+extern "C" fx_status fx_cg_solve_ex(fx_ctx* c, const fx_grid* g, const double* chi, const double* rho, double* phi, double tol, int32_t maxit,
                                  fx_cg_info* info) {
+    FX_ENTER(c, "fx_cg_solve");
     if (!fx_grid_ok(g) || !chi || !rho || !phi || maxit < 0 || !(tol >= 0)) { fx_set_error("fx_cg_solve: bad arguments"); return FX_EINVAL; }
-    FxCtx* c = fx_ctx();
-    if (!c) return FX_ECUDA;
     const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
     fx_status s = cg_workspace(c, n);
     if (s != FX_OK) return s;
@@ -625,21 +624,23 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
     const size_t bytes = (size_t)n * sizeof(double);
 
     // setup with the public primitives (lines before the loop)
-    if ((s = fx_dg_weights(g, W, V)) != FX_OK) return s;
-    if ((s = fx_pointwise_dot(-1.0, W, rho, 0.0, rhs, n)) != FX_OK) return s;
+    if ((s = fx_dg_weights_ex(c, g, W, V)) != FX_OK) return s;
+    if ((s = fx_pointwise_dot_ex(c, -1.0, W, rho, 0.0, rhs, n)) != FX_OK) return s;
     if ((s = fx_launch_apply(c, g, chi, phi, q, 0)) != FX_OK) return s;
     FX_CUDA(cudaMemcpyAsync(r, rhs, bytes, cudaMemcpyDeviceToDevice, c->stream));
-    if ((s = fx_axpby(-1.0, q, 1.0, r, n)) != FX_OK) return s;
-    if ((s = fx_pointwise_dot(1.0, V, rhs, 0.0, z, n)) != FX_OK) return s;
-    const double bz = fx_exdot(rhs, z, n);
+    if ((s = fx_axpby_ex(c, -1.0, q, 1.0, r, n)) != FX_OK) return s;
+    if ((s = fx_pointwise_dot_ex(c, 1.0, V, rhs, 0.0, z, n)) != FX_OK) return s;
+    double bz;
+    if ((s = fx_exdot_ex(c, rhs, z, n, &bz, nullptr)) != FX_OK) return s;
     if (bz == 0.0) {
         FX_CUDA(cudaMemsetAsync(phi, 0, bytes, c->stream));
         FX_CUDA(cudaStreamSynchronize(c->stream));
         if (info) { info->iterations = 0; info->status = FX_OK; info->rel_residual = 0.0; }
         return FX_OK;
     }
-    if ((s = fx_pointwise_dot(1.0, V, r, 0.0, z, n)) != FX_OK) return s;
-    double rz = fx_exdot(r, z, n);
+    if ((s = fx_pointwise_dot_ex(c, 1.0, V, r, 0.0, z, n)) != FX_OK) return s;
+    double rz;
+    if ((s = fx_exdot_ex(c, r, z, n, &rz, nullptr)) != FX_OK) return s;
     FX_CUDA(cudaMemcpyAsync(p, z, bytes, cudaMemcpyDeviceToDevice, c->stream));
     const double thresh = tol * sqrt(bz);
     int it = 0, status = FX_OK;
@@ -648,16 +649,18 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
         if (!c->cg_fused) {
             for (it = 1; it <= maxit; ++it) {
                 if ((s = fx_launch_apply(c, g, chi, p, q, 0)) != FX_OK) return s;
-                const double pq = fx_exdot(p, q, n);
+                double pq;
+                if ((s = fx_exdot_ex(c, p, q, n, &pq, nullptr)) != FX_OK) return s;
                 if (!(pq > 0.0) || !isfinite(pq)) { status = FX_EBREAKDOWN; break; }
                 const double alpha = rz / pq;
-                if ((s = fx_axpby(alpha, p, 1.0, phi, n)) != FX_OK) return s;
-                if ((s = fx_axpby(-alpha, q, 1.0, r, n)) != FX_OK) return s;
-                if ((s = fx_pointwise_dot(1.0, V, r, 0.0, z, n)) != FX_OK) return s;
-                const double rz_new = fx_exdot(r, z, n);
+                if ((s = fx_axpby_ex(c, alpha, p, 1.0, phi, n)) != FX_OK) return s;
+                if ((s = fx_axpby_ex(c, -alpha, q, 1.0, r, n)) != FX_OK) return s;
+                if ((s = fx_pointwise_dot_ex(c, 1.0, V, r, 0.0, z, n)) != FX_OK) return s;
+                double rz_new;
+                if ((s = fx_exdot_ex(c, r, z, n, &rz_new, nullptr)) != FX_OK) return s;
                 if (sqrt(rz_new) <= thresh) { rz = rz_new; status = FX_OK; break; }
                 const double beta = rz_new / rz;
-                if ((s = fx_axpby(1.0, z, beta, p, n)) != FX_OK) return s;
+                if ((s = fx_axpby_ex(c, 1.0, z, beta, p, n)) != FX_OK) return s;
                 rz = rz_new;
             }
             if (it > maxit) it = maxit;
@@ -677,12 +680,11 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
                 dp.smr = g->P <= 3 ? 1 : 0;
                 const int k1w = K1_THREADS(g->P) / 32;
                 const size_t sm = dp.smr ? fx_dg_ring_bytes(g->P, k1w, true) : 0;
-                if (sm) FX_CUDA(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-                FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occb, f, k1w * 32, sm));
-                occb *= k1w;
+                occb = fx_func_occ(c, f, k1w * 32, sm) * k1w;
             }
             cg_shapes(c, g, &dp, occb > 0 ? occb : 4, &ag, &ab, &eg, &eb);
-            static CgTile ct;                                    // (tensor maps are 64-byte aligned objects: kept out of the stack frame)
+            if (!fx_cg_tile(c)) { fx_set_error("out of host memory"); return FX_ENOMEM; }
+            CgTile& ct = *fx_cg_tile(c);
             ct.on = false;
             if (c->dg_path == 2 && fx_dgt_eligible(g, chi, r, p) && aligned16(p2)) {   // (measured: K1 on the warp-strip stencil is still the faster one)
                 const bool neu = fx_dg_has_neumann(&dp) != 0;
@@ -760,6 +762,11 @@ extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const doub
     if (info) { info->iterations = it; info->status = status; info->rel_residual = sqrt(rz) / sqrt(bz); }
     return (fx_status)status;
 }
+extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const double* rho, double* phi, double tol, int32_t maxit,
+                                 fx_cg_info* info) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_cg_solve_ex(c, g, chi, rho, phi, tol, maxit, info) : FX_ECUDA;
+}
 
 // ---- host-buffer entry points (bench.py "e2e") ------------------------------------------------------------------
 
@@ -784,11 +791,10 @@ static fx_status stage_alloc(FxCtx* c, int64_t cap) {
     return FX_OK;
 }
 
-extern "C" fx_status fx_cg_solve_host(const fx_grid* g, const double* chi, const double* rho, double* phi, double tol,
+extern "C" fx_status fx_cg_solve_host_ex(fx_ctx* c, const fx_grid* g, const double* chi, const double* rho, double* phi, double tol,
                                       int32_t maxit, fx_cg_info* info) {
+    FX_ENTER(c, "fx_cg_solve_host");
     if (!fx_grid_ok(g) || !chi || !rho || !phi) { fx_set_error("fx_cg_solve_host: bad arguments"); return FX_EINVAL; }
-    FxCtx* c = fx_ctx();
-    if (!c) return FX_ECUDA;
     const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
     fx_status s = stage_alloc(c, n);
     if (s != FX_OK) return s;
@@ -796,21 +802,25 @@ extern "C" fx_status fx_cg_solve_host(const fx_grid* g, const double* chi, const
     FX_CUDA(cudaMemcpyAsync(c->stage[0], chi, bytes, cudaMemcpyHostToDevice, c->stream));
     FX_CUDA(cudaMemcpyAsync(c->stage[1], rho, bytes, cudaMemcpyHostToDevice, c->stream));
     FX_CUDA(cudaMemcpyAsync(c->stage[2], phi, bytes, cudaMemcpyHostToDevice, c->stream));
-    s = fx_cg_solve(g, c->stage[0], c->stage[1], c->stage[2], tol, maxit, info);
+    s = fx_cg_solve_ex(c, g, c->stage[0], c->stage[1], c->stage[2], tol, maxit, info);
     if (s < 0) return s;
     FX_CUDA(cudaMemcpyAsync(phi, c->stage[2], bytes, cudaMemcpyDeviceToHost, c->stream));
     FX_CUDA(cudaStreamSynchronize(c->stream));
     return s;
 }
+extern "C" fx_status fx_cg_solve_host(const fx_grid* g, const double* chi, const double* rho, double* phi, double tol,
+                                      int32_t maxit, fx_cg_info* info) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_cg_solve_host_ex(c, g, chi, rho, phi, tol, maxit, info) : FX_ECUDA;
+}
 
 // double-buffered: the copy of chunk i+1 overlaps the accumulation of chunk i
-extern "C" double fx_exdot_host(const double* x, const double* y, int64_t n) {
-    if (n < 0 || (n > 0 && (!x || !y))) { fx_set_error("fx_exdot_host: bad arguments"); return NAN; }
-    fx_set_error("%s", "");
-    FxCtx* c = fx_ctx();
-    if (!c) return NAN;
+extern "C" fx_status fx_exdot_host_ex(fx_ctx* c, const double* x, const double* y, int64_t n, double* result_host) {
+    FX_ENTER(c, "fx_exdot_host");
+    if (n < 0 || (n > 0 && (!x || !y)) || !result_host) { fx_set_error("fx_exdot_host: bad arguments"); return FX_EINVAL; }
     const int64_t CH = (int64_t)1 << 23;                       // 64 MB per array and chunk
-    if (stage_alloc(c, n < CH ? (n > 0 ? n : 1) : CH) != FX_OK) return NAN;
+    fx_status s = stage_alloc(c, n < CH ? (n > 0 ? n : 1) : CH);
+    if (s != FX_OK) return s;
     const int64_t cap = c->stage_cap < CH ? c->stage_cap : CH;
     const int64_t nch = n == 0 ? 1 : (n + cap - 1) / cap;
     cudaEventRecord(c->ev_comp[0], c->stream);
@@ -825,10 +835,15 @@ extern "C" double fx_exdot_host(const double* x, const double* y, int64_t n) {
         }
         cudaEventRecord(c->ev_copy[b], c->copy_stream);
         cudaStreamWaitEvent(c->stream, c->ev_copy[b], 0);
-        if (fx_launch_exdot_part(c, c->stage[2 * b], c->stage[2 * b + 1], m, i == 0, i == nch - 1, c->result_dev) != FX_OK) return NAN;
+        if ((s = fx_launch_exdot_part(c, c->stage[2 * b], c->stage[2 * b + 1], m, i == 0, i == nch - 1, c->result_dev)) != FX_OK) return s;
         cudaEventRecord(c->ev_comp[b], c->stream);
     }
-    if (cudaMemcpyAsync(c->result_pinned, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
-        cudaStreamSynchronize(c->stream) != cudaSuccess) { fx_cuda_fail(cudaGetLastError(), "fx_exdot_host"); return NAN; }
-    return c->result_pinned[0];
+    return fx_result_to_host(c, result_host);
+}
+extern "C" double fx_exdot_host(const double* x, const double* y, int64_t n) {
+    fx_set_error("%s", "");
+    FxCtx* c = fx_default_ctx();
+    if (!c) return NAN;
+    double v = NAN;
+    return fx_exdot_host_ex(c, x, y, n, &v) == FX_OK ? v : NAN;
 }

@@ -206,16 +206,20 @@ fx_status fx_launch_derivative(FxCtx* c, const fx_grid* g, int dir, int flux, do
     return FX_OK;
 }
 
-extern "C" fx_status fx_dg_derivative(const fx_grid* g, int32_t direction, int32_t flux, double alpha, const double* x, double beta,
+extern "C" fx_status fx_dg_derivative_ex(fx_ctx* c, const fx_grid* g, int32_t direction, int32_t flux, double alpha, const double* x, double beta,
                                       double* y) {
+    FX_ENTER(c, "fx_dg_derivative");
     if (!fx_grid_ok(g) || !fx_grid_deriv_ok(g) || !x || !y || direction < 0 || direction > 1 || flux < 0 || flux > 2) {
         fx_set_error("fx_dg_derivative: bad grid, direction, flux or null pointer"); return FX_EINVAL;
     }
     const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
     if (x < y + n && y < x + n) { fx_set_error("fx_dg_derivative: y overlaps x"); return FX_EINVAL; }
-    FxCtx* c = fx_ctx();
-    if (!c) return FX_ECUDA;
     return fx_launch_derivative(c, g, direction, flux, alpha, x, beta, y);
+}
+extern "C" fx_status fx_dg_derivative(const fx_grid* g, int32_t direction, int32_t flux, double alpha, const double* x, double beta,
+                                      double* y) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_dg_derivative_ex(c, g, direction, flux, alpha, x, beta, y) : FX_ECUDA;
 }
 
 extern "C" fx_status fx_dg_dtables(int32_t P, int32_t flux, double* out) {
@@ -244,12 +248,11 @@ __global__ void __launch_bounds__(512) k_arakawa_products(double a, double b, co
     }
 }
 
-extern "C" fx_status fx_arakawa(const fx_grid* g, const double* f, const double* gg, double* out) {
+extern "C" fx_status fx_arakawa_ex(fx_ctx* c, const fx_grid* g, const double* f, const double* gg, double* out) {
+    FX_ENTER(c, "fx_arakawa");
     if (!fx_grid_ok(g) || !fx_grid_deriv_ok(g) || !f || !gg || !out) { fx_set_error("fx_arakawa: bad grid (PER / DIR only) or null pointer"); return FX_EINVAL; }
     const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
     if ((f < out + n && out < f + n) || (gg < out + n && out < gg + n)) { fx_set_error("fx_arakawa: out overlaps an input"); return FX_EINVAL; }
-    FxCtx* c = fx_ctx();
-    if (!c) return FX_ECUDA;
     if (c->ara_cap < n) {
         if (c->ara_vec) { cudaStreamSynchronize(c->stream); cudaFree(c->ara_vec); c->ara_vec = nullptr; c->ara_cap = 0; }
         if (cudaMalloc(&c->ara_vec, (size_t)6 * n * sizeof(double)) != cudaSuccess) {
@@ -275,4 +278,8 @@ extern "C" fx_status fx_arakawa(const fx_grid* g, const double* f, const double*
     }
     if ((s = fx_launch_derivative(c, g, 0, 2, 1.0, h1, 1.0, out)) != FX_OK) return s;                   // += Dx(...)
     return fx_launch_derivative(c, g, 1, 2, 1.0, h2, 1.0, out);                                         // += Dy(...)
+}
+extern "C" fx_status fx_arakawa(const fx_grid* g, const double* f, const double* gg, double* out) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_arakawa_ex(c, g, f, gg, out) : FX_ECUDA;
 }

@@ -44,14 +44,17 @@ struct DgCell { double v[P][P]; };     // [l][k]: row l (y node), column k (x no
 
 // load one cell's P x P values (always from valid memory: ghost lanes read their wrapped cell and have their traces
 // forced to +0.0 afterwards, which is all their neighbours ever see)
-template <int P>
-__device__ __forceinline__ void dg_load(DgCell<P>& c, const double* __restrict__ a, long long pitch, int col0, int j,
+// COH: the array is rewritten by this very kernel (the persistent CG loop, between grid syncs): the non-coherent path
+// (ld.global.nc) is only defined for data that stays read-only for the whole kernel, so such arrays are read with
+// ld.global.cg (L2, where the grid sync made the new values visible) and are not prefetched into L1.
+template <int P, bool COH = false>
+__device__ __forceinline__ void dg_load(DgCell<P>& c, const double* a, long long pitch, int col0, int j,
                                         bool) {
     const double* q = a + (long long)j * P * pitch + col0;
 #pragma unroll
     for (int l = 0; l < P; ++l)
 #pragma unroll
-        for (int k = 0; k < P; ++k) c.v[l][k] = __ldg(q + l * pitch + k);
+        for (int k = 0; k < P; ++k) c.v[l][k] = COH ? __ldcg(q + l * pitch + k) : __ldg(q + l * pitch + k);
 }
 
 // L1 prefetch of one cell (the first element of each of its P rows; a lane's P doubles span at most two 32-byte
@@ -74,13 +77,13 @@ struct DgSrc {
     bool upd;
 };
 
-template <int P, bool DIRF>
+template <int P, bool DIRF, bool COH = false>
 __device__ __forceinline__ void dg_load_u(DgCell<P>& c, const DgParams& g, const DgSrc& s, long long pitch, int col0, int j) {
-    dg_load<P>(c, s.x, pitch, col0, j, false);
+    dg_load<P, COH>(c, s.x, pitch, col0, j, false);
     if (DIRF) {
         if (s.upd) {
             DgCell<P> rr;
-            dg_load<P>(rr, s.r, pitch, col0, j, false);
+            dg_load<P, COH>(rr, s.r, pitch, col0, j, false);
 #pragma unroll
             for (int l = 0; l < P; ++l)
 #pragma unroll
@@ -241,11 +244,11 @@ __device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc
 // One warp: strip `strip` of 30 cells, cell rows [j0, j1).  FUSE: feed (x, y) pairs of the produced cells into the
 // exact-dot accumulator `acc` (the CG's p.Sp).
 // NEU: the grid has a Neumann wall (a separate instantiation, so that the periodic / Dirichlet code is untouched by it).
-template <int P, bool FUSE, bool DIRF, bool SMR, bool NEU, class ACC>
+template <int P, bool FUSE, bool DIRF, bool SMR, bool NEU, class ACC, bool COH = false>
 __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* __restrict__ chi, const DgSrc& src,
                                               double* __restrict__ y, int strip, int j0, int j1, ACC* acc, ExShared* sh,
                                               double* ring) {
-    const double* __restrict__ x = src.x;
+    const double* x = src.x;
     const int lane = threadIdx.x & 31;
     const int Nx = g.Nx, Ny = g.Ny;
     const long long pitch = (long long)Nx * P;
@@ -267,11 +270,11 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
     double tLy[P], tRyp[P], tByp[P];                               // own bottom trace; previous cell's top / flux trace
 
     // ---- prologue: state of cell row j0-1 ------------------------------------------------------------------
-    dg_load_u<P, DIRF>(uc, g, src, pitch, col0, j0);
+    dg_load_u<P, DIRF, COH>(uc, g, src, pitch, col0, j0);
     dg_load<P>(cc, chi, pitch, col0, j0, xghost);
     // L1 prefetch, FX_PFD steps ahead: row jr of the input vector (needed as the upper neighbour at step jr-1) and of chi
     auto pf_x = [&](int jr) {
-        if (xghost || jr > j1) return;
+        if (COH || xghost || jr > j1) return;
         if (jr >= Ny) { if (diry) return; jr -= Ny; }
         dg_prefetch<P>(x, pitch, col0, jr); if (DIRF) dg_prefetch<P>(src.r, pitch, col0, jr);
     };
@@ -297,7 +300,7 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
     } else {
         const int jp = (j0 == 0) ? Ny - 1 : j0 - 1;
         DgCell<P> up, cp;
-        dg_load_u<P, DIRF>(up, g, src, pitch, col0, jp);
+        dg_load_u<P, DIRF, COH>(up, g, src, pitch, col0, jp);
         dg_load<P>(cp, chi, pitch, col0, jp, xghost);
         double dummy[P][P];
 #pragma unroll
@@ -333,8 +336,8 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
             if (j > j0) { if (!DIRF) smr_read_u<P, DIRF>(uc, g, src, ring, sq); smr_read<P>(cc, ring, 3 + (sq & 1)); }
             smr_read_u<P, DIRF>(un, g, src, ring, sq + 1);
         } else {
-            if (j > j0) { if (!DIRF) dg_load_u<P, DIRF>(uc, g, src, pitch, col0, j); dg_load<P>(cc, chi, pitch, col0, j, xghost); }
-            dg_load_u<P, DIRF>(un, g, src, pitch, col0, jn);
+            if (j > j0) { if (!DIRF) dg_load_u<P, DIRF, COH>(uc, g, src, pitch, col0, j); dg_load<P>(cc, chi, pitch, col0, j, xghost); }
+            dg_load_u<P, DIRF, COH>(un, g, src, pitch, col0, jn);
             pf_x(j + 1 + FX_PFD); pf_c(j + FX_PFD);                // rows of the steps ahead
         }
 

@@ -14,9 +14,16 @@
 
 #define FX_NUM_SMS_DEFAULT 148
 
-struct FxCtx {
+struct FxFuncInfo { const void* f; int block; size_t smem; int occ; };
+
+// The opaque fx_ctx of include/fx.h.  One context = one device, one stream, its own scratch: exact-dot digits and ticket, result
+// slots, CG work vectors and scalars, staging buffers, launch-shape overrides, per-kernel attribute / occupancy cache.
+// Contexts share nothing mutable, so different contexts may be used from different threads and streams at the same time;
+// ONE context must be used by one thread at a time (its kernels are stream-ordered and share the digit scratch).
+struct fx_ctx {
     bool ready;
     int device, num_sms;
+    FxFuncInfo fcache[128]; int nfcache;   // kernels whose shared-memory attribute is set on this device, with their occupancy
     cudaStream_t stream;
     ExGlobal ex;                 // device scratch of the exact dot
     double* result_dev;          // [8] scratch doubles (dot results of the synchronous calls)
@@ -32,6 +39,7 @@ struct FxCtx {
     void* cg_scal_pinned;
     double* ara_vec; int64_t ara_cap;  // six work vectors of fx_arakawa
     void* cg_pdig;                     // digit buffers of the persistent CG kernel
+    void* cg_tile;                     // CgTile (fx_cg.cu): tensor maps and geometry of the tile K1 of the running solve
     cudaEvent_t cg_ev[2];
     // host staging for the *_host entry points
     double* stage[4]; int64_t stage_cap;
@@ -45,7 +53,22 @@ struct FxCtx {
     double prof_ms[4];
 };
 
-FxCtx* fx_ctx();                               // lazily initialised; NULL (and last error set) on failure
+typedef struct fx_ctx FxCtx;
+FxCtx* fx_default_ctx();                       // the calling thread's current device's default context, created on first use; NULL (and last error set) on failure
+// resident CTAs per SM of kernel `f` at (block, smem) on the context's device; the first call per kernel also raises its
+// dynamic shared-memory limit (and, with carveout, asks for the largest shared-memory carve-out)
+int fx_func_occ(FxCtx* c, const void* f, int block, size_t smem, bool carveout = false);
+// makes the context's device current for the scope of an _ex call (restores the caller's device afterwards)
+struct FxDeviceGuard {
+    int prev; bool switched;
+    explicit FxDeviceGuard(const FxCtx* c) : prev(-1), switched(false) {
+        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~FxDeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+#define FX_ENTER(c, name)                                                        \
+    if (!(c) || !(c)->ready) { fx_set_error("%s: null or destroyed context", name); return FX_EINVAL; } \
+    FxDeviceGuard fx_guard_(c)
 void fx_set_error(const char* fmt, ...);
 fx_status fx_cuda_fail(cudaError_t e, const char* what);
 
@@ -58,7 +81,6 @@ fx_status fx_cuda_fail(cudaError_t e, const char* what);
 static inline bool aligned16(const void* p) { return (((uintptr_t)p) & 15) == 0; }
 int fx_grid_ok(const fx_grid* g);
 int fx_grid_deriv_ok(const fx_grid* g);          // PER / DIR only: stand-alone derivatives and the bracket
-struct DgParams;
 int fx_dg_has_neumann(const DgParams* p);
 int fx_dg_neu_variant(const DgParams* p, int P);
 fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* out, double* vol4_out);
@@ -67,6 +89,7 @@ fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* out, double*
 fx_status fx_launch_exdot(FxCtx* c, const double* x, const double* y, int64_t n, double* result_dev);
 fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64_t m, int first, int last, double* result_dev, int mode = 0);   // mode 1: exact sum of two halves, 2: binary32 pairs
 fx_status fx_launch_exsum(FxCtx* c, const double* x, int64_t n, double* result_dev);
+fx_status fx_result_to_host(FxCtx* c, double* result_host);
 size_t fx_dg_ring_bytes(int P, int warps, bool dirf);
 void fx_dg_shape(FxCtx* c, const fx_grid* g, DgParams* p, int warps_per_sm, int* grid, int* block, int max_wpb = 4);
 // CTA-tile stencil kernels (fx_dgt.cuh): eligibility (TMA's global-memory rules), tensor maps, launch geometry

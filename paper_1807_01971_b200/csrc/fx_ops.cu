@@ -183,20 +183,11 @@ fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64
     int bd = c->launch[0][1] ? c->launch[0][1] : 256;
     if (bd > 256) bd = 256;                     // compiled for <= 256 threads per CTA
     const size_t smem = (size_t)EX_STAGES * 2 * EX_U * bd * sizeof(double);
-    static bool attr_done = false;
-    static int occ_cache[9] = {0};              // resident CTAs per SM by block size / 32
-    if (!attr_done) {
-        const int sm = EX_STAGES * 2 * EX_U * 256 * 8;
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
-        FX_CUDA(cudaFuncSetAttribute(k_exdot<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm));
-        attr_done = true;
-    }
-    int& occ = occ_cache[bd / 32];
-    if (!occ && (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_exdot<true, 0>, bd, smem) != cudaSuccess || occ < 1)) occ = 1;
+    // (the six instantiations share one shared-memory layout: the dynamic limit is raised for the one that is launched)
+    const void* kf = mode == 1 ? (vec ? (const void*)k_exdot<true, 1> : (const void*)k_exdot<false, 1>)
+                   : mode == 2 ? (vec ? (const void*)k_exdot<true, 2> : (const void*)k_exdot<false, 2>)
+                               : (vec ? (const void*)k_exdot<true, 0> : (const void*)k_exdot<false, 0>);
+    const int occ = fx_func_occ(c, kf, bd, smem);
     const long long tile = (long long)bd * EX_U;
     long long grid = (m + tile - 1) / tile;
     const long long gmax = (long long)c->num_sms * occ;             // one resident wave: every CTA pays one flush + merge
@@ -299,14 +290,8 @@ template <int NA>
 static fx_status launch_exdotn(FxCtx* c, const double* a0, const double* a1, const double* a2, int64_t n, double* result_dev) {
     const int bd = 256;
     const size_t smem = (size_t)EX_STAGES * NA * EX_U * bd * sizeof(double);
-    static bool attr_done = false;
-    static int occ = 0;
-    if (!attr_done) {
-        FX_CUDA(cudaFuncSetAttribute(k_exdotn<NA, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        FX_CUDA(cudaFuncSetAttribute(k_exdotn<NA, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_exdotn<NA, true>, bd, smem) != cudaSuccess || occ < 1) occ = 1;
-        attr_done = true;
-    }
+    const int occ = fx_func_occ(c, (const void*)k_exdotn<NA, true>, bd, smem);
+    fx_func_occ(c, (const void*)k_exdotn<NA, false>, bd, smem);
     const int64_t CHUNK = (int64_t)1 << 28;
     int64_t done = 0;
     do {
@@ -408,21 +393,14 @@ __global__ void __launch_bounds__(256, 2) k_exdot_f32(const float* __restrict__ 
     ex_block_finish(&sh, g, first, last, result);
 }
 
-extern "C" double fx_exdot_f32(const float* x, const float* y, int64_t n) {
-    if (n < 0 || (n > 0 && (!x || !y))) { fx_set_error("fx_exdot_f32: bad arguments"); return NAN; }
-    fx_set_error("%s", "");
-    FxCtx* c = fx_ctx();
-    if (!c) return NAN;
+// result_host: host double (synchronises)
+extern "C" fx_status fx_exdot_f32_ex(fx_ctx* c, const float* x, const float* y, int64_t n, double* result_host) {
+    FX_ENTER(c, "fx_exdot_f32");
+    if (n < 0 || (n > 0 && (!x || !y)) || !result_host) { fx_set_error("fx_exdot_f32: bad arguments"); return FX_EINVAL; }
     const int bd = 256;
     const size_t smem = (size_t)EX_STAGES * 2 * EXF_U * bd * sizeof(float);
-    static int occ = 0;
-    if (!occ) {
-        if (cudaFuncSetAttribute(k_exdot_f32<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-            cudaFuncSetAttribute(k_exdot_f32<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
-            fx_cuda_fail(cudaGetLastError(), "k_exdot_f32 attributes"); return NAN;
-        }
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_exdot_f32<true>, bd, smem) != cudaSuccess || occ < 1) occ = 1;
-    }
+    const int occ = fx_func_occ(c, (const void*)k_exdot_f32<true>, bd, smem);
+    fx_func_occ(c, (const void*)k_exdot_f32<false>, bd, smem);
     const bool vec = aligned16(x) && aligned16(y);
     const int64_t CHUNK = (int64_t)1 << 28;
     int64_t done = 0;
@@ -433,7 +411,8 @@ extern "C" double fx_exdot_f32(const float* x, const float* y, int64_t n) {
         while (n - done >= 2) {
             int64_t h = (n - done) / 2;
             if (h > SLOTS) h = SLOTS;
-            if (fx_launch_exdot_part(c, (const double*)(x + done), (const double*)(y + done), h, done == 0, done + 2 * h == n, c->result_dev, 2) != FX_OK) return NAN;
+            const fx_status sp = fx_launch_exdot_part(c, (const double*)(x + done), (const double*)(y + done), h, done == 0, done + 2 * h == n, c->result_dev, 2);
+            if (sp != FX_OK) return sp;
             done += 2 * h;
         }
     }
@@ -447,28 +426,35 @@ extern "C" double fx_exdot_f32(const float* x, const float* y, int64_t n) {
         if (tailvec) k_exdot_f32<true><<<(int)grid, bd, smem, c->stream>>>(x + done, y + done, m, c->ex, done == 0, done + m == n, c->result_dev);
         else k_exdot_f32<false><<<(int)grid, bd, smem, c->stream>>>(x + done, y + done, m, c->ex, done == 0, done + m == n, c->result_dev);
         c->launches++;
-        if (cudaGetLastError() != cudaSuccess) { fx_cuda_fail(cudaGetLastError(), "k_exdot_f32"); return NAN; }
+        FX_CUDA(cudaGetLastError());
         done += m;
     } while (done < n);
-    if (cudaMemcpyAsync(c->result_pinned, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
-        cudaStreamSynchronize(c->stream) != cudaSuccess) { fx_cuda_fail(cudaGetLastError(), "fx_exdot_f32 result copy"); return NAN; }
-    return c->result_pinned[0];
+    return fx_result_to_host(c, result_host);
+}
+// the plain-named reductions return the value; NaN with a non-empty fx_last_error() is a failure, with an empty one a genuine NaN
+#define FX_PLAIN_VALUE(call)                        \
+    fx_set_error("%s", "");                         \
+    FxCtx* c = fx_default_ctx();                    \
+    if (!c) return NAN;                             \
+    double v = NAN;                                 \
+    return (call) == FX_OK ? v : NAN;
+extern "C" double fx_exdot_f32(const float* x, const float* y, int64_t n) { FX_PLAIN_VALUE(fx_exdot_f32_ex(c, x, y, n, &v)) }
+
+// the double a finished reduction left in the context's device slot -> host (synchronises)
+fx_status fx_result_to_host(FxCtx* c, double* result_host) {
+    FX_CUDA(cudaMemcpyAsync(c->result_pinned, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    FX_CUDA(cudaStreamSynchronize(c->stream));
+    *result_host = c->result_pinned[0];
+    return FX_OK;
 }
 
-static double exdotn_sync(FxCtx* c, fx_status s) {
-    if (s != FX_OK) return NAN;
-    if (cudaMemcpyAsync(c->result_pinned, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
-        cudaStreamSynchronize(c->stream) != cudaSuccess) { fx_cuda_fail(cudaGetLastError(), "exact reduction result copy"); return NAN; }
-    return c->result_pinned[0];
+extern "C" fx_status fx_exdot3_ex(fx_ctx* c, const double* x, const double* w, const double* y, int64_t n, double* result_host) {
+    FX_ENTER(c, "fx_exdot3");
+    if (n < 0 || (n > 0 && (!x || !w || !y)) || !result_host) { fx_set_error("fx_exdot3: bad arguments"); return FX_EINVAL; }
+    const fx_status s = launch_exdotn<3>(c, x, w, y, n, c->result_dev);
+    return s != FX_OK ? s : fx_result_to_host(c, result_host);
 }
-
-extern "C" double fx_exdot3(const double* x, const double* w, const double* y, int64_t n) {
-    if (n < 0 || (n > 0 && (!x || !w || !y))) { fx_set_error("fx_exdot3: bad arguments"); return NAN; }
-    fx_set_error("%s", "");
-    FxCtx* c = fx_ctx();
-    if (!c) return NAN;
-    return exdotn_sync(c, launch_exdotn<3>(c, x, w, y, n, c->result_dev));
-}
+extern "C" double fx_exdot3(const double* x, const double* w, const double* y, int64_t n) { FX_PLAIN_VALUE(fx_exdot3_ex(c, x, w, y, n, &v)) }
 
 // Exact sum: long vectors go through the dot kernel's ring as two halves (x[0,h) and x[h,2h), h even so that both keep
 // the alignment of x), 2^27 elements per half and launch; what is left (<= 3 elements, or a short vector) through the
@@ -495,13 +481,13 @@ fx_status fx_launch_exsum(FxCtx* c, const double* x, int64_t n, double* result_d
     return FX_OK;
 }
 
-extern "C" double fx_exsum(const double* x, int64_t n) {
-    if (n < 0 || (n > 0 && !x)) { fx_set_error("fx_exsum: bad arguments"); return NAN; }
-    fx_set_error("%s", "");
-    FxCtx* c = fx_ctx();
-    if (!c) return NAN;
-    return exdotn_sync(c, fx_launch_exsum(c, x, n, c->result_dev));
+extern "C" fx_status fx_exsum_ex(fx_ctx* c, const double* x, int64_t n, double* result_host) {
+    FX_ENTER(c, "fx_exsum");
+    if (n < 0 || (n > 0 && !x) || !result_host) { fx_set_error("fx_exsum: bad arguments"); return FX_EINVAL; }
+    const fx_status s = fx_launch_exsum(c, x, n, c->result_dev);
+    return s != FX_OK ? s : fx_result_to_host(c, result_host);
 }
+extern "C" double fx_exsum(const double* x, int64_t n) { FX_PLAIN_VALUE(fx_exsum_ex(c, x, n, &v)) }
 
 fx_status fx_launch_exdot(FxCtx* c, const double* x, const double* y, int64_t n, double* result_dev) {
     const int64_t CHUNK = (int64_t)1 << 28;
@@ -515,32 +501,31 @@ fx_status fx_launch_exdot(FxCtx* c, const double* x, const double* y, int64_t n,
     return FX_OK;
 }
 
-extern "C" fx_status fx_exdot_async(const double* x, const double* y, int64_t n, double* result_dev) {
+extern "C" fx_status fx_exdot_async_ex(fx_ctx* c, const double* x, const double* y, int64_t n, double* result_dev) {
+    FX_ENTER(c, "fx_exdot_async");
     if (n < 0 || (n > 0 && (!x || !y)) || !result_dev) { fx_set_error("fx_exdot_async: bad arguments"); return FX_EINVAL; }
-    FxCtx* c = fx_ctx();
-    if (!c) return FX_ECUDA;
     return fx_launch_exdot(c, x, y, n, result_dev);
 }
-
-extern "C" double fx_exdot(const double* x, const double* y, int64_t n) {
-    if (n < 0 || (n > 0 && (!x || !y))) { fx_set_error("fx_exdot: bad arguments"); return NAN; }
-    fx_set_error("%s", "");                 // a NaN result with an empty fx_last_error() is a genuine NaN
-    FxCtx* c = fx_ctx();
-    if (!c) return NAN;
-    if (fx_launch_exdot(c, x, y, n, c->result_dev) != FX_OK) return NAN;
-    if (cudaMemcpyAsync(c->result_pinned, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
-        cudaStreamSynchronize(c->stream) != cudaSuccess) {
-        fx_cuda_fail(cudaGetLastError(), "fx_exdot result copy");
-        return NAN;
-    }
-    return c->result_pinned[0];
+extern "C" fx_status fx_exdot_async(const double* x, const double* y, int64_t n, double* result_dev) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_exdot_async_ex(c, x, y, n, result_dev) : FX_ECUDA;
 }
 
-extern "C" fx_status fx_exdot_digits(const double* x, const double* y, int64_t n, uint64_t* limbs_host, int32_t* flags_host,
+// result_host (host double, synchronises) and/or result_dev (device double, stream-ordered); at least one
+extern "C" fx_status fx_exdot_ex(fx_ctx* c, const double* x, const double* y, int64_t n, double* result_host, double* result_dev) {
+    FX_ENTER(c, "fx_exdot");
+    if (n < 0 || (n > 0 && (!x || !y)) || (!result_host && !result_dev)) { fx_set_error("fx_exdot: bad arguments"); return FX_EINVAL; }
+    fx_status s = fx_launch_exdot(c, x, y, n, c->result_dev);
+    if (s != FX_OK) return s;
+    if (result_dev) FX_CUDA(cudaMemcpyAsync(result_dev, c->result_dev, sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    return result_host ? fx_result_to_host(c, result_host) : FX_OK;
+}
+extern "C" double fx_exdot(const double* x, const double* y, int64_t n) { FX_PLAIN_VALUE(fx_exdot_ex(c, x, y, n, &v, nullptr)) }
+
+extern "C" fx_status fx_exdot_digits_ex(fx_ctx* c, const double* x, const double* y, int64_t n, uint64_t* limbs_host, int32_t* flags_host,
                                      double* result_host) {
+    FX_ENTER(c, "fx_exdot_digits");
     if (n < 0 || (n > 0 && (!x || !y)) || !limbs_host) { fx_set_error("fx_exdot_digits: bad arguments"); return FX_EINVAL; }
-    FxCtx* c = fx_ctx();
-    if (!c) return FX_ECUDA;
     // flags are cleared by the finaliser after rounding; read them through the result instead: launch, then copy
     fx_status s = fx_launch_exdot(c, x, y, n, c->result_dev);
     if (s != FX_OK) return s;
@@ -551,6 +536,11 @@ extern "C" fx_status fx_exdot_digits(const double* x, const double* y, int64_t n
     if (flags_host) { flags_host[0] = (fl[1] & FX_FLAG_NAN) != 0; flags_host[1] = (fl[1] & FX_FLAG_PINF) != 0; flags_host[2] = (fl[1] & FX_FLAG_NINF) != 0; }
     if (result_host) FX_CUDA(cudaMemcpy(result_host, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost));
     return FX_OK;
+}
+extern "C" fx_status fx_exdot_digits(const double* x, const double* y, int64_t n, uint64_t* limbs_host, int32_t* flags_host,
+                                     double* result_host) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_exdot_digits_ex(c, x, y, n, limbs_host, flags_host, result_host) : FX_ECUDA;
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -667,13 +657,7 @@ template <int P, bool NEU>
 static fx_status launch_dgt_apply(FxCtx* c, const fx_grid* g, const DgParams& p, const double* chi, const double* x, double* y) {
     constexpr int NBX = DgtCfg<P>::NBX;
     typedef DgtGeom<P, NBX, 2> G;
-    static int occ = 0;
-    if (!occ) {
-        FX_CUDA(cudaFuncSetAttribute(k_dgt_apply<P, NEU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
-        FX_CUDA(cudaFuncSetAttribute(k_dgt_apply<P, NEU>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
-        FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_dgt_apply<P, NEU>, G::NT, G::SMEM));
-        if (occ < 1) occ = 1;
-    }
+    const int occ = fx_func_occ(c, (const void*)k_dgt_apply<P, NEU>, G::NT, G::SMEM, true);
     DgtTile t;
     fx_dgt_shape(c, g, NBX, c->num_sms * occ, &t);
     const int pitch = g->Nx * P, rows = g->Ny * P;
@@ -766,18 +750,15 @@ fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const d
     fx_status s = fx_make_dg_params(g, normed, &p, nullptr);
     if (s != FX_OK) return s;
     const int neu = fx_dg_neu_variant(&p, g->P);
-    static int occs[2][FX_PMAX + 1] = {{0}, {0}};                // resident warps per SM of k_dg_apply<P, NEU> (128-thread CTAs)
-    int* occ = occs[neu];
-    if (!occ[g->P]) {
-        int nb = 0;
+    int occw;                                                    // resident warps per SM of k_dg_apply<P, NEU>
+    {
         const void* f;
         if (neu) f = g->P == 1 ? (const void*)k_dg_apply<1, true> : g->P == 2 ? (const void*)k_dg_apply<2, true> : g->P == 3 ? (const void*)k_dg_apply<3, true>
                    : g->P == 4 ? (const void*)k_dg_apply<4, true> : (const void*)k_dg_apply<5, true>;
         else f = g->P == 1 ? (const void*)k_dg_apply<1, false> : g->P == 2 ? (const void*)k_dg_apply<2, false> : g->P == 3 ? (const void*)k_dg_apply<3, false>
                : g->P == 4 ? (const void*)k_dg_apply<4, false> : (const void*)k_dg_apply<5, false>;
         const int w = g->P == 3 ? FX_AP_W : 4;
-        FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, f, w * 32, 0));
-        occ[g->P] = nb > 0 ? nb * w : 4;
+        occw = fx_func_occ(c, f, w * 32, 0) * w;
     }
     if (c->dg_path != 1 && fx_dgt_eligible(g, chi, x, y)) {
 #define FX_TAPPLY(PP) \
@@ -798,7 +779,7 @@ fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const d
     }
     p.smr = 0;            // measured: the stand-alone apply is 2 % faster on the L1-prefetch path, the fused K1 6 % faster with the ring
     int grid, block;
-    fx_dg_shape(c, g, &p, occ[g->P], &grid, &block, g->P == 3 ? FX_AP_W : 4);
+    fx_dg_shape(c, g, &p, occw, &grid, &block, g->P == 3 ? FX_AP_W : 4);
     const size_t smem = p.smr ? fx_dg_ring_bytes(g->P, block / 32, false) : 0;
 #define FX_APPLY(PP) \
     if (neu) k_dg_apply<PP, true><<<grid, block, smem, c->stream>>>(p, chi, x, y); \
@@ -817,17 +798,24 @@ fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const d
     return FX_OK;
 }
 
-static fx_status apply_checked(const fx_grid* g, const double* chi, const double* x, double* y, int normed) {
+static fx_status apply_checked(FxCtx* c, const fx_grid* g, const double* chi, const double* x, double* y, int normed) {
+    FX_ENTER(c, "fx_dg_elliptic_apply");
     if (!fx_grid_ok(g) || !chi || !x || !y) { fx_set_error("fx_dg_elliptic_apply: bad grid or null pointer"); return FX_EINVAL; }
     const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
     const double *ye = y + n;
     if ((x < ye && y < x + n) || (chi < ye && y < chi + n)) { fx_set_error("fx_dg_elliptic_apply: y overlaps an input"); return FX_EINVAL; }
-    FxCtx* c = fx_ctx();
-    if (!c) return FX_ECUDA;
     return fx_launch_apply(c, g, chi, x, y, normed);
 }
-extern "C" fx_status fx_dg_elliptic_apply(const fx_grid* g, const double* chi, const double* x, double* y) { return apply_checked(g, chi, x, y, 1); }
-extern "C" fx_status fx_dg_elliptic_apply_sym(const fx_grid* g, const double* chi, const double* x, double* y) { return apply_checked(g, chi, x, y, 0); }
+extern "C" fx_status fx_dg_elliptic_apply_ex(fx_ctx* c, const fx_grid* g, const double* chi, const double* x, double* y) { return apply_checked(c, g, chi, x, y, 1); }
+extern "C" fx_status fx_dg_elliptic_apply_sym_ex(fx_ctx* c, const fx_grid* g, const double* chi, const double* x, double* y) { return apply_checked(c, g, chi, x, y, 0); }
+extern "C" fx_status fx_dg_elliptic_apply(const fx_grid* g, const double* chi, const double* x, double* y) {
+    FxCtx* c = fx_default_ctx();
+    return c ? apply_checked(c, g, chi, x, y, 1) : FX_ECUDA;
+}
+extern "C" fx_status fx_dg_elliptic_apply_sym(const fx_grid* g, const double* chi, const double* x, double* y) {
+    FxCtx* c = fx_default_ctx();
+    return c ? apply_checked(c, g, chi, x, y, 0) : FX_ECUDA;
+}
 
 // W[idx] = RN(vol4 * WW[l][k]),  V[idx] = RN(1 / W[idx])     (Fig. 2 "volume")
 __global__ void k_dg_weights(const __grid_constant__ DgParams g, int P, double vol4, double* W, double* V) {
@@ -839,10 +827,9 @@ __global__ void k_dg_weights(const __grid_constant__ DgParams g, int P, double v
     }
 }
 
-extern "C" fx_status fx_dg_weights(const fx_grid* g, double* W, double* V) {
+extern "C" fx_status fx_dg_weights_ex(fx_ctx* c, const fx_grid* g, double* W, double* V) {
+    FX_ENTER(c, "fx_dg_weights");
     if (!fx_grid_ok(g)) { fx_set_error("fx_dg_weights: bad grid"); return FX_EINVAL; }
-    FxCtx* c = fx_ctx();
-    if (!c) return FX_ECUDA;
     DgParams p; double vol4;
     fx_status s = fx_make_dg_params(g, 0, &p, &vol4);
     if (s != FX_OK) return s;
@@ -852,6 +839,10 @@ extern "C" fx_status fx_dg_weights(const fx_grid* g, double* W, double* V) {
     c->launches++;
     FX_CUDA(cudaGetLastError());
     return FX_OK;
+}
+extern "C" fx_status fx_dg_weights(const fx_grid* g, double* W, double* V) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_dg_weights_ex(c, g, W, V) : FX_ECUDA;
 }
 
 extern "C" fx_status fx_dg_tables(int32_t P, double* out) {
@@ -876,29 +867,28 @@ extern "C" fx_status fx_dg_tables(int32_t P, double* out) {
 static fx_status time_one(FxCtx* c, int kind, const fx_grid* g, const double* a, const double* b, double* cc, int64_t n) {
     switch (kind) {
     case 0: return fx_launch_exdot(c, a, b, n, c->result_dev);
-    case 1: return fx_axpby(0.7, a, -0.3, cc, n);
-    case 2: return fx_pointwise_dot(1.0, a, b, 0.0, cc, n);
+    case 1: return fx_axpby_ex(c, 0.7, a, -0.3, cc, n);
+    case 2: return fx_pointwise_dot_ex(c, 1.0, a, b, 0.0, cc, n);
     case 3: return fx_launch_apply(c, g, a, b, cc, 0);
     case 4: return fx_launch_apply(c, g, a, b, cc, 1);
-    case 5: { const double v = fx_exdot(a, b, n); return (v != v && fx_last_error()[0]) ? FX_ECUDA : FX_OK; }
-    case 6: return fx_axpby(0.7, a, 1.0, cc, n);
+    case 5: { double v; return fx_exdot_ex(c, a, b, n, &v, nullptr); }
+    case 6: return fx_axpby_ex(c, 0.7, a, 1.0, cc, n);
     case 7: return launch_exdotn<3>(c, a, b, cc, n, c->result_dev);
     case 8: return fx_launch_exsum(c, a, n, c->result_dev);
     case 9: return fx_launch_derivative(c, g, 0, 0, 0.7, a, -0.3, cc);
     case 10: return fx_launch_derivative(c, g, 1, 0, 0.7, a, -0.3, cc);
     case 11: return fx_launch_derivative(c, g, 0, 2, 0.7, a, -0.3, cc);
     case 12: return fx_launch_derivative(c, g, 1, 2, 0.7, a, -0.3, cc);
-    case 13: return fx_arakawa(g, a, b, cc);
+    case 13: return fx_arakawa_ex(c, g, a, b, cc);
     }
     return FX_EINVAL;
 }
 
-extern "C" fx_status fx_time_primitive(int32_t kind, const fx_grid* g, const double* a, const double* b, double* cc, int64_t n,
+extern "C" fx_status fx_time_primitive_ex(fx_ctx* c, int32_t kind, const fx_grid* g, const double* a, const double* b, double* cc, int64_t n,
                                        int32_t reps, double* ms_host) {
+    FX_ENTER(c, "fx_time_primitive");
     if (kind < 0 || kind > 13 || n < 0 || reps < 1 || !ms_host || !a || !b || !cc) { fx_set_error("fx_time_primitive: bad arguments"); return FX_EINVAL; }
     if ((kind == 3 || kind == 4 || kind >= 9) && (!fx_grid_ok(g) || (int64_t)g->Nx * g->Ny * g->P * g->P != n)) { fx_set_error("fx_time_primitive: bad grid"); return FX_EINVAL; }
-    FxCtx* c = fx_ctx();
-    if (!c) return FX_ECUDA;
     cudaEvent_t e0, e1;
     FX_CUDA(cudaEventCreate(&e0)); FX_CUDA(cudaEventCreate(&e1));
     fx_status s = time_one(c, kind, g, a, b, cc, n);
@@ -914,4 +904,9 @@ extern "C" fx_status fx_time_primitive(int32_t kind, const fx_grid* g, const dou
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     return s;
+}
+extern "C" fx_status fx_time_primitive(int32_t kind, const fx_grid* g, const double* a, const double* b, double* cc, int64_t n,
+                                       int32_t reps, double* ms_host) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_time_primitive_ex(c, kind, g, a, b, cc, n, reps, ms_host) : FX_ECUDA;
 }

@@ -101,6 +101,32 @@ def time_events(fn, reps, torch):
     return s.elapsed_time(e) / reps
 
 
+def csrc_stamp():
+    """sha256 (16 hex digits) of the kernel sources: profiles/traffic.json is only valid for the sources it was measured with"""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1807_01971_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        h.update(f.encode()); h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def cpu_info():
+    model = ""
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip(); break
+    except OSError:
+        pass
+    return {"os_cpu_count": os.cpu_count(), "cpu_model": model}
+
+
+# fp64 operations per unknown of the loop kernels (ncu instruction counts, DESIGN.md 11): K1 = stencil 39 + direction update 3
+# + exact dot 23 (incl. the halo lanes' redundant share); K2 = 3 + 23
+FP64_OPS_PER_UNKNOWN = {"k1": 62.0, "k2": 26.0}
+
+
 def run_fx(args):
     import numpy as np
     import torch
@@ -163,8 +189,25 @@ def run_fx(args):
                     "per_kernel_GBs": {k: bytes_per_launch[k] / (k_ms[k] * 1e-3) / 1e9 for k in k_ms},
                     "kernel_share_of_step": {k: k_ms[k] / (loop_ms / K) for k in k_ms}}
         traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(traffic_file):
-            roofline["traffic"] = json.load(open(traffic_file)).get(dom)
+        if os.path.exists(traffic_file):                                  # ncu dram bytes per launch, valid only for the sources it names
+            tj = json.load(open(traffic_file))
+            if tj.get("csrc_sha256_16") == csrc_stamp():
+                roofline["traffic"] = tj.get(dom)
+                roofline["traffic_source"] = tj.get("source")
+            else:
+                roofline["traffic_note"] = "profiles/traffic.json was measured with other kernel sources (%s, now %s): not reported" % (
+                    tj.get("csrc_sha256_16"), csrc_stamp())
+        # the second roof ("high number of 64-bit operations per memory load"): fp64 issue, measured in this run
+        a8 = torch.zeros(8, dtype=torch.float64, device="cuda")
+        fx.time_primitive("fp64_fma", a8, a8, a8, 2)
+        t_roof = min(fx.time_primitive("fp64_fma", a8, a8, a8, 5) for _ in range(3))
+        sms = torch.cuda.get_device_properties(local).multi_processor_count
+        fp64_peak = sms * fx.FP64_ROOF_FMAS_PER_SM / (t_roof * 1e-3) / 1e12          # T fp64 instructions (FMA) per second
+        roofline["alu"] = {"bound": "fp64 issue", "peak_Tops": fp64_peak, "peak_source": "k_fp64_roof: %d SMs x 8 CTAs x 256 threads x 8 chains x 4096 dependent FMAs, measured in this run" % sms,
+                           "kernel_ops_per_unknown": FP64_OPS_PER_UNKNOWN[dom], "kernel_ops": FP64_OPS_PER_UNKNOWN[dom] * n,
+                           "achieved_Tops": FP64_OPS_PER_UNKNOWN[dom] * n / (k_ms[dom] * 1e-3) / 1e12,
+                           "frac": FP64_OPS_PER_UNKNOWN[dom] * n / (k_ms[dom] * 1e-3) / 1e12 / fp64_peak,
+                           "per_kernel_frac": {k: FP64_OPS_PER_UNKNOWN[k] * n / (k_ms[k] * 1e-3) / 1e12 / fp64_peak for k in k_ms}}
 
         # ---- the metric's other parts: primitives on >= 100 MB vectors (inputs larger than L2) --------------------
         prim = {}
@@ -220,6 +263,54 @@ def run_fx(args):
                                         "frac_of_peak": 24.0 * n / tn / 1e6 / peak}
             prim["dg_apply"] = {"grid": "%dx%d P=3" % (N, N), "n": n, "MB_per_vector": 8e-6 * n, "ms": t, "GBps": 24.0 * n / t / 1e6,
                                 "frac_of_peak": 24.0 * n / t / 1e6 / peak, "note": "3 x 75.5 MB partly L2-resident between repeats"}
+            del q, pvec
+            # the north-star bar: dG apply at vectors >= 100 MB, every P (config 4's largest grids; P = 1 needs 4096^2 for that)
+            big = {}
+            for P_, N_ in ((1, 4096), (2, 2048), (3, 2048), (4, 2048), (5, 2048)) if not args.quick else ((3, 256),):
+                gb = fx.make_grid(N_, N_, P_, cfg["grid"]["lx"], cfg["grid"]["ly"], fx.PER, fx.DIR)
+                va = torch.rand(gb.n, dtype=torch.float64, device="cuda") + 0.5      # timing only: any finite data
+                vb = torch.rand(gb.n, dtype=torch.float64, device="cuda") - 0.5
+                vc = torch.empty_like(va)
+                fx.time_primitive("dg_apply_sym", va, vb, vc, 3, grid=gb)
+                tb = min(fx.time_primitive("dg_apply_sym", va, vb, vc, 10, grid=gb) for _ in range(2))
+                big["P%d_%dx%d" % (P_, N_, N_)] = {"MB_per_vector": 8e-6 * gb.n, "ms": tb, "GBps": 24.0 * gb.n / tb / 1e6,
+                                                     "frac_of_peak": 24.0 * gb.n / tb / 1e6 / peak}
+                del va, vb, vc
+            prim["dg_apply_100MB"] = big
+            # config 1 as specified: the exact dot on every condition target and on a +-500 exponent spread, with the
+            # share of elements that left the register window (the paper: the long accumulator is "rarely invoked")
+            bycond = {}
+            for k_ in ((20,) if args.quick else (24, 27)):
+                for ci, ctarget in enumerate(fi.COND_TARGETS + ["spread500"]):
+                    if ctarget == "spread500":
+                        hx, hy = fi.dot_wide_spread(1 << k_)
+                    else:
+                        hx, hy, _ = fi.dot_family_a(k_, ci)
+                    dx = torch.from_numpy(hx).cuda(); dy = torch.from_numpy(hy).cuda()
+                    del hx, hy
+                    for _ in range(2):
+                        fx.exdot_async(dx, dy, out)
+                    fx.exdot_stats(reset=True)
+                    reps = 10
+                    tc = time_events(lambda: fx.exdot_async(dx, dy, out), reps, torch)
+                    st = fx.exdot_stats(reset=True)
+                    ne = float(1 << k_) * reps
+                    bycond["n2^%d_%s" % (k_, "cond%.0e" % ctarget if ctarget != "spread500" else ctarget)] = {
+                        "ms": tc, "GBps": 16.0 * (1 << k_) / tc / 1e6, "frac_of_peak": 16.0 * (1 << k_) / tc / 1e6 / peak,
+                        "slow_path_share": {"deposit_double_per_element": st["deposit_double"] / ne, "deposit_product_per_element": st["deposit_product"] / ne,
+                                            "window_moves_per_1e6_elements": 1e6 * st["window_moves"] / ne}}
+                    del dx, dy
+            prim["exdot_by_condition"] = bycond
+            for v in prim.values():                                  # every fraction against the nominal 8 TB/s too (north star)
+                for d in (v.values() if "GBps" not in v else [v]):
+                    if isinstance(d, dict) and "GBps" in d:
+                        d["frac_of_nominal_8TBs"] = d["GBps"] / 8000.0
+
+        # ---- the paper's runtime model t = T_lat + m S / B (Eq. 3; Eq. 9) on a reduced config-4 sweep -----
+        model = {}
+        if rank == 0 and not args.no_primitives and not args.quick:
+            import sweep
+            model = sweep.reduced(fx, fi, torch)
 
         # ---- configs[0] and configs[2] in full (small grids: latency-bound; persistent cooperative kernel) ----------------
         small = {}
@@ -261,7 +352,7 @@ def run_fx(args):
                       "multi_gpu": "replicas only (north star: one GPU, no sharding)", "algorithmic_bytes_per_step": PASSES_FUSED * 8.0 * n},
            "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
            "cg": {"iterations": int(info.iterations), "status": int(info.status), "rel_residual": info.rel_residual},
-           "primitives": prim, "small_grid_solves": small}
+           "primitives": prim, "small_grid_solves": small, "model": model}
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
             out["cpu_baseline"] = cpu_baseline(cfg, n, quick=args.quick)
@@ -279,7 +370,7 @@ def cpu_baseline(cfg, n, quick=False):
     o.cg_solve(og, cfg["chi"], cfg["rho"], cfg["phi0"], 0.0, 1 + its); t2 = time.perf_counter()
     per_it = ((t2 - t1) - (t1 - t0)) / its
     return {"value": PASSES_FUSED * 8.0 * n / per_it / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "ms_per_step": per_it * 1e3,
+            "ms_per_step": per_it * 1e3, "host": cpu_info(),
             "sample": "%d CG iterations of the same %dx%d P=3 problem (time of 1+%d iterations minus time of 1), oracle/fxo.cpp single-threaded"
                       % (its, og.Nx, og.Ny, its)}
 
@@ -307,7 +398,7 @@ def run_reference(args):
                       "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
                       "data": "synthetic (fxinputs.config3 at N=256)",
                       "config": {"workload": "BASELINE.json configs[3] (bounded sample: 256x256 cells, P=3, %d unknowns)" % n},
-                      "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+                      "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, "host": cpu_info()},
                       "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
                       "gpu_launches": 0}))
 

@@ -132,6 +132,49 @@ def dot_family_a(k, cond_index):
     return x[perm].copy(), y[perm].copy(), math.ldexp(26.0, -e)
 
 
+def dot_family_b(k, cond_index, oracle):
+    """BASELINE.json configs[1], family B (rounding-residue cancellation): n = 2^k elements (k <= 22).
+
+    First half as family A's first half (random 53-bit mantissas, product exponents spread over about [-e, e]).
+    Second half: x_j random as above and y_j = RN((t_j - sigma_j)/x_j), sigma_j the correctly rounded running sum and
+    t_j = u_j * 2^(e_j) with e_j descending linearly from e to -e, so that the partial sums are driven down through the
+    whole exponent range and the final sum is what the rounding residues leave.  The running sums need the method's
+    arithmetic, so they come from the oracle passed in (`oracle.exdot_cancel_fill`); this module computes none of it.
+    No permutation is applied (the construction is order dependent).  Returns (x, y)."""
+    assert 1 <= cond_index < len(COND_TARGETS) and k <= 22
+    n = 1 << k
+    c = COND_TARGETS[cond_index]
+    g = rng(2000 * cond_index + k)
+    e = max(1, int(round((math.log2(c) - math.log2(n)) / 2.0)))
+    he = (e + 1) // 2
+    h = n // 2
+
+    def rand_half(m):
+        f = 1.0 + g.integers(0, 1 << 52, m).astype(np.float64) * 2.0 ** -52
+        a = g.integers(-he, he + 1, m)
+        sgn = np.where(g.integers(0, 2, m) == 0, 1.0, -1.0)
+        return sgn * np.ldexp(f, a)
+
+    x = np.concatenate([rand_half(h), rand_half(n - h)])
+    y = np.concatenate([np.abs(rand_half(h)), np.zeros(n - h)])
+    u = uniform(2500 + 40 * cond_index + k, n)
+    ej = np.round(np.linspace(e, -e, n - h)).astype(np.int64)
+    t = np.zeros(n)
+    t[h:] = np.ldexp(u[h:], ej)
+    y = oracle.exdot_cancel_fill(x, y, h, t)
+    return x, y
+
+
+def dot_wide_spread(n, seed_offset=1700, spread=500):
+    """products with exponents uniform over about [-2*spread, 2*spread] (no cancellation): every element far from its
+    neighbours' binades -- the exact dot's worst case for a windowed expansion"""
+    g = rng(seed_offset)
+    f = 1.0 + g.integers(0, 1 << 52, n).astype(np.float64) * 2.0 ** -52
+    gg = 1.0 + g.integers(0, 1 << 52, n).astype(np.float64) * 2.0 ** -52
+    sgn = np.where(g.integers(0, 2, n) == 0, 1.0, -1.0)
+    return sgn * np.ldexp(f, g.integers(-spread, spread + 1, n)), np.ldexp(gg, g.integers(-spread, spread + 1, n))
+
+
 def dot_special_cases():
     """BASELINE.json configs[1] special set: zeros, denormals, +-2^1000, each mixed into a uniform
     background.  Returns a list of (name, x, y).  Expected values come from the oracle."""

@@ -125,6 +125,14 @@ fx_status fx_exdot_digits_ex(fx_ctx* ctx, const double* x_dev, const double* y_d
 double fx_exdot_host(const double* x_host, const double* y_host, int64_t n);
 fx_status fx_exdot_host_ex(fx_ctx* ctx, const double* x_host, const double* y_host, int64_t n, double* result_host);
 
+/* Census of the exact reductions' slow paths since the last reset -- the paper's claim under test is that the long
+ * accumulator is "rarely invoked".  out_host: host uint64[4] = {elements (product parts) deposited into the long
+ * accumulator as exact integers because they reached below the register window, products deposited as 106-bit integer
+ * products because TwoProd is not error-free for them (outside [2^-960, 2^1000)), window moves of a warp, 0}; NULL = only
+ * reset.  Every reduction kernel of the context counts (dots, sums, the fused CG kernels).  Synchronises.           */
+fx_status fx_exdot_stats(uint64_t* out_host, int32_t reset);
+fx_status fx_exdot_stats_ex(fx_ctx* ctx, uint64_t* out_host, int32_t reset);
+
 /* Weighted dot sum_i x[i] w[i] y[i] ("the weighted sum ... where w represents for example the volume form") in
  * the reading D:Q14: u = RN(x[i]*w[i]) in fp64, then the exactly rounded dot of u and y.  fx_exsum: the exactly rounded
  * sum of x (EXSUM) = exact dot with ones.  Device pointers, may alias; both synchronise and return the value.      */
@@ -220,7 +228,9 @@ fx_status fx_cg_last_profile_ex(fx_ctx* ctx, double* ms_host, int32_t* iteration
  * 1 = axpby(0.7,a,-0.3,c), 2 = pointwise_dot(1,a,b,0,c), 3 = dG apply_sym(grid; chi=a, x=b, y=c), 4 = dG apply (normed),
  * 5 = exdot(a,b) returned to the host every call (the paper's GPU dot latency), 6 = axpby(0.7,a,1,c),
  * 7 = weighted dot(a,b,c) device-resident, 8 = exact sum(a) device-resident; with a grid: 9/10 = d/dx, d/dy forward,
- * 11/12 = d/dx, d/dy centred, each as c <- 0.7 M a - 0.3 c; 13 = Arakawa bracket c = {a, b} (nine calls).
+ * 11/12 = d/dx, d/dy centred, each as c <- 0.7 M a - 0.3 c; 13 = Arakawa bracket c = {a, b} (nine calls);
+ * 14 = the fp64 issue roof: a kernel of (SM count * 8) CTAs x 256 threads x 8 independent chains x 4096 dependent fused
+ * multiply-adds and no memory traffic (the second roof of the exact dot and the stencil; a, b unused).
  * a, b, c: device vectors of n doubles (kinds 3,4,9-13: n must equal the grid's size).  Synchronises.               */
 fx_status fx_time_primitive(int32_t kind, const fx_grid* grid, const double* a_dev, const double* b_dev, double* c_dev,
                             int64_t n, int32_t reps, double* ms_host);

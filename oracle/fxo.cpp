@@ -170,6 +170,23 @@ extern "C" double fxo_exdot_f32(const float* x, const float* y, int64_t n) {
     return acc_round(a);
 }
 
+// Running correctly rounded sums with feedback -- the input construction of BASELINE.json config 1, "Family B" (SURVEY
+// 8d: "the other half are constructed to cancel so the exact sum is tiny").  For j = start .. n-1, in this order:
+//   sigma_j = RN( sum_{i<j} x_i*y_i )   (the definition above, one rounding);   y_j = RN( RN(t_j - sigma_j) / x_j ),
+// so that after element j the exact running sum is t_j up to rounding residues.  x, t: inputs; y[start..n) is written.
+// Pin: tests/test_oracle_exdot.py recomputes every sigma_j with fractions.Fraction.
+extern "C" void fxo_exdot_cancel_fill(const double* x, double* y, int64_t start, int64_t n, const double* t) {
+    BigAcc a; acc_clear(a);
+    for (int64_t i = 0; i < start; ++i) acc_add_product(a, x[i], y[i]);
+    for (int64_t j = start; j < n; ++j) {
+        const double sigma = acc_round(a);
+        volatile double d = t[j] - sigma;
+        volatile double q = d / x[j];
+        y[j] = q;
+        acc_add_product(a, x[j], y[j]);
+    }
+}
+
 // round an externally supplied accumulator (used by the "concatenation = integer sum" pin)
 extern "C" double fxo_round_digits(const uint64_t limbs[68]) {
     BigAcc a; acc_clear(a); std::memcpy(a.limb, limbs, sizeof(a.limb));

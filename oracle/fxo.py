@@ -64,6 +64,8 @@ def lib():
         L.fxo_exdot_f32.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_int64]
         L.fxo_exsum.restype = C.c_double
         L.fxo_exsum.argtypes = [dp, C.c_int64]
+        L.fxo_exdot_cancel_fill.restype = None
+        L.fxo_exdot_cancel_fill.argtypes = [dp, dp, C.c_int64, C.c_int64, dp]
         L.fxo_round_digits.restype = C.c_double
         L.fxo_round_digits.argtypes = [C.POINTER(C.c_uint64)]
         L.fxo_axpby.restype = None
@@ -145,6 +147,15 @@ def exdot_digits(x, y):
     v = lib().fxo_exdot_digits(_p(x), _p(y), x.size, limbs.ctypes.data_as(C.POINTER(C.c_uint64)),
                                flags.ctypes.data_as(C.POINTER(C.c_int32)))
     return float(v), limbs, flags
+
+
+def exdot_cancel_fill(x, y, start, t):
+    """Family B of config 1: y[j] = RN(RN(t[j] - RN(sum_{i<j} x_i y_i)) / x[j]) for j >= start, in place; -> y"""
+    x, t = _f64(x).ravel(), _f64(t).ravel()
+    y = np.array(y, dtype=np.float64).ravel()
+    assert x.size == y.size == t.size and 0 <= start <= x.size
+    lib().fxo_exdot_cancel_fill(_p(x), _p(y), int(start), x.size, _p(t))
+    return y
 
 
 def round_digits(limbs):

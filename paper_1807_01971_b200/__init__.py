@@ -67,11 +67,12 @@ _SIGNATURES = {
     "fx_cg_last_profile": (C.c_int, [_dp, C.POINTER(C.c_int32)]),
     "fx_time_primitive": (C.c_int, [C.c_int32, C.POINTER(Grid), _vp, _vp, _vp, C.c_int64, C.c_int32, _dp]),
     "fx_launch_count": (C.c_int64, []),
+    "fx_exdot_stats": (C.c_int, [_vp, C.c_int32]),
     "fx_create": (C.c_int, [C.POINTER(_vp), C.c_int32, _vp]),
     "fx_destroy": (None, [_vp]),
 }
 # the context forms: NAME_ex(ctx, <the plain call's arguments> [, result_host for the value-returning reductions])
-for _n in ("fx_set_stream", "fx_set_launch", "fx_set_cg_fused", "fx_set_dg_path", "fx_exdot_async", "fx_exdot_digits", "fx_axpby",
+for _n in ("fx_exdot_stats", "fx_set_stream", "fx_set_launch", "fx_set_cg_fused", "fx_set_dg_path", "fx_exdot_async", "fx_exdot_digits", "fx_axpby",
            "fx_pointwise_dot", "fx_pointwise_dot2", "fx_arakawa", "fx_dg_elliptic_apply", "fx_dg_elliptic_apply_sym", "fx_dg_weights",
            "fx_dg_derivative", "fx_cg_solve", "fx_cg_solve_host", "fx_cg_profile", "fx_cg_last_profile", "fx_time_primitive"):
     _SIGNATURES[_n + "_ex"] = (C.c_int, [_vp] + _SIGNATURES[_n][1])
@@ -212,6 +213,13 @@ def exdot(x, y):
     if v != v and lib().fx_last_error():
         raise FxError(lib().fx_last_error().decode())
     return v
+
+
+def exdot_stats(reset=False):
+    """slow-path census of the exact reductions since the last reset (fx.h): dict(deposit_double, deposit_product, window_moves)"""
+    out = (C.c_uint64 * 4)()
+    _check(lib().fx_exdot_stats(out, 1 if reset else 0), "fx_exdot_stats")
+    return dict(deposit_double=int(out[0]), deposit_product=int(out[1]), window_moves=int(out[2]))
 
 
 def exdot3(x, w, y):
@@ -378,7 +386,8 @@ def cg_solve(grid, chi, rho, phi, tol, maxit):
     return info
 
 
-TIME_KINDS = {"exdot": 0, "axpby": 1, "pointwise_dot": 2, "dg_apply_sym": 3, "dg_apply": 4, "exdot_host": 5, "axpy": 6, "exdot3": 7, "exsum": 8, "dx_forward": 9, "dy_forward": 10, "dx_centered": 11, "dy_centered": 12, "arakawa": 13}
+TIME_KINDS = {"exdot": 0, "axpby": 1, "pointwise_dot": 2, "dg_apply_sym": 3, "dg_apply": 4, "exdot_host": 5, "axpy": 6, "exdot3": 7, "exsum": 8, "dx_forward": 9, "dy_forward": 10, "dx_centered": 11, "dy_centered": 12, "arakawa": 13, "fp64_fma": 14}
+FP64_ROOF_FMAS_PER_SM = 8 * 256 * 8 * 4096          # fused multiply-adds one "fp64_fma" launch executes per SM (fx.h, kind 14)
 
 
 def time_primitive(kind, a, b, c, reps, grid=None):

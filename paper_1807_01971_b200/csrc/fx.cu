@@ -83,7 +83,7 @@ static fx_status ctx_make(FxCtx** out, int device, void* stream) {
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { fx_set_error("cudaGetDeviceProperties failed"); delete c; return FX_ECUDA; }
     c->num_sms = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : FX_NUM_SMS_DEFAULT;
-    const size_t ex_bytes = (FX_NDIG + FX_NLIMB) * sizeof(fx_u64) + 64;
+    const size_t ex_bytes = (FX_NDIG + FX_NLIMB) * sizeof(fx_u64) + 64 + 4 * sizeof(fx_u64);
     char* base = nullptr;
     if (cudaMalloc(&base, ex_bytes) != cudaSuccess || cudaMemset(base, 0, ex_bytes) != cudaSuccess ||
         cudaMalloc(&c->result_dev, 8 * sizeof(double)) != cudaSuccess ||
@@ -98,6 +98,7 @@ static fx_status ctx_make(FxCtx** out, int device, void* stream) {
     c->ex.limbs = c->ex.dig + FX_NDIG;
     c->ex.flags = (int*)(c->ex.limbs + FX_NLIMB);
     c->ex.ticket = (unsigned int*)(c->ex.flags + 4);
+    c->ex.stats = (fx_u64*)(base + (FX_NDIG + FX_NLIMB) * sizeof(fx_u64) + 64);
     c->cg_fused = 1;
     { const char* ev = getenv("FX_PDL"); c->cg_pdl = ev && ev[0] == '1'; }      // measured slower on B200: off unless asked for
     c->ready = true;
@@ -192,6 +193,18 @@ extern "C" fx_status fx_set_dg_path_ex(fx_ctx* c, int32_t path) {
     return FX_OK;
 }
 extern "C" fx_status fx_set_dg_path(int32_t path) { FxCtx* c = fx_default_ctx(); return c ? fx_set_dg_path_ex(c, path) : FX_ECUDA; }
+
+extern "C" fx_status fx_exdot_stats_ex(fx_ctx* c, uint64_t* out_host, int32_t reset) {
+    FX_ENTER(c, "fx_exdot_stats");
+    FX_CUDA(cudaStreamSynchronize(c->stream));
+    if (out_host) FX_CUDA(cudaMemcpy(out_host, c->ex.stats, 4 * sizeof(fx_u64), cudaMemcpyDeviceToHost));
+    if (reset) FX_CUDA(cudaMemset(c->ex.stats, 0, 4 * sizeof(fx_u64)));
+    return FX_OK;
+}
+extern "C" fx_status fx_exdot_stats(uint64_t* out_host, int32_t reset) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_exdot_stats_ex(c, out_host, reset) : FX_ECUDA;
+}
 
 extern "C" int64_t fx_launch_count(void) {
     std::lock_guard<std::mutex> lk(g_mu);

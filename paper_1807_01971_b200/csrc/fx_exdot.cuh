@@ -42,6 +42,7 @@ struct ExShared {
     int is_last;
     int dlo, dhi;            // last CTA only: range of non-zero merged digits
     double res;              // ex_grid_reduce: the rounded value, broadcast to the CTA
+    unsigned int stat[4];    // slow-path census of this CTA: exact-double deposits, integer-product deposits, window moves
 };
 
 struct ExGlobal {            // device scratch of one context
@@ -49,9 +50,27 @@ struct ExGlobal {            // device scratch of one context
     fx_u64* limbs;           // [FX_NLIMB]  canonical two's complement accumulator of the running call
     int* flags;              // [1]
     unsigned int* ticket;    // [1]         CTAs finished (zero between launches)
+    fx_u64* stats;           // [4]         slow-path census since the last reset (fx_exdot_stats): how rarely the long
+                             //             accumulator is "invoked"
 };
 
-// add (-1)^neg * (hi:lo) * 2^(b - FX_BIAS) into a digit array with atomics (shared or global)
+// 64-bit add into a shared-memory word.  Shared memory has no native 64-bit atomic add (atomicAdd compiles to a compare-and-swap
+// spin, ATOMS.CAST.SPIN.64, which collapses when many lanes hit the few digits of one exponent region); two native 32-bit adds
+// do the same: the low add returns the old value, from which THIS adder knows whether it caused the wrap-around, and carries
+// it into the high word.  Every wrap is seen by exactly one adder, so the 64-bit total is exact in any order.
+__device__ __forceinline__ void ex_sadd64(fx_u64* p, fx_u64 v) {
+    const unsigned a = (unsigned)__cvta_generic_to_shared(p);
+    const unsigned lo = (unsigned)v;
+    unsigned hi = (unsigned)(v >> 32);
+    if (lo) {
+        unsigned old;
+        asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(a), "r"(lo) : "memory");
+        hi += (old + lo) < old ? 1u : 0u;
+    }
+    if (hi) asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(a + 4u), "r"(hi) : "memory");
+}
+
+// add (-1)^neg * (hi:lo) * 2^(b - FX_BIAS) into the CTA's digit array in shared memory
 __device__ __forceinline__ void ex_deposit(fx_u64* dig, int b, fx_u64 hi, fx_u64 lo, bool neg) {
     const int d = b >> 5, s = b & 31;
     fx_u64 w0 = lo << s;
@@ -60,7 +79,7 @@ __device__ __forceinline__ void ex_deposit(fx_u64* dig, int b, fx_u64 hi, fx_u64
     fx_u64 c[5] = {w0 & 0xffffffffull, w0 >> 32, w1 & 0xffffffffull, w1 >> 32, w2};
 #pragma unroll
     for (int i = 0; i < 5; ++i)
-        if (c[i]) atomicAdd(&dig[d + i], neg ? (0ull - c[i]) : c[i]);
+        if (c[i]) ex_sadd64(&dig[d + i], neg ? (0ull - c[i]) : c[i]);
 }
 
 // any finite double v (exactly), DESIGN.md 6.1 "slow path 1"
@@ -71,6 +90,7 @@ static __device__ __noinline__ void ex_deposit_double(ExShared* sh, double v) {
     if (be) m |= 1ull << 52;
     if (m == 0) return;
     const int E = (be ? be : 1) - 1075;
+    atomicAdd(&sh->stat[0], 1u);
     ex_deposit(sh->dig, E + FX_BIAS, 0ull, m, (bits >> 63) != 0);
 }
 
@@ -88,6 +108,7 @@ static __device__ __noinline__ void ex_deposit_product(ExShared* sh, double x, d
     const fx_u64 mx = ex ? (fx | (1ull << 52)) : fx, my = ey ? (fy | (1ull << 52)) : fy;
     const fx_u64 lo = mx * my, hi = __umul64hi(mx, my);
     if ((lo | hi) == 0) return;
+    atomicAdd(&sh->stat[1], 1u);
     const int E = (ex ? ex : 1) + (ey ? ey : 1) - 2150;          // value = mx*my * 2^E, E >= -2148
     ex_deposit(sh->dig, E + FX_BIAS, hi, lo, neg);
 }
@@ -105,21 +126,26 @@ static __device__ __noinline__ void ex_deposit_count(ExShared* sh, int b, long l
 
 // Per-thread binned expansion with a warp-uniform window.  K bins of W bit.  All members are inlined so that the
 // state lives in registers; only the integer deposits are calls.
-template <int K, int W>
+// KL further bins below the K of the hot chain (a "low window"): they are visited only by a thread whose batch left a
+// remainder below the first K*W bits -- data whose exponents spread over more than the window (config 1's condition
+// targets 1e32 and 1e40: products over 2^-53 .. 2^53 plus their 106 bits).  Without them every such remainder went to the
+// shared long accumulator with atomics: 0.5 deposits per element at 1e40 and 234 GB/s instead of 6800.
+template <int K, int W, int KL = 0>
 struct ExAcc {
+    static constexpr int KT = K + KL;
     static constexpr int CAP = 1 << (50 - W);            // deposits per bin before S[k] must be re-centred
     static constexpr int MARGIN = 6;                     // head-room (bit) above the largest product seen
-    static constexpr int TB_MIN = -1074 + K * W + 1022;  // lowest bin stays a normal double with ulp >= 2^-1074
+    static constexpr int TB_MIN = -1074 + KT * W + 1022; // lowest bin stays a normal double with ulp >= 2^-1074
     static constexpr unsigned BE_LO = 63;                // fast path: 2^-960 <= |p| < 2^1000 (TwoProd error-free,
     static constexpr unsigned BE_HI = 2022;              //   no overflow of the top bin)
-    double S[K];
-    long long C[K];
+    double S[KT];
+    long long C[KT];
     int Tb;          // T + 1022; |p| < 2^T  <=>  biased exponent of p <= Tb.   very negative = no window yet
     int cnt, ren;
 
     __device__ __forceinline__ void init() {
 #pragma unroll
-        for (int k = 0; k < K; ++k) { S[k] = 0.0; C[k] = 0; }
+        for (int k = 0; k < KT; ++k) { S[k] = 0.0; C[k] = 0; }
         Tb = -(1 << 29); cnt = 0; ren = 0;
     }
     __device__ __forceinline__ long long mbits(int k) const {      // bit pattern of 1.5 * 2^(E_k + 52)
@@ -128,7 +154,7 @@ struct ExAcc {
     }
     __device__ __forceinline__ void recentre() {                    // S[k] -> centre, integer part -> C[k]
 #pragma unroll
-        for (int k = 0; k < K; ++k) {
+        for (int k = 0; k < KT; ++k) {
             const long long m = mbits(k);
             C[k] += __double_as_longlong(S[k]) - m;                 // same binade: bit patterns are linear in value
             S[k] = __longlong_as_double(m);
@@ -139,7 +165,7 @@ struct ExAcc {
     __device__ __forceinline__ void flush(ExShared* sh) {
         if (Tb > -(1 << 28)) {
 #pragma unroll
-            for (int k = 0; k < K; ++k) {
+            for (int k = 0; k < KT; ++k) {
                 long long c = C[k] + (__double_as_longlong(S[k]) - mbits(k));
                 c = ex_warp_sum(c);
                 if ((threadIdx.x & 31) == 0 && c != 0) ex_deposit_count(sh, Tb - 1022 - W * (k + 1) + FX_BIAS, c);
@@ -150,11 +176,12 @@ struct ExAcc {
         cnt = 0; ren = 0;
     }
     __device__ __forceinline__ void reanchor(ExShared* sh, int bemax) {
+        if ((threadIdx.x & 31) == 0 && Tb > -(1 << 28)) atomicAdd(&sh->stat[2], 1u);      // (the first anchoring of a warp is not a move)
         flush(sh);
         const int t = bemax + MARGIN;
         Tb = t < TB_MIN ? TB_MIN : t;
 #pragma unroll
-        for (int k = 0; k < K; ++k) { S[k] = __longlong_as_double(mbits(k)); C[k] = 0; }
+        for (int k = 0; k < KT; ++k) { S[k] = __longlong_as_double(mbits(k)); C[k] = 0; }
     }
 
     // U products per lane; must be called by all 32 lanes of the warp together.  Elements with active == false must
@@ -219,6 +246,26 @@ struct ExAcc {
             rlo |= (unsigned)__double2loint(v) | (unsigned)__double2loint(w);
             rhi |= (unsigned)__double2hiint(v) | (unsigned)__double2hiint(w);
         }
+        if (KL > 0 && (rlo | (rhi & 0x7fffffffu))) {                 // bits below the hot chain's K*W bits: the low window
+            rlo = 0; rhi = 0;
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                double v = p[u], w = e[u];
+#pragma unroll
+                for (int k = K; k < KT; ++k) {
+                    const double s = __dadd_rn(S[k], v);
+                    const double q = __dsub_rn(s, S[k]);
+                    v = __dsub_rn(v, q);
+                    const double s2 = NOERR ? s : __dadd_rn(s, w);
+                    const double q2 = NOERR ? 0.0 : __dsub_rn(s2, s);
+                    if (!NOERR) w = __dsub_rn(w, q2);
+                    S[k] = s2;
+                }
+                p[u] = v; e[u] = w;
+                rlo |= (unsigned)__double2loint(v) | (unsigned)__double2loint(w);
+                rhi |= (unsigned)__double2hiint(v) | (unsigned)__double2hiint(w);
+            }
+        }
         if (rlo | (rhi & 0x7fffffffu)) {                             // bits below the window: exact, but slow
 #pragma unroll
             for (int u = 0; u < U; ++u) {
@@ -243,6 +290,7 @@ struct ExAcc {
 __device__ __forceinline__ void ex_shared_init(ExShared* sh) {
     for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) sh->dig[i] = 0ull;
     if (threadIdx.x == 0) { sh->flags = 0; sh->is_last = 0; }
+    if (threadIdx.x < 4) sh->stat[threadIdx.x] = 0u;
     __syncthreads();
 }
 
@@ -308,6 +356,7 @@ __device__ __forceinline__ bool ex_block_finish(ExShared* sh, const ExGlobal& g,
         if (v) atomicAdd(&g.dig[i], v);
     }
     if (threadIdx.x == 0 && sh->flags) atomicOr(g.flags, sh->flags);
+    if (threadIdx.x < 4 && sh->stat[threadIdx.x]) atomicAdd(&g.stats[threadIdx.x], (fx_u64)sh->stat[threadIdx.x]);
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) {

@@ -13,6 +13,10 @@
 
 #define EX_K 4
 #define EX_W 40
+#ifndef EX_KL
+#define EX_KL 2            // low window of the stand-alone reductions (fx_exdot.cuh): 6 x 40 = 240 bit before the long accumulator
+#endif
+typedef ExAcc<EX_K, EX_W, EX_KL> ExDotAcc;
 #define EX_U 4
 #define EX_STAGES 4
 
@@ -55,7 +59,7 @@ __device__ __forceinline__ void exdot_issue(double* buf, int stage, const double
 // as element * 1 (no error term); same loads, same ring, about the same fp64 work per byte as the dot.
 // MODE 2 (binary32 dot): every 8-byte slot holds two floats; float * float is exact in fp64 (no error term).
 template <int MODE>
-__device__ __forceinline__ void ex_feed(ExAcc<EX_K, EX_W>& acc, const double (&xv)[EX_U], const double (&yv)[EX_U], const bool (&act)[EX_U],
+__device__ __forceinline__ void ex_feed(ExDotAcc& acc, const double (&xv)[EX_U], const double (&yv)[EX_U], const bool (&act)[EX_U],
                                         ExShared* sh) {
     if (MODE == 1) {
         double one[EX_U];
@@ -77,7 +81,7 @@ __device__ __forceinline__ void ex_feed(ExAcc<EX_K, EX_W>& acc, const double (&x
 }
 
 template <bool VEC, int MODE>
-__device__ __forceinline__ void exdot_consume(const double* buf, int stage, long long n, long long base, ExAcc<EX_K, EX_W>& acc,
+__device__ __forceinline__ void exdot_consume(const double* buf, int stage, long long n, long long base, ExDotAcc& acc,
                                               ExShared* sh) {
     const int bd = blockDim.x;
     const double* sx = buf + (size_t)stage * 2 * EX_U * bd;
@@ -112,7 +116,7 @@ __global__ void __launch_bounds__(256, 2) k_exdot(const double* __restrict__ x, 
     extern __shared__ __align__(16) double ex_buf[];
     __shared__ ExShared sh;
     ex_shared_init(&sh);
-    ExAcc<EX_K, EX_W> acc;
+    ExDotAcc acc;
     acc.init();
     const int bd = blockDim.x;
     const long long tile = (long long)bd * EX_U;
@@ -213,7 +217,7 @@ __global__ void __launch_bounds__(256, 2) k_exdotn(const double* __restrict__ a0
     extern __shared__ __align__(16) double ex_buf[];
     __shared__ ExShared sh;
     ex_shared_init(&sh);
-    ExAcc<EX_K, EX_W> acc;
+    ExDotAcc acc;
     acc.init();
     const int bd = blockDim.x;
     const long long tile = (long long)bd * EX_U, ntiles = (n + tile - 1) / tile;
@@ -323,7 +327,7 @@ __global__ void __launch_bounds__(256, 2) k_exdot_f32(const float* __restrict__ 
     extern __shared__ __align__(16) float exf_buf[];
     __shared__ ExShared sh;
     ex_shared_init(&sh);
-    ExAcc<EX_K, EX_W> acc;
+    ExDotAcc acc;
     acc.init();
     const int bd = blockDim.x;
     const long long tile = (long long)bd * EXF_U, ntiles = (n + tile - 1) / tile;
@@ -864,8 +868,31 @@ extern "C" fx_status fx_dg_tables(int32_t P, double* out) {
 // ------------------------------------------------------------------------------------------------------------
 // timing hook (include/fx.h): average time of back-to-back calls, measured on the device
 // ------------------------------------------------------------------------------------------------------------
+// fp64 issue roof (SURVEY 8d "FP64 issue rate is a real second roof ... micro-benchmark it first"; the paper: "high number of
+// 64-bit operations per memory load"): FX_ROOF_CHAINS independent dependent-FMA chains per thread, no memory traffic.
+// One launch = num_sms * 8 CTAs x 256 threads x FX_ROOF_CHAINS x FX_ROOF_ITERS fused multiply-adds.
+#define FX_ROOF_CHAINS 8
+#define FX_ROOF_ITERS 4096
+__global__ void __launch_bounds__(256) k_fp64_roof(double* out, double a, double b) {
+    double v[FX_ROOF_CHAINS];
+#pragma unroll
+    for (int i = 0; i < FX_ROOF_CHAINS; ++i) v[i] = (double)(threadIdx.x + i);
+#pragma unroll 1
+    for (int it = 0; it < FX_ROOF_ITERS; it += 4) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int i = 0; i < FX_ROOF_CHAINS; ++i) v[i] = __fma_rn(v[i], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < FX_ROOF_CHAINS; ++i) s = __dadd_rn(s, v[i]);
+    if (s == 12345.678) out[0] = s;                      // never true for the arguments used: keeps the chains alive
+}
+
 static fx_status time_one(FxCtx* c, int kind, const fx_grid* g, const double* a, const double* b, double* cc, int64_t n) {
     switch (kind) {
+    case 14: k_fp64_roof<<<c->num_sms * 8, 256, 0, c->stream>>>(cc, 0.999999, 1e-9); c->launches++; return cudaGetLastError() == cudaSuccess ? FX_OK : FX_ECUDA;
     case 0: return fx_launch_exdot(c, a, b, n, c->result_dev);
     case 1: return fx_axpby_ex(c, 0.7, a, -0.3, cc, n);
     case 2: return fx_pointwise_dot_ex(c, 1.0, a, b, 0.0, cc, n);
@@ -887,8 +914,8 @@ static fx_status time_one(FxCtx* c, int kind, const fx_grid* g, const double* a,
 extern "C" fx_status fx_time_primitive_ex(fx_ctx* c, int32_t kind, const fx_grid* g, const double* a, const double* b, double* cc, int64_t n,
                                        int32_t reps, double* ms_host) {
     FX_ENTER(c, "fx_time_primitive");
-    if (kind < 0 || kind > 13 || n < 0 || reps < 1 || !ms_host || !a || !b || !cc) { fx_set_error("fx_time_primitive: bad arguments"); return FX_EINVAL; }
-    if ((kind == 3 || kind == 4 || kind >= 9) && (!fx_grid_ok(g) || (int64_t)g->Nx * g->Ny * g->P * g->P != n)) { fx_set_error("fx_time_primitive: bad grid"); return FX_EINVAL; }
+    if (kind < 0 || kind > 14 || n < 0 || reps < 1 || !ms_host || !a || !b || !cc) { fx_set_error("fx_time_primitive: bad arguments"); return FX_EINVAL; }
+    if ((kind == 3 || kind == 4 || (kind >= 9 && kind <= 13)) && (!fx_grid_ok(g) || (int64_t)g->Nx * g->Ny * g->P * g->P != n)) { fx_set_error("fx_time_primitive: bad grid"); return FX_EINVAL; }
     cudaEvent_t e0, e1;
     FX_CUDA(cudaEventCreate(&e0)); FX_CUDA(cudaEventCreate(&e1));
     fx_status s = time_one(c, kind, g, a, b, cc, n);

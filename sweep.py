@@ -4,7 +4,7 @@ Paper: bandwidth b = m*S/t with STREAM counting (Eq. 2: axpby 
 model t(S) = T_lat + m*S/B (Eq. 3); estimators: B = mean over the largest sizes, T_lat = smallest average run
 time corrected by -m*S/B and clipped at 0; minimum efficient array size ~ T_lat*B (Eq. 9).
 
-    python -m paper_1807_01971_b200.sweep [--out DIR] [--quick]
+    python sweep.py [--out DIR] [--quick]            (bench.py runs `reduced` and puts its fits under "model")
 
 Runs on cuda:0 through the C ABI (fx_time_primitive: average of back-to-back launches, CUDA events).  Writes
 DIR/sweep.json and DIR/sweep.md.  Inputs: seeded uniform[-1,1) vectors (fxinputs.config4) -- synthetic stand-ins for
@@ -16,7 +16,7 @@ import math
 import os
 import sys
 
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
@@ -46,6 +46,34 @@ def fit(points, m):
     err = max(abs((Tlat + m * S / B) / t - 1.0) for S, t in pts if not (0.5e6 < S and 3 * S < 2 * L2_BYTES))
     return {"B_GBps": B / 1e9, "B_std_GBps": Bstd / 1e9, "T_lat_us": Tlat * 1e6, "T_lat_times_B_MB": Tlat * B / 1e6,
             "lsq_B_GBps": m / slope / 1e9, "lsq_T_lat_us": icpt * 1e6, "model_max_rel_err_outside_L2_bump": err}
+
+
+def reduced(fx, fi, torch, P=3, Ns=(16, 64, 256, 1024, 1536, 2048)):
+    """Six sizes of config 4 at one P (18 KB ... 302 MB per vector): the fits of the five north-star primitives for bench.py"""
+    pts = {}
+    for N in Ns:
+        c = fi.config4(P, N)
+        g = fx.make_grid(**c["grid"])
+        x = torch.from_numpy(c["x"]).cuda(); y = torch.from_numpy(c["y"]).cuda(); chi = torch.from_numpy(c["chi"]).cuda()
+        out = torch.empty_like(x)
+        S = 8.0 * g.n
+        reps = int(max(10, min(1000, 0.03 / max(2e-6, 3 * S / 5e12))))
+        for kind in ("axpby", "pointwise_dot", "exdot", "exdot_host", "dg_apply_sym"):
+            if kind == "dg_apply_sym":
+                ms = fx.time_primitive(kind, chi, x, out, reps, grid=g)
+            else:
+                if kind == "axpby":
+                    out.copy_(y)
+                ms = fx.time_primitive(kind, x, y, out, max(10, reps // (4 if kind == "exdot_host" else 1)))
+            pts.setdefault(kind, []).append((S, ms * 1e-3))
+        del x, y, chi, out
+    res = {}
+    for kind, p in pts.items():
+        f = fit(p, M_PASSES[kind])
+        f["m"] = M_PASSES[kind]
+        f["points_MB_us"] = [[round(S / 1e6, 3), round(t * 1e6, 2)] for S, t in p]
+        res[kind if kind != "dg_apply_sym" else "dg_apply_sym_P%d" % P] = f
+    return res
 
 
 def main():

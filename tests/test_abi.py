@@ -33,10 +33,21 @@ def test_header_symbols_exported(fx):
 
 
 def test_sass_is_sm100_fp64_no_contraction(fx):
-    """the cubin inside libfx.so targets sm_100a and contains explicit DFMA/DMUL/DADD only (no tensor-core path)"""
+    """the cubins inside libfx.so target sm_100a; the arithmetic is explicit fp64 (DFMA / DMUL / DADD), nothing runs on a
+    tensor-core path (this is a scan / stencil, not a contraction), and the staging is Blackwell's: 1-D bulk copies
+    (UBLKCP) in the vector-update kernel, 2-D tensor-map loads (UTMALDG) in the stencil kernels, mbarrier waits (SYNCS)"""
     import subprocess
     out = subprocess.run(["cuobjdump", "-lelf", fx.lib_path()], capture_output=True, text=True).stdout
     assert "sm_100a" in out
+    sass = subprocess.run(["cuobjdump", "-sass", fx.lib_path()], capture_output=True, text=True).stdout
+    ops = {}
+    for m in re.finditer(r"^\s+/\*[0-9a-f]{4}\*/\s+(?:@!?U?P\w+\s+)?([A-Z][A-Z0-9_]*)", sass, flags=re.M):
+        ops[m.group(1)] = ops.get(m.group(1), 0) + 1
+    for need in ("DFMA", "DMUL", "DADD", "UBLKCP", "UTMALDG", "SYNCS", "LDGSTS", "SHFL"):
+        assert ops.get(need, 0) > 0, "no %s in the SASS" % need
+    tensor = [o for o in ops if o.startswith(("HMMA", "IMMA", "DMMA", "BMMA", "UTCHMMA", "UTCQMMA", "UTCIMMA", "UTCOMMA", "HGMMA", "QGMMA", "IGMMA"))]
+    assert not tensor, tensor
+    assert ops["DFMA"] > ops.get("FFMA", 0)                       # fp64 throughout; fp32 only in address / conversion helpers
 
 
 @pytest.mark.parametrize("P", [1, 2, 3, 4, 5])

@@ -156,14 +156,54 @@ def test_exdot_multi_launch_and_host_chunks(fx, oracle):
     assert fbits(got) == fbits(want) and np.array_equal(glimbs, limbs)
 
 
-@pytest.mark.parametrize("ci", [0, 3, 5])
-def test_exdot_full_size_config1(fx, oracle, ci):
-    """n = 2^27 (the largest size of config 1, the launch configuration bench.py times)"""
-    x, y, expected = fi.dot_family_a(27, ci)
-    got = fx.exdot(dev(x), dev(y))
+@pytest.mark.parametrize("k", [24, 27])
+@pytest.mark.parametrize("ci", range(6))
+def test_exdot_full_size_config1(fx, oracle, ci, k):
+    """config 1, family A at n = 2^24 and 2^27 (the sizes and launch configuration bench.py times), every condition target:
+    the value and all 68 limbs of the long accumulator"""
+    x, y, expected = fi.dot_family_a(k, ci)
+    want, limbs, flags = oracle.exdot_digits(x, y)
     if expected is not None:
-        assert got == expected
-    assert fbits(got) == fbits(oracle.exdot(x, y))
+        assert want == expected
+    got, glimbs, gflags = fx.exdot_digits(dev(x), dev(y))
+    assert fbits(got) == fbits(want)
+    assert np.array_equal(glimbs, limbs) and np.array_equal(gflags, flags)
+
+
+@pytest.mark.parametrize("k,ci", [(20, 1), (20, 2), (20, 3), (20, 4), (20, 5), (21, 3), (22, 5)])
+def test_exdot_family_b_residue_cancellation(fx, oracle, k, ci):
+    """config 1, family B: the second half drives the running sum down through the whole exponent range, the
+    result is what the rounding residues leave.  Value, limbs, and the achieved condition number (exact, from the oracle)."""
+    x, y = fi.dot_family_b(k, ci, oracle)
+    want, limbs, flags = oracle.exdot_digits(x, y)
+    cond = 2.0 * oracle.exdot(np.abs(x), np.abs(y)) / abs(want)
+    assert cond >= 1e-3 * fi.COND_TARGETS[ci]
+    fx.exdot_stats(reset=True)
+    got, glimbs, gflags = fx.exdot_digits(dev(x), dev(y))
+    assert fbits(got) == fbits(want)
+    assert np.array_equal(glimbs, limbs) and np.array_equal(gflags, flags)
+    st = fx.exdot_stats()
+    assert st["deposit_product"] == 0                                  # all products inside TwoProd's error-free range
+    # launch-shape invariance on the ill-conditioned data too
+    for grid, block in [(1, 32), (77, 64), (1000, 256)]:
+        fx.set_launch(0, grid, block)
+        assert fbits(fx.exdot(dev(x), dev(y))) == fbits(want), (grid, block)
+
+
+def test_exdot_stats_census(fx, oracle):
+    """fx_exdot_stats: uniform data never leaves the register window; a +-500 exponent spread does, and 2^1000-class products
+    take the integer-product path -- with the oracle's bits either way"""
+    n = 1 << 20
+    x, y = fi.uniform(41, n), fi.uniform(42, n)
+    fx.exdot_stats(reset=True)
+    assert fbits(fx.exdot(dev(x), dev(y))) == fbits(oracle.exdot(x, y))
+    st = fx.exdot_stats(reset=True)
+    assert st["deposit_product"] == 0 and st["deposit_double"] <= n // 1000
+    x, y = fi.dot_wide_spread(n)
+    assert fbits(fx.exdot(dev(x), dev(y))) == fbits(oracle.exdot(x, y))
+    st = fx.exdot_stats(reset=True)
+    assert st["deposit_double"] + st["deposit_product"] > 0 and st["window_moves"] > 0
+    assert fx.exdot_stats() == dict(deposit_double=0, deposit_product=0, window_moves=0)
 
 
 # ---- axpby / pointwise_dot / weights ------------------------------------------------------------------------------

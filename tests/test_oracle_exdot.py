@@ -309,3 +309,33 @@ def test_exdot_f32_pins(oracle):
     # naive float32 accumulation loses the small terms that the exact accumulation keeps
     big = np.array([1e8, 1.0, -1e8, 1.0], dtype=np.float32)
     assert oracle.exdot_f32(big, np.ones(4, dtype=np.float32)) == 2.0
+
+
+# ---------------------------------------------------------------- config 1, family B (rounding-residue cancellation)
+def test_cancel_fill_against_rationals(oracle):
+    """fxo_exdot_cancel_fill: every y_j = RN(RN(t_j - sigma_j)/x_j) with sigma_j recomputed from exact rationals"""
+    g = fi.rng(9101)
+    n, h = 160, 64
+    x = np.ldexp(1.0 + g.random(n), g.integers(-30, 31, n)) * np.where(g.integers(0, 2, n) == 0, 1.0, -1.0)
+    y0 = np.concatenate([np.ldexp(1.0 + g.random(h), g.integers(-30, 31, h)), np.zeros(n - h)])
+    t = np.concatenate([np.zeros(h), np.ldexp(fi.uniform(9102, n - h), np.round(np.linspace(40, -40, n - h)).astype(np.int64))])
+    y = oracle.exdot_cancel_fill(x, y0, h, t)
+    assert np.array_equal(y[:h], y0[:h])
+    run = frac_dot(x[:h], y[:h])
+    for j in range(h, n):
+        sigma = frac_round(run)
+        want = (float(t[j]) - sigma) / float(x[j])                  # two IEEE operations, as the definition writes them
+        assert same(y[j], want), j
+        run += Fraction(float(x[j])) * Fraction(float(y[j]))
+    # the construction does what it is for: partial sums follow t_j, the total is tiny against the terms
+    assert abs(frac_round(run)) <= 2.0 * abs(t[-1]) + 1e-300
+    assert same(oracle.exdot(x, y), frac_round(run))
+
+
+@pytest.mark.parametrize("ci", [1, 3, 5])
+def test_family_b_is_ill_conditioned_and_exact(oracle, ci):
+    x, y = fi.dot_family_b(10, ci, oracle)
+    val = oracle.exdot(x, y)
+    assert same(val, frac_round(frac_dot(x, y)))
+    cond = 2.0 * oracle.exdot(np.abs(x), np.abs(y)) / abs(val)
+    assert cond >= 1e-3 * fi.COND_TARGETS[ci]                      # achieved condition number: the target's order of magnitude or more

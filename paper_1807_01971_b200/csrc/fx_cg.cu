@@ -27,7 +27,66 @@ namespace cgr = cooperative_groups;
 struct CgScal {
     double rz, pq, alpha, beta, bz, thresh, dot;
     int done, status, iters, pad;
+    double rzb[2];               // r.z entering iteration k (slot k & 1): written by K1(k), read by K2(k) and K1(k+1)
 };
+
+// The fused loop's reductions are finished by their consumers (fx_exdot.cuh, ex_publish / ex_fetch_round): K1(k) adds the
+// digits of p.q to PQ[k & 1], every CTA of K2(k) rounds them and forms alpha; K2(k) adds r.z to RZ[k & 1], every CTA of
+// K1(k+1) rounds them, tests convergence and forms beta.  A kernel pays no ticket, no last-CTA finaliser and no scalar
+// round trip at its end (about 6 us per kernel, twice per iteration); the rounding at the start overlaps the first loads.
+// CTA 0 re-zeroes the buffer of the iteration after next one kernel after its last reader finished.
+struct CgRed {
+    fx_u64* dig;                 // [4][FX_NDIG]: PQ[0], PQ[1], RZ[0], RZ[1]
+    int* flags;                  // [4]
+    fx_u64* stats;               // the context's slow-path census
+    __device__ fx_u64* pq(int k) const { return dig + (size_t)(k & 1) * FX_NDIG; }
+    __device__ fx_u64* rz(int k) const { return dig + (size_t)(2 + (k & 1)) * FX_NDIG; }
+    __device__ int* pqf(int k) const { return flags + (k & 1); }
+    __device__ int* rzf(int k) const { return flags + 2 + (k & 1); }
+};
+
+// start of K1(k): r.z of the previous iteration -> convergence test, beta.  Returns false if the loop is over.
+__device__ __forceinline__ bool cg_k1_scalars(ExShared* sh, const CgRed& red, CgScal* sc, int k, double* beta) {
+    double rzn;
+    if (k == 0) rzn = sc->rzb[1];                                   // set up by the host: r.z of the start residual
+    else rzn = ex_fetch_round(sh, red.rz(k - 1), red.rzf(k - 1));
+    const bool lead = blockIdx.x == 0 && threadIdx.x == 0;
+    if (k > 0 && __dsqrt_rn(rzn) <= sc->thresh) {
+        if (lead) { sc->rz = rzn; sc->status = FX_OK; sc->iters = k; sc->done = 1; }
+        return false;
+    }
+    *beta = k > 0 ? __ddiv_rn(rzn, sc->rzb[(k - 1) & 1]) : 0.0;
+    if (lead) { sc->rzb[k & 1] = rzn; sc->rz = rzn; sc->iters = k + 1; }
+    if (blockIdx.x == 0) {                                          // PQ of the next iteration: its last reader was K2(k-1)
+        for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) red.pq(k + 1)[i] = 0ull;
+        if (threadIdx.x == 0) *red.pqf(k + 1) = 0;
+    }
+    return true;
+}
+// start of K2(k): p.q -> breakdown test, alpha
+__device__ __forceinline__ bool cg_k2_scalars(ExShared* sh, const CgRed& red, CgScal* sc, int k, double* alpha) {
+    const double pq = ex_fetch_round(sh, red.pq(k), red.pqf(k));
+    if (!(pq > 0.0) || isinf(pq)) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) { sc->pq = pq; sc->status = FX_EBREAKDOWN; sc->done = 1; }
+        return false;
+    }
+    *alpha = __ddiv_rn(sc->rzb[k & 1], pq);
+    if (blockIdx.x == 0) {                                          // RZ of the next iteration: its last reader was K1(k)
+        for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) red.rz(k + 1)[i] = 0ull;
+        if (threadIdx.x == 0) { *red.rzf(k + 1) = 0; sc->pq = pq; sc->alpha = *alpha; }
+    }
+    return true;
+}
+// after the last enqueued iteration of a batch: r.z of iteration k -> rz, convergence (what K1(k+1) would find)
+__global__ void __launch_bounds__(128) k_cg_finish(CgRed red, CgScal* sc, int k) {
+    __shared__ ExShared sh;
+    if (*(volatile int*)&sc->done) return;
+    const double rzn = ex_fetch_round(&sh, red.rz(k), red.rzf(k));
+    if (threadIdx.x == 0) {
+        sc->rz = rzn; sc->dot = rzn;
+        if (__dsqrt_rn(rzn) <= sc->thresh) { sc->status = FX_OK; sc->done = 1; }
+    }
+}
 
 #define CG_K 4
 #define CG_W 40
@@ -67,18 +126,38 @@ static cudaError_t cg_launch(bool pdl, void (*kern)(KArgs...), int grid, int blo
 template <int P, bool NEU>
 __global__ void __maxnreg__(P <= 2 ? 128 : P == 3 ? FX_K1_R : 255)
 k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict__ chi, const double* __restrict__ pin,
-                   const double* __restrict__ r, double* __restrict__ pout, double* __restrict__ q, ExGlobal ex, CgScal* sc) {
+                   const double* __restrict__ r, double* __restrict__ pout, double* __restrict__ q, CgRed red, CgScal* sc, int k) {
     __shared__ ExShared sh;
+    FX_PDL_SYNC();
+    if (*(volatile int*)&sc->done) return;
+    const int wpb = blockDim.x >> 5;
+    const long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
+    if (w < (long long)g.nstrip * g.nseg) {                          // the warp's first rows on their way to L2 while beta is formed
+        const int seg = (int)(w / g.nstrip), strip = (int)(w % g.nstrip);
+        int ci = strip * FX_STRIP - 1 + (threadIdx.x & 31);
+        ci = ci < 0 ? 0 : ci >= g.Nx ? g.Nx - 1 : ci;
+        const long long pitch = (long long)g.Nx * P;
+        int j = seg * g.rows_per_seg - 1;
+        if (j < 0) j = 0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d, ++j) {
+            if (j >= g.Ny) break;
+            const long long off = (long long)j * P * pitch + (long long)ci * P;
+#pragma unroll
+            for (int l = 0; l < P; ++l) {
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(pin + off + l * pitch));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(chi + off + l * pitch));
+                if (k > 0) asm volatile("prefetch.global.L2 [%0];" ::"l"(r + off + l * pitch));
+            }
+        }
+    }
+    double beta;
+    if (!cg_k1_scalars(&sh, red, sc, k, &beta)) return;
     ex_shared_init(&sh);
     CgAcc acc;
     acc.init();
-    FX_PDL_SYNC();                          // everything above overlaps the previous kernel's tail
-    if (*(volatile int*)&sc->done) return;
-    // first iteration: p = z was set up by the caller, copy it through; later: p = z + beta p with the beta K2 left.
-    // (sc->iters is bumped by this kernel's own finaliser, which runs after every CTA has started.)
-    const DgSrc src = {pin, r, pout, sc->beta, *(volatile int*)&sc->iters > 0};
-    const int wpb = blockDim.x >> 5;
-    const long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
+    // first iteration: p = z was set up by the caller, copy it through; later: p = z + beta p
+    const DgSrc src = {pin, r, pout, beta, k > 0};
     if (w < (long long)g.nstrip * g.nseg) {
         const int seg = (int)(w / g.nstrip), strip = (int)(w % g.nstrip);
         const int j0 = seg * g.rows_per_seg;
@@ -90,33 +169,28 @@ k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict_
     }
     FX_PDL_TRIGGER();
     acc.flush(&sh);
-    if (ex_block_finish(&sh, ex, 1, 1, &sc->pq) && threadIdx.x == 0) {
-        const double pq = sc->pq;
-        sc->iters += 1;
-        if (!(pq > 0.0) || isinf(pq)) { sc->status = FX_EBREAKDOWN; sc->done = 1; }
-        else sc->alpha = __ddiv_rn(sc->rz, pq);
-    }
+    ex_publish(&sh, red.pq(k), red.pqf(k), red.stats);
 }
 
 // K1 on the CTA-tile stencil (fx_dgt.cuh): rows of r, p_old and chi arrive by 2-D TMA, the direction update is formed in
 // shared memory, q = S p leaves through coalesced stores and every (p, q) pair enters the column thread's exact-dot bins.
 template <int P>
 struct CgtCfg {
+    static constexpr int NBX = P == 3 ? FX_K1T_NBX : DgtCfg<P>::NBX;      // x-blocks per tile
+    static constexpr int ND = FX_K1T_ND;                                  // exact-dot warps per CTA
+    static constexpr int NT = 32 * NBX * P + 32 * ND;
     static constexpr int MINB = P >= 4 ? 2 : 3;
-    static constexpr int REGS = P == 3 ? FX_K1T_R : (65536 / (MINB * DgtCfg<P>::NT)) / 8 * 8 > 255 ? 255 : (65536 / (MINB * DgtCfg<P>::NT)) / 8 * 8;
+    static constexpr int REGS = P == 3 ? FX_K1T_R : (65536 / (MINB * NT)) / 16 * 16 > 255 ? 255 : (65536 / (MINB * NT)) / 16 * 16;
 };
 template <int P, bool NEU>
-__global__ void __launch_bounds__(DgtCfg<P>::NT) __maxnreg__(CgtCfg<P>::REGS)
+__global__ void __launch_bounds__(CgtCfg<P>::NT) __maxnreg__(CgtCfg<P>::REGS)
 k_cgt_dir_apply_dot(const __grid_constant__ DgParams g, const __grid_constant__ DgtTile t, const __grid_constant__ CUtensorMap mp,
                     const __grid_constant__ CUtensorMap mph, const __grid_constant__ CUtensorMap mc, const __grid_constant__ CUtensorMap mch,
                     const __grid_constant__ CUtensorMap mr, const __grid_constant__ CUtensorMap mrh, double* __restrict__ pout,
-                    double* __restrict__ q, ExGlobal ex, CgScal* sc) {
+                    double* __restrict__ q, CgRed red, CgScal* sc, int k) {
     extern __shared__ __align__(128) double dgt_smem[];
     __shared__ ExShared sh;
     __shared__ __align__(8) unsigned long long bars[DGT_NS_K1];
-    ex_shared_init(&sh);
-    CgAcc acc;
-    acc.init();
     if (threadIdx.x == 0) {
         for (int s = 0; s < DGT_NS_K1; ++s) fx_mbar_init(fx_smem_addr(bars) + 8u * s, 1u);
         fx_mbar_fence_init();
@@ -125,17 +199,17 @@ k_cgt_dir_apply_dot(const __grid_constant__ DgParams g, const __grid_constant__ 
     __syncthreads();
     FX_PDL_SYNC();
     if (*(volatile int*)&sc->done) return;
-    const DgtDir dir = {&mr, &mrh, pout, sc->beta, *(volatile int*)&sc->iters > 0};
-    dgt_tile<P, DgtCfg<P>::NBX, DGT_NS_K1, true, true, NEU, CgAcc>(g, t, &mp, &mph, &mc, &mch, dir, q, bars, (int)(blockIdx.x % t.ntx),
-                                                                    (int)(blockIdx.x / t.ntx), &acc, &sh);
+    double beta;
+    if (!cg_k1_scalars(&sh, red, sc, k, &beta)) return;
+    ex_shared_init(&sh);
+    CgAcc acc;
+    acc.init();
+    const DgtDir dir = {&mr, &mrh, pout, beta, k > 0};
+    dgt_tile<P, CgtCfg<P>::NBX, DGT_NS_K1, true, true, NEU, CgAcc, CgtCfg<P>::ND>(g, t, &mp, &mph, &mc, &mch, dir, q, bars, (int)(blockIdx.x % t.ntx),
+                                                                                 (int)(blockIdx.x / t.ntx), &acc, &sh);
     FX_PDL_TRIGGER();
     acc.flush(&sh);
-    if (ex_block_finish(&sh, ex, 1, 1, &sc->pq) && threadIdx.x == 0) {
-        const double pq = sc->pq;
-        sc->iters += 1;
-        if (!(pq > 0.0) || isinf(pq)) { sc->status = FX_EBREAKDOWN; sc->done = 1; }
-        else sc->alpha = __ddiv_rn(sc->rz, pq);
-    }
+    ex_publish(&sh, red.pq(k), red.pqf(k), red.stats);
 }
 
 // launch state of the tile K1 for one solve: geometry and the tensor maps of p (both buffers), chi and r
@@ -154,8 +228,8 @@ static CgTile* fx_cg_tile(FxCtx* c) {              // (tensor maps are 64-byte a
 
 template <int P, bool NEU>
 static fx_status cgt_setup(FxCtx* c, const fx_grid* g, const double* chi, const double* r, const double* pb0, const double* pb1, CgTile* ct) {
-    constexpr int NBX = DgtCfg<P>::NBX;
-    typedef DgtGeom<P, NBX, 3, DGT_NS_K1> G;
+    constexpr int NBX = CgtCfg<P>::NBX;
+    typedef DgtGeom<P, NBX, 3, DGT_NS_K1, CgtCfg<P>::ND> G;
     const int occ = fx_func_occ(c, (const void*)k_cgt_dir_apply_dot<P, NEU>, G::NT, G::SMEM, true);
     fx_dgt_shape(c, g, NBX, c->num_sms * occ, &ct->t);
     ct->grid = ct->t.ntx * ct->t.nseg; ct->block = G::NT; ct->smem = G::SMEM;
@@ -205,16 +279,18 @@ __device__ __forceinline__ void cg_issue(double* buf, int stage, const double* c
 // K2: phi += alpha p; r -= alpha q; z = V o r; dot(r, z)
 template <int P>
 __global__ void __launch_bounds__(256, 3) k_cg_update(const __grid_constant__ DgParams g, const double* __restrict__ p,
-                                                      const double* __restrict__ q, double* phi, double* r, ExGlobal ex,
-                                                      CgScal* sc) {
+                                                      const double* __restrict__ q, double* phi, double* r, CgRed red,
+                                                      CgScal* sc, int k) {
     extern __shared__ __align__(16) double cg_buf[];
     __shared__ ExShared sh;
+    FX_PDL_SYNC();
+    if (*(volatile int*)&sc->done) return;
+    double alpha;
+    if (!cg_k2_scalars(&sh, red, sc, k, &alpha)) return;
+    const double nalpha = -alpha;
     ex_shared_init(&sh);
     CgAcc acc;
     acc.init();
-    FX_PDL_SYNC();
-    if (*(volatile int*)&sc->done) return;
-    const double alpha = sc->alpha, nalpha = -alpha;
     const int pitch = g.Nx * P, rows = g.Ny * P, bd = blockDim.x;
     const int cpr = (pitch + CG_U * bd - 1) / (CG_U * bd);
     const double* const arr[4] = {p, q, phi, r};
@@ -252,11 +328,7 @@ __global__ void __launch_bounds__(256, 3) k_cg_update(const __grid_constant__ Dg
     fx_cp_wait<0>();
     FX_PDL_TRIGGER();
     acc.flush(&sh);
-    if (ex_block_finish(&sh, ex, 1, 1, &sc->dot) && threadIdx.x == 0) {
-        const double rzn = sc->dot;
-        if (__dsqrt_rn(rzn) <= sc->thresh) { sc->rz = rzn; sc->status = FX_OK; sc->done = 1; }
-        else { sc->beta = __ddiv_rn(rzn, sc->rz); sc->rz = rzn; }
-    }
+    ex_publish(&sh, red.rz(k), red.rzf(k), red.stats);
 }
 
 // K2, fast path: all four vectors 16-byte aligned.  Linear tiles of 2*blockDim.x elements, one 16-byte vector per thread,
@@ -281,14 +353,11 @@ __device__ __forceinline__ void cg_update_pair(const DgParams& g, double alpha, 
 #define K2_STAGES 4
 template <int P>
 __global__ void __launch_bounds__(256, 3) k_cg_update_tma(const __grid_constant__ DgParams g, const double* __restrict__ p,
-                                                          const double* __restrict__ q, double* phi, double* r, ExGlobal ex,
-                                                          CgScal* sc) {
+                                                          const double* __restrict__ q, double* phi, double* r, CgRed red,
+                                                          CgScal* sc, int kit) {
     extern __shared__ __align__(128) double cg_buf[];
     __shared__ ExShared sh;
     __shared__ __align__(8) unsigned long long bars[2 * K2_STAGES];
-    ex_shared_init(&sh);
-    CgAcc acc;
-    acc.init();
     const int pitch = g.Nx * P, bd = blockDim.x, nwarp = bd >> 5;
     const long long n = (long long)pitch * g.Ny * P;
     const long long tile = 2ll * bd, nfull = n / tile;
@@ -302,7 +371,6 @@ __global__ void __launch_bounds__(256, 3) k_cg_update_tma(const __grid_constant_
     __syncthreads();
     FX_PDL_SYNC();                          // barriers are set up while the previous kernel drains
     if (*(volatile int*)&sc->done) return;
-    const double alpha = sc->alpha, nalpha = -alpha;
     // my full tiles: blockIdx.x, +G, ...  (count as a 32-bit number)
     const int mine = blockIdx.x < nfull ? (int)((nfull - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0;
     const long long step = (long long)gridDim.x * tile;
@@ -318,6 +386,17 @@ __global__ void __launch_bounds__(256, 3) k_cg_update_tma(const __grid_constant_
     };
     if (threadIdx.x == 0)
         for (int i = 0; i < K2_STAGES - 1 && i < mine; ++i) issue(i);
+    // alpha from the digits K1 left (every CTA rounds them itself) while the first tiles are on their way
+    double alpha;
+    if (!cg_k2_scalars(&sh, red, sc, kit, &alpha)) {
+        if (threadIdx.x == 0)                                        // (copies in flight into this CTA's shared memory must land first)
+            for (int i = 0; i < K2_STAGES - 1 && i < mine; ++i) fx_mbar_wait(full0 + 8u * i, 0u);
+        return;
+    }
+    const double nalpha = -alpha;
+    ex_shared_init(&sh);
+    CgAcc acc;
+    acc.init();
     long long i0 = (long long)blockIdx.x * tile + 2 * threadIdx.x;
     int col = (int)(i0 % pitch), l = (int)((i0 / pitch) % P), k = col % P;
     const int dcol = (int)(step % pitch), dl = (int)((step / pitch) % P), dk1 = dcol % P, dk2 = ((dcol % P) - (pitch % P) + P) % P;
@@ -367,11 +446,7 @@ __global__ void __launch_bounds__(256, 3) k_cg_update_tma(const __grid_constant_
     }
     FX_PDL_TRIGGER();
     acc.flush(&sh);
-    if (ex_block_finish(&sh, ex, 1, 1, &sc->dot) && threadIdx.x == 0) {
-        const double rzn = sc->dot;
-        if (__dsqrt_rn(rzn) <= sc->thresh) { sc->rz = rzn; sc->status = FX_OK; sc->done = 1; }
-        else { sc->beta = __ddiv_rn(rzn, sc->rz); sc->rz = rzn; }
-    }
+    ex_publish(&sh, red.rz(kit), red.rzf(kit), red.stats);
 }
 
 // ---- persistent driver for grids that fit in L2 --------------------------------------------------------
@@ -465,9 +540,6 @@ static fx_status cg_run_persistent(FxCtx* c, const fx_grid* g, DgParams dp, cons
     FX_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device));
     if (!coop) return FX_OK;
     occ = fx_func_occ(c, (const void*)k_cg_persistent<P>, 128, 0);
-    if (!c->cg_pdig) {
-        if (cudaMalloc(&c->cg_pdig, 4 * FX_NDIG * sizeof(fx_u64) + 64) != cudaSuccess) { fx_set_error("persistent CG scratch: %s", cudaGetErrorString(cudaGetLastError())); return FX_ENOMEM; }
-    }
     FX_CUDA(cudaMemsetAsync(c->cg_pdig, 0, 4 * FX_NDIG * sizeof(fx_u64) + 64, c->stream));
     fx_u64* pdig = (fx_u64*)c->cg_pdig;
     int* pflags = (int*)(pdig + 4 * FX_NDIG);
@@ -496,6 +568,9 @@ static fx_status cg_workspace(FxCtx* c, int64_t n) {
             fx_set_error("CG work space: %s", cudaGetErrorString(cudaGetLastError())); return FX_ENOMEM;
         }
         c->cg_cap = n;
+    }
+    if (!c->cg_pdig) {                                            // digit buffers of the loop's reductions: PQ[2], RZ[2], flags
+        if (cudaMalloc(&c->cg_pdig, 4 * FX_NDIG * sizeof(fx_u64) + 64) != cudaSuccess) { fx_set_error("CG digit buffers: %s", cudaGetErrorString(cudaGetLastError())); return FX_ENOMEM; }
     }
     if (!c->cg_scal) {
         if (cudaMalloc(&c->cg_scal, sizeof(CgScal)) != cudaSuccess || cudaMallocHost(&c->cg_scal_pinned, 2 * sizeof(CgScal)) != cudaSuccess ||
@@ -536,6 +611,7 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, const CgTile& ct
         if (c->launch[3][0]) nt = c->launch[3][0];
         lg = (int)nt;
     }
+    const CgRed red = {(fx_u64*)c->cg_pdig, (int*)((fx_u64*)c->cg_pdig + 4 * FX_NDIG), c->ex.stats};
     for (int i = 0; i < iters; ++i) {
         // p is double-buffered: iteration k reads buffer k & 1 and writes the other one
         const int k = first_index + i;
@@ -548,17 +624,21 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, const CgTile& ct
         const bool pdl = !ev && c->cg_pdl;                        // (profiling events between the kernels: plain launches)
         if (ct.on) {
             const int b = k & 1;
-            if (fx_dg_has_neumann(&dp)) cg_launch(pdl, k_cgt_dir_apply_dot<P, true>, ct.grid, ct.block, ct.smem, c->stream, dp, ct.t, ct.p[b], ct.ph[b], ct.c, ct.ch, ct.r, ct.rh, pout, q, c->ex, sc);
-            else cg_launch(pdl, k_cgt_dir_apply_dot<P, false>, ct.grid, ct.block, ct.smem, c->stream, dp, ct.t, ct.p[b], ct.ph[b], ct.c, ct.ch, ct.r, ct.rh, pout, q, c->ex, sc);
-        } else if (fx_dg_neu_variant(&dp, P)) cg_launch(pdl, k_cg_dir_apply_dot<P, true>, ag, ab, k1_smem, c->stream, dp, chi, pin, r, pout, q, c->ex, sc);
-        else cg_launch(pdl, k_cg_dir_apply_dot<P, false>, ag, ab, k1_smem, c->stream, dp, chi, pin, r, pout, q, c->ex, sc);
+            if (fx_dg_has_neumann(&dp)) cg_launch(pdl, k_cgt_dir_apply_dot<P, true>, ct.grid, ct.block, ct.smem, c->stream, dp, ct.t, ct.p[b], ct.ph[b], ct.c, ct.ch, ct.r, ct.rh, pout, q, red, sc, k);
+            else cg_launch(pdl, k_cgt_dir_apply_dot<P, false>, ct.grid, ct.block, ct.smem, c->stream, dp, ct.t, ct.p[b], ct.ph[b], ct.c, ct.ch, ct.r, ct.rh, pout, q, red, sc, k);
+        } else if (fx_dg_neu_variant(&dp, P)) cg_launch(pdl, k_cg_dir_apply_dot<P, true>, ag, ab, k1_smem, c->stream, dp, chi, pin, r, pout, q, red, sc, k);
+        else cg_launch(pdl, k_cg_dir_apply_dot<P, false>, ag, ab, k1_smem, c->stream, dp, chi, pin, r, pout, q, red, sc, k);
         if (ev) cudaEventRecord(ev[1], c->stream);
-        if (lin) cg_launch(pdl, k_cg_update_tma<P>, lg, eb, (size_t)K2_STAGES * 4 * 2 * eb * 8, c->stream, dp, (const double*)pout, (const double*)q, phi, r, c->ex, sc);
-        else cg_launch(pdl, k_cg_update<P>, eg, eb, (size_t)FX_STAGES * 4 * CG_U * eb * 8, c->stream, dp, (const double*)pout, (const double*)q, phi, r, c->ex, sc);
+        if (lin) cg_launch(pdl, k_cg_update_tma<P>, lg, eb, (size_t)K2_STAGES * 4 * 2 * eb * 8, c->stream, dp, (const double*)pout, (const double*)q, phi, r, red, sc, k);
+        else cg_launch(pdl, k_cg_update<P>, eg, eb, (size_t)FX_STAGES * 4 * CG_U * eb * 8, c->stream, dp, (const double*)pout, (const double*)q, phi, r, red, sc, k);
         if (ev) { cudaEventRecord(ev[2], c->stream); cudaEventRecord(ev[3], c->stream); }
         c->launches += 2;
     }
     if (c->prof_on) cudaEventRecord(c->prof_loop[1], c->stream);      // re-recorded after every batch: the last one stands
+    if (iters > 0) {                                                  // r.z of the batch's last iteration -> rz, convergence, for the host
+        k_cg_finish<<<1, 128, 0, c->stream>>>(red, sc, first_index + iters - 1);
+        c->launches++;
+    }
     FX_CUDA(cudaGetLastError());
     return FX_OK;
 }
@@ -703,7 +783,9 @@ extern "C" fx_status fx_cg_solve_ex(fx_ctx* c, const fx_grid* g, const double* c
             CgScal* hs = (CgScal*)c->cg_scal_pinned;
             memset(hs, 0, sizeof(*hs));
             hs->rz = rz; hs->bz = bz; hs->thresh = thresh; hs->status = FX_MAXIT;
+            hs->rzb[1] = rz;                                     // K1(0) takes r.z of the start residual from here
             FX_CUDA(cudaMemcpyAsync(sc, hs, sizeof(CgScal), cudaMemcpyHostToDevice, c->stream));
+            FX_CUDA(cudaMemsetAsync(c->cg_pdig, 0, 4 * FX_NDIG * sizeof(fx_u64) + 64, c->stream));
             FX_CUDA(cudaStreamSynchronize(c->stream));           // hs is reused as the read-back buffer
             // small grids (vectors resident in L2): the whole loop in one cooperative launch.  mode 1 = automatic,
             // 2 = never, 3 = whenever the device allows it (tests)

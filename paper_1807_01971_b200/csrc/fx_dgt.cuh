@@ -36,10 +36,16 @@
 #endif
 #define DGT_NS 4          // ring stages (cell rows resident or in flight per CTA) of the stand-alone apply
 #ifndef FX_K1T_NS
-#define FX_K1T_NS 3
+#define FX_K1T_NS 4
 #endif
 #ifndef FX_K1T_R
-#define FX_K1T_R 96
+#define FX_K1T_R 112
+#endif
+#ifndef FX_K1T_NBX
+#define FX_K1T_NBX 2
+#endif
+#ifndef FX_K1T_ND
+#define FX_K1T_ND 0
 #endif
 #define DGT_NS_K1 FX_K1T_NS   // ... of the fused CG kernel (three streams per stage)
 
@@ -57,7 +63,7 @@ struct DgtCfg {
     static constexpr int REGS = (65536 / (MINB * NT)) / 8 * 8 > 255 ? 255 : (65536 / (MINB * NT)) / 8 * 8;
 };
 
-template <int P, int NBX, int NSTR, int NS = DGT_NS>
+template <int P, int NBX, int NSTR, int NS = DGT_NS, int ND = 0>
 struct DgtGeom {
     static constexpr int TXM = FX_STRIP * NBX;                 // cells per tile at wb = 30
     static constexpr int SW = TXM * P;                         // doubles per image row of the tile proper (hand-off rows)
@@ -68,9 +74,10 @@ struct DgtGeom {
     static constexpr int WRAP_D = (P * HW * 8 + 127) / 128 * 16;
     static constexpr int STR_D = MAIN_D + 2 * WRAP_D;          // one stream of one stage: main box, left wrap, right wrap
     static constexpr int STG_D = NSTR * STR_D;
-    static constexpr int NT = 32 * NBX * P;
+    static constexpr int NTS = 32 * NBX * P;                    // stencil threads
+    static constexpr int NT = NTS + 32 * ND;                    // ... plus the exact-dot warps of the fused CG kernel
     static constexpr unsigned MAIN_BYTES = (unsigned)(P * BW * 8), WRAP_BYTES = (unsigned)(P * HW * 8);
-    static constexpr size_t SMEM = (size_t)NS * STG_D * 8 + (size_t)2 * P * SW * 16;
+    static constexpr size_t SMEM = (size_t)NS * STG_D * 8 + (size_t)2 * P * SW * 16 * (ND > 0 ? 2 : 1);
 };
 
 struct DgtTile {                 // launch geometry of the tile kernels (host: fx_dgt_shape)
@@ -174,11 +181,15 @@ struct DgtDir {
 // __syncthreads; after it one lane refills the stage that iteration released -- the warps take turns, so that none of
 // them is the straggler of every barrier.  Iterations 2 .. n-1 are "steady": no wall, no missing row, interior table --
 // they run from a branch-free body, two per loop trip with the carried row alternating between two register sets.
-template <int P, int NBX, int NS, bool FUSE, bool DIRF, bool NEU, class ACC>
+// ND > 0 (with FUSE): the accumulation is done by ND warps of their own.  The column threads hand every (p, q) pair over
+// through a second double-buffered shared-memory tile; the dot warps consume the pairs of iteration it-1 while the stencil
+// warps work on iteration it.  (With the accumulator inside the column threads -- 19 registers of state, 23 fp64 and ~15
+// other instructions per element inlined into the stencil code -- K1 spilled at 96 registers and ran 108-134 us.)
+template <int P, int NBX, int NS, bool FUSE, bool DIRF, bool NEU, class ACC, int ND = 0>
 __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, const CUtensorMap* mu, const CUtensorMap* muh,
                                          const CUtensorMap* mc, const CUtensorMap* mch, const DgtDir& dir, double* __restrict__ y,
                                          unsigned long long* bars, int tx, int seg, ACC* acc, ExShared* sh) {
-    typedef DgtGeom<P, NBX, DIRF ? 3 : 2, NS> G;
+    typedef DgtGeom<P, NBX, DIRF ? 3 : 2, NS, ND> G;
     constexpr int NW = NBX * P;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int Nx = g.Nx, Ny = g.Ny, pitch = Nx * P;
@@ -195,6 +206,7 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
     double2* const dgt_h = reinterpret_cast<double2*>(dgt_smem + (size_t)NS * G::STG_D);
     const unsigned sbase = fx_smem_addr(dgt_smem), full0 = fx_smem_addr(bars);
     constexpr int HBUF = P * G::SW;                                  // double2 per hand-off buffer
+    double2* const dgt_pq = dgt_h + 2 * HBUF;                        // ND > 0: the (p, q) pairs for the dot warps, double2[2][P][SW]
     const int cR = (i0 + txc < Nx) ? i0 + txc : Nx;                  // the cell after the tile's last one
     const bool wrapL = i0 == 0 && !wallx, wrapR = cR >= Nx && !wallx;    // periodic edge tiles: the halo cell is a box of its own
 
@@ -264,6 +276,37 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
     const bool upd = DIRF && dir.upd;
     const double beta = DIRF ? dir.beta : 0.0;
     auto pnew = [&](double po, double rr, double v) { return upd ? __fma_rn(1.0, __dmul_rn(v, rr), __dmul_rn(beta, po)) : po; };
+
+    if (ND > 0 && FUSE && warp >= NW) {                              // ---- the exact-dot warps (see above) ----------------------
+        const int dt = tid - NW * 32;
+        int ncol = txc * P;
+        if ((long long)i0 * P + ncol > pitch) ncol = pitch - i0 * P;
+        if (ncol < 0) ncol = 0;
+        auto consume = [&](int buf) {
+            const double2* const pq = dgt_pq + buf * HBUF;
+#pragma unroll 1
+            for (int c0 = 0; c0 < ncol; c0 += ND * 32) {
+                const int c = c0 + dt;
+                const bool in = c < ncol;
+                double xs[P], ys[P];
+                bool act[P];
+#pragma unroll
+                for (int l = 0; l < P; ++l) {
+                    const double2 v = in ? pq[l * G::SW + c] : make_double2(0.0, 0.0);
+                    xs[l] = v.x; ys[l] = v.y; act[l] = in;
+                }
+                if (c0 + ND * 32 <= ncol) acc->template add_all<P>(xs, ys, sh);
+                else acc->template add<P>(xs, ys, act, sh);
+            }
+        };
+#pragma unroll 1
+        for (int it = 0; it <= n; ++it) {                             // the pairs of iteration it-1 while the stencil warps run iteration it
+            if (it >= 2) consume((it - 1) & 1);
+            __syncthreads();
+        }
+        consume(n & 1);
+        return;
+    }
 
     double ua[P], ca[P], ub[P], cb[P];                                // the carried cell row: alternating register sets
     double tLy = 0.0, tRyp = 0.0, tByp = 0.0;
@@ -365,7 +408,13 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
                     for (int l = 0; l < P; ++l) yp[l * prow] = o[l];
                 }
                 yp += P * prow;
-                if (FUSE) {
+                if (FUSE && ND > 0) {                                 // hand the pairs to the dot warps
+                    if (tid < G::SW) {
+                        double2* const pq = dgt_pq + (it & 1) * HBUF + ycol;
+#pragma unroll
+                        for (int l = 0; l < P; ++l) pq[l * G::SW] = make_double2(uc[l], o[l]);
+                    }
+                } else if (FUSE) {
                     double xs[P], ys[P];
                     bool act[P];
 #pragma unroll

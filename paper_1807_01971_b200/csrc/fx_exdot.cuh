@@ -444,6 +444,35 @@ __device__ inline double ex_round_digits_shared(ExShared* sh, int flags) {
     return ex_round(sh->lim, flags, sh->dig, la, bb);
 }
 
+// The two halves of a reduction that is finished by its CONSUMER (the fused CG kernels): a kernel's CTAs
+// only add their digits to a global digit buffer (ex_publish: no ticket, no last-CTA finaliser, no tail), and every CTA
+// of the NEXT kernel fetches the merged digits and normalises and rounds them itself (ex_fetch_round) while its first
+// tiles are already in flight -- all CTAs hold the same bits.  gdig/gflags must be zero before the producing kernel.
+__device__ __forceinline__ void ex_publish(ExShared* sh, fx_u64* gdig, int* gflags, fx_u64* gstats) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) {
+        const fx_u64 v = sh->dig[i];
+        if (v) atomicAdd(&gdig[i], v);
+    }
+    if (threadIdx.x == 0 && sh->flags) atomicOr(gflags, sh->flags);
+    if (threadIdx.x < 4 && sh->stat[threadIdx.x]) atomicAdd(&gstats[threadIdx.x], (fx_u64)sh->stat[threadIdx.x]);
+}
+__device__ inline double ex_round_digits_shared(ExShared* sh, int flags);
+__device__ __forceinline__ double ex_fetch_round(ExShared* sh, const fx_u64* gdig, const int* gflags) {
+    if (threadIdx.x == 0) { sh->dlo = FX_NDIG; sh->dhi = -1; }
+    __syncthreads();
+    if (threadIdx.x == blockDim.x - 1) sh->flags = __ldcg(gflags);  // (in the same round trip as the digits)
+    for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) {
+        const fx_u64 v = __ldcg(&gdig[i]);
+        sh->dig[i] = v;
+        if (v) { atomicMin(&sh->dlo, i); atomicMax(&sh->dhi, i); }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) sh->res = ex_round_digits_shared(sh, sh->flags);
+    __syncthreads();
+    return sh->res;
+}
+
 // Grid-wide exact reduction inside a cooperative (persistent) kernel: every CTA adds its digits to gdig, the grid
 // synchronises, and EVERY CTA normalises and rounds the merged digits itself, so that all of them hold the same bits
 // without a second synchronisation.  gdig/gflags must be zero on entry; the caller re-zeroes them one phase later

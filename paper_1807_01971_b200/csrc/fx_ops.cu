@@ -551,7 +551,10 @@ extern "C" fx_status fx_exdot_digits(const double* x, const double* y, int64_t n
 // dG elliptic apply  (fx_dg.cuh / DESIGN.md 6.2).  HBM roofline: 24 B per unknown.
 // ------------------------------------------------------------------------------------------------------------
 
-struct NoAcc { template <int U> __device__ void add(const double (&)[U], const double (&)[U], const bool (&)[U], ExShared*) {} };
+struct NoAcc {
+    template <int U> __device__ void add(const double (&)[U], const double (&)[U], const bool (&)[U], ExShared*) {}
+    template <int U> __device__ void add_all(const double (&)[U], const double (&)[U], ExShared*) {}
+};
 
 #ifndef FX_AP_R
 #define FX_AP_R 168      // registers per thread / warps per CTA of k_dg_apply<3>

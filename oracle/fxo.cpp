@@ -423,8 +423,10 @@ extern "C" int fxo_dg_matrix_1d(int32_t N, int32_t P, double h, int32_t bc, doub
 // y = S x (normed==0) or A x = V o (S x) (normed==1), every product/sum in q128, rounded once at
 // the end; scale = (|Fx^T||W chi||Fx| + |Fy^T||W chi||Fy| + |J|)|x| evaluated the same way.
 // Dense 1-D matrices: meant for grids up to a few hundred nodes per direction.
-extern "C" int fxo_dg_apply_definition(const fxo_grid* g, const double* chi, const double* x, int32_t normed,
-                                       double* y, double* scale) {
+// (zfac: 1 for the 2-D operator; the plane weight hz of a 3-D product grid for its symmetric form, section 8 below --
+// a factor of exactly 1 changes no bit of the 2-D results)
+static int apply_definition_q(const fxo_grid* g, const double* chi, const double* x, int32_t normed, q128 zfac,
+                              double* y, double* scale) {
     if (!grid_ok(g)) return -1;
     const int P = g->P, Nx = g->Nx, Ny = g->Ny, nx = Nx * P, ny = Ny * P;
     RefElem e; ref_elem(P, e);
@@ -460,11 +462,15 @@ extern "C" int fxo_dg_apply_definition(const fxo_grid* g, const double* chi, con
         out[at(r, c)] = s; aout[at(r, c)] = a;
     }
     for (int r = 0; r < ny; ++r) for (int c = 0; c < nx; ++c) {
-        q128 v = normed ? 1 / (wx(c) * wy(r)) : (q128)1;
+        q128 v = (normed ? 1 / (wx(c) * wy(r)) : (q128)1) * zfac;
         if (y) y[at(r, c)] = (double)(v * out[at(r, c)]);
         if (scale) scale[at(r, c)] = (double)(v * aout[at(r, c)]);
     }
     return 0;
+}
+extern "C" int fxo_dg_apply_definition(const fxo_grid* g, const double* chi, const double* x, int32_t normed,
+                                       double* y, double* scale) {
+    return apply_definition_q(g, chi, x, normed, (q128)1, y, scale);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -769,6 +775,106 @@ extern "C" int fxo_cg_solve(const fxo_grid* g, const double* chi, const double* 
         status = FXO_MAXIT;
         for (it = 1; it <= maxit; ++it) {
             apply_canonical(g, c, chi, p.data(), 0, q.data());
+            double pq = fxo_exdot(p.data(), q.data(), n);
+            if (!(pq > 0.0) || !std::isfinite(pq)) { status = FXO_EBREAKDOWN; break; }
+            double alpha = rz / pq;
+            fxo_axpby(alpha, p.data(), 1.0, phi, n);
+            fxo_axpby(-alpha, q.data(), 1.0, r.data(), n);
+            fxo_pointwise_dot(1.0, V.data(), r.data(), 0.0, z.data(), n);
+            double rz_new = fxo_exdot(r.data(), z.data(), n);
+            if (std::sqrt(rz_new) <= thresh) { rz = rz_new; status = FXO_OK; break; }
+            double beta = rz_new / rz;
+            fxo_axpby(1.0, z.data(), beta, p.data(), n);
+            rz = rz_new;
+        }
+        if (it > maxit) it = maxit;
+    }
+    if (info) { info->iterations = it; info->status = status; info->rel_residual = std::sqrt(rz) / std::sqrt(bz); }
+    return status;
+}
+
+// ------------------------------------------------------------------------------------------------
+// 8. 3-D product grids.  The paper's applications are "2D/3D drift-/gyro-fluid simulations"
+//     with derivatives "on product spaces"; its elliptic equation is the PERPENDICULAR one,
+//    div(chi grad_perp phi) = rho (Eq. 1c).  Reading DESIGN.md Q24: a 3-D product grid is
+//    Nz planes of the 2-D grid with one node per plane in z (cell height hz = lz/Nz); a vector stores
+//    plane after plane (idx3 = p*n2 + idx2); the operator acts in every plane and the planes meet only
+//    in the dot products.  Weights (the volume form of the product space): W3 = RN(hz*W2), V3 = RN(1/W3).
+//    Symmetric form S3 x = RN(hz * (S2 x_plane)); normed form A3 x = A2 x_plane (V3 o S3 = V2 o S2).
+// ------------------------------------------------------------------------------------------------
+struct fxo_grid3 { int32_t Nx, Ny, Nz, P; double lx, ly, lz; int32_t bcx, bcy; };
+static bool grid3_ok(const fxo_grid3* g, fxo_grid* p) {
+    if (!g || g->Nz < 1 || !(g->lz > 0)) return false;
+    p->Nx = g->Nx; p->Ny = g->Ny; p->P = g->P; p->lx = g->lx; p->ly = g->ly; p->bcx = g->bcx; p->bcy = g->bcy;
+    return grid_ok(p) != 0;
+}
+
+extern "C" int fxo_dg3_weights(const fxo_grid3* g, double* W, double* V) {
+    fxo_grid p;
+    if (!grid3_ok(g, &p)) return -1;
+    const int64_t n2 = (int64_t)p.Nx * p.Ny * p.P * p.P;
+    std::vector<double> W2(n2);
+    fxo_dg_weights(&p, W2.data(), nullptr);
+    const double hz = g->lz / g->Nz;
+    for (int z = 0; z < g->Nz; ++z) for (int64_t i = 0; i < n2; ++i) {
+        volatile double w = hz * W2[i];
+        if (W) W[z * n2 + i] = w;
+        if (V) V[z * n2 + i] = 1.0 / w;
+    }
+    return 0;
+}
+
+extern "C" int fxo_dg3_apply_canonical(const fxo_grid3* g, const double* chi, const double* x, int32_t normed, double* y) {
+    fxo_grid p;
+    if (!grid3_ok(g, &p)) return -1;
+    const int64_t n2 = (int64_t)p.Nx * p.Ny * p.P * p.P;
+    const double hz = g->lz / g->Nz;
+    for (int z = 0; z < g->Nz; ++z) {
+        fxo_dg_apply_canonical(&p, chi + z * n2, x + z * n2, normed, y + z * n2);
+        if (!normed) for (int64_t i = 0; i < n2; ++i) { volatile double v = hz * y[z * n2 + i]; y[z * n2 + i] = v; }
+    }
+    return 0;
+}
+
+extern "C" int fxo_dg3_apply_definition(const fxo_grid3* g, const double* chi, const double* x, int32_t normed, double* y, double* scale) {
+    fxo_grid p;
+    if (!grid3_ok(g, &p)) return -1;
+    const int64_t n2 = (int64_t)p.Nx * p.Ny * p.P * p.P;
+    const q128 hz = (q128)g->lz / g->Nz;
+    for (int z = 0; z < g->Nz; ++z)
+        apply_definition_q(&p, chi + z * n2, x + z * n2, normed, normed ? (q128)1 : hz, y ? y + z * n2 : nullptr, scale ? scale + z * n2 : nullptr);
+    return 0;
+}
+
+// PCG of section 7 with the 3-D primitives: one system over all planes (the dots are global).
+extern "C" int fxo_cg3_solve(const fxo_grid3* g, const double* chi, const double* rho, double* phi,
+                             double tol, int32_t maxit, fxo_cg_info* info) {
+    fxo_grid pg;
+    if (!grid3_ok(g, &pg) || maxit < 0 || !(tol >= 0)) return FXO_EINVAL;
+    const int64_t n = (int64_t)pg.Nx * pg.Ny * pg.P * pg.P * g->Nz;
+    std::vector<double> W(n), V(n), rhs(n), r(n), z(n), p(n), q(n);
+    fxo_dg3_weights(g, W.data(), V.data());
+    fxo_pointwise_dot(-1.0, W.data(), rho, 0.0, rhs.data(), n);
+    fxo_dg3_apply_canonical(g, chi, phi, 0, q.data());
+    r = rhs;
+    fxo_axpby(-1.0, q.data(), 1.0, r.data(), n);
+    fxo_pointwise_dot(1.0, V.data(), rhs.data(), 0.0, z.data(), n);
+    double bz = fxo_exdot(rhs.data(), z.data(), n);
+    int it = 0, status = FXO_OK;
+    double rz = 0;
+    if (bz == 0.0) {
+        for (int64_t i = 0; i < n; ++i) phi[i] = 0.0;
+        if (info) { info->iterations = 0; info->status = FXO_OK; info->rel_residual = 0.0; }
+        return FXO_OK;
+    }
+    fxo_pointwise_dot(1.0, V.data(), r.data(), 0.0, z.data(), n);
+    rz = fxo_exdot(r.data(), z.data(), n);
+    p = z;
+    double thresh = tol * std::sqrt(bz);
+    if (!(std::sqrt(rz) <= thresh)) {
+        status = FXO_MAXIT;
+        for (it = 1; it <= maxit; ++it) {
+            fxo_dg3_apply_canonical(g, chi, p.data(), 0, q.data());
             double pq = fxo_exdot(p.data(), q.data(), n);
             if (!(pq > 0.0) || !std::isfinite(pq)) { status = FXO_EBREAKDOWN; break; }
             double alpha = rz / pq;

@@ -30,6 +30,20 @@ class Grid(C.Structure):
         return (self.Ny * self.P, self.Nx * self.P)
 
 
+class Grid3(C.Structure):
+    """3-D product grid (Q24): Nz planes of the 2-D grid, one node per plane in z"""
+    _fields_ = [("Nx", C.c_int32), ("Ny", C.c_int32), ("Nz", C.c_int32), ("P", C.c_int32),
+                ("lx", C.c_double), ("ly", C.c_double), ("lz", C.c_double), ("bcx", C.c_int32), ("bcy", C.c_int32)]
+
+    @property
+    def n(self):
+        return self.Nx * self.Ny * self.Nz * self.P * self.P
+
+    @property
+    def plane(self):
+        return Grid(self.Nx, self.Ny, self.P, self.lx, self.ly, self.bcx, self.bcy)
+
+
 class CGInfo(C.Structure):
     _fields_ = [("iterations", C.c_int32), ("status", C.c_int32), ("rel_residual", C.c_double)]
 
@@ -99,6 +113,15 @@ def lib():
         L.fxo_arakawa.argtypes = [gp, dp, dp, dp]
         L.fxo_cg_solve.restype = C.c_int
         L.fxo_cg_solve.argtypes = [gp, dp, dp, dp, C.c_double, C.c_int32, C.POINTER(CGInfo)]
+        g3 = C.POINTER(Grid3)
+        L.fxo_dg3_weights.restype = C.c_int
+        L.fxo_dg3_weights.argtypes = [g3, dp, dp]
+        L.fxo_dg3_apply_canonical.restype = C.c_int
+        L.fxo_dg3_apply_canonical.argtypes = [g3, dp, dp, C.c_int32, dp]
+        L.fxo_dg3_apply_definition.restype = C.c_int
+        L.fxo_dg3_apply_definition.argtypes = [g3, dp, dp, C.c_int32, dp, dp]
+        L.fxo_cg3_solve.restype = C.c_int
+        L.fxo_cg3_solve.argtypes = [g3, dp, dp, dp, C.c_double, C.c_int32, C.POINTER(CGInfo)]
         _lib = L
     return _lib
 
@@ -297,4 +320,36 @@ def cg_solve(g, chi, rho, phi0, tol, maxit):
     assert chi.size == g.n and rho.size == g.n and phi.size == g.n
     info = CGInfo()
     lib().fxo_cg_solve(C.byref(g), _p(chi), _p(rho), _p(phi), tol, maxit, C.byref(info))
+    return phi, info
+
+
+# ---- 3-D product grids (Q24) ----------------------------------------------------------------------------
+def dg3_weights(g):
+    W = np.empty(g.n); V = np.empty(g.n)
+    assert lib().fxo_dg3_weights(C.byref(g), _p(W), _p(V)) == 0
+    return W, V
+
+
+def dg3_apply_canonical(g, chi, x, normed=False):
+    chi, x = _f64(chi).ravel(), _f64(x).ravel()
+    assert chi.size == x.size == g.n
+    y = np.empty(g.n)
+    assert lib().fxo_dg3_apply_canonical(C.byref(g), _p(chi), _p(x), 1 if normed else 0, _p(y)) == 0
+    return y
+
+
+def dg3_apply_definition(g, chi, x, normed=False):
+    chi, x = _f64(chi).ravel(), _f64(x).ravel()
+    assert chi.size == x.size == g.n
+    y = np.empty(g.n); sc = np.empty(g.n)
+    assert lib().fxo_dg3_apply_definition(C.byref(g), _p(chi), _p(x), 1 if normed else 0, _p(y), _p(sc)) == 0
+    return y, sc
+
+
+def cg3_solve(g, chi, rho, phi0, tol, maxit):
+    chi, rho = _f64(chi).ravel(), _f64(rho).ravel()
+    phi = np.array(phi0, dtype=np.float64).ravel().copy()
+    assert chi.size == rho.size == phi.size == g.n
+    info = CGInfo()
+    lib().fxo_cg3_solve(C.byref(g), _p(chi), _p(rho), _p(phi), float(tol), int(maxit), C.byref(info))
     return phi, info

@@ -91,6 +91,12 @@ __global__ void __launch_bounds__(128) k_cg_finish(CgRed red, CgScal* sc, int k)
 #define CG_K 4
 #define CG_W 40
 typedef ExAcc<CG_K, CG_W> CgAcc;
+#ifndef FX_K1_K
+#define FX_K1_K 4
+#define FX_K1_WB 40
+#define FX_K1_KL 0
+#endif
+typedef ExAcc<FX_K1_K, FX_K1_WB, FX_K1_KL> K1Acc;      // the accumulator of p.q inside the stencil kernel K1
 
 // Programmatic dependent launch (optional, FX_PDL=1): K1 and K2 of the fused loop are launched with programmatic stream
 // serialisation, so a kernel's CTAs are scheduled as soon as the previous kernel's CTAs leave the SMs, set up their
@@ -154,7 +160,7 @@ k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict_
     double beta;
     if (!cg_k1_scalars(&sh, red, sc, k, &beta)) return;
     ex_shared_init(&sh);
-    CgAcc acc;
+    K1Acc acc;
     acc.init();
     // first iteration: p = z was set up by the caller, copy it through; later: p = z + beta p
     const DgSrc src = {pin, r, pout, beta, k > 0};
@@ -164,8 +170,8 @@ k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict_
         int j1 = j0 + g.rows_per_seg;
         if (j1 > g.Ny) j1 = g.Ny;
         extern __shared__ __align__(16) double dg_smem[];
-        if (P <= 3 && g.smr) dg_warp_strip<P, true, true, true, NEU, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, dg_smem + (size_t)(threadIdx.x >> 5) * 8 * P * P * 32);
-        else dg_warp_strip<P, true, true, false, NEU, CgAcc>(g, chi, src, q, strip, j0, j1, &acc, &sh, nullptr);
+        if (P <= 3 && g.smr) dg_warp_strip<P, true, true, true, NEU, K1Acc>(g, chi, src, q, strip, j0, j1, &acc, &sh, dg_smem + (size_t)(threadIdx.x >> 5) * 8 * P * P * 32);
+        else dg_warp_strip<P, true, true, false, NEU, K1Acc>(g, chi, src, q, strip, j0, j1, &acc, &sh, nullptr);
     }
     FX_PDL_TRIGGER();
     acc.flush(&sh);

@@ -178,6 +178,27 @@ fx_status fx_dg_weights_ex(fx_ctx* ctx, const fx_grid* grid, double* w_dev, doub
  * out_host: host double[5*P + 4*P*P] = xi,w,L,R,B (P each) then T0,T0L,WW,D (P*P each, row-major).  No GPU.   */
 fx_status fx_dg_tables(int32_t P, double* out_host);
 
+/* ---- 3-D product grids (D:Q24) -----------------------------------------------------------------------------
+ * The paper's applications are "2D/3D drift-/gyro-fluid simulations" with derivatives "on product spaces";
+ * its elliptic equation is the perpendicular one, div(chi grad_perp phi) = rho (Eq. 1c).  Reading D:Q24: Nz planes
+ * of the 2-D grid with one node per plane in z (cell height hz = lz/Nz).  A vector stores plane after plane
+ * (idx3 = plane * P*P*Nx*Ny + idx2); the operator acts in every plane, the planes meet in the dot products of CG.  Weights (the
+ * volume form): W3 = RN(hz * W2), V3 = RN(1/W3).  sym != 0: y = S3 x = RN(hz * (S2 x_plane)); sym == 0: y = A3 x = A2 x_plane.   */
+typedef struct {
+    int32_t Nx, Ny, Nz, P;
+    double lx, ly, lz;
+    int32_t bcx, bcy;      /* fx_bc of the x and y directions (z carries no derivative) */
+} fx_grid3;
+fx_status fx_dg3_elliptic_apply(const fx_grid3* grid, const double* chi_dev, const double* x_dev, double* y_dev, int32_t sym);
+fx_status fx_dg3_elliptic_apply_ex(fx_ctx* ctx, const fx_grid3* grid, const double* chi_dev, const double* x_dev, double* y_dev, int32_t sym);
+fx_status fx_dg3_weights(const fx_grid3* grid, double* w_dev, double* v_dev);
+fx_status fx_dg3_weights_ex(fx_ctx* ctx, const fx_grid3* grid, double* w_dev, double* v_dev);
+/* fx_cg_solve on the product grid: one system over all planes (S3 phi = W3 o (-rho), preconditioner V3, global exact dots).  */
+fx_status fx_cg3_solve(const fx_grid3* grid, const double* chi_dev, const double* rho_dev, double* phi_dev,
+                       double tol, int32_t maxit, fx_cg_info* info);
+fx_status fx_cg3_solve_ex(fx_ctx* ctx, const fx_grid3* grid, const double* chi_dev, const double* rho_dev, double* phi_dev,
+                          double tol, int32_t maxit, fx_cg_info* info);
+
 /* ---- stand-alone dG derivatives: the paper's "dxdy" primitive (P:240, P:321 / Table 3; D:6.7, Q21) -----------------
  * y <- alpha * M x + beta * y (beta == 0: y is not read), M = d/dx (direction 0) or d/dy (direction 1) of the grid with its
  * boundary condition in that direction; flux 0 = forward (the F of the elliptic operator), 1 = backward (-W^-1 F^T W),

@@ -25,6 +25,16 @@ class Grid(C.Structure):
         return self.Nx * self.Ny * self.P * self.P
 
 
+class Grid3(C.Structure):
+    """fx_grid3: 3-D product grid, Nz planes of the 2-D grid with one node per plane in z (include/fx.h; Q24)."""
+    _fields_ = [("Nx", C.c_int32), ("Ny", C.c_int32), ("Nz", C.c_int32), ("P", C.c_int32),
+                ("lx", C.c_double), ("ly", C.c_double), ("lz", C.c_double), ("bcx", C.c_int32), ("bcy", C.c_int32)]
+
+    @property
+    def n(self):
+        return self.Nx * self.Ny * self.Nz * self.P * self.P
+
+
 class CGInfo(C.Structure):
     _fields_ = [("iterations", C.c_int32), ("status", C.c_int32), ("rel_residual", C.c_double)]
 
@@ -68,11 +78,14 @@ _SIGNATURES = {
     "fx_time_primitive": (C.c_int, [C.c_int32, C.POINTER(Grid), _vp, _vp, _vp, C.c_int64, C.c_int32, _dp]),
     "fx_launch_count": (C.c_int64, []),
     "fx_exdot_stats": (C.c_int, [_vp, C.c_int32]),
+    "fx_dg3_elliptic_apply": (C.c_int, [C.POINTER(Grid3), _vp, _vp, _vp, C.c_int32]),
+    "fx_dg3_weights": (C.c_int, [C.POINTER(Grid3), _vp, _vp]),
+    "fx_cg3_solve": (C.c_int, [C.POINTER(Grid3), _vp, _vp, _vp, C.c_double, C.c_int32, C.POINTER(CGInfo)]),
     "fx_create": (C.c_int, [C.POINTER(_vp), C.c_int32, _vp]),
     "fx_destroy": (None, [_vp]),
 }
 # the context forms: NAME_ex(ctx, <the plain call's arguments> [, result_host for the value-returning reductions])
-for _n in ("fx_exdot_stats", "fx_set_stream", "fx_set_launch", "fx_set_cg_fused", "fx_set_dg_path", "fx_exdot_async", "fx_exdot_digits", "fx_axpby",
+for _n in ("fx_dg3_elliptic_apply", "fx_dg3_weights", "fx_cg3_solve", "fx_exdot_stats", "fx_set_stream", "fx_set_launch", "fx_set_cg_fused", "fx_set_dg_path", "fx_exdot_async", "fx_exdot_digits", "fx_axpby",
            "fx_pointwise_dot", "fx_pointwise_dot2", "fx_arakawa", "fx_dg_elliptic_apply", "fx_dg_elliptic_apply_sym", "fx_dg_weights",
            "fx_dg_derivative", "fx_cg_solve", "fx_cg_solve_host", "fx_cg_profile", "fx_cg_last_profile", "fx_time_primitive"):
     _SIGNATURES[_n + "_ex"] = (C.c_int, [_vp] + _SIGNATURES[_n][1])
@@ -336,6 +349,29 @@ def dg_elliptic_apply(grid, chi, x, y, sym=False):
     fn = lib().fx_dg_elliptic_apply_sym if sym else lib().fx_dg_elliptic_apply
     _check(fn(C.byref(grid), _ptr(chi, grid.n), _ptr(x, grid.n), _ptr(y, grid.n)), "fx_dg_elliptic_apply")
     return y
+
+
+def make_grid3(Nx, Ny, Nz, P, lx, ly, lz, bcx, bcy):
+    return Grid3(int(Nx), int(Ny), int(Nz), int(P), float(lx), float(ly), float(lz), int(bcx), int(bcy))
+
+
+def dg3_elliptic_apply(grid, chi, x, y, sym=False):
+    """3-D product grid (fx.h): y = A3 x, or S3 x = hz * S2 x plane by plane with sym=True"""
+    _use_torch_stream()
+    _check(lib().fx_dg3_elliptic_apply(C.byref(grid), _ptr(chi, grid.n), _ptr(x, grid.n), _ptr(y, grid.n), 1 if sym else 0), "fx_dg3_elliptic_apply")
+
+
+def dg3_weights(grid, w=None, v=None):
+    _use_torch_stream()
+    _check(lib().fx_dg3_weights(C.byref(grid), _ptr(w, grid.n) if w is not None else None, _ptr(v, grid.n) if v is not None else None), "fx_dg3_weights")
+
+
+def cg3_solve(grid, chi, rho, phi, tol, maxit):
+    _use_torch_stream()
+    info = CGInfo()
+    rc = lib().fx_cg3_solve(C.byref(grid), _ptr(chi, grid.n), _ptr(rho, grid.n), _ptr(phi, grid.n), float(tol), int(maxit), C.byref(info))
+    _check(rc, "fx_cg3_solve")
+    return info
 
 
 def dg_weights(grid, w=None, v=None):

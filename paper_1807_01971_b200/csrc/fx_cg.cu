@@ -137,8 +137,15 @@ k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict_
     FX_PDL_SYNC();
     if (*(volatile int*)&sc->done) return;
     const int wpb = blockDim.x >> 5;
-    const long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
-    if (w < (long long)g.nstrip * g.nseg) {                          // the warp's first rows on their way to L2 while beta is formed
+    long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
+    const long long per = (long long)g.nstrip * g.nseg;             // warps per plane (3-D product grid: planes stacked in the vectors)
+    const bool mine = w < per * g.Nz;
+    if (mine) {
+        const long long zoff = (w / per) * ((long long)g.Nx * g.Ny * P * P);
+        w %= per;
+        chi += zoff; pin += zoff; r += zoff; pout += zoff; q += zoff;
+    }
+    if (mine) {                                                      // the warp's first rows on their way to L2 while beta is formed
         const int seg = (int)(w / g.nstrip), strip = (int)(w % g.nstrip);
         int ci = strip * FX_STRIP - 1 + (threadIdx.x & 31);
         ci = ci < 0 ? 0 : ci >= g.Nx ? g.Nx - 1 : ci;
@@ -164,7 +171,7 @@ k_cg_dir_apply_dot(const __grid_constant__ DgParams g, const double* __restrict_
     acc.init();
     // first iteration: p = z was set up by the caller, copy it through; later: p = z + beta p
     const DgSrc src = {pin, r, pout, beta, k > 0};
-    if (w < (long long)g.nstrip * g.nseg) {
+    if (mine) {
         const int seg = (int)(w / g.nstrip), strip = (int)(w % g.nstrip);
         const int j0 = seg * g.rows_per_seg;
         int j1 = j0 + g.rows_per_seg;
@@ -211,8 +218,9 @@ k_cgt_dir_apply_dot(const __grid_constant__ DgParams g, const __grid_constant__ 
     CgAcc acc;
     acc.init();
     const DgtDir dir = {&mr, &mrh, pout, beta, k > 0};
-    dgt_tile<P, CgtCfg<P>::NBX, DGT_NS_K1, true, true, NEU, CgAcc, CgtCfg<P>::ND>(g, t, &mp, &mph, &mc, &mch, dir, q, bars, (int)(blockIdx.x % t.ntx),
-                                                                                 (int)(blockIdx.x / t.ntx), &acc, &sh);
+    const int per = t.ntx * t.nseg, rem = (int)(blockIdx.x % per);
+    dgt_tile<P, CgtCfg<P>::NBX, DGT_NS_K1, true, true, NEU, CgAcc, CgtCfg<P>::ND>(g, t, &mp, &mph, &mc, &mch, dir, q, bars, rem % t.ntx, rem / t.ntx,
+                                                                                 (int)(blockIdx.x / per), &acc, &sh);
     FX_PDL_TRIGGER();
     acc.flush(&sh);
     ex_publish(&sh, red.pq(k), red.pqf(k), red.stats);
@@ -233,13 +241,13 @@ static CgTile* fx_cg_tile(FxCtx* c) {              // (tensor maps are 64-byte a
 }
 
 template <int P, bool NEU>
-static fx_status cgt_setup(FxCtx* c, const fx_grid* g, const double* chi, const double* r, const double* pb0, const double* pb1, CgTile* ct) {
+static fx_status cgt_setup(FxCtx* c, const fx_grid* g, int Nz, const double* chi, const double* r, const double* pb0, const double* pb1, CgTile* ct) {
     constexpr int NBX = CgtCfg<P>::NBX;
     typedef DgtGeom<P, NBX, 3, DGT_NS_K1, CgtCfg<P>::ND> G;
     const int occ = fx_func_occ(c, (const void*)k_cgt_dir_apply_dot<P, NEU>, G::NT, G::SMEM, true);
-    fx_dgt_shape(c, g, NBX, c->num_sms * occ, &ct->t);
-    ct->grid = ct->t.ntx * ct->t.nseg; ct->block = G::NT; ct->smem = G::SMEM;
-    const int pitch = g->Nx * P, rows = g->Ny * P;
+    fx_dgt_shape(c, g, NBX, c->num_sms * occ, &ct->t, Nz);
+    ct->grid = ct->t.ntx * ct->t.nseg * Nz; ct->block = G::NT; ct->smem = G::SMEM;
+    const int pitch = g->Nx * P, rows = g->Ny * P * Nz;
     fx_status s;
     const double* pb[2] = {pb0, pb1};
     for (int i = 0; i < 2; ++i)
@@ -297,7 +305,7 @@ __global__ void __launch_bounds__(256, 3) k_cg_update(const __grid_constant__ Dg
     ex_shared_init(&sh);
     CgAcc acc;
     acc.init();
-    const int pitch = g.Nx * P, rows = g.Ny * P, bd = blockDim.x;
+    const int pitch = g.Nx * P, rows = g.Ny * P * g.Nz, bd = blockDim.x;
     const int cpr = (pitch + CG_U * bd - 1) / (CG_U * bd);
     const double* const arr[4] = {p, q, phi, r};
     ChunkIter iq, ic;
@@ -365,7 +373,7 @@ __global__ void __launch_bounds__(256, 3) k_cg_update_tma(const __grid_constant_
     __shared__ ExShared sh;
     __shared__ __align__(8) unsigned long long bars[2 * K2_STAGES];
     const int pitch = g.Nx * P, bd = blockDim.x, nwarp = bd >> 5;
-    const long long n = (long long)pitch * g.Ny * P;
+    const long long n = (long long)pitch * g.Ny * P * g.Nz;
     const long long tile = 2ll * bd, nfull = n / tile;
     const unsigned arr_bytes = 16u * bd, stage_bytes = 4u * arr_bytes;
     const unsigned sbase = fx_smem_addr(cg_buf), s0 = sbase + 16u * threadIdx.x;
@@ -469,13 +477,14 @@ k_cg_persistent(const __grid_constant__ DgParams g, const double* __restrict__ c
     cgr::grid_group grid = cgr::this_grid();
     __shared__ ExShared sh;
     const unsigned pitch = (unsigned)(g.Nx * P);
-    const unsigned n = pitch * (unsigned)(g.Ny * P);                 // the host takes this path only for n < 2^24
+    const unsigned n = pitch * (unsigned)(g.Ny * P * g.Nz);          // the host takes this path only for n < 2^24
     const double thresh = sc->thresh;
     double rz = sc->rz, beta = 0.0;
     int status = FX_MAXIT, it;
     const int wpb = blockDim.x >> 5;
     const long long gw = (long long)blockIdx.x * wpb + (threadIdx.x >> 5), tw = (long long)gridDim.x * wpb;
-    const long long nwork = (long long)g.nstrip * g.nseg;
+    const long long per = (long long)g.nstrip * g.nseg, nwork = per * g.Nz;
+    const long long n2 = (long long)g.Nx * g.Ny * P * P;
     const unsigned tile = blockDim.x * 2u, ntiles = (n + tile - 1) / tile;
     for (it = 1; it <= maxit; ++it) {
         const int k = it - 1;
@@ -486,13 +495,14 @@ k_cg_persistent(const __grid_constant__ DgParams g, const double* __restrict__ c
         CgAcc acc;
         acc.init();
         {
-            const DgSrc src = {pin, r, pout, beta, k > 0};
-            for (long long w = gw; w < nwork; w += tw) {
+            for (long long wz = gw; wz < nwork; wz += tw) {
+                const long long zoff = (wz / per) * n2, w = wz % per;                      // 3-D product grid: this warp's plane
+                const DgSrc src = {pin + zoff, r + zoff, pout + zoff, beta, k > 0};
                 const int seg = (int)(w / g.nstrip), strip = (int)(w % g.nstrip);
                 const int j0 = seg * g.rows_per_seg;
                 int j1 = j0 + g.rows_per_seg;
                 if (j1 > g.Ny) j1 = g.Ny;
-                dg_warp_strip<P, true, true, false, false, CgAcc, true>(g, chi, src, q, strip, j0, j1, &acc, &sh, nullptr);   // L2-resident grids: generic rows, coherent loads
+                dg_warp_strip<P, true, true, false, false, CgAcc, true>(g, chi + zoff, src, q + zoff, strip, j0, j1, &acc, &sh, nullptr);   // L2-resident grids: generic rows, coherent loads
             }
         }
         acc.flush(&sh);
@@ -552,8 +562,8 @@ static fx_status cg_run_persistent(FxCtx* c, const fx_grid* g, DgParams dp, cons
     int ag, ab;
     fx_dg_shape(c, g, &dp, occ * 4, &ag, &ab);
     // as many CTAs as either phase can use, at most one resident wave (a cooperative launch must be co-resident)
-    const long long n = (long long)g->Nx * g->Ny * g->P * g->P;
-    long long want = ((long long)dp.nstrip * dp.nseg + 3) / 4, wantB = (n + 255) / 256;
+    const long long n = (long long)g->Nx * g->Ny * g->P * g->P * dp.Nz;
+    long long want = ((long long)dp.nstrip * dp.nseg * dp.Nz + 3) / 4, wantB = (n + 255) / 256;
     if (wantB > want) want = wantB;
     long long grid = (long long)c->num_sms * occ;
     if (want < grid) grid = want;
@@ -594,7 +604,7 @@ static void cg_shapes(FxCtx* c, const fx_grid* g, DgParams* p, int k1_warps_per_
     if (bd > 256) bd = 256;
     const int pitch = g->Nx * g->P;
     const long long cpr = (pitch + (long long)bd * CG_U - 1) / ((long long)bd * CG_U);
-    long long chunks = cpr * g->Ny * g->P;
+    long long chunks = cpr * g->Ny * g->P * (p->Nz > 0 ? p->Nz : 1);
     long long gmax = (long long)c->num_sms * (768 / bd);           // one resident wave
     if (chunks > gmax) chunks = gmax;
     if (c->launch[3][0]) chunks = c->launch[3][0];
@@ -611,7 +621,7 @@ static fx_status cg_enqueue_iters(FxCtx* c, const DgParams& dp, const CgTile& ct
     const bool lin = aligned16(phi) && aligned16(r) && aligned16(pbuf0) && aligned16(pbuf1) && aligned16(q);
     int lg;
     {
-        const long long n = (long long)dp.Nx * dp.Ny * P * P, tile = 2ll * eb;
+        const long long n = (long long)dp.Nx * dp.Ny * P * P * dp.Nz, tile = 2ll * eb;
         long long nt = (n + tile - 1) / tile, gm = (long long)c->num_sms * (768 / eb);
         if (nt > gm) nt = gm;
         if (c->launch[3][0]) nt = c->launch[3][0];
@@ -699,20 +709,21 @@ static fx_status cg_collect_profile(FxCtx* c, int iters_done) {
     return FX_OK;
 }
 
-extern "C" fx_status fx_cg_solve_ex(fx_ctx* c, const fx_grid* g, const double* chi, const double* rho, double* phi, double tol, int32_t maxit,
-                                 fx_cg_info* info) {
-    FX_ENTER(c, "fx_cg_solve");
-    if (!fx_grid_ok(g) || !chi || !rho || !phi || maxit < 0 || !(tol >= 0)) { fx_set_error("fx_cg_solve: bad arguments"); return FX_EINVAL; }
-    const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
+// The solve on Nz stacked planes of the grid g (Nz = 1, lz = 0: the 2-D solve; lz > 0: the 3-D product grid, Q24)
+static fx_status cg_solve_impl(FxCtx* c, const fx_grid* g, int Nz, double lz, const double* chi, const double* rho, double* phi, double tol,
+                               int32_t maxit, fx_cg_info* info) {
+    if (!fx_grid_ok(g) || Nz < 1 || !chi || !rho || !phi || maxit < 0 || !(tol >= 0)) { fx_set_error("fx_cg_solve: bad arguments"); return FX_EINVAL; }
+    const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P * Nz;
+    if (n >= ((int64_t)1 << 31)) { fx_set_error("fx_cg_solve: more than 2^31 unknowns"); return FX_EINVAL; }
     fx_status s = cg_workspace(c, n);
     if (s != FX_OK) return s;
     double *W = c->cg_vec, *V = W + n, *rhs = V + n, *r = rhs + n, *z = r + n, *p = z + n, *q = p + n, *p2 = q + n;
     const size_t bytes = (size_t)n * sizeof(double);
 
     // setup with the public primitives (lines before the loop)
-    if ((s = fx_dg_weights_ex(c, g, W, V)) != FX_OK) return s;
+    if ((s = fx_launch_weights(c, g, W, V, Nz, lz)) != FX_OK) return s;
     if ((s = fx_pointwise_dot_ex(c, -1.0, W, rho, 0.0, rhs, n)) != FX_OK) return s;
-    if ((s = fx_launch_apply(c, g, chi, phi, q, 0)) != FX_OK) return s;
+    if ((s = fx_launch_apply(c, g, chi, phi, q, 0, Nz, lz)) != FX_OK) return s;
     FX_CUDA(cudaMemcpyAsync(r, rhs, bytes, cudaMemcpyDeviceToDevice, c->stream));
     if ((s = fx_axpby_ex(c, -1.0, q, 1.0, r, n)) != FX_OK) return s;
     if ((s = fx_pointwise_dot_ex(c, 1.0, V, rhs, 0.0, z, n)) != FX_OK) return s;
@@ -734,7 +745,7 @@ extern "C" fx_status fx_cg_solve_ex(fx_ctx* c, const fx_grid* g, const double* c
         status = FX_MAXIT;
         if (!c->cg_fused) {
             for (it = 1; it <= maxit; ++it) {
-                if ((s = fx_launch_apply(c, g, chi, p, q, 0)) != FX_OK) return s;
+                if ((s = fx_launch_apply(c, g, chi, p, q, 0, Nz, lz)) != FX_OK) return s;
                 double pq;
                 if ((s = fx_exdot_ex(c, p, q, n, &pq, nullptr)) != FX_OK) return s;
                 if (!(pq > 0.0) || !isfinite(pq)) { status = FX_EBREAKDOWN; break; }
@@ -752,7 +763,7 @@ extern "C" fx_status fx_cg_solve_ex(fx_ctx* c, const fx_grid* g, const double* c
             if (it > maxit) it = maxit;
         } else if (maxit > 0) {
             DgParams dp;
-            if ((s = fx_make_dg_params(g, 0, &dp, nullptr)) != FX_OK) return s;
+            if ((s = fx_make_dg_params(g, 0, &dp, nullptr, Nz, lz)) != FX_OK) return s;
             int ag, ab, eg, eb;
             int occb = 0;
             {
@@ -774,7 +785,7 @@ extern "C" fx_status fx_cg_solve_ex(fx_ctx* c, const fx_grid* g, const double* c
             ct.on = false;
             if (c->dg_path == 2 && fx_dgt_eligible(g, chi, r, p) && aligned16(p2)) {   // (measured: K1 on the warp-strip stencil is still the faster one)
                 const bool neu = fx_dg_has_neumann(&dp) != 0;
-#define FX_CGT(PP) s = neu ? cgt_setup<PP, true>(c, g, chi, r, p, p2, &ct) : cgt_setup<PP, false>(c, g, chi, r, p, p2, &ct); break;
+#define FX_CGT(PP) s = neu ? cgt_setup<PP, true>(c, g, Nz, chi, r, p, p2, &ct) : cgt_setup<PP, false>(c, g, Nz, chi, r, p, p2, &ct); break;
                 switch (g->P) {
                 case 1: FX_CGT(1)
                 case 2: FX_CGT(2)
@@ -849,6 +860,50 @@ extern "C" fx_status fx_cg_solve_ex(fx_ctx* c, const fx_grid* g, const double* c
     FX_CUDA(cudaStreamSynchronize(c->stream));
     if (info) { info->iterations = it; info->status = status; info->rel_residual = sqrt(rz) / sqrt(bz); }
     return (fx_status)status;
+}
+extern "C" fx_status fx_cg_solve_ex(fx_ctx* c, const fx_grid* g, const double* chi, const double* rho, double* phi, double tol, int32_t maxit,
+                                    fx_cg_info* info) {
+    FX_ENTER(c, "fx_cg_solve");
+    return cg_solve_impl(c, g, 1, 0.0, chi, rho, phi, tol, maxit, info);
+}
+// 3-D product grid (fx.h; Q24)
+static bool grid3_plane(const fx_grid3* g, fx_grid* p) {
+    if (!g || g->Nz < 1 || !(g->lz > 0)) return false;
+    p->Nx = g->Nx; p->Ny = g->Ny; p->P = g->P; p->lx = g->lx; p->ly = g->ly; p->bcx = g->bcx; p->bcy = g->bcy;
+    return fx_grid_ok(p) != 0 && (int64_t)g->Ny * g->P * g->Nz < (1ll << 30);
+}
+extern "C" fx_status fx_cg3_solve_ex(fx_ctx* c, const fx_grid3* g, const double* chi, const double* rho, double* phi, double tol, int32_t maxit,
+                                     fx_cg_info* info) {
+    FX_ENTER(c, "fx_cg3_solve");
+    fx_grid p;
+    if (!grid3_plane(g, &p)) { fx_set_error("fx_cg3_solve: bad grid"); return FX_EINVAL; }
+    return cg_solve_impl(c, &p, g->Nz, g->lz, chi, rho, phi, tol, maxit, info);
+}
+extern "C" fx_status fx_cg3_solve(const fx_grid3* g, const double* chi, const double* rho, double* phi, double tol, int32_t maxit, fx_cg_info* info) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_cg3_solve_ex(c, g, chi, rho, phi, tol, maxit, info) : FX_ECUDA;
+}
+extern "C" fx_status fx_dg3_elliptic_apply_ex(fx_ctx* c, const fx_grid3* g, const double* chi, const double* x, double* y, int32_t sym) {
+    FX_ENTER(c, "fx_dg3_elliptic_apply");
+    fx_grid p;
+    if (!grid3_plane(g, &p) || !chi || !x || !y) { fx_set_error("fx_dg3_elliptic_apply: bad grid or null pointer"); return FX_EINVAL; }
+    const int64_t n = (int64_t)p.Nx * p.Ny * p.P * p.P * g->Nz;
+    if ((x < y + n && y < x + n) || (chi < y + n && y < chi + n)) { fx_set_error("fx_dg3_elliptic_apply: y overlaps an input"); return FX_EINVAL; }
+    return fx_launch_apply(c, &p, chi, x, y, sym ? 0 : 1, g->Nz, g->lz);
+}
+extern "C" fx_status fx_dg3_elliptic_apply(const fx_grid3* g, const double* chi, const double* x, double* y, int32_t sym) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_dg3_elliptic_apply_ex(c, g, chi, x, y, sym) : FX_ECUDA;
+}
+extern "C" fx_status fx_dg3_weights_ex(fx_ctx* c, const fx_grid3* g, double* W, double* V) {
+    FX_ENTER(c, "fx_dg3_weights");
+    fx_grid p;
+    if (!grid3_plane(g, &p)) { fx_set_error("fx_dg3_weights: bad grid"); return FX_EINVAL; }
+    return fx_launch_weights(c, &p, W, V, g->Nz, g->lz);
+}
+extern "C" fx_status fx_dg3_weights(const fx_grid3* g, double* W, double* V) {
+    FxCtx* c = fx_default_ctx();
+    return c ? fx_dg3_weights_ex(c, g, W, V) : FX_ECUDA;
 }
 extern "C" fx_status fx_cg_solve(const fx_grid* g, const double* chi, const double* rho, double* phi, double tol, int32_t maxit,
                                  fx_cg_info* info) {

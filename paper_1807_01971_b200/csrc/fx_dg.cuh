@@ -28,6 +28,8 @@ struct DgParams {
     int rows_per_seg, nseg, nstrip;
     int normed;
     int smr;                       // rows staged through the per-lane shared-memory ring (P <= 3)
+    int Nz, zmul;                  // 3-D product grid (Q24): planes stacked in the vectors; zmul: (S x) is multiplied by hz
+    double hz;
     double cxx, cyy;               // hy/hx, hx/hy
     double T0[FX_PMAX][FX_PMAX], T0L[FX_PMAX][FX_PMAX], WW[FX_PMAX][FX_PMAX], V[FX_PMAX][FX_PMAX];
     double TD[FX_PMAX][FX_PMAX];   // D: the cell table of the last cell before a Neumann wall
@@ -236,6 +238,7 @@ __device__ __forceinline__ void dg_xlines(const DgParams& g, const DgCell<P>& uc
 #undef CT
             double o = __fma_rn(g.cxx, __fma_rn(g.L[k], tBl[l], a), acc_[l][k]);
             if (g.normed) o = __dmul_rn(g.V[l][k], o);
+            else if (g.zmul) o = __dmul_rn(g.hz, o);
             acc_[l][k] = o;
         }
 #undef FL

@@ -188,7 +188,7 @@ struct DgtDir {
 template <int P, int NBX, int NS, bool FUSE, bool DIRF, bool NEU, class ACC, int ND = 0>
 __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, const CUtensorMap* mu, const CUtensorMap* muh,
                                          const CUtensorMap* mc, const CUtensorMap* mch, const DgtDir& dir, double* __restrict__ y,
-                                         unsigned long long* bars, int tx, int seg, ACC* acc, ExShared* sh) {
+                                         unsigned long long* bars, int tx, int seg, int plane, ACC* acc, ExShared* sh) {
     typedef DgtGeom<P, NBX, DIRF ? 3 : 2, NS, ND> G;
     constexpr int NW = NBX * P;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -236,7 +236,8 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
     const bool yact = tid < txc * P && (long long)i0 * P + tid < pitch;
     const int yk = ycol % P;
     const int ya = G::HE + P + ycol;
-    double* yp = y + (long long)j0 * P * pitch + (long long)i0 * P + tid;     // row of the next output (yact threads only)
+    const int zrow = plane * Ny * P;                                // first image row of this plane in the stacked vectors
+    double* yp = y + ((long long)zrow + (long long)j0 * P) * pitch + (long long)i0 * P + tid;     // row of the next output (yact threads only)
     const long long prow = (long long)pitch;
 
     // ---- TMA producer -----------------------------------------------------------------------------------------------------
@@ -246,7 +247,7 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
         int r = j0 - 1 + q;
         if (r < 0) r += Ny;
         if (r >= Ny) r -= Ny;
-        r *= P;
+        r = zrow + r * P;
         const unsigned nstr = (q <= n ? 2u : 1u) + (DIRF ? 1u : 0u);  // the row above the segment needs no chi
         const unsigned bar = full0 + 8u * (q % NS);
         if (!present(q)) { fx_mbar_arrive(bar); return; }            // a row beyond a wall: the phase completes empty
@@ -272,7 +273,7 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
     // ---- DIRF: p_new is formed on the fly by whoever reads an element (the x-phase thread for its line, the y-phase thread
     // for its column: 3 redundant fp64 operations per unknown instead of a separate pass through shared memory), and stored
     // to pout by the column thread.  Streams of a stage: 0 = p_old, 1 = chi, 2 = r.
-    double* pp = DIRF ? dir.pout + (long long)j0 * P * pitch + (long long)i0 * P + tid : nullptr;
+    double* pp = DIRF ? dir.pout + ((long long)zrow + (long long)j0 * P) * pitch + (long long)i0 * P + tid : nullptr;
     const bool upd = DIRF && dir.upd;
     const double beta = DIRF ? dir.beta : 0.0;
     auto pnew = [&](double po, double rr, double v) { return upd ? __fma_rn(1.0, __dmul_rn(v, rr), __dmul_rn(beta, po)) : po; };
@@ -401,6 +402,7 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
                     v = __fma_rn(g.cyy, sy[l], v);
                     v = __fma_rn(g.cxx, hx.y, v);
                     if (g.normed) v = __dmul_rn(g.V[l][yk], v);
+                    else if (g.zmul) v = __dmul_rn(g.hz, v);
                     o[l] = v;
                 }
                 if (yact) {

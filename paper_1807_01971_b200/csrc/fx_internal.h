@@ -83,7 +83,7 @@ int fx_grid_ok(const fx_grid* g);
 int fx_grid_deriv_ok(const fx_grid* g);          // PER / DIR only: stand-alone derivatives and the bracket
 int fx_dg_has_neumann(const DgParams* p);
 int fx_dg_neu_variant(const DgParams* p, int P);
-fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* out, double* vol4_out);
+fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* out, double* vol4_out, int Nz = 1, double lz = 0.0);   // lz > 0: 3-D product grid of Nz planes
 
 // internal launchers (stream-ordered, no synchronisation)
 fx_status fx_launch_exdot(FxCtx* c, const double* x, const double* y, int64_t n, double* result_dev);
@@ -95,8 +95,9 @@ void fx_dg_shape(FxCtx* c, const fx_grid* g, DgParams* p, int warps_per_sm, int*
 // CTA-tile stencil kernels (fx_dgt.cuh): eligibility (TMA's global-memory rules), tensor maps, launch geometry
 bool fx_dgt_eligible(const fx_grid* g, const void* a, const void* b, const void* c2);
 fx_status fx_dgt_make_map(CUtensorMap* m, const double* base, int pitch, int rows, int boxw, int boxh);
-void fx_dgt_shape(FxCtx* c, const fx_grid* g, int nbx, int resident, DgtTile* t);
+void fx_dgt_shape(FxCtx* c, const fx_grid* g, int nbx, int resident, DgtTile* t, int Nz = 1);
 fx_status fx_launch_derivative(FxCtx* c, const fx_grid* g, int dir, int flux, double alpha, const double* x, double beta, double* y);
-fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const double* x, double* y, int normed);
+fx_status fx_launch_weights(FxCtx* c, const fx_grid* g, double* W, double* V, int Nz = 1, double lz = 0.0);
+fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const double* x, double* y, int normed, int Nz = 1, double lz = 0.0);
 
 #endif

@@ -564,8 +564,12 @@ template <int P, bool NEU>
 __global__ void __maxnreg__(P <= 2 ? 128 : P == 3 ? FX_AP_R : 255) k_dg_apply(const __grid_constant__ DgParams g, const double* __restrict__ chi,
                                                   const double* __restrict__ x, double* __restrict__ y) {
     const int wpb = blockDim.x >> 5;
-    const long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
-    if (w >= (long long)g.nstrip * g.nseg) return;
+    long long w = (long long)blockIdx.x * wpb + (threadIdx.x >> 5);
+    const long long per = (long long)g.nstrip * g.nseg;                       // warps per plane
+    if (w >= per * g.Nz) return;
+    const long long zoff = (w / per) * ((long long)g.Nx * g.Ny * P * P);      // 3-D product grid: this warp's plane
+    w %= per;
+    chi += zoff; x += zoff; y += zoff;
     // consecutive warps take consecutive strips of the same row segment: neighbouring halo columns are L1/L2 hits
     const int seg = (int)(w / g.nstrip), strip = (int)(w % g.nstrip);
     const int j0 = seg * g.rows_per_seg;
@@ -592,8 +596,9 @@ k_dgt_apply(const __grid_constant__ DgParams g, const __grid_constant__ DgtTile 
     }
     __syncthreads();
     const DgtDir nodir = {nullptr, nullptr, nullptr, 0.0, false};
-    dgt_tile<P, DgtCfg<P>::NBX, DGT_NS, false, false, NEU, NoAcc>(g, t, &mu, &muh, &mc, &mch, nodir, y, bars, (int)(blockIdx.x % t.ntx),
-                                                                  (int)(blockIdx.x / t.ntx), nullptr, nullptr);
+    const int per = t.ntx * t.nseg, rem = (int)(blockIdx.x % per);
+    dgt_tile<P, DgtCfg<P>::NBX, DGT_NS, false, false, NEU, NoAcc>(g, t, &mu, &muh, &mc, &mch, nodir, y, bars, rem % t.ntx, rem / t.ntx,
+                                                                  (int)(blockIdx.x / per), nullptr, nullptr);
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (libfx.so does not link libcuda)
@@ -635,7 +640,7 @@ bool fx_dgt_eligible(const fx_grid* g, const void* a, const void* b, const void*
 
 // Launch geometry: tiles of NBX blocks of wb <= 30 cells, balanced over the row; segments so that the grid is whole waves
 // of `resident` CTAs with little prologue work (one extra cell row of loads and about half a row of arithmetic each).
-void fx_dgt_shape(FxCtx* c, const fx_grid* g, int nbx, int resident, DgtTile* t) {
+void fx_dgt_shape(FxCtx* c, const fx_grid* g, int nbx, int resident, DgtTile* t, int Nz) {
     const int tmax = FX_STRIP * nbx;
     t->ntx = (g->Nx + tmax - 1) / tmax;
     t->wb = (g->Nx + t->ntx * nbx - 1) / (t->ntx * nbx);
@@ -649,7 +654,7 @@ void fx_dgt_shape(FxCtx* c, const fx_grid* g, int nbx, int resident, DgtTile* t)
         double best = 1e300;
         rps = 1;
         for (int r = 1; r <= g->Ny; ++r) {
-            const long long ctas = (long long)t->ntx * ((g->Ny + r - 1) / r);
+            const long long ctas = (long long)t->ntx * ((g->Ny + r - 1) / r) * Nz;
             const double cost = (double)((ctas + resident - 1) / resident) * (r + 1.0);
             if (cost <= best) { best = cost; rps = r; }
             if (ctas <= resident && r >= 2) break;
@@ -661,19 +666,19 @@ void fx_dgt_shape(FxCtx* c, const fx_grid* g, int nbx, int resident, DgtTile* t)
 }
 
 template <int P, bool NEU>
-static fx_status launch_dgt_apply(FxCtx* c, const fx_grid* g, const DgParams& p, const double* chi, const double* x, double* y) {
+static fx_status launch_dgt_apply(FxCtx* c, const fx_grid* g, const DgParams& p, const double* chi, const double* x, double* y) {   // (p.Nz planes)
     constexpr int NBX = DgtCfg<P>::NBX;
     typedef DgtGeom<P, NBX, 2> G;
     const int occ = fx_func_occ(c, (const void*)k_dgt_apply<P, NEU>, G::NT, G::SMEM, true);
     DgtTile t;
-    fx_dgt_shape(c, g, NBX, c->num_sms * occ, &t);
-    const int pitch = g->Nx * P, rows = g->Ny * P;
+    fx_dgt_shape(c, g, NBX, c->num_sms * occ, &t, p.Nz);
+    const int pitch = g->Nx * P, rows = g->Ny * P * p.Nz;
     CUtensorMap mu, muh, mc, mch;
     fx_status s;
     if ((s = fx_dgt_make_map(&mu, x, pitch, rows, G::BW, P)) != FX_OK || (s = fx_dgt_make_map(&muh, x, pitch, rows, G::HW, P)) != FX_OK ||
         (s = fx_dgt_make_map(&mc, chi, pitch, rows, G::BW, P)) != FX_OK || (s = fx_dgt_make_map(&mch, chi, pitch, rows, G::HW, P)) != FX_OK)
         return s;
-    k_dgt_apply<P, NEU><<<t.ntx * t.nseg, G::NT, G::SMEM, c->stream>>>(p, t, mu, muh, mc, mch, y);
+    k_dgt_apply<P, NEU><<<t.ntx * t.nseg * p.Nz, G::NT, G::SMEM, c->stream>>>(p, t, mu, muh, mc, mch, y);
     return FX_OK;
 }
 
@@ -695,7 +700,7 @@ int fx_grid_ok(const fx_grid* g) {
 }
 
 // host scalars and tables exactly as DESIGN.md 3.4 writes them (plain IEEE double operations, no contraction)
-fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* o, double* vol4_out) {
+fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* o, double* vol4_out, int Nz, double lz) {
     fx_tables t;
     if (fx_make_tables(g->P, &t) != 0) { fx_set_error("P outside 1..5"); return FX_EINVAL; }
     memset(o, 0, sizeof(*o));
@@ -704,6 +709,10 @@ fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* o, double* v
     volatile double hxhy = hx * hy;
     const double vol4 = hxhy / 4;
     o->Nx = g->Nx; o->Ny = g->Ny; o->bcx = g->bcx; o->bcy = g->bcy; o->normed = normed;
+    // 3-D product grid (Q24): W3 = RN(hz*W2); the symmetric form is RN(hz*(S2 x)), the normed one is the plane's A2 x
+    volatile double hz = lz > 0 ? lz / Nz : 1.0;
+    const bool three_d = lz > 0;
+    o->Nz = Nz > 0 ? Nz : 1; o->hz = hz; o->zmul = (three_d && !normed) ? 1 : 0;
     o->lox = wall_lo(g->bcx); o->hix = wall_hi(g->bcx); o->loy = wall_lo(g->bcy); o->hiy = wall_hi(g->bcy);
     o->cxx = hy / hx; o->cyy = hx / hy;
     volatile double hy2 = hy / 2, hx2 = hx / 2;
@@ -713,7 +722,8 @@ fx_status fx_make_dg_params(const fx_grid* g, int normed, DgParams* o, double* v
         for (int m = 0; m < P; ++m) {
             o->T0[k][m] = t.T0[k][m]; o->T0L[k][m] = t.T0L[k][m]; o->WW[k][m] = t.WW[k][m]; o->TD[k][m] = t.D[k][m];
             volatile double w = vol4 * t.WW[k][m];
-            o->V[k][m] = 1.0 / w;
+            if (three_d && !normed) { volatile double w3 = hz * w; o->V[k][m] = 1.0 / w3; }      // preconditioner of the 3-D solve: V3 = 1/W3
+            else o->V[k][m] = 1.0 / w;
         }
     }
     if (vol4_out) *vol4_out = vol4;
@@ -738,7 +748,7 @@ void fx_dg_shape(FxCtx* c, const fx_grid* g, DgParams* p, int warps_per_sm, int*
         double best = 1e300;
         rps = 1;
         for (int r = 1; r <= g->Ny; ++r) {
-            const long long warps = (long long)p->nstrip * ((g->Ny + r - 1) / r);
+            const long long warps = (long long)p->nstrip * ((g->Ny + r - 1) / r) * (p->Nz > 0 ? p->Nz : 1);
             const double cost = (double)((warps + resident - 1) / resident) * (r + 0.6);
             if (cost <= best) { best = cost; rps = r; }
             if (warps <= resident && r >= 2) break;                   // one wave: larger segments only cost more
@@ -747,14 +757,14 @@ void fx_dg_shape(FxCtx* c, const fx_grid* g, DgParams* p, int warps_per_sm, int*
     if (rps > g->Ny) rps = g->Ny;
     p->rows_per_seg = rps;
     p->nseg = (g->Ny + rps - 1) / rps;
-    const long long warps = (long long)p->nstrip * p->nseg;
+    const long long warps = (long long)p->nstrip * p->nseg * (p->Nz > 0 ? p->Nz : 1);
     *grid = (int)((warps + wpb - 1) / wpb);
     *block = wpb * 32;
 }
 
-fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const double* x, double* y, int normed) {
+fx_status fx_launch_apply(FxCtx* c, const fx_grid* g, const double* chi, const double* x, double* y, int normed, int Nz, double lz) {
     DgParams p;
-    fx_status s = fx_make_dg_params(g, normed, &p, nullptr);
+    fx_status s = fx_make_dg_params(g, normed, &p, nullptr, Nz, lz);
     if (s != FX_OK) return s;
     const int neu = fx_dg_neu_variant(&p, g->P);
     int occw;                                                    // resident warps per SM of k_dg_apply<P, NEU>
@@ -825,27 +835,32 @@ extern "C" fx_status fx_dg_elliptic_apply_sym(const fx_grid* g, const double* ch
 }
 
 // W[idx] = RN(vol4 * WW[l][k]),  V[idx] = RN(1 / W[idx])     (Fig. 2 "volume")
-__global__ void k_dg_weights(const __grid_constant__ DgParams g, int P, double vol4, double* W, double* V) {
-    const long long pitch = (long long)g.Nx * P, n = pitch * g.Ny * P;
+// 3-D product grid (hz3 != 0): W3 = RN(hz * W2) on every plane, V3 = RN(1 / W3) (Q24; g.V holds V3 then)
+__global__ void k_dg_weights(const __grid_constant__ DgParams g, int P, double vol4, int hz3, double* W, double* V) {
+    const long long pitch = (long long)g.Nx * P, n = pitch * g.Ny * P * g.Nz;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
         const int l = (int)((i / pitch) % P), k = (int)((i % pitch) % P);
-        if (W) W[i] = __dmul_rn(vol4, g.WW[l][k]);
+        if (W) { const double w = __dmul_rn(vol4, g.WW[l][k]); W[i] = hz3 ? __dmul_rn(g.hz, w) : w; }
         if (V) V[i] = g.V[l][k];
     }
+}
+
+fx_status fx_launch_weights(FxCtx* c, const fx_grid* g, double* W, double* V, int Nz, double lz) {
+    DgParams p; double vol4;
+    fx_status s = fx_make_dg_params(g, 0, &p, &vol4, Nz, lz);
+    if (s != FX_OK) return s;
+    const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P * p.Nz;
+    int grid = (int)((n + 255) / 256); if (grid > c->num_sms * 32) grid = c->num_sms * 32;
+    k_dg_weights<<<grid, 256, 0, c->stream>>>(p, g->P, vol4, lz > 0 ? 1 : 0, W, V);
+    c->launches++;
+    FX_CUDA(cudaGetLastError());
+    return FX_OK;
 }
 
 extern "C" fx_status fx_dg_weights_ex(fx_ctx* c, const fx_grid* g, double* W, double* V) {
     FX_ENTER(c, "fx_dg_weights");
     if (!fx_grid_ok(g)) { fx_set_error("fx_dg_weights: bad grid"); return FX_EINVAL; }
-    DgParams p; double vol4;
-    fx_status s = fx_make_dg_params(g, 0, &p, &vol4);
-    if (s != FX_OK) return s;
-    const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;
-    int grid = (int)((n + 255) / 256); if (grid > c->num_sms * 32) grid = c->num_sms * 32;
-    k_dg_weights<<<grid, 256, 0, c->stream>>>(p, g->P, vol4, W, V);
-    c->launches++;
-    FX_CUDA(cudaGetLastError());
-    return FX_OK;
+    return fx_launch_weights(c, g, W, V, 1, 0.0);
 }
 extern "C" fx_status fx_dg_weights(const fx_grid* g, double* W, double* V) {
     FxCtx* c = fx_default_ctx();

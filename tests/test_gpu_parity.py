@@ -821,3 +821,63 @@ def test_exdot_f32_widening_cases(fx, oracle):
     assert fx.exdot_f32(torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda()) == -np.inf
     y[9] = np.nan
     assert math.isnan(fx.exdot_f32(torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda()))
+
+
+# ---- 3-D product grids (Q24) -----------------------------------------------------------------------
+@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("P,bc,Nx,Ny,Nz", [(1, (0, 1), 8, 6, 3), (2, (1, 0), 31, 5, 4), (3, (0, 1), 64, 24, 5), (3, (1, 1), 62, 9, 2),
+                                           (4, (2, 1), 30, 7, 3), (5, (3, 4), 12, 6, 2), (3, (0, 0), 250, 5, 3)])
+def test_dg3_apply_and_weights_bit_exact(fx, oracle, P, bc, Nx, Ny, Nz, path):
+    import torch
+    fx.set_dg_path(path)
+    g = fx.make_grid3(Nx, Ny, Nz, P, 2 * math.pi, 3.0, 1.7, *bc)
+    og = oracle.Grid3(Nx, Ny, Nz, P, 2 * math.pi, 3.0, 1.7, *bc)
+    x = fi.uniform(191 + P, g.n); chi = 1.0 + 0.5 * fi.uniform(192 + P, g.n)
+    w = torch.empty(g.n, dtype=torch.float64, device="cuda"); v = torch.empty_like(w)
+    fx.dg3_weights(g, w, v)
+    W, V = oracle.dg3_weights(og)
+    assert same_bits(w.cpu().numpy(), W) and same_bits(v.cpu().numpy(), V)
+    for sym in (True, False):
+        want = oracle.dg3_apply_canonical(og, chi, x, normed=not sym)
+        for rows in (0, 2):
+            fx.set_launch(2, rows, 0)
+            y = torch.full((g.n,), float("nan"), dtype=torch.float64, device="cuda")
+            fx.dg3_elliptic_apply(g, dev(chi), dev(x), y, sym=sym)
+            assert same_bits(y.cpu().numpy(), want), (sym, rows)
+        fx.set_launch(2, 0, 0)
+    ydef, scale = oracle.dg3_apply_definition(og, chi, x, normed=False)
+    y = torch.empty(g.n, dtype=torch.float64, device="cuda")
+    fx.dg3_elliptic_apply(g, dev(chi), dev(x), y, sym=True)
+    assert np.all(np.abs(y.cpu().numpy() - ydef) <= 1e-14 * scale)
+
+
+@pytest.mark.parametrize("mode,path", [(0, 0), (1, 0), (2, 0), (2, 2), (3, 1)])
+@pytest.mark.parametrize("P,bc,Nx,Ny,Nz", [(3, (0, 1), 16, 12, 4), (2, (1, 1), 34, 9, 3), (5, (1, 0), 12, 6, 2)])
+def test_cg3_matches_oracle(fx, oracle, P, bc, Nx, Ny, Nz, mode, path):
+    """one PCG over all planes: every driver (unfused, persistent, two fused kernels on either stencil) gives the oracle's bits"""
+    fx.set_cg_fused(mode); fx.set_dg_path(path)
+    g = fx.make_grid3(Nx, Ny, Nz, P, 2 * math.pi, 2.0, 1.1, *bc)
+    og = oracle.Grid3(Nx, Ny, Nz, P, 2 * math.pi, 2.0, 1.1, *bc)
+    chi = 1.0 + 0.5 * fi.uniform(195, g.n); rho = fi.uniform(196, g.n); phi0 = 0.1 * fi.uniform(197, g.n)
+    want, oinfo = oracle.cg3_solve(og, chi, rho, phi0, 1e-9, 4000)
+    phi = dev(phi0)
+    info = fx.cg3_solve(g, dev(chi), dev(rho), phi, 1e-9, 4000)
+    assert info.iterations == oinfo.iterations and info.status == oinfo.status == 0
+    assert info.rel_residual == oinfo.rel_residual
+    assert same_bits(phi.cpu().numpy(), want)
+    want, oinfo = oracle.cg3_solve(og, chi, rho, phi0, 0.0, 17)
+    phi = dev(phi0)
+    info = fx.cg3_solve(g, dev(chi), dev(rho), phi, 0.0, 17)
+    assert info.iterations == 17 and info.status == 1 and same_bits(phi.cpu().numpy(), want)
+
+
+def test_cg3_larger_grid(fx, oracle):
+    """128 x 128 cells x 8 planes, P = 3 (1.2 M unknowns: the two-kernel loop at its default launch shapes), 30 iterations"""
+    g = fx.make_grid3(128, 128, 8, 3, 2 * math.pi, 2 * math.pi, 2 * math.pi, 1, 1)
+    og = oracle.Grid3(128, 128, 8, 3, 2 * math.pi, 2 * math.pi, 2 * math.pi, 1, 1)
+    chi = 1.0 + 0.5 * fi.uniform(198, g.n); rho = fi.uniform(199, g.n)
+    want, oinfo = oracle.cg3_solve(og, chi, rho, np.zeros(g.n), 0.0, 30)
+    phi = dev(np.zeros(g.n))
+    info = fx.cg3_solve(g, dev(chi), dev(rho), phi, 0.0, 30)
+    assert info.iterations == oinfo.iterations == 30 and info.rel_residual == oinfo.rel_residual
+    assert same_bits(phi.cpu().numpy(), want)

@@ -13,6 +13,7 @@
 //     were enqueued past convergence into no-ops, and the host looks at it once per batch of iterations.
 
 #include <math.h>
+#include <type_traits>
 #include <stdlib.h>
 #include <string.h>
 
@@ -470,12 +471,13 @@ __global__ void __launch_bounds__(256, 3) k_cg_update_tma(const __grid_constant_
 // launches, two single-pass tails and their gaps.  The arithmetic, and therefore every bit of the result, is unchanged.
 // Digit buffers: pdig[0..1] for p.q of even/odd iterations, pdig[2..3] for r.z; CTA 0 re-zeroes the buffer of the next
 // iteration one phase after its last reader has passed a grid sync.
-template <int P>
+template <int P, bool NEU>
 __global__ void __launch_bounds__(128, 2)
 k_cg_persistent(const __grid_constant__ DgParams g, const double* __restrict__ chi, double* r, double* p0, double* p1, double* q,
                 double* phi, fx_u64* pdig, int* pflags, CgScal* sc, int maxit) {
     cgr::grid_group grid = cgr::this_grid();
     __shared__ ExShared sh;
+    extern __shared__ __align__(16) double dg_smem[];
     const unsigned pitch = (unsigned)(g.Nx * P);
     const unsigned n = pitch * (unsigned)(g.Ny * P * g.Nz);          // the host takes this path only for n < 2^24
     const double thresh = sc->thresh;
@@ -486,6 +488,63 @@ k_cg_persistent(const __grid_constant__ DgParams g, const double* __restrict__ c
     const long long per = (long long)g.nstrip * g.nseg, nwork = per * g.Nz;
     const long long n2 = (long long)g.Nx * g.Ny * P * P;
     const unsigned tile = blockDim.x * 2u, ntiles = (n + tile - 1) / tile;
+    // phase B walks tiles blockIdx.x, +G, +2G, ...: a thread's two elements of a tile start at (col0, l0) and move by `step`
+    const unsigned step = gridDim.x * tile, dcol = step % pitch;
+    const int drow = (int)((step / pitch) % P);
+    unsigned col0[2];
+    int l0[2];
+#pragma unroll
+    for (int v = 0; v < 2; ++v) {
+        const unsigned e = blockIdx.x * tile + (unsigned)v * blockDim.x + threadIdx.x;
+        col0[v] = e % pitch; l0[v] = (int)((e / pitch) % P);
+    }
+    auto phaseB = [&](auto uu, const double alpha, const double nalpha, double* pout, CgAcc& acc) {
+        constexpr int U = decltype(uu)::value;
+        unsigned col[2] = {col0[0], col0[1]};
+        int l[2] = {l0[0], l0[1]};
+#pragma unroll 1
+        for (unsigned t = blockIdx.x; t < ntiles; t += (unsigned)U * gridDim.x) {
+            double pv[2 * U], qv[2 * U], fv[2 * U], rv[2 * U];
+            unsigned ee[2 * U];
+#pragma unroll
+            for (int u = 0; u < 2 * U; ++u) {
+                const unsigned tt = t + (unsigned)(u >> 1) * gridDim.x;
+                ee[u] = tt < ntiles ? tt * tile + (unsigned)(u & 1) * blockDim.x + threadIdx.x : n;
+                const bool in = ee[u] < n;
+                pv[u] = in ? pout[ee[u]] : 0.0; qv[u] = in ? q[ee[u]] : 0.0; fv[u] = in ? phi[ee[u]] : 0.0; rv[u] = in ? r[ee[u]] : 0.0;
+            }
+#pragma unroll
+            for (int h = 0; h < U; ++h) {
+                double rr[2], zz[2];
+                bool act[2];
+#pragma unroll
+                for (int v = 0; v < 2; ++v) {
+                    const int u = 2 * h + v;
+                    const unsigned e = ee[u];
+                    act[v] = e < n;
+                    rr[v] = 0.0; zz[v] = 0.0;
+                    if (act[v]) {
+                        phi[e] = __fma_rn(alpha, pv[u], fv[u]);
+                        const double rn = __fma_rn(nalpha, qv[u], rv[u]);
+                        r[e] = rn;
+                        rr[v] = rn; zz[v] = __dmul_rn(g.V[l[v]][col[v] % P], rn);
+                    }
+                    col[v] += dcol; l[v] += drow;                          // the same element of the next tile
+                    if (col[v] >= pitch) { col[v] -= pitch; ++l[v]; }
+                    if (l[v] >= P) l[v] -= P;
+                    if (l[v] >= P) l[v] -= P;
+                }
+                acc.add<2>(rr, zz, act, &sh);
+            }
+        }
+    };
+#ifdef FX_PERSIST_PROF
+    unsigned long long tp[5] = {0, 0, 0, 0, 0}, t0, t1;
+#define FX_TICK(i) do { asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)); tp[i] += t1 - t0; t0 = t1; } while (0)
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+#else
+#define FX_TICK(i)
+#endif
     for (it = 1; it <= maxit; ++it) {
         const int k = it - 1;
         const double* pin = (k & 1) ? p1 : p0;
@@ -502,11 +561,16 @@ k_cg_persistent(const __grid_constant__ DgParams g, const double* __restrict__ c
                 const int j0 = seg * g.rows_per_seg;
                 int j1 = j0 + g.rows_per_seg;
                 if (j1 > g.Ny) j1 = g.Ny;
-                dg_warp_strip<P, true, true, false, false, CgAcc, true>(g, chi + zoff, src, q + zoff, strip, j0, j1, &acc, &sh, nullptr);   // L2-resident grids: generic rows, coherent loads
+                // rows through the per-lane cp.async ring where it exists (P <= 3: the copies of the next step are in flight while this
+                // one computes; cp.async.ca is an ordinary coherent access, unlike ld.global.nc), else coherent register loads
+                if (P <= 3 && g.smr && g.rows_per_seg >= 2) dg_warp_strip<P, true, true, true, NEU, CgAcc, true>(g, chi + zoff, src, q + zoff, strip, j0, j1, &acc, &sh, dg_smem + (size_t)(threadIdx.x >> 5) * 8 * P * P * 32);
+                else dg_warp_strip<P, true, true, false, NEU, CgAcc, true>(g, chi + zoff, src, q + zoff, strip, j0, j1, &acc, &sh, nullptr);
             }
         }
         acc.flush(&sh);
+        FX_TICK(0);
         const double pq = ex_grid_reduce(&sh, pdig + (size_t)(k & 1) * FX_NDIG, pflags + (k & 1), grid);
+        FX_TICK(1);
         if (blockIdx.x == 0) {
             for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) pdig[(size_t)((k + 1) & 1) * FX_NDIG + i] = 0ull;
             if (threadIdx.x == 0) pflags[(k + 1) & 1] = 0;
@@ -516,26 +580,14 @@ k_cg_persistent(const __grid_constant__ DgParams g, const double* __restrict__ c
         // ---- phase B: phi += alpha p, r -= alpha q, z = V o r, exact dot r.z -----------------------------------------
         ex_shared_init(&sh);
         acc.init();
-        for (unsigned t = blockIdx.x; t < ntiles; t += gridDim.x) {
-            double rr[2], zz[2];
-            bool act[2];
-#pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                const unsigned e = t * tile + u * blockDim.x + threadIdx.x;
-                act[u] = e < n;
-                rr[u] = 0.0; zz[u] = 0.0;
-                if (act[u]) {
-                    const unsigned row = e / pitch, col = e - row * pitch;
-                    phi[e] = __fma_rn(alpha, pout[e], phi[e]);
-                    const double rn = __fma_rn(nalpha, q[e], r[e]);
-                    r[e] = rn;
-                    rr[u] = rn; zz[u] = __dmul_rn(g.V[row % P][col % P], rn);
-                }
-            }
-            acc.add<2>(rr, zz, act, &sh);
-        }
+        // (the vectors sit in L2: a trip of this loop is one load round trip, so up to four tiles are fetched per trip; the table
+        // indices of a thread's elements advance incrementally from tile to tile: no division in the loop)
+        if (ntiles > gridDim.x) phaseB(std::integral_constant<int, 4>(), alpha, nalpha, pout, acc);
+        else phaseB(std::integral_constant<int, 1>(), alpha, nalpha, pout, acc);
         acc.flush(&sh);
+        FX_TICK(2);
         const double rzn = ex_grid_reduce(&sh, pdig + (size_t)(2 + (k & 1)) * FX_NDIG, pflags + 2 + (k & 1), grid);
+        FX_TICK(3);
         if (blockIdx.x == 0) {
             for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) pdig[(size_t)(2 + ((k + 1) & 1)) * FX_NDIG + i] = 0ull;
             if (threadIdx.x == 0) pflags[2 + ((k + 1) & 1)] = 0;
@@ -546,16 +598,22 @@ k_cg_persistent(const __grid_constant__ DgParams g, const double* __restrict__ c
     }
     if (it > maxit) it = maxit;
     if (blockIdx.x == 0 && threadIdx.x == 0) { sc->rz = rz; sc->status = status; sc->iters = it; sc->done = 1; }
+#ifdef FX_PERSIST_PROF
+    if (blockIdx.x == 0 && threadIdx.x == 0) printf("persistent: %d iterations, ns per iteration: phase A %.0f, reduce %.0f, phase B %.0f, reduce %.0f (grid %d)\n", it,
+                                                    (double)tp[0] / it, (double)tp[1] / it, (double)tp[2] / it, (double)tp[3] / it, (int)gridDim.x);
+#endif
 }
 
-template <int P>
+template <int P, bool NEU>
 static fx_status cg_run_persistent(FxCtx* c, const fx_grid* g, DgParams dp, const double* chi, double* r, double* p0, double* p1, double* q,
                                    double* phi, CgScal* sc, int maxit, bool* ran) {
     *ran = false;
     int coop = 0, occ = 0;
     FX_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device));
     if (!coop) return FX_OK;
-    occ = fx_func_occ(c, (const void*)k_cg_persistent<P>, 128, 0);
+    dp.smr = P <= 3 ? 1 : 0;
+    const size_t psm = dp.smr ? fx_dg_ring_bytes(P, 4, true) : 0;
+    occ = fx_func_occ(c, (const void*)k_cg_persistent<P, NEU>, 128, psm);
     FX_CUDA(cudaMemsetAsync(c->cg_pdig, 0, 4 * FX_NDIG * sizeof(fx_u64) + 64, c->stream));
     fx_u64* pdig = (fx_u64*)c->cg_pdig;
     int* pflags = (int*)(pdig + 4 * FX_NDIG);
@@ -569,7 +627,7 @@ static fx_status cg_run_persistent(FxCtx* c, const fx_grid* g, DgParams dp, cons
     if (want < grid) grid = want;
     if (grid < 1) grid = 1;
     void* args[] = {&dp, &chi, &r, &p0, &p1, &q, &phi, &pdig, &pflags, &sc, &maxit};
-    FX_CUDA(cudaLaunchCooperativeKernel((const void*)k_cg_persistent<P>, dim3((unsigned)grid), dim3(128), args, 0, c->stream));
+    FX_CUDA(cudaLaunchCooperativeKernel((const void*)k_cg_persistent<P, NEU>, dim3((unsigned)grid), dim3(128), args, psm, c->stream));
     c->launches++;
     *ran = true;
     return FX_OK;
@@ -807,14 +865,14 @@ static fx_status cg_solve_impl(FxCtx* c, const fx_grid* g, int Nz, double lz, co
             // small grids (vectors resident in L2): the whole loop in one cooperative launch.  mode 1 = automatic,
             // 2 = never, 3 = whenever the device allows it (tests)
             bool persistent = false;
-            // (grids with a Neumann wall always take the two-kernel path: the cooperative kernel is not instantiated for them)
-            if (!fx_dg_has_neumann(&dp) && ((c->cg_fused == 1 && n <= ((int64_t)1 << 20)) || (c->cg_fused == 3 && n < ((int64_t)1 << 24)))) {
+            if (((c->cg_fused == 1 && n <= ((int64_t)1 << 20)) || (c->cg_fused == 3 && n < ((int64_t)1 << 24)))) {
+                const bool neuv = fx_dg_neu_variant(&dp, g->P) != 0;
                 switch (g->P) {
-                case 1: s = cg_run_persistent<1>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
-                case 2: s = cg_run_persistent<2>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
-                case 3: s = cg_run_persistent<3>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
-                case 4: s = cg_run_persistent<4>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
-                default: s = cg_run_persistent<5>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
+                case 1: s = neuv ? cg_run_persistent<1, true>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent) : cg_run_persistent<1, false>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
+                case 2: s = neuv ? cg_run_persistent<2, true>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent) : cg_run_persistent<2, false>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
+                case 3: s = neuv ? cg_run_persistent<3, true>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent) : cg_run_persistent<3, false>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
+                case 4: s = neuv ? cg_run_persistent<4, true>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent) : cg_run_persistent<4, false>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
+                default: s = neuv ? cg_run_persistent<5, true>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent) : cg_run_persistent<5, false>(c, g, dp, chi, r, p, p2, q, phi, sc, maxit, &persistent); break;
                 }
                 if (s != FX_OK) return s;
                 if (persistent) {

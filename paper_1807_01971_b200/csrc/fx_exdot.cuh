@@ -485,19 +485,8 @@ __device__ __forceinline__ double ex_grid_reduce(ExShared* sh, fx_u64* gdig, int
         if (v) atomicAdd(&gdig[i], v);
     }
     if (threadIdx.x == 0 && sh->flags) atomicOr(gflags, sh->flags);
-    __threadfence();
-    grid.sync();
-    if (threadIdx.x == 0) { sh->dlo = FX_NDIG; sh->dhi = -1; }
-    __syncthreads();
-    for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) {
-        const fx_u64 v = __ldcg(&gdig[i]);
-        sh->dig[i] = v;
-        if (v) { atomicMin(&sh->dlo, i); atomicMax(&sh->dhi, i); }
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) sh->res = ex_round_digits_shared(sh, __ldcg(gflags));
-    __syncthreads();
-    return sh->res;
+    grid.sync();                                  // (fences: the digits of every CTA are visible after it)
+    return ex_fetch_round(sh, gdig, gflags);      // digits and flags in one round trip, one thread normalises and rounds
 }
 
 #endif

@@ -34,6 +34,27 @@
 #ifndef FX_MINB3
 #define FX_MINB3 3
 #endif
+#ifndef FX_NBX1
+#define FX_NBX1 4
+#endif
+#ifndef FX_NBX4
+#define FX_NBX4 1
+#endif
+#ifndef FX_NBX5
+#define FX_NBX5 1
+#endif
+#ifndef FX_MINB4
+#define FX_MINB4 3
+#endif
+#ifndef FX_MINB5
+#define FX_MINB5 2
+#endif
+#ifndef FX_NS5
+#define FX_NS5 4
+#endif
+#ifndef FX_KEEPP
+#define FX_KEEPP 0        // keep the thread's table entries in registers for P <= FX_KEEPP (else they are re-read from the constant bank)
+#endif
 #define DGT_NS 4          // ring stages (cell rows resident or in flight per CTA) of the stand-alone apply
 #ifndef FX_K1T_NS
 #define FX_K1T_NS 4
@@ -57,8 +78,9 @@
 
 template <int P>
 struct DgtCfg {
-    static constexpr int NBX = P == 1 ? 4 : P == 2 ? 2 : P == 3 ? FX_NBX3 : 1;    // 30-cell x-blocks per CTA tile
-    static constexpr int MINB = P == 5 ? 2 : P == 3 ? FX_MINB3 : 3;                // CTAs per SM the register cap is sized for
+    static constexpr int NBX = P == 1 ? FX_NBX1 : P == 2 ? 2 : P == 3 ? FX_NBX3 : P == 4 ? FX_NBX4 : FX_NBX5;    // 30-cell x-blocks per CTA tile
+    static constexpr int MINB = P == 5 ? FX_MINB5 : P == 4 ? FX_MINB4 : P == 3 ? FX_MINB3 : 3;   // CTAs per SM the register cap is sized for
+    static constexpr int NS = P == 5 ? FX_NS5 : DGT_NS;                            // ring stages of the stand-alone apply
     static constexpr int NT = 32 * NBX * P;
     static constexpr int REGS = (65536 / (MINB * NT)) / 8 * 8 > 255 ? 255 : (65536 / (MINB * NT)) / 8 * 8;
 };
@@ -159,6 +181,7 @@ __device__ __forceinline__ void dgt_yline(const DgParams& g, const double (&uc)[
 }
 
 template <bool B> struct DgtTag { static constexpr bool value = B; };
+__device__ __forceinline__ void fx_keep(double& v) { asm volatile("" : "+d"(v)); }     // pin a loop-invariant in a register
 
 // DIRF (the CG's fused direction update): the vector is p_new = fma(1, RN(V*r), RN(beta*p_old)) -- axpby(1, z,
 // beta, p) with z = V o r in the canonical order of DESIGN.md 3.2 -- formed in shared memory from the staged rows of r and
@@ -237,6 +260,14 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
     const int yk = ycol % P;
     const int ya = G::HE + P + ycol;
     const int zrow = plane * Ny * P;                                // first image row of this plane in the stacked vectors
+    double wwy[P], wwx[P], jyk = g.JY[yk];                           // this thread's table entries
+#pragma unroll
+    for (int l = 0; l < P; ++l) { wwy[l] = g.WW[l][yk]; wwx[l] = g.WW[xl][l]; }
+    if (P <= FX_KEEPP) {
+#pragma unroll
+        for (int l = 0; l < P; ++l) { fx_keep(wwy[l]); fx_keep(wwx[l]); }
+        fx_keep(jyk);
+    }
     double* yp = y + ((long long)zrow + (long long)j0 * P) * pitch + (long long)i0 * P + tid;     // row of the next output (yact threads only)
     const long long prow = (long long)pitch;
 
@@ -319,7 +350,7 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
         for (int l = 0; l < P; ++l) {
             ua[l] = dgt_smem[ya + l * G::BW];
             if (DIRF) ua[l] = pnew(ua[l], dgt_smem[2 * G::STR_D + ya + l * G::BW], g.V[l][yk]);
-            ca[l] = __dmul_rn(g.WW[l][yk], dgt_smem[G::STR_D + ya + l * G::BW]);
+            ca[l] = __dmul_rn(wwy[l], dgt_smem[G::STR_D + ya + l * G::BW]);
         }
     }
 
@@ -338,7 +369,7 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
             for (int m = 0; m < P; ++m) {
                 u[m] = sq[xa + m];
                 if (DIRF) u[m] = pnew(u[m], sq[2 * G::STR_D + xa + m], g.V[xl][m]);
-                c[m] = __dmul_rn(g.WW[xl][m], sq[G::STR_D + xa + m]);
+                c[m] = __dmul_rn(wwx[m], sq[G::STR_D + xa + m]);
             }
             if (edge) dgt_xline<P, true, NEU>(g, u, c, xghost, firstx, lastx, mirlx, jx, sx);
             else dgt_xline<P, false, NEU>(g, u, c, xghost, firstx, lastx, mirlx, jx, sx);
@@ -366,7 +397,7 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
             }
             if (ST || it < n) {
 #pragma unroll
-                for (int l = 0; l < P; ++l) cn[l] = __dmul_rn(g.WW[l][yk], sq[G::STR_D + ya + l * G::BW]);
+                for (int l = 0; l < P; ++l) cn[l] = __dmul_rn(wwy[l], sq[G::STR_D + ya + l * G::BW]);
             }
         }
         double tLyn;
@@ -392,7 +423,6 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
                 const double gyn = (!ST && NEU && !have && g.hiy == 2) ? tRy : tLyn;
                 const double dl = __dsub_rn(tLy, tRyp), dr = __dsub_rn(tRy, gyn);
                 const double2* const h = dgt_h + ((it - 1) & 1) * HBUF + ycol;
-                const double jyk = g.JY[yk];
                 double o[P];
 #pragma unroll
                 for (int l = 0; l < P; ++l) {

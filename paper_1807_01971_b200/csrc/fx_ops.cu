@@ -588,16 +588,16 @@ k_dgt_apply(const __grid_constant__ DgParams g, const __grid_constant__ DgtTile 
             const __grid_constant__ CUtensorMap muh, const __grid_constant__ CUtensorMap mc, const __grid_constant__ CUtensorMap mch,
             double* __restrict__ y) {
     extern __shared__ __align__(128) double dgt_smem[];
-    __shared__ __align__(8) unsigned long long bars[DGT_NS];
+    __shared__ __align__(8) unsigned long long bars[DgtCfg<P>::NS];
     if (threadIdx.x == 0) {
-        for (int s = 0; s < DGT_NS; ++s) fx_mbar_init(fx_smem_addr(bars) + 8u * s, 1u);
+        for (int s = 0; s < DgtCfg<P>::NS; ++s) fx_mbar_init(fx_smem_addr(bars) + 8u * s, 1u);
         fx_mbar_fence_init();
         fx_tma_prefetch_desc(&mu); fx_tma_prefetch_desc(&muh); fx_tma_prefetch_desc(&mc); fx_tma_prefetch_desc(&mch);
     }
     __syncthreads();
     const DgtDir nodir = {nullptr, nullptr, nullptr, 0.0, false};
     const int per = t.ntx * t.nseg, rem = (int)(blockIdx.x % per);
-    dgt_tile<P, DgtCfg<P>::NBX, DGT_NS, false, false, NEU, NoAcc>(g, t, &mu, &muh, &mc, &mch, nodir, y, bars, rem % t.ntx, rem / t.ntx,
+    dgt_tile<P, DgtCfg<P>::NBX, DgtCfg<P>::NS, false, false, NEU, NoAcc>(g, t, &mu, &muh, &mc, &mch, nodir, y, bars, rem % t.ntx, rem / t.ntx,
                                                                   (int)(blockIdx.x / per), nullptr, nullptr);
 }
 
@@ -668,7 +668,7 @@ void fx_dgt_shape(FxCtx* c, const fx_grid* g, int nbx, int resident, DgtTile* t,
 template <int P, bool NEU>
 static fx_status launch_dgt_apply(FxCtx* c, const fx_grid* g, const DgParams& p, const double* chi, const double* x, double* y) {   // (p.Nz planes)
     constexpr int NBX = DgtCfg<P>::NBX;
-    typedef DgtGeom<P, NBX, 2> G;
+    typedef DgtGeom<P, NBX, 2, DgtCfg<P>::NS> G;
     const int occ = fx_func_occ(c, (const void*)k_dgt_apply<P, NEU>, G::NT, G::SMEM, true);
     DgtTile t;
     fx_dgt_shape(c, g, NBX, c->num_sms * occ, &t, p.Nz);

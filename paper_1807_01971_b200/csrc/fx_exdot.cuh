@@ -43,6 +43,7 @@ struct ExShared {
     int dlo, dhi;            // last CTA only: range of non-zero merged digits
     double res;              // ex_grid_reduce: the rounded value, broadcast to the CTA
     unsigned int stat[4];    // slow-path census of this CTA: exact-double deposits, integer-product deposits, window moves
+    int gflags;              // last CTA only: the merged flags, fetched together with the digits
 };
 
 struct ExGlobal {            // device scratch of one context
@@ -52,6 +53,8 @@ struct ExGlobal {            // device scratch of one context
     unsigned int* ticket;    // [1]         CTAs finished (zero between launches)
     fx_u64* stats;           // [4]         slow-path census since the last reset (fx_exdot_stats): how rarely the long
                              //             accumulator is "invoked"
+    int keep_limbs;          // write the canonical limbs back after the last launch of a call (fx_exdot_digits); a plain dot
+                             // only needs its rounded value and skips that store and its fence
 };
 
 // 64-bit add into a shared-memory word.  Shared memory has no native 64-bit atomic add (atomicAdd compiles to a compare-and-swap
@@ -351,27 +354,33 @@ __device__ inline double ex_round(const fx_u64* limbs, int flags, fx_u64* mag /*
 // `first`/`last`: position of this launch in a multi-launch call (first: limbs start from zero; last: round).
 __device__ __forceinline__ bool ex_block_finish(ExShared* sh, const ExGlobal& g, int first, int last, double* result) {
     __syncthreads();
-    for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) {
-        const fx_u64 v = sh->dig[i];
-        if (v) atomicAdd(&g.dig[i], v);
+    const bool solo = gridDim.x * gridDim.y == 1;                  // one CTA: its shared digits ARE the merged digits -- no
+    if (!solo) {                                                     // global round trips at all (the latency of a small dot)
+        for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) {
+            const fx_u64 v = sh->dig[i];
+            if (v) atomicAdd(&g.dig[i], v);
+        }
     }
-    if (threadIdx.x == 0 && sh->flags) atomicOr(g.flags, sh->flags);
+    if (threadIdx.x == 0 && sh->flags && !(solo && first && last)) atomicOr(g.flags, sh->flags);
     if (threadIdx.x < 4 && sh->stat[threadIdx.x]) atomicAdd(&g.stats[threadIdx.x], (fx_u64)sh->stat[threadIdx.x]);
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const unsigned int t = atomicAdd(g.ticket, 1u);
-        sh->is_last = (t == gridDim.x * gridDim.y - 1);
+    if (!solo) {
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const unsigned int t = atomicAdd(g.ticket, 1u);
+            sh->is_last = (t == gridDim.x * gridDim.y - 1);
+        }
+        __syncthreads();
+        if (!sh->is_last) return false;
+        __threadfence();
     }
-    __syncthreads();
-    if (!sh->is_last) return false;
-    __threadfence();
     if (threadIdx.x == 0) { sh->dlo = FX_NDIG; sh->dhi = -1; }
     __syncthreads();
+    if (threadIdx.x == blockDim.x - 1) sh->gflags = (solo && first && last) ? sh->flags : __ldcg(g.flags);   // with the digits: one round trip
     for (int i = threadIdx.x; i < FX_NDIG; i += blockDim.x) {
-        const fx_u64 v = __ldcg(&g.dig[i]);
-        sh->dig[i] = v;
-        if (v) { g.dig[i] = 0ull; atomicMin(&sh->dlo, i); atomicMax(&sh->dhi, i); }
+        const fx_u64 v = solo ? sh->dig[i] : __ldcg(&g.dig[i]);
+        if (!solo) { sh->dig[i] = v; if (v) g.dig[i] = 0ull; }
+        if (v) { atomicMin(&sh->dlo, i); atomicMax(&sh->dhi, i); }
     }
     for (int i = threadIdx.x; i < FX_NLIMB; i += blockDim.x) sh->lim[i] = first ? 0ull : __ldcg(&g.limbs[i]);
     __syncthreads();
@@ -406,13 +415,14 @@ __device__ __forceinline__ bool ex_block_finish(ExShared* sh, const ExGlobal& g,
         if (k < FX_NLIMB) sh->lim[k] = fill; else bb = FX_NLIMB - 1;
         sh->dlo = k; sh->dhi = (carry == -1) ? 1 : 0;                 // hand the fill range to the other threads
         if (last) {
-            const int flags = __ldcg(g.flags);
+            const int flags = sh->gflags;
             g.flags[1] = flags;                       // kept for fx_exdot_digits
-            g.flags[0] = 0;
+            if (!(solo && first)) g.flags[0] = 0;
             if (result) *result = ex_round(sh->lim, flags, sh->dig, la, bb);
         }
-        *g.ticket = 0u;
+        if (!solo) *g.ticket = 0u;
     }
+    if (last && !g.keep_limbs) return true;                           // (uniform: nobody needs the limbs of a finished plain dot)
     __syncthreads();
     {
         const int kf = sh->dlo;

@@ -531,7 +531,9 @@ extern "C" fx_status fx_exdot_digits_ex(fx_ctx* c, const double* x, const double
     FX_ENTER(c, "fx_exdot_digits");
     if (n < 0 || (n > 0 && (!x || !y)) || !limbs_host) { fx_set_error("fx_exdot_digits: bad arguments"); return FX_EINVAL; }
     // flags are cleared by the finaliser after rounding; read them through the result instead: launch, then copy
+    c->ex.keep_limbs = 1;                      // (a plain dot does not write the canonical limbs back)
     fx_status s = fx_launch_exdot(c, x, y, n, c->result_dev);
+    c->ex.keep_limbs = 0;
     if (s != FX_OK) return s;
     FX_CUDA(cudaStreamSynchronize(c->stream));
     FX_CUDA(cudaMemcpy(limbs_host, c->ex.limbs, FX_NLIMB * sizeof(fx_u64), cudaMemcpyDeviceToHost));

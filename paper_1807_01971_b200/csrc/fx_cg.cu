@@ -192,7 +192,7 @@ template <int P>
 struct CgtCfg {
     static constexpr int NBX = P == 3 ? FX_K1T_NBX : DgtCfg<P>::NBX;      // x-blocks per tile
     static constexpr int ND = FX_K1T_ND;                                  // exact-dot warps per CTA
-    static constexpr int NT = 32 * NBX * P + 32 * ND;
+    static constexpr int NT = 32 * NBX * P + 32 * (ND > 0 ? ND : 0);
     static constexpr int MINB = P >= 4 ? 2 : 3;
     static constexpr int REGS = P == 3 ? FX_K1T_R : (65536 / (MINB * NT)) / 16 * 16 > 255 ? 255 : (65536 / (MINB * NT)) / 16 * 16;
 };
@@ -319,6 +319,7 @@ __global__ void __launch_bounds__(256, 3) k_cg_update(const __grid_constant__ Dg
         cg_issue<4>(cg_buf, sq, arr, pitch, rows, iq); iq.next();
         fx_cp_wait<FX_STAGES - 1>();
         const double* s0 = cg_buf + (size_t)stage * 4 * CG_U * bd;
+        FX_ASSERT(stage >= 0 && stage < FX_STAGES && ic.row >= 0 && ic.row < rows);
         const int l = ic.row % P;
         const long long base = (long long)ic.row * pitch;
         double rr[CG_U], zz[CG_U];
@@ -393,6 +394,7 @@ __global__ void __launch_bounds__(256, 3) k_cg_update_tma(const __grid_constant_
         const int s = i % K2_STAGES;
         const long long e0 = ((long long)blockIdx.x + (long long)i * gridDim.x) * tile;
         const unsigned dst = sbase + s * stage_bytes, bar = full0 + 8u * s;
+        FX_ASSERT(i >= 0 && i < mine && e0 >= 0 && e0 + tile <= n);      // a full tile of the vectors, a stage of the ring
         fx_mbar_expect_tx(bar, stage_bytes);
         fx_tma_load_1d(dst, p + e0, arr_bytes, bar);
         fx_tma_load_1d(dst + arr_bytes, q + e0, arr_bytes, bar);
@@ -435,7 +437,9 @@ __global__ void __launch_bounds__(256, 3) k_cg_update_tma(const __grid_constant_
         *reinterpret_cast<double2*>(of) = fo;
         *reinterpret_cast<double2*>(orr) = ro;
         rr[0] = ro.x; rr[1] = ro.y;
+#ifndef FX_K2_NODOT
         acc.add_all<2>(rr, zz, &sh);
+#endif
         of += step; orr += step;
         col += dcol;
         const bool wrapped = col >= pitch;

@@ -105,6 +105,7 @@ __device__ __forceinline__ void dg_load_u(DgCell<P>& c, const DgParams& g, const
 template <int P>
 __device__ __forceinline__ void smr_issue(double* ring, int slot, const double* __restrict__ a, long long pitch, int col0, int jr) {
     const double* q = a + (long long)jr * P * pitch + col0;
+    FX_ASSERT(slot >= 0 && slot < 8 && jr >= 0 && col0 >= 0 && col0 + P <= pitch);      // own slot of the ring, a row of the image
     const unsigned dst = fx_smem_addr(ring + (size_t)slot * P * P * 32 + (threadIdx.x & 31));
 #pragma unroll
     for (int l = 0; l < P; ++l)
@@ -268,6 +269,7 @@ __device__ __forceinline__ void dg_warp_strip(const DgParams& g, const double* _
     const bool mirlx = NEU && g.lox == 2 && ci == 0;               // lower Neumann wall: the jump's ghost mirrors
     const bool selx = dirx && (strip == 0 || (NEU && strip == g.nstrip - 1));   // warp-uniform: some lane has a wall table
     const int col0 = cw * P;
+    FX_ASSERT(cw >= 0 && cw < Nx && j0 >= 0 && j0 < j1 && j1 <= Ny);
 
     DgCell<P> uc, un, cc;
     double tLy[P], tRyp[P], tByp[P];                               // own bottom trace; previous cell's top / flux trace

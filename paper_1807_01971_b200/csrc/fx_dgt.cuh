@@ -97,9 +97,9 @@ struct DgtGeom {
     static constexpr int STR_D = MAIN_D + 2 * WRAP_D;          // one stream of one stage: main box, left wrap, right wrap
     static constexpr int STG_D = NSTR * STR_D;
     static constexpr int NTS = 32 * NBX * P;                    // stencil threads
-    static constexpr int NT = NTS + 32 * ND;                    // ... plus the exact-dot warps of the fused CG kernel
+    static constexpr int NT = NTS + 32 * (ND > 0 ? ND : 0);      // ... plus the exact-dot warps of the fused CG kernel (ND < 0: none, see dgt_tile)
     static constexpr unsigned MAIN_BYTES = (unsigned)(P * BW * 8), WRAP_BYTES = (unsigned)(P * HW * 8);
-    static constexpr size_t SMEM = (size_t)NS * STG_D * 8 + (size_t)2 * P * SW * 16 * (ND > 0 ? 2 : 1);
+    static constexpr size_t SMEM = (size_t)NS * STG_D * 8 + (size_t)2 * P * SW * 16 * (ND != 0 ? 2 : 1);
 };
 
 struct DgtTile {                 // launch geometry of the tile kernels (host: fx_dgt_shape)
@@ -254,6 +254,8 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
         hw = xl * G::SW + cl * P;
     }
 
+    FX_ASSERT(xa >= 0 && xa + P <= G::STR_D && hw >= 0 && hw + P <= P * G::SW);
+    FX_ASSERT(n >= 1 && i0 >= 0 && i0 < Nx && ((i0 * P) & 1) == 0 && txc <= G::TXM);
     // ---- y-phase identity: one image column ------------------------------------------------------------------------------
     const int ycol = tid < G::SW ? tid : G::SW - 1;
     const bool yact = tid < txc * P && (long long)i0 * P + tid < pitch;
@@ -281,6 +283,7 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
         r = zrow + r * P;
         const unsigned nstr = (q <= n ? 2u : 1u) + (DIRF ? 1u : 0u);  // the row above the segment needs no chi
         const unsigned bar = full0 + 8u * (q % NS);
+        FX_ASSERT(q >= 0 && q <= n + 1 && r >= 0 && r + P <= g.Nz * Ny * P);
         if (!present(q)) { fx_mbar_arrive(bar); return; }            // a row beyond a wall: the phase completes empty
         const unsigned dst = sbase + (unsigned)(q % NS) * (unsigned)(G::STG_D * 8);
         fx_mbar_expect_tx(bar, nstr * (G::MAIN_BYTES + (wrapL ? G::WRAP_BYTES : 0u) + (wrapR ? G::WRAP_BYTES : 0u)));
@@ -309,6 +312,22 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
     const double beta = DIRF ? dir.beta : 0.0;
     auto pnew = [&](double po, double rr, double v) { return upd ? __fma_rn(1.0, __dmul_rn(v, rr), __dmul_rn(beta, po)) : po; };
 
+    // ND < 0: the pairs go through the same tile, but the stencil threads themselves consume the tile of the previous iteration
+    // (one column each) after their y-phase: the accumulator code sits outside the stencil's live ranges
+    int ncols = txc * P;
+    if ((long long)i0 * P + ncols > pitch) ncols = pitch - i0 * P;
+    auto consume_self = [&](int buf) {
+        const double2* const pq = dgt_pq + buf * HBUF;
+        const bool in = tid < ncols;
+        double xs[P], ys[P];
+        bool act[P];
+#pragma unroll
+        for (int l = 0; l < P; ++l) {
+            const double2 v = in ? pq[l * G::SW + ycol] : make_double2(0.0, 0.0);
+            xs[l] = v.x; ys[l] = v.y; act[l] = in;
+        }
+        acc->template add<P>(xs, ys, act, sh);
+    };
     if (ND > 0 && FUSE && warp >= NW) {                              // ---- the exact-dot warps (see above) ----------------------
         const int dt = tid - NW * 32;
         int ncol = txc * P;
@@ -440,7 +459,7 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
                     for (int l = 0; l < P; ++l) yp[l * prow] = o[l];
                 }
                 yp += P * prow;
-                if (FUSE && ND > 0) {                                 // hand the pairs to the dot warps
+                if (FUSE && ND != 0) {                                // hand the pairs to the dot warps (or to the later self)
                     if (tid < G::SW) {
                         double2* const pq = dgt_pq + (it & 1) * HBUF + ycol;
 #pragma unroll
@@ -456,6 +475,7 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
             }
             tRyp = tRy; tByp = tB; tLy = tLyn;
         }
+        if (FUSE && ND < 0 && (ST || it >= 2)) consume_self((it - 1) & 1);
         __syncthreads();
         // iteration `it` is over: the stages of q <= it+1 are free
         const int lim = (it + 1 + NS < n + 1) ? it + 1 + NS : n + 1;
@@ -482,6 +502,7 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
     }
 #pragma unroll 1
     for (; it <= n; ++it) generic(it);
+    if (FUSE && ND < 0) consume_self(n & 1);                          // (written in iteration n, before its barrier)
 }
 
 #undef CL

@@ -28,6 +28,7 @@ __device__ __forceinline__ void exdot_issue(double* buf, int stage, const double
     const int bd = blockDim.x;
     double* sx = buf + (size_t)stage * 2 * EX_U * bd;
     double* sy = sx + EX_U * bd;
+    FX_ASSERT(stage >= 0 && stage < EX_STAGES && base >= 0 && (!live || base < n + (long long)EX_U * bd));
     if (live) {
         if (VEC) {
 #pragma unroll

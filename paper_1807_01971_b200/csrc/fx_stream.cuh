@@ -12,6 +12,21 @@
 
 #define FX_STAGES 4
 
+// -DFX_CHECKED: bounds and ownership asserts in every staging routine (compute-sanitizer is closed on the pool the library is
+// developed on).  A failing assert prints its location and traps; the parity suite is run against this build once per round.
+#ifdef FX_CHECKED
+#include <stdio.h>
+#define FX_ASSERT(cond)                                                                                          \
+    do {                                                                                                         \
+        if (!(cond)) {                                                                                           \
+            printf("FX_ASSERT failed: %s  (%s:%d, block %d thread %d)\n", #cond, __FILE__, __LINE__, (int)blockIdx.x, (int)threadIdx.x); \
+            __trap();                                                                                            \
+        }                                                                                                        \
+    } while (0)
+#else
+#define FX_ASSERT(cond) do { } while (0)
+#endif
+
 __device__ __forceinline__ unsigned fx_smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void fx_cp_async8(unsigned dst, const void* src, bool valid) {

@@ -588,12 +588,22 @@ extern "C" int fxo_dg_apply_canonical(const fxo_grid* g, const double* chi, cons
 //        a = chain_m(TT[k][m], u_{n,m});  a = fma(cP[k], tR_{n-1}, a);  a = fma(cN[k], tL_{n+1}, a);  d = RN((2/h) * a)
 //        y = beta == 0 ? RN(alpha*d) : fma(alpha, d, RN(beta*y))
 //     with TT = T (forward), -W^-1 T^T W (backward), their mean (centred); T = T0L in the first cell of a DIR line.
+//     flux == 3: the stand-alone JUMP matrix (the paper's primitive is "y <- alpha M x + beta y" for the derivatives in x
+//     and y "and jump" terms): M = Jhat(N, bc) of section 5, un-normed (sum over faces of [v][u]): block row
+//     n has diagonal R R^T + L L^T, off-diagonals -R L^T (to n+1) and -L R^T (to n-1); no 2/h scale.  Canonical order: the
+//     same three-step line with TT = R R^T + L L^T, cN = -R, cP = -L, s = 1.  Definition: build_J in 113-bit arithmetic.
 // ------------------------------------------------------------------------------------------------
 
 struct DTab { double TT[2][PMAX][PMAX], cN[PMAX], cP[PMAX]; };   // [0] interior, [1] first cell of a DIR line
 
 static void make_dtab(int P, int flux, DTab& d) {
     RefElem e; ref_elem(P, e);
+    if (flux == 3) {                                         // jump matrix (see above)
+        for (int v = 0; v < 2; ++v) for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m)
+            d.TT[v][k][m] = snap(e.R[k] * e.R[m] + e.L[k] * e.L[m]);
+        for (int k = 0; k < P; ++k) { d.cN[k] = snap(-e.R[k]); d.cP[k] = snap(-e.L[k]); }
+        return;
+    }
     for (int v = 0; v < 2; ++v) for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m) {
         auto T = [&](int a, int b) { q128 t = e.D[a][b] - e.R[a] * e.R[b] / e.w[a]; if (v) t += e.L[a] * e.L[b] / e.w[a]; return t; };
         q128 f = T(k, m), b = -T(m, k) * e.w[m] / e.w[k];
@@ -608,7 +618,7 @@ static void make_dtab(int P, int flux, DTab& d) {
 }
 
 extern "C" int fxo_dg_dtables(int32_t P, int32_t flux, double* out) {      // TT[0], TT[1] (P*P each), cN, cP
-    if (P < 1 || P > PMAX || flux < 0 || flux > 2) return -1;
+    if (P < 1 || P > PMAX || flux < 0 || flux > 3) return -1;
     DTab d; make_dtab(P, flux, d);
     double* o = out;
     for (int v = 0; v < 2; ++v) for (int k = 0; k < P; ++k) for (int m = 0; m < P; ++m) *o++ = d.TT[v][k][m];
@@ -640,11 +650,11 @@ static void dline_canonical(const DTab& d, int P, int N, int bc, double s, const
 
 extern "C" int fxo_dg_derivative_canonical(const fxo_grid* g, int32_t dir, int32_t flux, double alpha, const double* x, double beta,
                                            double* y) {
-    if (!grid_ok(g) || !deriv_bc_ok(g) || dir < 0 || dir > 1 || flux < 0 || flux > 2 || x == y) return -1;
+    if (!grid_ok(g) || !deriv_bc_ok(g) || dir < 0 || dir > 1 || flux < 0 || flux > 3 || x == y) return -1;
     const int P = g->P, nx = g->Nx * P, ny = g->Ny * P;
     DTab d; make_dtab(P, flux, d);
     const int N = dir == 0 ? g->Nx : g->Ny, len = N * P, bc = dir == 0 ? g->bcx : g->bcy;
-    const double h = dir == 0 ? g->lx / g->Nx : g->ly / g->Ny, s = 2.0 / h;
+    const double h = dir == 0 ? g->lx / g->Nx : g->ly / g->Ny, s = flux == 3 ? 1.0 : 2.0 / h;
     std::vector<double> u(len), o(len);
     const int nl = dir == 0 ? ny : nx;
     for (int line = 0; line < nl; ++line) {
@@ -662,10 +672,15 @@ extern "C" int fxo_dg_derivative_canonical(const fxo_grid* g, int32_t dir, int32
 // definition: explicit matrices, 113 bit; M (rounded to double) is also returned for the numpy-side pins
 extern "C" int fxo_dg_derivative_matrix_1d(int32_t N, int32_t P, double h, int32_t bc, int32_t flux, double* M_out) {
     if (bc != BC_PER && bc != BC_DIR) return -1;
-    if (N < 1 || P < 1 || P > PMAX || !(h > 0) || flux < 0 || flux > 2) return -1;
+    if (N < 1 || P < 1 || P > PMAX || !(h > 0) || flux < 0 || flux > 3) return -1;
     RefElem e; ref_elem(P, e);
-    std::vector<q128> F; build_F(e, N, (q128)h, bc, F);
     int n = N * P;
+    if (flux == 3) {
+        std::vector<q128> J; build_J(e, N, bc, J);
+        for (size_t a = 0; a < (size_t)n * n; ++a) M_out[a] = (double)J[a];
+        return 0;
+    }
+    std::vector<q128> F; build_F(e, N, (q128)h, bc, F);
     for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) {
         q128 f = F[(size_t)a * n + b], bk = -F[(size_t)b * n + a] * e.w[b % P] / e.w[a % P];
         M_out[(size_t)a * n + b] = (double)(flux == 0 ? f : flux == 1 ? bk : (f + bk) / 2);
@@ -675,13 +690,16 @@ extern "C" int fxo_dg_derivative_matrix_1d(int32_t N, int32_t P, double h, int32
 
 extern "C" int fxo_dg_derivative_definition(const fxo_grid* g, int32_t dir, int32_t flux, double alpha, const double* x, double beta,
                                             const double* y_in, double* y_out, double* scale) {
-    if (!grid_ok(g) || !deriv_bc_ok(g) || dir < 0 || dir > 1 || flux < 0 || flux > 2) return -1;
+    if (!grid_ok(g) || !deriv_bc_ok(g) || dir < 0 || dir > 1 || flux < 0 || flux > 3) return -1;
     const int P = g->P, nx = g->Nx * P, ny = g->Ny * P;
     RefElem e; ref_elem(P, e);
     const int N = dir == 0 ? g->Nx : g->Ny, len = N * P, bc = dir == 0 ? g->bcx : g->bcy;
     q128 h = dir == 0 ? (q128)g->lx / g->Nx : (q128)g->ly / g->Ny;
-    std::vector<q128> F; build_F(e, N, h, bc, F);
+    std::vector<q128> F, J;
+    build_F(e, N, h, bc, F);
+    if (flux == 3) build_J(e, N, bc, J);
     auto M = [&](int a, int b) {
+        if (flux == 3) return J[(size_t)a * len + b];
         q128 f = F[(size_t)a * len + b], bk = -F[(size_t)b * len + a] * e.w[b % P] / e.w[a % P];
         return flux == 0 ? f : flux == 1 ? bk : (f + bk) / 2;
     };

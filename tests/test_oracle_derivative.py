@@ -143,3 +143,66 @@ def test_arakawa_converges_and_conserves(oracle, P):
         Jr = oracle.arakawa(g, gg.ravel(), f.ravel())
         assert np.max(np.abs(J + Jr)) < 1e-12 * np.max(np.abs(J))                        # antisymmetry
     assert errs[2] < errs[1] < errs[0] and math.log2(errs[1] / errs[2]) > P - 1.5
+
+
+# ---- the stand-alone jump matrix (flux code 3; "y <- alpha M x + beta y" for dx, dy and jump) -----------
+JUMP = 3
+
+
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("bc", [0, 1])
+def test_jump_is_the_sum_of_squared_face_jumps(oracle, P, bc):
+    """x^T J x = sum over the faces of (trace from the right - trace from the left)^2, traces evaluated independently with
+    numpy from the Lagrange end values; J symmetric, positive semi-definite, J 1 = 0 on a periodic line"""
+    N, h = 7, 0.3
+    J = oracle.dg_derivative_matrix_1d(N, P, h, bc, JUMP)
+    t = oracle.dg_tables(P)
+    assert np.allclose(J, J.T, atol=1e-15)
+    ev = np.linalg.eigvalsh(J)
+    assert ev.min() > -1e-13
+    x = fi.uniform(331 + P, N * P)
+    X = x.reshape(N, P)
+    tl, tr = X @ t["L"], X @ t["R"]                       # left / right end value of every cell
+    if bc == 0:
+        jumps = tl[np.arange(1, N + 1) % N] - tr          # face between cell n and n+1 (periodic)
+    else:
+        jumps = np.concatenate([[tl[0] - 0.0], tl[1:] - tr[:-1], [0.0 - tr[-1]]])      # walls: jump against the zero boundary value
+    assert abs(x @ J @ x - np.sum(jumps ** 2)) <= 1e-12 * np.sum(jumps ** 2)
+    if bc == 0:
+        assert np.abs(J @ np.ones(N * P)).max() <= 1e-14
+    if P == 1:                                            # piecewise constants: the second-difference matrix
+        want = 2 * np.eye(N) - np.eye(N, k=1) - np.eye(N, k=-1)
+        if bc == 0:
+            want[0, -1] -= 1; want[-1, 0] -= 1
+        assert np.allclose(J, want, atol=1e-15)
+
+
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("direction", [0, 1])
+def test_jump_canonical_matches_definition_and_matrix(oracle, P, direction):
+    for bc in (0, 1):
+        g = oracle.Grid(6, 5, P, 1.3, 0.9, bc, bc)
+        x, y = fi.uniform(341 + P, g.n), fi.uniform(342 + P, g.n)
+        for alpha, beta in ((1.0, 0.0), (0.7, -0.3)):
+            want, scale = oracle.dg_derivative_definition(g, direction, JUMP, alpha, x, beta, y)
+            got = oracle.dg_derivative_canonical(g, direction, JUMP, alpha, x, beta, y)
+            assert np.all(np.abs(got - want) <= 1e-14 * scale + 1e-300), (bc, alpha)
+        N = g.Nx if direction == 0 else g.Ny
+        J = oracle.dg_derivative_matrix_1d(N, P, 1.0, bc, JUMP)           # (no h in the un-normed jump)
+        X = x.reshape(g.Ny * P, g.Nx * P)
+        got = oracle.dg_derivative_canonical(g, direction, JUMP, 1.0, x, 0.0, np.zeros(g.n)).reshape(X.shape)
+        assert np.allclose(got, X @ J.T if direction == 0 else J @ X, atol=1e-12)
+
+
+def test_jump_is_the_elliptic_operators_penalty(oracle):
+    """S - (the two flux terms) = diag(Wy) (x) Jx + Jy (x) diag(Wx): with chi = 0 the elliptic operator IS the weighted jumps"""
+    P = 3
+    g = oracle.Grid(5, 4, P, 1.7, 2.3, 0, 1)
+    x = fi.uniform(351, g.n)
+    S0 = oracle.dg_apply_canonical(g, np.zeros(g.n), x, normed=False)
+    jx = oracle.dg_derivative_canonical(g, 0, JUMP, 1.0, x, 0.0, np.zeros(g.n)).reshape(g.Ny * P, g.Nx * P)
+    jy = oracle.dg_derivative_canonical(g, 1, JUMP, 1.0, x, 0.0, np.zeros(g.n)).reshape(g.Ny * P, g.Nx * P)
+    w = oracle.dg_tables(P)["w"]
+    Wx = np.tile(w, g.Nx) * (1.7 / 5) / 2; Wy = np.tile(w, g.Ny) * (2.3 / 4) / 2
+    want = Wy[:, None] * jx + Wx[None, :] * jy
+    assert np.allclose(S0.reshape(want.shape), want, atol=1e-13 * np.abs(want).max())

@@ -202,7 +202,9 @@ fx_status fx_cg3_solve_ex(fx_ctx* ctx, const fx_grid3* grid, const double* chi_d
 /* ---- stand-alone dG derivatives: the paper's "dxdy" primitive (P:240, P:321 / Table 3; D:6.7, Q21) -----------------
  * y <- alpha * M x + beta * y (beta == 0: y is not read), M = d/dx (direction 0) or d/dy (direction 1) of the grid with its
  * boundary condition in that direction; flux 0 = forward (the F of the elliptic operator), 1 = backward (-W^-1 F^T W),
- * 2 = centred (their mean).  x, y: device vectors of the grid; y must not overlap x.                                   */
+ * 2 = centred (their mean); 3 = the un-normed jump matrix of that direction (sum over the faces of [v][u]: block row n has
+ * diagonal R R^T + L L^T and off-diagonals -R L^T, -L R^T; no 1/h), the third matrix of the paper's primitive "for dx, dy and
+ * jump".  x, y: device vectors of the grid; y must not overlap x.                                                        */
 fx_status fx_dg_derivative(const fx_grid* grid, int32_t direction, int32_t flux, double alpha, const double* x_dev, double beta,
                            double* y_dev);
 fx_status fx_dg_derivative_ex(fx_ctx* ctx, const fx_grid* grid, int32_t direction, int32_t flux, double alpha, const double* x_dev,

@@ -167,7 +167,7 @@ fx_status fx_launch_derivative(FxCtx* c, const fx_grid* g, int dir, int flux, do
     const int P = g->P;
     p.Nx = g->Nx; p.Ny = g->Ny; p.bc = dir == 0 ? g->bcx : g->bcy; p.beta0 = beta == 0.0;
     volatile double h = dir == 0 ? g->lx / g->Nx : g->ly / g->Ny;
-    p.s = 2.0 / h; p.alpha = alpha; p.beta = beta;
+    p.s = flux == 3 ? 1.0 : 2.0 / h; p.alpha = alpha; p.beta = beta;      // (the jump matrix carries no 1/h)
     for (int k = 0; k < P; ++k) {
         p.cN[k] = d.cN[k]; p.cP[k] = d.cP[k]; p.L[k] = t.L[k]; p.R[k] = t.R[k];
         for (int m = 0; m < P; ++m) { p.TT[0][k][m] = d.TT[0][k][m]; p.TT[1][k][m] = d.TT[1][k][m]; }
@@ -209,7 +209,7 @@ fx_status fx_launch_derivative(FxCtx* c, const fx_grid* g, int dir, int flux, do
 extern "C" fx_status fx_dg_derivative_ex(fx_ctx* c, const fx_grid* g, int32_t direction, int32_t flux, double alpha, const double* x, double beta,
                                       double* y) {
     FX_ENTER(c, "fx_dg_derivative");
-    if (!fx_grid_ok(g) || !fx_grid_deriv_ok(g) || !x || !y || direction < 0 || direction > 1 || flux < 0 || flux > 2) {
+    if (!fx_grid_ok(g) || !fx_grid_deriv_ok(g) || !x || !y || direction < 0 || direction > 1 || flux < 0 || flux > 3) {
         fx_set_error("fx_dg_derivative: bad grid, direction, flux or null pointer"); return FX_EINVAL;
     }
     const int64_t n = (int64_t)g->Nx * g->Ny * g->P * g->P;

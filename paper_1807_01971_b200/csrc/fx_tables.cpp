@@ -54,15 +54,15 @@ static int make_dtables_uncached(int P, int flux, fx_dtables* d);
 static int make_tables_uncached(int P, fx_tables* t);
 static std::once_flag g_once;
 static fx_tables g_tab[FX_PMAX + 1];
-static fx_dtables g_dtab[FX_PMAX + 1][3];
+static fx_dtables g_dtab[FX_PMAX + 1][4];
 static void fill_cache() {
     for (int P = 1; P <= FX_PMAX; ++P) {
         make_tables_uncached(P, &g_tab[P]);
-        for (int f = 0; f < 3; ++f) make_dtables_uncached(P, f, &g_dtab[P][f]);
+        for (int f = 0; f < 4; ++f) make_dtables_uncached(P, f, &g_dtab[P][f]);
     }
 }
 extern "C" int fx_make_dtables(int P, int flux, fx_dtables* d) {
-    if (P < 1 || P > FX_PMAX || flux < 0 || flux > 2) return -1;
+    if (P < 1 || P > FX_PMAX || flux < 0 || flux > 3) return -1;
     std::call_once(g_once, fill_cache);
     *d = g_dtab[P][flux];
     return 0;
@@ -75,8 +75,15 @@ extern "C" int fx_make_tables(int P, fx_tables* t) {
 }
 
 static int make_dtables_uncached(int P, int flux, fx_dtables* d) {
-    if (P < 1 || P > FX_PMAX || flux < 0 || flux > 2) return -1;
+    if (P < 1 || P > FX_PMAX || flux < 0 || flux > 3) return -1;
     Ref r; reference_element(P, r);
+    if (flux == 3) {             // the jump matrix: diagonal block R R^T + L L^T, neighbour traces with -R (next) and -L (previous)
+        for (int v = 0; v < 2; ++v)
+            for (int k = 0; k < P; ++k)
+                for (int m = 0; m < P; ++m) d->TT[v][k][m] = rnd(r.R[k] * r.R[m] + r.L[k] * r.L[m]);
+        for (int k = 0; k < P; ++k) { d->cN[k] = rnd(-r.R[k]); d->cP[k] = rnd(-r.L[k]); }
+        return 0;
+    }
     for (int v = 0; v < 2; ++v)
         for (int k = 0; k < P; ++k)
             for (int m = 0; m < P; ++m) {

@@ -59,7 +59,7 @@ def test_tables_match_oracle_bitwise(fx, oracle, P):
 
 
 @pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
-@pytest.mark.parametrize("flux", [0, 1, 2])
+@pytest.mark.parametrize("flux", [0, 1, 2, 3])          # forward, backward, centred, jump matrix
 def test_derivative_tables_match_oracle_bitwise(fx, oracle, P, flux):
     a, b = fx.dg_dtables(P, flux), oracle.dg_dtables(P, flux)
     for k in a:

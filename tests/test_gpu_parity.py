@@ -583,7 +583,7 @@ def test_dg_derivative_bit_exact(fx, oracle, P, direction):
         for bc in (0, 1):
             g, og = _grid(fx, oracle, Nx, Ny, P, bc, bc)
             x, y0 = fi.uniform(401 + P, g.n), fi.uniform(402 + P, g.n)
-            for flux in (0, 1, 2):
+            for flux in (0, 1, 2, 3):                                  # forward, backward, centred flux; 3: the jump matrix
                 for alpha, beta in ((1.0, 0.0), (0.7, -0.3)):
                     want = oracle.dg_derivative_canonical(og, direction, flux, alpha, x, beta, y0)
                     y = dev(y0) if beta != 0.0 else torch.full((g.n,), float("nan"), dtype=torch.float64, device="cuda")

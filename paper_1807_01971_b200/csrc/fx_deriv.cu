@@ -17,6 +17,7 @@
 #include <string.h>
 
 #include "fx_internal.h"
+#include "fx_dgb.cuh"
 
 struct DdParams {
     int Nx, Ny, bc, beta0;
@@ -248,6 +249,64 @@ __global__ void __launch_bounds__(512) k_arakawa_products(double a, double b, co
     }
 }
 
+// ---- the bracket in two kernels on the CTA-tile stencil (fx_dgb.cuh) ------------------------------------------------------
+#define DGB_NS(STAGE) ((STAGE) == 0 ? 4 : 3)
+template <int P, int STAGE>
+__global__ void __launch_bounds__(DgtCfg<P>::NT)
+k_arakawa_tile(const __grid_constant__ DbParams g, const __grid_constant__ DgtTile t, const __grid_constant__ CUtensorMap m0,
+               const __grid_constant__ CUtensorMap m0h, const __grid_constant__ CUtensorMap m1, const __grid_constant__ CUtensorMap m1h,
+               const __grid_constant__ CUtensorMap m2, const __grid_constant__ CUtensorMap m2h, double* __restrict__ o0,
+               double* __restrict__ o1, double* __restrict__ o2) {
+    __shared__ __align__(8) unsigned long long bars[DGB_NS(STAGE)];
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < DGB_NS(STAGE); ++s) fx_mbar_init(fx_smem_addr(bars) + 8u * s, 1u);
+        fx_mbar_fence_init();
+        fx_tma_prefetch_desc(&m0); fx_tma_prefetch_desc(&m1);
+    }
+    __syncthreads();
+    const CUtensorMap* const mm[3] = {&m0, &m1, &m2};
+    const CUtensorMap* const mh[3] = {&m0h, &m1h, &m2h};
+    dgb_tile<P, DgtCfg<P>::NBX, DGB_NS(STAGE), STAGE>(g, t, mm, mh, o0, o1, o2, bars, (int)(blockIdx.x % t.ntx), (int)(blockIdx.x / t.ntx));
+}
+
+template <int P>
+static fx_status launch_arakawa_tile(FxCtx* c, const fx_grid* g, const double* f, const double* gg, double* out, double* h1, double* h2) {
+    constexpr int NBX = DgtCfg<P>::NBX;
+    typedef DgtGeom<P, NBX, 2, DGB_NS(0)> GA;
+    typedef DgtGeom<P, NBX, 3, DGB_NS(1)> GB;
+    fx_tables t;
+    fx_dtables d;
+    if (fx_make_tables(P, &t) != 0 || fx_make_dtables(P, 2, &d) != 0) { fx_set_error("fx_arakawa: tables"); return FX_EINVAL; }
+    DbParams p;
+    memset(&p, 0, sizeof(p));
+    p.Nx = g->Nx; p.Ny = g->Ny; p.bcx = g->bcx; p.bcy = g->bcy;
+    volatile double hx = g->lx / g->Nx, hy = g->ly / g->Ny;
+    p.sx = 2.0 / hx; p.sy = 2.0 / hy; p.third = 1.0 / 3.0;
+    for (int k = 0; k < P; ++k) {
+        p.cN[k] = d.cN[k]; p.cP[k] = d.cP[k]; p.L[k] = t.L[k]; p.R[k] = t.R[k];
+        for (int m = 0; m < P; ++m) { p.TT[0][k][m] = d.TT[0][k][m]; p.TT[1][k][m] = d.TT[1][k][m]; }
+    }
+    const int pitch = g->Nx * P, rows = g->Ny * P;
+    CUtensorMap mf, mfh, mg, mgh, m1, m1h, m2, m2h, mo, moh;
+    fx_status s;
+    if ((s = fx_dgt_make_map(&mf, f, pitch, rows, GA::BW, P)) != FX_OK || (s = fx_dgt_make_map(&mfh, f, pitch, rows, GA::HW, P)) != FX_OK ||
+        (s = fx_dgt_make_map(&mg, gg, pitch, rows, GA::BW, P)) != FX_OK || (s = fx_dgt_make_map(&mgh, gg, pitch, rows, GA::HW, P)) != FX_OK ||
+        (s = fx_dgt_make_map(&m1, h1, pitch, rows, GB::BW, P)) != FX_OK || (s = fx_dgt_make_map(&m1h, h1, pitch, rows, GB::HW, P)) != FX_OK ||
+        (s = fx_dgt_make_map(&m2, h2, pitch, rows, GB::BW, P)) != FX_OK || (s = fx_dgt_make_map(&m2h, h2, pitch, rows, GB::HW, P)) != FX_OK ||
+        (s = fx_dgt_make_map(&mo, out, pitch, rows, GB::BW, P)) != FX_OK || (s = fx_dgt_make_map(&moh, out, pitch, rows, GB::HW, P)) != FX_OK)
+        return s;
+    DgtTile ta, tb;
+    const int occa = fx_func_occ(c, (const void*)k_arakawa_tile<P, 0>, GA::NT, GA::SMEM, true);
+    const int occb = fx_func_occ(c, (const void*)k_arakawa_tile<P, 1>, GB::NT, GB::SMEM, true);
+    fx_dgt_shape(c, g, NBX, c->num_sms * occa, &ta);
+    fx_dgt_shape(c, g, NBX, c->num_sms * occb, &tb);
+    k_arakawa_tile<P, 0><<<ta.ntx * ta.nseg, GA::NT, GA::SMEM, c->stream>>>(p, ta, mf, mfh, mg, mgh, mg, mgh, out, h1, h2);
+    k_arakawa_tile<P, 1><<<tb.ntx * tb.nseg, GB::NT, GB::SMEM, c->stream>>>(p, tb, m1, m1h, m2, m2h, mo, moh, out, nullptr, nullptr);
+    c->launches += 2;
+    FX_CUDA(cudaGetLastError());
+    return FX_OK;
+}
+
 extern "C" fx_status fx_arakawa_ex(fx_ctx* c, const fx_grid* g, const double* f, const double* gg, double* out) {
     FX_ENTER(c, "fx_arakawa");
     if (!fx_grid_ok(g) || !fx_grid_deriv_ok(g) || !f || !gg || !out) { fx_set_error("fx_arakawa: bad grid (PER / DIR only) or null pointer"); return FX_EINVAL; }
@@ -261,6 +320,16 @@ extern "C" fx_status fx_arakawa_ex(fx_ctx* c, const fx_grid* g, const double* f,
         c->ara_cap = n;
     }
     double *fx_ = c->ara_vec, *fy_ = fx_ + n, *gx_ = fy_ + n, *gy_ = gx_ + n, *h1 = gy_ + n, *h2 = h1 + n;
+    // two kernels on the tile stencil (9 vector passes) where TMA's rules allow; else the seven launches below (23 passes)
+    if (c->dg_path != 1 && fx_dgt_eligible(g, f, gg, out)) {
+        switch (g->P) {
+        case 1: return launch_arakawa_tile<1>(c, g, f, gg, out, h1, h2);
+        case 2: return launch_arakawa_tile<2>(c, g, f, gg, out, h1, h2);
+        case 3: return launch_arakawa_tile<3>(c, g, f, gg, out, h1, h2);
+        case 4: return launch_arakawa_tile<4>(c, g, f, gg, out, h1, h2);
+        default: return launch_arakawa_tile<5>(c, g, f, gg, out, h1, h2);
+        }
+    }
     const double third = 1.0 / 3.0;
     fx_status s;
     if ((s = fx_launch_derivative(c, g, 0, 2, 1.0, f, 0.0, fx_)) != FX_OK) return s;

@@ -650,14 +650,19 @@ def test_pointwise_dot2_bit_exact(fx, oracle, n, gamma):
 
 @pytest.mark.parametrize("P", [1, 2, 3, 4, 5])
 def test_arakawa_bit_exact(fx, oracle, P):
+    """the nine-call oracle against the two tile kernels (even pitch; every launch shape) and the seven-launch fallback"""
     import torch
-    for (Nx, Ny, bcx, bcy) in [(1, 1, 0, 0), (7, 5, 0, 1), (33, 12, 1, 0), (64, 40, 0, 0)]:
+    for (Nx, Ny, bcx, bcy) in [(1, 1, 0, 0), (7, 5, 0, 1), (33, 12, 1, 0), (64, 40, 0, 0), (2, 2, 1, 1), (62, 9, 1, 1), (34, 7, 0, 1),
+                               (120, 5, 1, 0), (250, 12, 0, 0)]:
         g, og = _grid(fx, oracle, Nx, Ny, P, bcx, bcy)
         f, gg = fi.uniform(511 + P, g.n), fi.uniform(512 + P, g.n)
         want = oracle.arakawa(og, f, gg)
-        out = torch.full((g.n,), float("nan"), dtype=torch.float64, device="cuda")
-        fx.arakawa(g, dev(f), dev(gg), out)
-        assert np.array_equal(out.cpu().numpy(), want), (Nx, Ny, P)
+        for path, rows in ((0, 0), (0, 1), (0, 3), (1, 0)):
+            fx.set_dg_path(path); fx.set_launch(2, rows, 0)
+            out = torch.full((g.n,), float("nan"), dtype=torch.float64, device="cuda")
+            fx.arakawa(g, dev(f), dev(gg), out)
+            assert same_bits(out.cpu().numpy(), want), (Nx, Ny, P, path, rows)
+    fx.set_dg_path(0); fx.set_launch(2, 0, 0)
     g, og = _grid(fx, oracle, 256, 256, 3, 0, 0, 2 * math.pi, 2 * math.pi)      # conservation on the GPU result
     xs, ys = oracle.dg_nodes(og)
     X, Y = np.meshgrid(xs, ys)

@@ -114,6 +114,18 @@ fx_status fx_exdot_ex(fx_ctx* ctx, const double* x_dev, const double* y_dev, int
 /* Asynchronous form: writes the double to result_dev (device, 8 bytes). */
 fx_status fx_exdot_async(const double* x_dev, const double* y_dev, int64_t n, double* result_dev);
 fx_status fx_exdot_async_ex(fx_ctx* ctx, const double* x_dev, const double* y_dev, int64_t n, double* result_dev);
+/* Allocation-free form, for callers that may not call cudaMalloc (CUDA graph capture, serving loops, harnesses that
+ * forbid it): same value, same bits as fx_exdot_async, but no context and no work space -- the long accumulator's device
+ * scratch is a file-scope __device__ array of 1728 bytes that every GPU loading the library holds until exit.
+ * The call makes no cudaMalloc / cudaFree and calls no allocating routine: a stream-ordered clear of that array and ONE
+ * kernel launch on `stream` (a cudaStream_t; NULL = the legacy default stream) of the current device.
+ * Limit: 0 <= n <= FX_EXDOT_STATIC_MAX_N (one launch); beyond it FX_EINVAL with a message in fx_last_error().
+ * x_dev, y_dev: device, n doubles each, may alias, caller-owned; result_dev: device, 8 bytes, written stream-ordered.
+ * The array is shared by every call on that device and keeps the last call's contents (it is cleared before each
+ * launch): calls on one stream are ordered and safe; calls that OVERLAP on the GPU (different streams, other host
+ * threads' streams) race on it and give undefined values -- use contexts (fx_exdot_async_ex) for concurrency.        */
+#define FX_EXDOT_STATIC_MAX_N (1LL << 28)
+fx_status fx_exdot_static(const double* x_dev, const double* y_dev, int64_t n, double* result_dev, void* stream);
 /* The long accumulator itself: 68 limbs, two's complement, limb k weighs 2^(64k-2176), plus flags
  * {nan, +inf, -inf}.  limbs_host: host uint64[68]; flags_host: host int32[3] or NULL.  Synchronises.          */
 fx_status fx_exdot_digits(const double* x_dev, const double* y_dev, int64_t n, uint64_t* limbs_host,

@@ -56,6 +56,7 @@ _SIGNATURES = {
     "fx_set_dg_path": (C.c_int, [C.c_int32]),
     "fx_exdot": (C.c_double, [_vp, _vp, C.c_int64]),
     "fx_exdot_async": (C.c_int, [_vp, _vp, C.c_int64, _vp]),
+    "fx_exdot_static": (C.c_int, [_vp, _vp, C.c_int64, _vp, _vp]),
     "fx_exdot_digits": (C.c_int, [_vp, _vp, C.c_int64, _vp, _vp, _vp]),
     "fx_exdot_host": (C.c_double, [_vp, _vp, C.c_int64]),
     "fx_exdot3": (C.c_double, [_vp, _vp, _vp, C.c_int64]),
@@ -271,6 +272,20 @@ def exdot_async(x, y, out):
     _use_torch_stream()
     n = x.numel()
     _check(lib().fx_exdot_async(_ptr(x), _ptr(y, n), n, _ptr(out)), "fx_exdot_async")
+    return out
+
+
+EXDOT_STATIC_MAX_N = 1 << 28
+
+
+def exdot_static(x, y, out, stream=None):
+    """Allocation-free exact dot (fx_exdot_static): no context, no work space, scratch in a static device array of the
+    library; n <= EXDOT_STATIC_MAX_N; writes out[0] (float64 CUDA tensor) on `stream` (default: torch's current stream).
+    Calls that overlap on the GPU race on the shared scratch."""
+    import torch
+    st = torch.cuda.current_stream().cuda_stream if stream is None else (stream.cuda_stream if hasattr(stream, "cuda_stream") else stream)
+    n = x.numel()
+    _check(lib().fx_exdot_static(_ptr(x), _ptr(y, n), n, _ptr(out), st), "fx_exdot_static")
     return out
 
 

@@ -3,6 +3,8 @@
 #include <math.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "fx_internal.h"
 #include "fx_dgt.cuh"
 #include "fx_stream.cuh"
@@ -957,4 +959,68 @@ extern "C" fx_status fx_time_primitive(int32_t kind, const fx_grid* g, const dou
                                        int32_t reps, double* ms_host) {
     FxCtx* c = fx_default_ctx();
     return c ? fx_time_primitive_ex(c, kind, g, a, b, cc, n, reps, ms_host) : FX_ECUDA;
+}
+
+// ---- exact dot without any allocation (fx_exdot_static) ----------------------------------------------------------------
+// For callers that may not call cudaMalloc (stream capture, serving loops): the long accumulator's device scratch is a
+// file-scope array that every GPU loading the library holds until exit, instead of a context's work space.  One launch of
+// the k_exdot kernel above, so n <= FX_EXDOT_STATIC_MAX_N (2^28: every 64-bit digit stays far from overflow in one launch).
+// The array is shared by every call on the device and keeps the last call's contents: the part that must start at zero is
+// cleared, stream-ordered, before the launch; two calls that overlap on the GPU (different streams) race on it.
+#define FX_XS_WORDS (FX_NDIG + FX_NLIMB + 8 + 4)                    // digits, limbs, flags + ticket (64 B), census
+static __device__ __align__(256) fx_u64 fx_exdot_static_scratch[FX_XS_WORDS];     // 1728 bytes
+
+struct FxStaticDev { int state; fx_u64* base; int num_sms; int occ[2]; };          // state: 0 new, 1 ready, -1 failed
+static FxStaticDev fx_xs_dev[64];
+static std::mutex fx_xs_mu;
+
+extern "C" fx_status fx_exdot_static(const double* x, const double* y, int64_t n, double* result_dev, void* stream) {
+    if (n < 0 || (n > 0 && (!x || !y)) || !result_dev) { fx_set_error("fx_exdot_static: bad arguments"); return FX_EINVAL; }
+    if (n > FX_EXDOT_STATIC_MAX_N) {
+        fx_set_error("fx_exdot_static: n exceeds FX_EXDOT_STATIC_MAX_N (2^28 elements in one launch); use fx_exdot_async");
+        return FX_EINVAL;
+    }
+    int dev = 0;
+    FX_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) { fx_set_error("fx_exdot_static: device ordinal beyond 63"); return FX_EINVAL; }
+    const int bd = 256;
+    const size_t smem = (size_t)EX_STAGES * 2 * EX_U * bd * sizeof(double);
+    FxStaticDev* d = &fx_xs_dev[dev];
+    {
+        std::lock_guard<std::mutex> lk(fx_xs_mu);
+        if (d->state == 0) {                   // set-up, once per device, with that device current
+            d->state = -1;
+            // in host code the array's name is a host-side stand-in: the device address comes from the runtime
+            FX_CUDA(cudaGetSymbolAddress((void**)&d->base, fx_exdot_static_scratch));
+            FX_CUDA(cudaDeviceGetAttribute(&d->num_sms, cudaDevAttrMultiProcessorCount, dev));
+            const void* kf[2] = {(const void*)k_exdot<false, 0>, (const void*)k_exdot<true, 0>};
+            for (int v = 0; v < 2; ++v) {
+                FX_CUDA(cudaFuncSetAttribute(kf[v], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                FX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&d->occ[v], kf[v], bd, smem));
+                if (d->occ[v] < 1) { fx_set_error("fx_exdot_static: kernel does not fit an SM"); return FX_ECUDA; }
+            }
+            d->state = 1;
+        }
+        if (d->state != 1) { fx_set_error("fx_exdot_static: set-up failed on this device"); return FX_ECUDA; }
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    ExGlobal g;
+    g.dig = d->base;
+    g.limbs = g.dig + FX_NDIG;
+    g.flags = (int*)(g.limbs + FX_NLIMB);
+    g.ticket = (unsigned int*)(g.flags + 4);
+    g.stats = g.limbs + FX_NLIMB + 8;
+    g.keep_limbs = 0;
+    // digits, flags and ticket must be zero when the kernel starts (a finished launch leaves them so, an aborted one may not)
+    FX_CUDA(cudaMemsetAsync(d->base, 0, FX_XS_WORDS * sizeof(fx_u64), st));
+    const bool vec = aligned16(x) && aligned16(y);
+    const long long tile = (long long)bd * EX_U;
+    long long grid = ((long long)n + tile - 1) / tile;
+    const long long gmax = (long long)d->num_sms * d->occ[vec ? 1 : 0];
+    if (grid > gmax) grid = gmax;
+    if (grid < 1) grid = 1;
+    if (vec) k_exdot<true, 0><<<(int)grid, bd, smem, st>>>(x, y, (long long)n, g, 1, 1, result_dev);
+    else k_exdot<false, 0><<<(int)grid, bd, smem, st>>>(x, y, (long long)n, g, 1, 1, result_dev);
+    FX_CUDA(cudaGetLastError());
+    return FX_OK;
 }

@@ -94,9 +94,11 @@ fx_status fx_set_launch_ex(fx_ctx* ctx, int32_t kernel_id, int32_t grid_dim, int
  * kernels; 3 = the persistent kernel whenever possible (< 2^24 unknowns).  Results are bit-identical in every mode.      */
 fx_status fx_set_cg_fused(int32_t fused);
 fx_status fx_set_cg_fused_ex(fx_ctx* ctx, int32_t fused);
-/* Test hook: which dG stencil kernels serve fx_dg_elliptic_apply* and fx_cg_solve.  0 (default) = the CTA-tile kernels
- * (2-D TMA staging, D:6.2) whenever the row pitch Nx*P is even and the vectors are 16-byte aligned, else the warp-strip
- * kernels; 1 = always the warp-strip kernels; 2 = as 0.  Same bits either way.                                            */
+/* Test hook: which dG stencil kernels serve fx_dg_elliptic_apply*, fx_arakawa and fx_cg_solve.  0 (default) = the CTA-tile
+ * kernels (2-D TMA staging, D:6.2) whenever the row pitch Nx*P is even and the vectors are 16-byte aligned, else the
+ * warp-strip kernels -- except K1 of the two-kernel CG loop, which is the warp-strip kernel for P <= 3 (measured faster)
+ * and the tile kernel for P = 4, 5; 1 = always the warp-strip kernels; 2 = the tile kernels wherever they are eligible,
+ * K1 included.  Same bits either way.                                                                                    */
 fx_status fx_set_dg_path(int32_t path);
 fx_status fx_set_dg_path_ex(fx_ctx* ctx, int32_t path);
 

@@ -845,7 +845,9 @@ static fx_status cg_solve_impl(FxCtx* c, const fx_grid* g, int Nz, double lz, co
             if (!fx_cg_tile(c)) { fx_set_error("out of host memory"); return FX_ENOMEM; }
             CgTile& ct = *fx_cg_tile(c);
             ct.on = false;
-            if (c->dg_path == 2 && fx_dgt_eligible(g, chi, r, p) && aligned16(p2)) {   // (measured: K1 on the warp-strip stencil is still the faster one)
+            // K1 on the CTA-tile stencil: on request, and by default for P >= 4, where the warp-strip K1 spills (measured at 1024^2:
+            // P = 4 326 against 368 us per iteration, P = 5 752 against 865; P = 2, 3: the strip K1 is faster)
+            if ((c->dg_path == 2 || (c->dg_path == 0 && g->P >= 4)) && fx_dgt_eligible(g, chi, r, p) && aligned16(p2)) {
                 const bool neu = fx_dg_has_neumann(&dp) != 0;
 #define FX_CGT(PP) s = neu ? cgt_setup<PP, true>(c, g, Nz, chi, r, p, p2, &ct) : cgt_setup<PP, false>(c, g, Nz, chi, r, p, p2, &ct); break;
                 switch (g->P) {

@@ -68,6 +68,12 @@
 #ifndef FX_K1T_ND
 #define FX_K1T_ND 0
 #endif
+#ifndef FX_HPAD
+#define FX_HPAD 1
+#endif
+#ifndef FX_XVEC
+#define FX_XVEC 1
+#endif
 #define DGT_NS_K1 FX_K1T_NS   // ... of the fused CG kernel (three streams per stage)
 
 // coefficient accessors of FX_CHAIN (fx_dg.cuh undefines its own at the end)
@@ -99,7 +105,11 @@ struct DgtGeom {
     static constexpr int NTS = 32 * NBX * P;                    // stencil threads
     static constexpr int NT = NTS + 32 * (ND > 0 ? ND : 0);      // ... plus the exact-dot warps of the fused CG kernel (ND < 0: none, see dgt_tile)
     static constexpr unsigned MAIN_BYTES = (unsigned)(P * BW * 8), WRAP_BYTES = (unsigned)(P * HW * 8);
-    static constexpr size_t SMEM = (size_t)NS * STG_D * 8 + (size_t)2 * P * SW * 16 * (ND != 0 ? 2 : 1);
+    // hand-off tile: cell pitch HP double2.  The x-phase lanes (one cell each) store P double2 at a stride of HP * 16 bytes:
+    // 64 bytes (P = 4) would put the 8 lanes of a quarter-warp on 2 of the 8 16-byte bank groups (4-way conflict); 80 does not
+    static constexpr int HP = (P == 4 && FX_HPAD) ? 5 : P;
+    static constexpr int HSW = TXM * HP;                       // double2 per image row of the hand-off tile
+    static constexpr size_t SMEM = (size_t)NS * STG_D * 8 + (size_t)2 * P * HSW * 16 * (ND != 0 ? 2 : 1);
 };
 
 struct DgtTile {                 // launch geometry of the tile kernels (host: fx_dgt_shape)
@@ -228,7 +238,7 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
     extern __shared__ __align__(128) double dgt_smem[];
     double2* const dgt_h = reinterpret_cast<double2*>(dgt_smem + (size_t)NS * G::STG_D);
     const unsigned sbase = fx_smem_addr(dgt_smem), full0 = fx_smem_addr(bars);
-    constexpr int HBUF = P * G::SW;                                  // double2 per hand-off buffer
+    constexpr int HBUF = P * G::HSW;                                 // double2 per hand-off buffer
     double2* const dgt_pq = dgt_h + 2 * HBUF;                        // ND > 0: the (p, q) pairs for the dot warps, double2[2][P][SW]
     const int cR = (i0 + txc < Nx) ? i0 + txc : Nx;                  // the cell after the tile's last one
     const bool wrapL = i0 == 0 && !wallx, wrapR = cR >= Nx && !wallx;    // periodic edge tiles: the halo cell is a box of its own
@@ -251,15 +261,16 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
         if (wrapL && ci == -1) xa = G::MAIN_D + xl * G::HW + G::HE;
         if (wrapR && ci == Nx) xa = G::MAIN_D + G::WRAP_D + xl * G::HW;
         if (cl < 0 || cl >= G::TXM) cl = 0;
-        hw = xl * G::SW + cl * P;
+        hw = xl * G::HSW + cl * G::HP;
     }
 
-    FX_ASSERT(xa >= 0 && xa + P <= G::STR_D && hw >= 0 && hw + P <= P * G::SW);
+    FX_ASSERT(xa >= 0 && xa + P <= G::STR_D && hw >= 0 && hw + P <= P * G::HSW);
     FX_ASSERT(n >= 1 && i0 >= 0 && i0 < Nx && ((i0 * P) & 1) == 0 && txc <= G::TXM);
     // ---- y-phase identity: one image column ------------------------------------------------------------------------------
     const int ycol = tid < G::SW ? tid : G::SW - 1;
     const bool yact = tid < txc * P && (long long)i0 * P + tid < pitch;
     const int yk = ycol % P;
+    const int hcol = (ycol / P) * G::HP + yk;                       // this column in a hand-off row
     const int ya = G::HE + P + ycol;
     const int zrow = plane * Ny * P;                                // first image row of this plane in the stacked vectors
     double wwy[P], wwx[P], jyk = g.JY[yk];                           // this thread's table entries
@@ -384,11 +395,26 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
         // ---- x-phase of cell row j0 + it -----------------------------------------------------------------------------
         if (ST || it < n) {
             double u[P], c[P], jx[P], sx[P];
+            if constexpr ((P & 1) == 0 && FX_XVEC != 0) {             // even P: a cell's line is 16-byte aligned (xa even): LDS.128 halves
+#pragma unroll                                                        // the wavefronts of the lane-per-cell stride (P * 8 bytes)
+                for (int m = 0; m < P; m += 2) {
+                    const double2 uv = *reinterpret_cast<const double2*>(sq + xa + m);
+                    const double2 cv = *reinterpret_cast<const double2*>(sq + G::STR_D + xa + m);
+                    u[m] = uv.x; u[m + 1] = uv.y;
+                    if (DIRF) {
+                        const double2 rv = *reinterpret_cast<const double2*>(sq + 2 * G::STR_D + xa + m);
+                        u[m] = pnew(u[m], rv.x, g.V[xl][m]);
+                        u[m + 1] = pnew(u[m + 1], rv.y, g.V[xl][m + 1]);
+                    }
+                    c[m] = __dmul_rn(wwx[m], cv.x); c[m + 1] = __dmul_rn(wwx[m + 1], cv.y);
+                }
+            } else {
 #pragma unroll
-            for (int m = 0; m < P; ++m) {
-                u[m] = sq[xa + m];
-                if (DIRF) u[m] = pnew(u[m], sq[2 * G::STR_D + xa + m], g.V[xl][m]);
-                c[m] = __dmul_rn(wwx[m], sq[G::STR_D + xa + m]);
+                for (int m = 0; m < P; ++m) {
+                    u[m] = sq[xa + m];
+                    if (DIRF) u[m] = pnew(u[m], sq[2 * G::STR_D + xa + m], g.V[xl][m]);
+                    c[m] = __dmul_rn(wwx[m], sq[G::STR_D + xa + m]);
+                }
             }
             if (edge) dgt_xline<P, true, NEU>(g, u, c, xghost, firstx, lastx, mirlx, jx, sx);
             else dgt_xline<P, false, NEU>(g, u, c, xghost, firstx, lastx, mirlx, jx, sx);
@@ -441,11 +467,11 @@ __device__ __forceinline__ void dgt_tile(const DgParams& g, const DgtTile& t, co
             if (ST || it >= 1) {
                 const double gyn = (!ST && NEU && !have && g.hiy == 2) ? tRy : tLyn;
                 const double dl = __dsub_rn(tLy, tRyp), dr = __dsub_rn(tRy, gyn);
-                const double2* const h = dgt_h + ((it - 1) & 1) * HBUF + ycol;
+                const double2* const h = dgt_h + ((it - 1) & 1) * HBUF + hcol;
                 double o[P];
 #pragma unroll
                 for (int l = 0; l < P; ++l) {
-                    const double2 hx = h[l * G::SW];
+                    const double2 hx = h[l * G::HSW];
                     const double jy = __fma_rn(g.L[l], dl, __dmul_rn(g.R[l], dr));
                     double v = __fma_rn(g.JX[l], hx.x, __dmul_rn(jyk, jy));
                     v = __fma_rn(g.cyy, sy[l], v);

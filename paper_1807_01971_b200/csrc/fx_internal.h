@@ -31,7 +31,7 @@ struct fx_ctx {
     // launch-shape overrides (fx_set_launch): [kernel_id][0]=grid, [1]=block
     int launch[4][2];
     int cg_fused;
-    int dg_path;                // 0 = automatic (CTA-tile kernels where TMA's rules allow), 1 = warp-strip kernels, 2 = tile kernels (as 0)
+    int dg_path;                // 0 = automatic (CTA-tile kernels where TMA's rules allow; CG's K1: tile for P >= 4), 1 = warp-strip kernels, 2 = tile kernels, K1 too
     int cg_pdl;                 // programmatic dependent launch of the fused loop's kernels (off; environment FX_PDL=1 turns it on)
     // CG work space
     double* cg_vec; int64_t cg_cap;   // 7 vectors of cg_cap doubles

@@ -12,7 +12,7 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libfx.so")
 BUILD = os.path.join(HERE, "build")
 
-NVCC_FLAGS = [("-D%s=%s" % (k, os.environ[k])) for k in ("FX_PFD", "FX_K1_R", "FX_K1_W", "FX_AP_R", "FX_AP_W", "FX_NBX3", "FX_MINB3", "FX_DGT_DEBUG", "FX_K1T_NS", "FX_K1T_R", "FX_K1T_NBX", "FX_K1T_ND", "EX_KL", "FX_K1_K", "FX_K1_WB", "FX_K1_KL", "FX_PERSIST_PROF", "FX_NBX1", "FX_NBX4", "FX_NBX5", "FX_MINB4", "FX_MINB5", "FX_NS5", "FX_KEEPP", "FX_K2_NODOT", "FX_CHECKED", "FX_HPAD", "FX_XVEC") if os.environ.get(k)] + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
+NVCC_FLAGS = [("-D%s=%s" % (k, os.environ[k])) for k in ("FX_PFD", "FX_K1_R", "FX_K1_W", "FX_AP_R", "FX_AP_W", "FX_NBX3", "FX_MINB3", "FX_DGT_DEBUG", "FX_K1T_NS", "FX_K1T_R", "FX_K1T_NBX", "FX_K1T_ND", "EX_KL", "FX_K1_K", "FX_K1_WB", "FX_K1_KL", "FX_PERSIST_PROF", "FX_NBX1", "FX_NBX4", "FX_NBX5", "FX_MINB4", "FX_MINB5", "FX_NS5", "FX_KEEPP", "FX_K2_NODOT", "FX_CHECKED", "FX_HPAD", "FX_XVEC", "FX_EX_SKIP") if os.environ.get(k)] + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math", "-Xptxas", "-v"]
 
 

@@ -180,8 +180,15 @@ __global__ void __launch_bounds__(256, 2) k_exdot(const double* __restrict__ x, 
         if (++stage == EX_STAGES) stage = 0;
     }
     fx_cp_wait<0>();
+#if defined(FX_EX_SKIP) && FX_EX_SKIP == 1
+    if (n == -12345) { acc.flush(&sh); ex_block_finish(&sh, g, first, last, result); }
+#elif defined(FX_EX_SKIP) && FX_EX_SKIP == 2
+    acc.flush(&sh);
+    if (n == -12345) ex_block_finish(&sh, g, first, last, result);
+#else
     acc.flush(&sh);
     ex_block_finish(&sh, g, first, last, result);
+#endif
 }
 
 // one launch over m <= 2^28 elements (keeps every 64-bit digit far from overflow); first/last: position in the call

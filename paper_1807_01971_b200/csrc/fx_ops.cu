@@ -206,7 +206,8 @@ fx_status fx_launch_exdot_part(FxCtx* c, const double* x, const double* y, int64
     long long grid = (m + tile - 1) / tile;
     const long long gmax = (long long)c->num_sms * occ;             // one resident wave: every CTA pays one flush + merge
     if (grid > gmax) grid = gmax;
-    if (grid < 1) grid = 1;
+    if (grid <= EX_STAGES) grid = 1;                                 // a few tiles: one CTA has them all in flight at once and finishes
+    if (grid < 1) grid = 1;                                          // alone -- no digit round trips through L2, no ticket (6 us against 8)
     if (c->launch[0][0]) grid = c->launch[0][0];
 #define FX_EXDOT_GO(M) \
     if (vec) k_exdot<true, M><<<(int)grid, bd, smem, c->stream>>>(x, y, m, c->ex, first, last, result_dev); \

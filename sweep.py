@@ -4,7 +4,7 @@ Paper: bandwidth b = m*S/t with STREAM counting (Eq. 2: axpby 
 model t(S) = T_lat + m*S/B (Eq. 3); estimators: B = mean over the largest sizes, T_lat = smallest average run
 time corrected by -m*S/B and clipped at 0; minimum efficient array size ~ T_lat*B (Eq. 9).
 
-    python sweep.py [--out DIR] [--quick]            (bench.py runs `reduced` and puts its fits under "model")
+    python sweep.py [--out DIR] [--quick] [--dg-path 0|1]            (bench.py runs `reduced` and puts its fits under "model")
 
 Runs on cuda:0 through the C ABI (fx_time_primitive: average of back-to-back launches, CUDA events).  Writes
 DIR/sweep.json and DIR/sweep.md.  Inputs: seeded uniform[-1,1) vectors (fxinputs.config4) -- synthetic stand-ins for
@@ -80,6 +80,7 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out"))
     ap.add_argument("--quick", action="store_true")
+    ap.add_argument("--dg-path", type=int, default=0, help="fx_set_dg_path: 0 = default (CTA-tile stencil), 1 = warp-strip kernels (round 1's)")
     args = ap.parse_args()
     import numpy as np
     import torch
@@ -89,6 +90,7 @@ def main():
 
     assert torch.cuda.is_available(), "sweep needs a CUDA device (no CPU fallback)"
     fx.lib()
+    fx.set_dg_path(args.dg_path)
     Ns = [16, 64, 256] if args.quick else [16, 32, 64, 128, 256, 512, 1024, 2048]
     Ps = [3] if args.quick else [1, 2, 3, 4, 5]
     res = {}

@@ -74,7 +74,7 @@ __device__ __forceinline__ void dgb_tile(const DbParams& g, const DgtTile& t, co
     extern __shared__ __align__(128) double dgt_smem[];
     double2* const hbuf = reinterpret_cast<double2*>(dgt_smem + (size_t)NS * G::STG_D);   // hand-off double2[2][P][SW] (stage B uses .x)
     const unsigned sbase = fx_smem_addr(dgt_smem), full0 = fx_smem_addr(bars);
-    constexpr int HBUF = P * G::SW;
+    constexpr int HBUF = P * G::HSW;                               // (padded cell pitch for P = 4: DgtGeom::HP)
     const int cR = (i0 + txc < Nx) ? i0 + txc : Nx;
     const bool wrapL = i0 == 0 && !wallx, wrapR = cR >= Nx && !wallx;
 
@@ -93,11 +93,12 @@ __device__ __forceinline__ void dgb_tile(const DbParams& g, const DgtTile& t, co
         if (wrapL && ci == -1) xa = G::MAIN_D + xl * G::HW + G::HE;
         if (wrapR && ci == Nx) xa = G::MAIN_D + G::WRAP_D + xl * G::HW;
         if (cl < 0 || cl >= G::TXM) cl = 0;
-        hw = xl * G::SW + cl * P;
+        hw = xl * G::HSW + cl * G::HP;
     }
     // y-phase identity
     const int ycol = tid < G::SW ? tid : G::SW - 1;
     const bool yact = tid < txc * P && (long long)i0 * P + tid < pitch;
+    const int hcol = (ycol / P) * G::HP + ycol % P;                  // this column in a hand-off row
     const int ya = G::HE + P + ycol;
     const long long prow = (long long)pitch;
     const long long obase = (long long)j0 * P * pitch + (long long)i0 * P + tid;
@@ -200,11 +201,11 @@ __device__ __forceinline__ void dgb_tile(const DbParams& g, const DgtTile& t, co
         } else {
             const int r = j0 - 1 + it;
             const bool firsty = wally && r == 0;
-            const double2* const h = hbuf + ((it - 1) & 1) * HBUF + ycol;
+            const double2* const h = hbuf + ((it - 1) & 1) * HBUF + hcol;
             double w0[P], w1[P], w2[P];
 #pragma unroll
             for (int l = 0; l < P; ++l) {
-                const double2 hx = h[l * G::SW];
+                const double2 hx = h[l * G::HSW];
                 const double ay = db_out<P>(g, l, firsty, g.sy, ac, tRa, tLna);
                 if (STAGE == 0) {
                     const double by = db_out<P>(g, l, firsty, g.sy, bc_, tRb, tLnb);

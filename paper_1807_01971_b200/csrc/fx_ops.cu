@@ -83,6 +83,24 @@ __device__ __forceinline__ void ex_feed(ExDotAcc& acc, const double (&xv)[EX_U],
     } else acc.add<EX_U>(xv, yv, act, sh);
 }
 
+// the same for a full tile (the hot loop): no activity flags, and the 2 * EX_U values of the sum as ONE batch (one range test
+// and one branch per 8 values instead of two batches with selects: the sum is issue-bound; 5.3 -> 5.9 TB/s at 2^26)
+template <int MODE>
+__device__ __forceinline__ void ex_feed_full(ExDotAcc& acc, const double (&xv)[EX_U], const double (&yv)[EX_U], ExShared* sh) {
+    if (MODE == 1) {
+        double v[2 * EX_U], one[2 * EX_U];
+        bool all[2 * EX_U];
+#pragma unroll
+        for (int u = 0; u < EX_U; ++u) { v[u] = xv[u]; v[EX_U + u] = yv[u]; one[u] = 1.0; one[EX_U + u] = 1.0; all[u] = true; all[EX_U + u] = true; }
+        acc.add<2 * EX_U, true, true>(v, one, all, sh);
+    } else if (MODE == 2) {                                          // (the binary32 dot measured 2 % slower as one flag-free batch)
+        bool act[EX_U];
+#pragma unroll
+        for (int u = 0; u < EX_U; ++u) act[u] = true;
+        ex_feed<2>(acc, xv, yv, act, sh);
+    } else acc.add_all<EX_U>(xv, yv, sh);
+}
+
 template <bool VEC, int MODE>
 __device__ __forceinline__ void exdot_consume(const double* buf, int stage, long long n, long long base, ExDotAcc& acc,
                                               ExShared* sh) {
@@ -160,13 +178,7 @@ __global__ void __launch_bounds__(256, 2) k_exdot(const double* __restrict__ x, 
                 fx_lds128(b, s0 + so + arr_bytes + u * u_bytes);
                 xv[2 * u] = a.x; xv[2 * u + 1] = a.y; yv[2 * u] = b.x; yv[2 * u + 1] = b.y;
             }
-            if (MODE == 0) acc.add_all<EX_U>(xv, yv, &sh);           // consumed tile < issued tile: full as well
-            else {
-                bool act[EX_U];
-#pragma unroll
-                for (int u = 0; u < EX_U; ++u) act[u] = true;
-                ex_feed<MODE>(acc, xv, yv, act, &sh);
-            }
+            ex_feed_full<MODE>(acc, xv, yv, &sh);                    // consumed tile < issued tile: full as well
             sqo = so;
             so += stage_bytes; if (so == EX_STAGES * stage_bytes) so = 0;
             if (++stage == EX_STAGES) stage = 0;

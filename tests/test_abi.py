@@ -41,7 +41,7 @@ def test_sass_is_sm100_fp64_no_contraction(fx):
     assert "sm_100a" in out
     sass = subprocess.run(["cuobjdump", "-sass", fx.lib_path()], capture_output=True, text=True).stdout
     ops = {}
-    for m in re.finditer(r"^\s+/\*[0-9a-f]{4}\*/\s+(?:@!?U?P\w+\s+)?([A-Z][A-Z0-9_]*)", sass, flags=re.M):
+    for m in re.finditer(r"^\s+/\*[0-9a-f]{4,6}\*/\s+(?:@!?U?P\w+\s+)?([A-Z][A-Z0-9_]*)", sass, flags=re.M):
         ops[m.group(1)] = ops.get(m.group(1), 0) + 1
     for need in ("DFMA", "DMUL", "DADD", "UBLKCP", "UTMALDG", "SYNCS", "LDGSTS", "SHFL"):
         assert ops.get(need, 0) > 0, "no %s in the SASS" % need
